@@ -1,0 +1,334 @@
+// CPU ORACLE -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, scalar C++17 restatement of the thermochemistry of arXiv 2503.24286
+// (Pyrometheus), Appendix A, point by point, in the order and notation of the paper.
+// Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+// legs may call it.  It shares no code, header, table or constant with the CUDA
+// library (paper_2503_24286_b200/csrc); it has its own mechanism struct and is built
+// with g++ -O2 -ffp-contract=off (no FMA contraction, no fast-math, no blocking or
+// reordering).  The only concession to speed is `#pragma omp parallel for` over the
+// independent points ("no loop-carried dependencies").
+//
+// Every function is instantiated for Real = double (the oracle proper) and
+// Real = long double (80-bit; the arbiter of pin P14).
+//
+// What pins each function (tests/test_oracle_pins.py):
+//   species_thermo      P1 continuity at T_mid, P2 c_p = dh/dT, P3 c_p/T = ds/dT, W2 g/RT values
+//   mixture_e / cv      P4 c_v = de/dT, W4 closed form
+//   get_temperature     P8 recovers generating T, W4 one-step convergence
+//   rate coefficient    W1 (the Arrhenius triple printed at PAPER.md:205-208)
+//   equilibrium const   W2 hand computation, P7 K_c(fwd) K_c(bwd) = 1, P6 detailed balance
+//   third body/falloff  W3 hand computation, P9 [M] = p/RT, P10 Lindemann limits, P11 Troe -> Lindemann
+//   production rates    P5 mass + element conservation, P12 scaling, P15 dense nu brute force, P16
+//   No function is "parity unpinned".
+//
+// Readings of garbled / silent passages are
+// marked (Gn) where they are used.
+//
+// Units: SI with kmol.  R = 8314.46261815324 J/(kmol K), p0 = 101325 Pa (G5).
+
+#include <cmath>
+#include <cstdint>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" {
+// The oracle's own description of a mechanism: borrowed host pointers.
+struct oracle_mech {
+    int32_t n_species, n_reactions;
+    const double *mol_weight;            // [n_species] kg/kmol
+    const double *nasa_lo, *nasa_hi;     // [n_species][7]  a1..a7
+    const double *t_mid;                 // [n_species]
+    const int32_t *reac_ptr, *reac_species, *reac_coeff;   // nu'  (CSR over reactions)
+    const int32_t *prod_ptr, *prod_species, *prod_coeff;   // nu''
+    const double *A, *b, *theta;         // [n_reactions]
+    const uint8_t *type;                 // 0 elementary, 1 three-body, 2 Lindemann, 3 Troe
+    const uint8_t *reversible;
+    const double *eff_default;           // [n_reactions]
+    const int32_t *eff_ptr, *eff_species;
+    const double *eff_value;
+    const double *A0, *b0, *theta0;      // low-pressure limit (type >= 2)
+    const double *troe;                  // [n_reactions][4] alpha, T***, T*, T**
+};
+}
+
+namespace {
+
+template <class Real> struct Const {
+    static constexpr Real R = Real(8314.46261815324L);   // J/(kmol K)            (G5)
+    static constexpr Real p0 = Real(101325.0L);          // Pa, 1 atm
+};
+
+// NASA-7 polynomials of species k at temperature T.
+//   (A.31; G3)  cp/R = a1 + a2 T + a3 T^2 + a4 T^3 + a5 T^4
+//   (A.12)      h/RT = a1 + a2/2 T + a3/3 T^2 + a4/4 T^3 + a5/5 T^4 + a6/T
+//   (A.13; G2)  s/R  = a1 ln T + a2 T + a3/2 T^2 + a4/3 T^3 + a5/4 T^4 + a7
+//   (A.11)      g/RT = h/RT - s/R
+// Range choice (G10): T < T_mid ? low : high.
+template <class Real>
+void species_thermo(const oracle_mech &m, int k, Real T, Real &cp_R, Real &h_RT, Real &s_R, Real &g_RT) {
+    const double *c = (T < Real(m.t_mid[k])) ? (m.nasa_lo + 7 * k) : (m.nasa_hi + 7 * k);
+    const Real a1 = c[0], a2 = c[1], a3 = c[2], a4 = c[3], a5 = c[4], a6 = c[5], a7 = c[6];
+    const Real T2 = T * T, T3 = T2 * T, T4 = T3 * T;
+    cp_R = a1 + a2 * T + a3 * T2 + a4 * T3 + a5 * T4;
+    h_RT = a1 + a2 / Real(2) * T + a3 / Real(3) * T2 + a4 / Real(4) * T3 + a5 / Real(5) * T4 + a6 / T;
+    s_R = a1 * std::log(T) + a2 * T + a3 / Real(2) * T2 + a4 / Real(3) * T3 + a5 / Real(4) * T4 + a7;
+    g_RT = h_RT - s_R;
+}
+
+// (A.25), (A.26): e = sum_k Y_k e_k,  e_k = (h_k - R T)/W_k = (h_RT_k - 1) R T / W_k
+template <class Real>
+Real mixture_e(const oracle_mech &m, Real T, const Real *Y, int64_t ld) {
+    Real e = 0;
+    for (int k = 0; k < m.n_species; ++k) {
+        Real cp_R, h_RT, s_R, g_RT;
+        species_thermo<Real>(m, k, T, cp_R, h_RT, s_R, g_RT);
+        e += Y[k * ld] * (h_RT - Real(1)) * Const<Real>::R * T / Real(m.mol_weight[k]);
+    }
+    return e;
+}
+
+// (A.29), (A.30) per unit mass (G4): c_v = sum_k Y_k (c_p,k - R)/W_k
+template <class Real>
+Real mixture_cv(const oracle_mech &m, Real T, const Real *Y, int64_t ld) {
+    Real cv = 0;
+    for (int k = 0; k < m.n_species; ++k) {
+        Real cp_R, h_RT, s_R, g_RT;
+        species_thermo<Real>(m, k, T, cp_R, h_RT, s_R, g_RT);
+        cv += Y[k * ld] * (cp_R - Real(1)) * Const<Real>::R / Real(m.mol_weight[k]);
+    }
+    return cv;
+}
+
+// (A.27), (A.28); listing 22; per-point stop rule (G11):
+// apply the update, then test |dT| < tol; cap max_iter; last iterate returned.
+template <class Real>
+void get_temperature_point(const oracle_mech &m, Real e, const Real *Y, int64_t ld, Real T_guess, Real tol,
+                           int max_iter, Real &T_out, int &iters, int &converged) {
+    Real T = T_guess;
+    iters = 0;
+    converged = 0;
+    for (int it = 1; it <= max_iter; ++it) {
+        const Real dT = -(mixture_e<Real>(m, T, Y, ld) - e) / mixture_cv<Real>(m, T, Y, ld);
+        T = T + dT;
+        iters = it;
+        if (std::fabs(dT) < tol) {
+            converged = 1;
+            break;
+        }
+    }
+    T_out = T;
+}
+
+// Everything the rate of one reaction is made of, for the pins.
+template <class Real> struct ReactionDetail {
+    Real kf;       // effective forward rate coefficient (after falloff)
+    Real k_inf;    // A T^b exp(-theta/T)
+    Real k0;       // low-pressure coefficient (falloff) else 0
+    Real M;        // third-body concentration
+    Real Pr;       // reduced pressure (falloff) else 0
+    Real F;        // broadening factor (falloff) else 1
+    Real Kc;       // equilibrium constant (reversible) else 0
+    Real qf, qr;   // forward / reverse rates of progress (after the three-body factor)
+};
+
+// One reaction at one point, following SURVEY.md 8(c) "Oracle algorithm".
+//   C[k]  molar concentrations (A.8),  g[k] = g_k/(R T) (A.11)
+template <class Real>
+ReactionDetail<Real> reaction_rate(const oracle_mech &m, int j, Real T, const Real *C, const Real *g) {
+    ReactionDetail<Real> d{};
+    // (A.9): k = A T^b exp(-theta/T)  -- literal form with pow (G13, G15)
+    Real kf = Real(m.A[j]) * std::pow(T, Real(m.b[j])) * std::exp(-Real(m.theta[j]) / T);
+    d.k_inf = kf;
+    // third-body concentration [M] = sum_k eff_jk C_k, eff = default unless listed (G6)
+    Real M = 0;
+    {
+        int q = m.eff_ptr[j];
+        const int qend = m.eff_ptr[j + 1];
+        for (int k = 0; k < m.n_species; ++k) {
+            Real eff = Real(m.eff_default[j]);
+            if (q < qend && m.eff_species[q] == k) {
+                eff = Real(m.eff_value[q]);
+                ++q;
+            }
+            M += eff * C[k];
+        }
+    }
+    d.M = M;
+    d.F = 1;
+    const int type = m.type[j];
+    if (type >= 2) {   // falloff (G6-G9)
+        const Real k0 = Real(m.A0[j]) * std::pow(T, Real(m.b0[j])) * std::exp(-Real(m.theta0[j]) / T);
+        const Real Pr = k0 * M / kf;   // kf is k_inf here
+        Real F = 1;                    // Lindemann
+        if (type == 3) {               // Troe
+            const Real alpha = m.troe[4 * j + 0], T3 = m.troe[4 * j + 1], T1 = m.troe[4 * j + 2],
+                       T2 = m.troe[4 * j + 3];
+            Real Fc = (Real(1) - alpha) * std::exp(-T / T3) + alpha * std::exp(-T / T1);
+            if (std::isfinite(m.troe[4 * j + 3])) Fc += std::exp(-T2 / T);   // 4-parameter form (G7)
+            const Real lFc = std::log10(Fc);
+            const Real c = Real(-0.4L) - Real(0.67L) * lFc;
+            const Real n = Real(0.75L) - Real(1.27L) * lFc;
+            const Real lPr = std::log10(Pr) + c;
+            const Real f1 = lPr / (n - Real(0.14L) * lPr);
+            F = std::pow(Real(10), lFc / (Real(1) + f1 * f1));
+        }
+        d.k0 = k0;
+        d.Pr = Pr;
+        d.F = F;
+        kf = kf * (Pr / (Real(1) + Pr)) * F;
+    }
+    d.kf = kf;
+    // (A.7) forward: kf prod C^nu'   (integer powers by repeated multiplication, G16)
+    Real qf = kf;
+    for (int q = m.reac_ptr[j]; q < m.reac_ptr[j + 1]; ++q)
+        for (int r = 0; r < m.reac_coeff[q]; ++r) qf *= C[m.reac_species[q]];
+    Real qr = 0;
+    if (m.reversible[j]) {
+        // (A.10; G1): Kc = (p0/RT)^(sum nu) exp(-sum nu g/RT)
+        int dnu = 0;
+        Real dg = 0;
+        for (int q = m.prod_ptr[j]; q < m.prod_ptr[j + 1]; ++q) {
+            dnu += m.prod_coeff[q];
+            dg += Real(m.prod_coeff[q]) * g[m.prod_species[q]];
+        }
+        for (int q = m.reac_ptr[j]; q < m.reac_ptr[j + 1]; ++q) {
+            dnu -= m.reac_coeff[q];
+            dg -= Real(m.reac_coeff[q]) * g[m.reac_species[q]];
+        }
+        const Real Kc = std::pow(Const<Real>::p0 / (Const<Real>::R * T), Real(dnu)) * std::exp(-dg);
+        d.Kc = Kc;
+        qr = kf / Kc;
+        for (int q = m.prod_ptr[j]; q < m.prod_ptr[j + 1]; ++q)
+            for (int r = 0; r < m.prod_coeff[q]; ++r) qr *= C[m.prod_species[q]];
+    }
+    if (type == 1) {   // three-body: R = [M](qf - qr)  (G8)
+        qf *= M;
+        qr *= M;
+    }
+    d.qf = qf;
+    d.qr = qr;
+    return d;
+}
+
+// omega_i = sum_j nu_ij R_j (A.5), nu = nu'' - nu' (A.6), summed in reaction order (G22);
+// bound_i = sum_j |nu_ij| (|r_f,j| + |r_r,j|) is the scale of the parity tolerance (north_star).
+template <class Real>
+void production_rates_point(const oracle_mech &m, Real rho, Real T, const Real *Y, int64_t ld, Real *omega,
+                            Real *bound, int64_t ldo, Real *rf_out, Real *rr_out, int64_t ldr) {
+    const int ns = m.n_species, nr = m.n_reactions;
+    std::vector<Real> C(ns), g(ns), nu(ns);
+    for (int k = 0; k < ns; ++k) {
+        C[k] = rho * Y[k * ld] / Real(m.mol_weight[k]);   // (A.8)
+        Real cp_R, h_RT, s_R;
+        species_thermo<Real>(m, k, T, cp_R, h_RT, s_R, g[k]);
+        omega[k * ldo] = 0;
+        if (bound) bound[k * ldo] = 0;
+    }
+    for (int j = 0; j < nr; ++j) {
+        const ReactionDetail<Real> d = reaction_rate<Real>(m, j, T, C.data(), g.data());
+        if (rf_out) rf_out[j * ldr] = d.qf;
+        if (rr_out) rr_out[j * ldr] = d.qr;
+        const Real Rj = d.qf - d.qr;   // (A.7)
+        // net coefficients of this reaction
+        for (int q = m.reac_ptr[j]; q < m.reac_ptr[j + 1]; ++q) nu[m.reac_species[q]] = 0;
+        for (int q = m.prod_ptr[j]; q < m.prod_ptr[j + 1]; ++q) nu[m.prod_species[q]] = 0;
+        for (int q = m.reac_ptr[j]; q < m.reac_ptr[j + 1]; ++q) nu[m.reac_species[q]] -= Real(m.reac_coeff[q]);
+        for (int q = m.prod_ptr[j]; q < m.prod_ptr[j + 1]; ++q) nu[m.prod_species[q]] += Real(m.prod_coeff[q]);
+        auto add = [&](int k) {
+            if (nu[k] == Real(0)) return;
+            omega[k * ldo] += nu[k] * Rj;
+            if (bound) bound[k * ldo] += std::fabs(nu[k]) * (std::fabs(d.qf) + std::fabs(d.qr));
+            nu[k] = 0;   // a species listed on both sides is visited once
+        };
+        for (int q = m.reac_ptr[j]; q < m.reac_ptr[j + 1]; ++q) add(m.reac_species[q]);
+        for (int q = m.prod_ptr[j]; q < m.prod_ptr[j + 1]; ++q) add(m.prod_species[q]);
+    }
+}
+
+template <class Real>
+void get_net_production_rates(const oracle_mech &m, int64_t n, int64_t ld, const Real *rho, const Real *T,
+                              const Real *Y, Real *omega, Real *bound, Real *rf, Real *rr) {
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < n; ++p)
+        production_rates_point<Real>(m, rho[p], T[p], Y + p, ld, omega + p, bound ? bound + p : nullptr, ld,
+                                     rf ? rf + p : nullptr, rr ? rr + p : nullptr, ld);
+}
+
+template <class Real>
+void get_temperature(const oracle_mech &m, int64_t n, int64_t ld, const Real *e, const Real *Y,
+                     const Real *T_guess, Real tol, int max_iter, Real *T, int32_t *iters, int32_t *conv) {
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < n; ++p) {
+        int it, cv;
+        get_temperature_point<Real>(m, e[p], Y + p, ld, T_guess[p], tol, max_iter, T[p], it, cv);
+        if (iters) iters[p] = it;
+        if (conv) conv[p] = cv;
+    }
+}
+
+template <class Real>
+void reaction_detail(const oracle_mech &m, int j, Real rho, Real T, const Real *Y, Real *out9) {
+    const int ns = m.n_species;
+    std::vector<Real> C(ns), g(ns);
+    for (int k = 0; k < ns; ++k) {
+        C[k] = rho * Y[k] / Real(m.mol_weight[k]);
+        Real cp_R, h_RT, s_R;
+        species_thermo<Real>(m, k, T, cp_R, h_RT, s_R, g[k]);
+    }
+    const ReactionDetail<Real> d = reaction_rate<Real>(m, j, T, C.data(), g.data());
+    out9[0] = d.kf; out9[1] = d.k_inf; out9[2] = d.k0; out9[3] = d.M; out9[4] = d.Pr;
+    out9[5] = d.F; out9[6] = d.Kc; out9[7] = d.qf; out9[8] = d.qr;
+}
+
+}   // namespace
+
+extern "C" {
+
+int oracle_num_threads() {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+void oracle_set_num_threads(int n) {
+#ifdef _OPENMP
+    omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
+int oracle_sizeof_real80() { return (int)sizeof(long double); }
+
+#define ORACLE_API(SUFFIX, Real)                                                                              \
+    void oracle_species_thermo_##SUFFIX(const oracle_mech *m, int k, Real T, Real *out4) {                    \
+        species_thermo<Real>(*m, k, T, out4[0], out4[1], out4[2], out4[3]);                                   \
+    }                                                                                                         \
+    Real oracle_mixture_e_##SUFFIX(const oracle_mech *m, Real T, const Real *Y) {                             \
+        return mixture_e<Real>(*m, T, Y, 1);                                                                  \
+    }                                                                                                         \
+    Real oracle_mixture_cv_##SUFFIX(const oracle_mech *m, Real T, const Real *Y) {                            \
+        return mixture_cv<Real>(*m, T, Y, 1);                                                                 \
+    }                                                                                                         \
+    void oracle_reaction_detail_##SUFFIX(const oracle_mech *m, int j, Real rho, Real T, const Real *Y,        \
+                                         Real *out9) {                                                        \
+        reaction_detail<Real>(*m, j, rho, T, Y, out9);                                                        \
+    }                                                                                                         \
+    void oracle_get_temperature_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *e,          \
+                                         const Real *Y, const Real *T_guess, Real tol, int max_iter, Real *T, \
+                                         int32_t *iters, int32_t *converged) {                                \
+        get_temperature<Real>(*m, n, ld, e, Y, T_guess, tol, max_iter, T, iters, converged);                  \
+    }                                                                                                         \
+    void oracle_get_net_production_rates_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld,                \
+                                                  const Real *rho, const Real *T, const Real *Y, Real *omega, \
+                                                  Real *bound, Real *rf, Real *rr) {                          \
+        get_net_production_rates<Real>(*m, n, ld, rho, T, Y, omega, bound, rf, rr);                           \
+    }
+
+ORACLE_API(f64, double)
+ORACLE_API(f80, long double)
+
+}   // extern "C"
