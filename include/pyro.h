@@ -1,0 +1,139 @@
+/* pyro.h -- C ABI of libpyro: per-point combustion thermochemistry on one NVIDIA B200 (sm_100a).
+ *
+ * The data-parallel hot path of Pyrometheus (arXiv 2503.24286, Appendix A; citations are
+ * PAPER.md:LINE of the extracted paper text):
+ *   - NASA-7 species thermodynamics                          (A.11)-(A.13), (A.31)
+ *   - Newton inversion of temperature from internal energy   (A.25)-(A.30)
+ *   - net production rates  omega_i = sum_j nu_ij R_j        (A.5)-(A.10)
+ *     with Arrhenius, third-body, Lindemann/Troe falloff rate coefficients
+ *     and reverse rates from equilibrium constants           (A.10)
+ *
+ * Conventions
+ *   Units: SI with kmol. W kg/kmol, C kmol/m^3, omega kmol/(m^3 s), e J/kg, T K, rho kg/m^3,
+ *          R = 8314.46261815324 J/(kmol K), p0 = 101325 Pa.
+ *   Fields: FP64, structure of arrays [species][points]: species k of point p is X[k*ld + p],
+ *          ld >= n in doubles.  "device" pointers are CUDA device memory on the mechanism's
+ *          device; "host" pointers are ordinary (preferably pinned) host memory.
+ *   Every function returns a pyro_status (0 = PYRO_OK); nothing throws or aborts across the ABI.
+ *   Device calls enqueue on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
+ *   stream) and return without synchronising; they allocate nothing and copy nothing
+ *   (exception: the first launch after a *different* mechanism used the constant-memory
+ *   table bank re-uploads <= 64 KB on that stream, ordered after earlier launches by events).
+ *   Concurrent calls on one handle from several host threads are allowed.
+ *   There is no CPU fallback: without a CUDA device pyro_mech_create fails with PYRO_ERR_CUDA.
+ */
+#ifndef PYRO_H
+#define PYRO_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    PYRO_OK = 0,
+    PYRO_ERR_NULL = 1,        /* a required pointer is NULL                                         */
+    PYRO_ERR_BAD_SIZE = 2,    /* n < 0, ld < n, n_species < 1, n_reactions < 0, max_iter < 1 ...     */
+    PYRO_ERR_BAD_MECH = 3,    /* index out of range, A <= 0, W <= 0, bad Troe temperature,
+                                 coefficient <= 0, more than 3 molecules on a side, CSR not monotone,
+                                 unknown reaction type                                              */
+    PYRO_ERR_TOO_LARGE = 4,   /* species / reactions beyond what the on-chip staging can hold        */
+    PYRO_ERR_ALIGN = 5,       /* a field pointer is not 8-byte aligned                               */
+    PYRO_ERR_CUDA = 6,        /* CUDA runtime error (text via pyro_last_error_string)                */
+    PYRO_ERR_UNSUPPORTED = 7  /* valid input that this build has no kernel for                      */
+} pyro_status;
+
+/* reaction types */
+enum { PYRO_ELEMENTARY = 0, PYRO_THREE_BODY = 1, PYRO_FALLOFF_LINDEMANN = 2, PYRO_FALLOFF_TROE = 3 };
+
+typedef struct pyro_mech pyro_mech; /* opaque; owns the device tables of one mechanism on one device */
+
+/* Host description of a mechanism.  All pointers are HOST memory, borrowed only for the
+ * duration of pyro_mech_create (the caller may free everything afterwards).
+ * Reaction j reads  sum_i nu'_ij S_i <=> sum_i nu''_ij S_i  (A.4) PAPER.md:903. */
+typedef struct {
+    int32_t n_species, n_reactions, n_elements; /* n_elements may be 0                             */
+    const double *mol_weight;                   /* [n_species] kg/kmol, > 0                        */
+    const double *nasa_lo, *nasa_hi;            /* [n_species][7] a1..a7 for T < T_mid / T >= T_mid */
+    const double *t_mid;                        /* [n_species] K                                   */
+    const int32_t *elem_comp;                   /* [n_species][n_elements] or NULL; if given, every
+                                                   reaction must be element balanced              */
+    const int32_t *reac_ptr, *reac_species, *reac_coeff; /* CSR of nu' : ptr[n_reactions+1]       */
+    const int32_t *prod_ptr, *prod_species, *prod_coeff; /* CSR of nu''                           */
+    const double *A, *b, *theta; /* [n_reactions] k = A T^b exp(-theta/T) (A.9): A > 0 in
+                                    (m^3/kmol)^(order-1)/s, theta = Ea/R in K (any sign);
+                                    for falloff reactions this is the high-pressure limit          */
+    const uint8_t *type;         /* [n_reactions] PYRO_ELEMENTARY ... PYRO_FALLOFF_TROE            */
+    const uint8_t *reversible;   /* [n_reactions] 1: reverse rate from K_c (A.10); 0: r_r = 0      */
+    const double *eff_default;   /* [n_reactions] default third-body efficiency (usually 1)        */
+    const int32_t *eff_ptr, *eff_species; /* CSR of non-default efficiencies: ptr[n_reactions+1]   */
+    const double *eff_value;
+    const double *A0, *b0, *theta0; /* [n_reactions] low-pressure limit, read when type >= 2       */
+    const double *troe; /* [n_reactions][4] alpha, T***, T*, T** read when type == 3;
+                           T* or T** = +inf drops that term (3-parameter form when T** = +inf)     */
+} pyro_mech_desc;
+
+/* Validate `desc`, flatten it into device tables (packed rate and equilibrium coefficients,
+ * fixed-width species slots, efficiency lists, falloff parameters, NASA energy tables) and
+ * upload them to CUDA device `device`.  *out receives the handle.  On error *out = NULL. */
+int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out);
+
+/* Free the device tables.  pyro_mech_destroy(NULL) is a no-op returning PYRO_OK.  The caller
+ * must make sure no launch that uses the handle is still running. */
+int pyro_mech_destroy(pyro_mech *mech);
+
+/* Newton controls of pyro_get_temperature: stop when |dT| < abs_tol_K after the update,
+ * at most max_iter iterations.  Defaults 1e-6 K and 10 (BASELINE.json configs[4]). */
+int pyro_mech_set_newton(pyro_mech *mech, double abs_tol_K, int max_iter);
+
+/* Temperature from internal energy: solves  sum_k Y_k e_k(T) = e  per point by Newton's
+ * method, T <- T - (Y.e(T) - e)/c_v(T,Y)   (A.25)-(A.30) PAPER.md:1008-1029, listing 22 :672.
+ *   rho      [n]            device, may be NULL (the ideal-gas caloric EOS does not use it)
+ *   e        [n]            device, J/kg
+ *   Y        [n_species][ld] device, mass fractions (not clipped, not renormalised)
+ *   T_guess  [n]            device, K, > 0
+ *   T        [n]            device, out; may alias T_guess
+ *   n_not_converged         device int32 or NULL: incremented once per point that hit max_iter
+ *                           (the last iterate is still written; this is not an error)
+ * n == 0 returns PYRO_OK and launches nothing. */
+int pyro_get_temperature(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e,
+                         const double *Y, const double *T_guess, double *T, int32_t *n_not_converged,
+                         void *cuda_stream);
+
+/* Net molar production rates omega[k*ld+p] = sum_j nu_kj R_j  (A.5)-(A.10) PAPER.md:908-934 from
+ *   rho [n], T [n], Y [n_species][ld]   (device; T > 0, rho > 0, Y >= 0 are preconditions)
+ *   omega [n_species][ld]               (device, out; must not alias Y) */
+int pyro_get_net_production_rates(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho,
+                                  const double *T, const double *Y, double *omega, void *cuda_stream);
+
+/* The whole source-term step from HOST buffers: (rho, e, Y, T_guess) -> (T, omega).  Copies the
+ * inputs to the device in slabs of points, runs the temperature solve and the rates kernel on
+ * each slab and copies T and omega back, the three stages overlapped on separate streams.
+ * All pointers are host memory (pinned memory gives asynchronous copies); layouts as above
+ * with leading dimension `ld`.  Blocks until the results are in T and omega.
+ * *n_not_converged (host, may be NULL) receives the Newton non-convergence count. */
+int pyro_source_terms_host(pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e,
+                           const double *Y, const double *T_guess, double *T, double *omega,
+                           int64_t *n_not_converged);
+
+/* Facts about a packed mechanism, for reports: fills up to `cap` int64 values
+ *   [0] n_species  [1] n_reactions  [2] reactions in the plain class  [3] in the extended class
+ *   [4] table bytes  [5] 1 if tables live in __constant__ memory, 0 if in global memory
+ *   [6] threads per block of the rates kernel  [7] dynamic shared memory per block (bytes)
+ *   [8] resident blocks per SM (occupancy query)  [9] registers per thread of the rates kernel
+ *   [10] local (spill) bytes per thread  [11] SM count of the device
+ * returns the number of values written (negative pyro_status on error). */
+int pyro_mech_info(const pyro_mech *mech, int64_t *out, int cap);
+
+/* Measures the FP64 FMA peak of `device`: independent DFMA chains on every SM for about
+ * `millis` ms; *tflops = 2 * FMAs / time.  Used as the roofline denominator cross-check. */
+int pyro_probe_fp64_peak(int device, double millis, double *tflops);
+
+const char *pyro_status_string(int status); /* static text for a pyro_status                       */
+const char *pyro_last_error_string(void);   /* detail of the last error on this thread (may be "") */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PYRO_H */

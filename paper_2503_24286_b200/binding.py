@@ -1,0 +1,208 @@
+"""Thin ctypes binding of libpyro.so (include/pyro.h): argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C ABI; PyTorch is used
+here for device memory and streams.  There is no CPU fallback: if libpyro.so is missing
+or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpyro.so")
+
+EXPORTS = (
+    "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
+    "pyro_get_net_production_rates", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
+    "pyro_status_string", "pyro_last_error_string",
+)
+
+PYRO_OK = 0
+STATUS_NAMES = {0: "PYRO_OK", 1: "PYRO_ERR_NULL", 2: "PYRO_ERR_BAD_SIZE", 3: "PYRO_ERR_BAD_MECH",
+                4: "PYRO_ERR_TOO_LARGE", 5: "PYRO_ERR_ALIGN", 6: "PYRO_ERR_CUDA", 7: "PYRO_ERR_UNSUPPORTED"}
+
+
+class PyroError(RuntimeError):
+    def __init__(self, status, detail):
+        self.status = int(status)
+        super().__init__(f"{STATUS_NAMES.get(self.status, self.status)}: {detail}")
+
+
+class MechDesc(C.Structure):
+    """Mirror of pyro_mech_desc."""
+    _fields_ = [
+        ("n_species", C.c_int32), ("n_reactions", C.c_int32), ("n_elements", C.c_int32),
+        ("mol_weight", C.c_void_p), ("nasa_lo", C.c_void_p), ("nasa_hi", C.c_void_p), ("t_mid", C.c_void_p),
+        ("elem_comp", C.c_void_p),
+        ("reac_ptr", C.c_void_p), ("reac_species", C.c_void_p), ("reac_coeff", C.c_void_p),
+        ("prod_ptr", C.c_void_p), ("prod_species", C.c_void_p), ("prod_coeff", C.c_void_p),
+        ("A", C.c_void_p), ("b", C.c_void_p), ("theta", C.c_void_p),
+        ("type", C.c_void_p), ("reversible", C.c_void_p),
+        ("eff_default", C.c_void_p), ("eff_ptr", C.c_void_p), ("eff_species", C.c_void_p),
+        ("eff_value", C.c_void_p),
+        ("A0", C.c_void_p), ("b0", C.c_void_p), ("theta0", C.c_void_p), ("troe", C.c_void_p),
+    ]
+
+
+_lib = None
+
+
+def load_library():
+    """Loads libpyro.so (building it with nvcc first if the sources are newer)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        from . import build
+        build.build_libpyro()
+    lib = C.CDLL(LIB_PATH)
+    vp, i64, dbl = C.c_void_p, C.c_int64, C.c_double
+    lib.pyro_mech_create.argtypes = [C.POINTER(MechDesc), C.c_int, C.POINTER(vp)]
+    lib.pyro_mech_destroy.argtypes = [vp]
+    lib.pyro_mech_set_newton.argtypes = [vp, dbl, C.c_int]
+    lib.pyro_get_temperature.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
+    lib.pyro_get_net_production_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+    lib.pyro_source_terms_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]
+    lib.pyro_mech_info.argtypes = [vp, C.POINTER(i64), C.c_int]
+    lib.pyro_probe_fp64_peak.argtypes = [C.c_int, dbl, C.POINTER(dbl)]
+    lib.pyro_status_string.argtypes = [C.c_int]
+    lib.pyro_status_string.restype = C.c_char_p
+    lib.pyro_last_error_string.restype = C.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(status):
+    if status != PYRO_OK:
+        raise PyroError(status, load_library().pyro_last_error_string().decode())
+
+
+def make_desc(mech):
+    """pyro_mech_desc from an object with the attributes of `inputs.Mechanism`.
+    Returns (desc, keepalive)."""
+    keep = []
+
+    def arr(x, dt):
+        if x is None:
+            return None
+        a = np.ascontiguousarray(np.asarray(x), dtype=dt)
+        keep.append(a)
+        return a.ctypes.data
+
+    d = MechDesc()
+    d.n_species = int(mech.n_species)
+    d.n_reactions = int(mech.n_reactions)
+    ec = getattr(mech, "elem_comp", None)
+    d.n_elements = 0 if ec is None else int(np.asarray(ec).shape[1])
+    d.elem_comp = arr(ec, np.int32) if d.n_elements else None
+    for name in ("mol_weight", "nasa_lo", "nasa_hi", "t_mid", "A", "b", "theta", "eff_default", "eff_value",
+                 "A0", "b0", "theta0", "troe"):
+        setattr(d, name, arr(getattr(mech, name), np.float64))
+    for name in ("reac_ptr", "reac_species", "reac_coeff", "prod_ptr", "prod_species", "prod_coeff",
+                 "eff_ptr", "eff_species"):
+        setattr(d, name, arr(getattr(mech, name), np.int32))
+    d.type = arr(mech.rtype, np.uint8)
+    d.reversible = arr(mech.reversible, np.uint8)
+    return d, keep
+
+
+_INFO_KEYS = ("n_species", "n_reactions", "n_plain", "n_extended", "table_bytes", "tables_in_constant",
+              "block_threads", "smem_bytes", "blocks_per_sm", "registers", "local_bytes", "sm_count")
+
+
+def _ptr(t):
+    return None if t is None else t.data_ptr()
+
+
+def _stream(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return s.cuda_stream
+
+
+class Mechanism:
+    """Owns a pyro_mech handle.  Field arguments are torch CUDA float64 tensors
+    (Y, omega of shape [n_species, ld] with points contiguous)."""
+
+    def __init__(self, mech, device=0):
+        lib = load_library()
+        desc, keep = make_desc(mech)
+        h = C.c_void_p()
+        _check(lib.pyro_mech_create(C.byref(desc), int(device), C.byref(h)))
+        self._h = h
+        self._lib = lib
+        self.device = int(device)
+        self.n_species = int(mech.n_species)
+        self.n_reactions = int(mech.n_reactions)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.pyro_mech_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def info(self):
+        out = (C.c_int64 * 12)()
+        n = self._lib.pyro_mech_info(self._h, out, 12)
+        if n < 0:
+            _check(-n)
+        return dict(zip(_INFO_KEYS, [int(v) for v in out[:n]]))
+
+    def set_newton(self, abs_tol_K=1e-6, max_iter=10):
+        _check(self._lib.pyro_mech_set_newton(self._h, float(abs_tol_K), int(max_iter)))
+
+    def get_temperature(self, e, Y, T_guess, rho=None, out=None, n_not_converged=None, stream=None):
+        """pyro_get_temperature: T from (e, Y, T_guess); returns T."""
+        import torch
+        n = e.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        if out is None:
+            out = torch.empty_like(e)
+        _check(self._lib.pyro_get_temperature(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T_guess),
+                                              _ptr(out), _ptr(n_not_converged), _stream(stream)))
+        return out
+
+    def get_net_production_rates(self, rho, T, Y, out=None, stream=None):
+        """pyro_get_net_production_rates: omega from (rho, T, Y); returns omega."""
+        import torch
+        n = rho.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        if out is None:
+            out = torch.empty_like(Y)
+        assert out.stride(0) == ld or n == 0
+        _check(self._lib.pyro_get_net_production_rates(self._h, n, ld, _ptr(rho), _ptr(T), _ptr(Y), _ptr(out),
+                                                       _stream(stream)))
+        return out
+
+    def source_terms_host(self, rho, e, Y, T_guess, T_out, omega_out):
+        """pyro_source_terms_host on HOST buffers (numpy arrays or CPU torch tensors, float64,
+        preferably pinned).  Returns the Newton non-convergence count."""
+        def hp(x):
+            return x.ctypes.data if isinstance(x, np.ndarray) else x.data_ptr()
+
+        def ld_of(x, n):
+            if isinstance(x, np.ndarray):
+                return x.strides[0] // 8 if x.ndim == 2 and n > 0 else n
+            return x.stride(0) if x.dim() == 2 and n > 0 else n
+        n = rho.shape[0]
+        ld = ld_of(Y, n)
+        assert ld_of(omega_out, n) == ld
+        bad = C.c_int64(0)
+        _check(self._lib.pyro_source_terms_host(self._h, n, ld, hp(rho), hp(e), hp(Y), hp(T_guess), hp(T_out),
+                                                hp(omega_out), C.byref(bad)))
+        return int(bad.value)
+
+
+def probe_fp64_peak(device=0, millis=200.0):
+    """Measured DFMA peak of the device in TFLOP/s (2 flops per FMA)."""
+    out = C.c_double(0.0)
+    _check(load_library().pyro_probe_fp64_peak(int(device), float(millis), C.byref(out)))
+    return float(out.value)

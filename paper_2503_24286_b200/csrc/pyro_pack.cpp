@@ -1,0 +1,311 @@
+// Mechanism packer (host): validates a pyro_mech_desc and flattens it into the device
+// tables of pyro_tables.h.  Row a0 of the hot path.
+#include "pyro_pack.h"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <map>
+
+namespace pyro {
+namespace {
+
+constexpr long double kR = 8314.46261815324L;   // J/(kmol K)
+constexpr long double kP0 = 101325.0L;          // Pa
+const long double kLog2e = 1.0L / std::log(2.0L);
+
+struct Fail {
+    int status;
+    std::string msg;
+};
+
+#define PYRO_REQUIRE(cond, status, ...)                  \
+    do {                                                 \
+        if (!(cond)) {                                   \
+            char buf_[256];                              \
+            std::snprintf(buf_, sizeof buf_, __VA_ARGS__); \
+            throw Fail{status, buf_};                    \
+        }                                                \
+    } while (0)
+
+bool finite(double x) { return std::isfinite(x); }
+
+template <class T> void put(std::vector<unsigned char> &blob, uint32_t off, const T *src, size_t count) {
+    if (count) std::memcpy(blob.data() + off, src, count * sizeof(T));
+}
+
+uint32_t align8(uint32_t x) { return (x + 7u) & ~7u; }
+
+// coefficients of  sum_i nu_i g_i/(RT)  on the features (1, ln T, 1/T, T, T^2, T^3, T^4):
+//   g/RT = a1 (1 - ln T) - a2/2 T - a3/6 T^2 - a4/12 T^3 - a5/20 T^4 + a6/T - a7
+// which is h/RT - s/R of (A.12), (A.13) with the readings G2, G3.
+void add_gibbs(long double c[7], long double nu, const double *a) {
+    c[0] += nu * ((long double)a[0] - (long double)a[6]);
+    c[1] += nu * (-(long double)a[0]);
+    c[2] += nu * (long double)a[5];
+    c[3] += nu * (-(long double)a[1] / 2);
+    c[4] += nu * (-(long double)a[2] / 6);
+    c[5] += nu * (-(long double)a[3] / 12);
+    c[6] += nu * (-(long double)a[4] / 20);
+}
+
+}   // namespace
+
+int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
+    try {
+        PYRO_REQUIRE(d != nullptr, PYRO_ERR_NULL, "desc is NULL");
+        const int ns = d->n_species, nr = d->n_reactions, ne = d->n_elements;
+        PYRO_REQUIRE(ns >= 1, PYRO_ERR_BAD_SIZE, "n_species = %d", ns);
+        PYRO_REQUIRE(nr >= 0, PYRO_ERR_BAD_SIZE, "n_reactions = %d", nr);
+        PYRO_REQUIRE(ne >= 0, PYRO_ERR_BAD_SIZE, "n_elements = %d", ne);
+        PYRO_REQUIRE(d->mol_weight && d->nasa_lo && d->nasa_hi && d->t_mid, PYRO_ERR_NULL, "species table is NULL");
+        if (nr > 0) {
+            PYRO_REQUIRE(d->reac_ptr && d->reac_species && d->reac_coeff && d->prod_ptr && d->prod_species &&
+                             d->prod_coeff,
+                         PYRO_ERR_NULL, "stoichiometry CSR is NULL");
+            PYRO_REQUIRE(d->A && d->b && d->theta && d->type && d->reversible, PYRO_ERR_NULL,
+                         "rate table is NULL");
+        }
+        PYRO_REQUIRE(ns <= kMaxSpecies, PYRO_ERR_TOO_LARGE, "n_species %d > %d (on-chip staging limit)", ns,
+                     kMaxSpecies);
+        PYRO_REQUIRE(nr <= kMaxReactions, PYRO_ERR_TOO_LARGE, "n_reactions %d > %d", nr, kMaxReactions);
+
+        // ---- species
+        for (int k = 0; k < ns; ++k) {
+            PYRO_REQUIRE(finite(d->mol_weight[k]) && d->mol_weight[k] > 0, PYRO_ERR_BAD_MECH,
+                         "mol_weight[%d] is not positive", k);
+            PYRO_REQUIRE(finite(d->t_mid[k]) && d->t_mid[k] > 0, PYRO_ERR_BAD_MECH, "t_mid[%d] is not positive", k);
+            for (int m = 0; m < 7; ++m)
+                PYRO_REQUIRE(finite(d->nasa_lo[7 * k + m]) && finite(d->nasa_hi[7 * k + m]), PYRO_ERR_BAD_MECH,
+                             "NASA coefficient of species %d is not finite", k);
+        }
+        bool single_tmid = true;
+        for (int k = 1; k < ns; ++k) single_tmid = single_tmid && d->t_mid[k] == d->t_mid[0];
+        PYRO_REQUIRE(single_tmid, PYRO_ERR_UNSUPPORTED,
+                     "species with different T_mid: this build folds the Gibbs sums per reaction and needs one "
+                     "T_mid per mechanism");
+
+        // ---- reactions: validation
+        bool any_special = false;
+        for (int j = 0; j < nr; ++j) {
+            for (int side = 0; side < 2; ++side) {
+                const int32_t *ptr = side ? d->prod_ptr : d->reac_ptr;
+                const int32_t *sp = side ? d->prod_species : d->reac_species;
+                const int32_t *co = side ? d->prod_coeff : d->reac_coeff;
+                PYRO_REQUIRE(ptr[0] == 0 && ptr[j + 1] >= ptr[j], PYRO_ERR_BAD_MECH, "CSR pointer of reaction %d", j);
+                int molecules = 0;
+                for (int q = ptr[j]; q < ptr[j + 1]; ++q) {
+                    PYRO_REQUIRE(sp[q] >= 0 && sp[q] < ns, PYRO_ERR_BAD_MECH,
+                                 "species index %d out of range in reaction %d", sp[q], j);
+                    PYRO_REQUIRE(co[q] >= 1, PYRO_ERR_BAD_MECH, "stoichiometric coefficient %d in reaction %d",
+                                 co[q], j);
+                    for (int q2 = ptr[j]; q2 < q; ++q2)
+                        PYRO_REQUIRE(sp[q2] != sp[q], PYRO_ERR_BAD_MECH, "species %d listed twice on one side of reaction %d", sp[q], j);
+                    molecules += co[q];
+                }
+                PYRO_REQUIRE(molecules >= 1, PYRO_ERR_BAD_MECH, "reaction %d has an empty side", j);
+                PYRO_REQUIRE(molecules <= kMaxSide, PYRO_ERR_BAD_MECH,
+                             "reaction %d has %d molecules on one side (slot width %d)", j, molecules, kMaxSide);
+            }
+            PYRO_REQUIRE(finite(d->A[j]) && d->A[j] > 0, PYRO_ERR_BAD_MECH, "A[%d] must be positive (ln A is taken)", j);
+            PYRO_REQUIRE(finite(d->b[j]) && finite(d->theta[j]), PYRO_ERR_BAD_MECH, "b/theta of reaction %d", j);
+            PYRO_REQUIRE(d->type[j] <= PYRO_FALLOFF_TROE, PYRO_ERR_BAD_MECH, "type[%d] = %d", j, d->type[j]);
+            if (d->type[j] != PYRO_ELEMENTARY) {
+                any_special = true;
+                PYRO_REQUIRE(d->eff_default && d->eff_ptr, PYRO_ERR_NULL, "efficiency tables are NULL");
+                PYRO_REQUIRE(finite(d->eff_default[j]), PYRO_ERR_BAD_MECH, "eff_default[%d]", j);
+            }
+            if (d->type[j] >= PYRO_FALLOFF_LINDEMANN) {
+                PYRO_REQUIRE(d->A0 && d->b0 && d->theta0, PYRO_ERR_NULL, "low-pressure tables are NULL");
+                PYRO_REQUIRE(finite(d->A0[j]) && d->A0[j] > 0, PYRO_ERR_BAD_MECH, "A0[%d] must be positive", j);
+                PYRO_REQUIRE(finite(d->b0[j]) && finite(d->theta0[j]), PYRO_ERR_BAD_MECH, "b0/theta0 of reaction %d", j);
+            }
+            if (d->type[j] == PYRO_FALLOFF_TROE) {
+                PYRO_REQUIRE(d->troe, PYRO_ERR_NULL, "troe table is NULL");
+                const double *t = d->troe + 4 * j;
+                PYRO_REQUIRE(finite(t[0]), PYRO_ERR_BAD_MECH, "Troe alpha of reaction %d", j);
+                for (int m = 1; m < 4; ++m)
+                    PYRO_REQUIRE(t[m] > 0 && !std::isnan(t[m]), PYRO_ERR_BAD_MECH,
+                                 "Troe temperature %d of reaction %d is not positive", m, j);
+                PYRO_REQUIRE(finite(t[1]), PYRO_ERR_BAD_MECH, "Troe T*** of reaction %d must be finite", j);
+            }
+        }
+        if (any_special) {
+            PYRO_REQUIRE(d->eff_ptr[0] == 0, PYRO_ERR_BAD_MECH, "eff_ptr[0] != 0");
+            for (int j = 0; j < nr; ++j) {
+                PYRO_REQUIRE(d->eff_ptr[j + 1] >= d->eff_ptr[j], PYRO_ERR_BAD_MECH, "eff_ptr of reaction %d", j);
+                if (d->eff_ptr[j + 1] > d->eff_ptr[j])
+                    PYRO_REQUIRE(d->eff_species && d->eff_value, PYRO_ERR_NULL, "efficiency lists are NULL");
+                for (int q = d->eff_ptr[j]; q < d->eff_ptr[j + 1]; ++q) {
+                    PYRO_REQUIRE(d->eff_species[q] >= 0 && d->eff_species[q] < ns, PYRO_ERR_BAD_MECH,
+                                 "efficiency species %d out of range in reaction %d", d->eff_species[q], j);
+                    PYRO_REQUIRE(finite(d->eff_value[q]), PYRO_ERR_BAD_MECH, "efficiency value in reaction %d", j);
+                    for (int q2 = d->eff_ptr[j]; q2 < q; ++q2)
+                        PYRO_REQUIRE(d->eff_species[q2] != d->eff_species[q], PYRO_ERR_BAD_MECH,
+                                     "efficiency of species %d listed twice in reaction %d", d->eff_species[q], j);
+                }
+            }
+        }
+        if (d->elem_comp && ne > 0) {
+            for (int j = 0; j < nr; ++j)
+                for (int e = 0; e < ne; ++e) {
+                    long long bal = 0;
+                    for (int q = d->reac_ptr[j]; q < d->reac_ptr[j + 1]; ++q)
+                        bal -= (long long)d->reac_coeff[q] * d->elem_comp[d->reac_species[q] * ne + e];
+                    for (int q = d->prod_ptr[j]; q < d->prod_ptr[j + 1]; ++q)
+                        bal += (long long)d->prod_coeff[q] * d->elem_comp[d->prod_species[q] * ne + e];
+                    PYRO_REQUIRE(bal == 0, PYRO_ERR_BAD_MECH, "reaction %d does not balance element %d", j, e);
+                }
+        }
+
+        // ---- reactions: records
+        std::vector<RxnE> recE;
+        std::vector<RxnX> recX;
+        std::vector<double> eff_delta;
+        std::vector<uint16_t> eff_species;
+        out.order.clear();
+        std::vector<int> orderX;
+        bool needs_ctot = false;
+        for (int j = 0; j < nr; ++j) {
+            RxnE e;
+            std::memset(&e, 0, sizeof e);
+            for (int s = 0; s < 6; ++s) e.slot[s] = kNoSpecies;
+            std::map<int, int> net;
+            bool both_sides = false;
+            int nreac = 0, nprod = 0;
+            for (int q = d->reac_ptr[j]; q < d->reac_ptr[j + 1]; ++q) {
+                for (int r = 0; r < d->reac_coeff[q]; ++r) e.slot[nreac++] = (uint16_t)d->reac_species[q];
+                net[d->reac_species[q]] -= d->reac_coeff[q];
+            }
+            for (int q = d->prod_ptr[j]; q < d->prod_ptr[j + 1]; ++q) {
+                for (int r = 0; r < d->prod_coeff[q]; ++r) e.slot[3 + nprod++] = (uint16_t)d->prod_species[q];
+                if (net.count(d->prod_species[q])) both_sides = true;
+                net[d->prod_species[q]] += d->prod_coeff[q];
+            }
+            e.nreac = (uint8_t)nreac;
+            e.nprod = (uint8_t)nprod;
+            e.reversible = d->reversible[j] ? 1 : 0;
+            // (A.9): log2 k_f = log2 A + b log2 T - theta log2e / T
+            e.f[0] = (double)(std::log((long double)d->A[j]) * kLog2e);
+            e.f[1] = d->b[j];
+            e.f[2] = (double)(-(long double)d->theta[j] * kLog2e);
+            if (e.reversible) {
+                // (A.10), G1: ln K_c = dnu ln(p0/(R T)) - sum_i nu_i g_i/(RT);  ln k_r = ln k_f - ln K_c
+                const int dnu = nprod - nreac;
+                for (int range = 0; range < 2; ++range) {
+                    long double c[7] = {0, 0, 0, 0, 0, 0, 0};
+                    const double *nasa = range ? d->nasa_hi : d->nasa_lo;
+                    for (auto &kv : net) add_gibbs(c, (long double)kv.second, nasa + 7 * kv.first);
+                    // ln k_r on (1, ln T, 1/T, T..T^4)
+                    c[0] += std::log((long double)d->A[j]) - dnu * std::log(kP0 / kR);
+                    c[1] += (long double)d->b[j] + dnu;
+                    c[2] += -(long double)d->theta[j];
+                    double *dst = range ? e.rhi : e.rlo;
+                    for (int m = 0; m < 7; ++m) dst[m] = (double)(m == 1 ? c[m] : c[m] * kLog2e);
+                }
+            }
+            const int type = d->type[j];
+            if (type == PYRO_ELEMENTARY && !both_sides) {
+                recE.push_back(e);
+                out.order.push_back(j);
+                continue;
+            }
+            RxnX x;
+            std::memset(&x, 0, sizeof x);
+            x.e = e;
+            x.type = (uint8_t)type;
+            for (int s = 0; s < 6; ++s) x.sc_species[s] = kNoSpecies;
+            int nsc = 0;
+            for (auto &kv : net)
+                if (kv.second != 0) {
+                    x.sc_species[nsc] = (uint16_t)kv.first;
+                    x.sc_coef[nsc] = (double)kv.second;
+                    ++nsc;
+                }
+            x.n_scatter = (uint8_t)nsc;
+            x.eff_default = 1.0;
+            if (type != PYRO_ELEMENTARY) {
+                needs_ctot = true;
+                x.eff_default = d->eff_default[j];
+                x.eff_begin = (uint32_t)eff_delta.size();
+                const int cnt = d->eff_ptr[j + 1] - d->eff_ptr[j];
+                PYRO_REQUIRE(cnt <= 65535, PYRO_ERR_TOO_LARGE, "too many efficiencies in reaction %d", j);
+                x.eff_count = (uint16_t)cnt;
+                for (int q = d->eff_ptr[j]; q < d->eff_ptr[j + 1]; ++q) {
+                    eff_delta.push_back(d->eff_value[q] - d->eff_default[j]);
+                    eff_species.push_back((uint16_t)d->eff_species[q]);
+                }
+            }
+            if (type >= PYRO_FALLOFF_LINDEMANN) {
+                x.l[0] = (double)(std::log((long double)d->A0[j]) * kLog2e);
+                x.l[1] = d->b0[j];
+                x.l[2] = (double)(-(long double)d->theta0[j] * kLog2e);
+            }
+            if (type == PYRO_FALLOFF_TROE) {
+                const double *t = d->troe + 4 * j;
+                x.troe_alpha = t[0];
+                x.troe_t3 = (double)(-kLog2e / (long double)t[1]);
+                x.troe_t1 = std::isinf(t[2]) ? 0.0 : (double)(-kLog2e / (long double)t[2]);
+                x.troe_has_t2 = std::isinf(t[3]) ? 0 : 1;
+                x.troe_t2 = x.troe_has_t2 ? (double)(-kLog2e * (long double)t[3]) : 0.0;
+            }
+            recX.push_back(x);
+            orderX.push_back(j);
+        }
+        out.order.insert(out.order.end(), orderX.begin(), orderX.end());
+
+        // ---- blob
+        TableLayout &lay = out.lay;
+        std::memset(&lay, 0, sizeof lay);
+        lay.n_species = ns;
+        lay.n_e = (int)recE.size();
+        lay.n_x = (int)recX.size();
+        lay.n_eff = (int)eff_delta.size();
+        lay.needs_ctot = needs_ctot ? 1 : 0;
+        lay.t_mid = d->t_mid[0];
+        uint32_t off = 0;
+        lay.off_inv_w = off;
+        off = align8(off + (uint32_t)(ns * sizeof(double)));
+        lay.off_rxn_e = off;
+        off = align8(off + (uint32_t)(recE.size() * sizeof(RxnE)));
+        lay.off_rxn_x = off;
+        off = align8(off + (uint32_t)(recX.size() * sizeof(RxnX)));
+        lay.off_eff_delta = off;
+        off = align8(off + (uint32_t)(eff_delta.size() * sizeof(double)));
+        lay.off_eff_species = off;
+        off = align8(off + (uint32_t)(eff_species.size() * sizeof(uint16_t)));
+        lay.bytes = off;
+        out.blob.assign(off, 0);
+        std::vector<double> inv_w(ns);
+        for (int k = 0; k < ns; ++k) inv_w[k] = (double)(1.0L / (long double)d->mol_weight[k]);
+        put(out.blob, lay.off_inv_w, inv_w.data(), inv_w.size());
+        put(out.blob, lay.off_rxn_e, recE.data(), recE.size());
+        put(out.blob, lay.off_rxn_x, recX.data(), recX.size());
+        put(out.blob, lay.off_eff_delta, eff_delta.data(), eff_delta.size());
+        put(out.blob, lay.off_eff_species, eff_species.data(), eff_species.size());
+
+        // ---- energy table of the temperature solve
+        out.energy.assign(ns, EnergyRow{});
+        for (int k = 0; k < ns; ++k) {
+            const long double rw = kR / (long double)d->mol_weight[k];
+            for (int range = 0; range < 2; ++range) {
+                const double *a = (range ? d->nasa_hi : d->nasa_lo) + 7 * k;
+                double *c = range ? out.energy[k].hi : out.energy[k].lo;
+                c[0] = (double)((long double)a[5] * rw);
+                c[1] = (double)(((long double)a[0] - 1) * rw);
+                for (int m = 2; m <= 5; ++m) c[m] = (double)((long double)a[m - 1] / m * rw);
+            }
+        }
+        out.n_species = ns;
+        out.n_reactions = nr;
+        return PYRO_OK;
+    } catch (const Fail &f) {
+        err = f.msg;
+        return f.status;
+    } catch (const std::exception &ex) {
+        err = ex.what();
+        return PYRO_ERR_BAD_MECH;
+    }
+}
+
+}   // namespace pyro

@@ -381,7 +381,10 @@ def config_mechanism(cfg):
 
 def _mean_weight(mech, Y):
     """(A.3): W = 1 / sum(Y_k / W_k); Y is [n_species][n]."""
-    return 1.0 / (Y / mech.mol_weight[:, None]).sum(axis=0)
+    acc = np.zeros(Y.shape[1])
+    for k in range(mech.n_species):   # no [n_species][n] temporary (7 GB at 256^3 x 53)
+        acc += Y[k] / mech.mol_weight[k]
+    return 1.0 / acc
 
 
 def mixture_energy(mech, T, Y, dtype=np.longdouble):

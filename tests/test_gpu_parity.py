@@ -1,0 +1,272 @@
+"""GPU parity: the CUDA path, called through the C ABI of libpyro.so, against the CPU oracle on
+the same seeded inputs, element by element (tolerances of north_star, see parity.py)."""
+import ctypes as C
+import os
+
+import numpy as np
+import pytest
+
+import hand_cases
+import parity
+from oracle import oracle
+from paper_2503_24286_b200 import binding, inputs
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+def dev(x):
+    return torch.from_numpy(np.ascontiguousarray(x)).cuda()
+
+
+@pytest.fixture(scope="module")
+def mechs():
+    cache = {}
+
+    def get(cfg):
+        if cfg not in cache:
+            m = inputs.config_mechanism(cfg)
+            cache[cfg] = (m, binding.Mechanism(m), oracle.Oracle(m))
+        return cache[cfg]
+    return get
+
+
+def gpu_rates(gm, rho, T, Y, **kw):
+    om = gm.get_net_production_rates(dev(rho), dev(T), dev(Y), **kw)
+    torch.cuda.synchronize()
+    return om.cpu().numpy()
+
+
+# ------------------------------------------------------------------ small sizes: every element
+@pytest.mark.parametrize("cfg,n", [(0, 4096), (1, 3001), (2, 2500), (3, 700)])
+def test_rates_every_point(mechs, cfg, n):
+    """Several blocks and a ragged tail; every (species, point) entry compared."""
+    mech, gm, orc = mechs(cfg)
+    st = inputs.config_states(cfg, n=n)
+    om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+    om = gpu_rates(gm, st["rho"], st["T"], st["Y"])
+    parity.assert_omega_parity(om, om_ref, bound)
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 4096), (2, 2500), (3, 700), (4, 13**3)])
+def test_temperature_every_point(mechs, cfg, n):
+    mech, gm, orc = mechs(cfg)
+    st = inputs.config_states(cfg, n=n)
+    T_ref, it, conv = orc.get_temperature(st["e"], st["Y"], st["T_guess"])
+    bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T = gm.get_temperature(dev(st["e"]), dev(st["Y"]), dev(st["T_guess"]), rho=dev(st["rho"]), n_not_converged=bad)
+    torch.cuda.synchronize()
+    parity.assert_T_parity(T.cpu().numpy(), T_ref)
+    assert int(bad.item()) == 0 and conv.all()
+    # generated e came from T in long double: the solve recovers it
+    assert np.max(np.abs(T.cpu().numpy() - st["T"]) / st["T"]) < 1e-12
+
+
+def test_hand_mechanism_every_reaction_class(mechs):
+    mech = hand_cases.all_paths_mechanism()
+    gm = binding.Mechanism(mech)
+    rho, T, Y = hand_cases.random_states(mech, 777)
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+    parity.assert_omega_parity(gpu_rates(gm, rho, T, Y), om_ref, bound)
+
+
+# ------------------------------------------------------------------ full sizes, bench launch configuration
+def _sample(n, count, seed=5):
+    rng = np.random.default_rng(seed)
+    idx = np.unique(np.concatenate([rng.integers(0, n, size=count), [0, 1, n - 2, n - 1]]))
+    return idx
+
+
+@pytest.mark.parametrize("cfg,count", [(1, 20000), (2, 4096), (3, 1024)])
+def test_rates_full_size_sampled(mechs, cfg, count):
+    """BASELINE.json sizes (2^24 / 2^22 / 2^20 points), one launch as bench.py issues it; the oracle
+    evaluates a random sample of points one by one."""
+    mech, gm, orc = mechs(cfg)
+    n = inputs.CONFIG_POINTS[cfg]
+    st = inputs.config_states(cfg)
+    assert st["rho"].shape[0] == n
+    d_rho, d_T, d_Y = dev(st["rho"]), dev(st["T"]), dev(st["Y"])
+    om = gm.get_net_production_rates(d_rho, d_T, d_Y)
+    torch.cuda.synchronize()
+    idx = _sample(n, count)
+    om_s = om[:, torch.from_numpy(idx).cuda()].cpu().numpy()
+    om_ref, bound = orc.get_net_production_rates(st["rho"][idx], st["T"][idx], st["Y"][:, idx])
+    parity.assert_omega_parity(om_s, om_ref, bound)
+    # properties that hold at any size: finite everywhere, mass conservation sum_i W_i omega_i = 0
+    assert bool(torch.isfinite(om).all())
+    W = dev(mech.mol_weight)[:, None]
+    mass = (W * om).sum(0).abs()
+    scale = (W * om.abs()).sum(0)
+    assert bool((mass <= 1e-9 * scale + 1e-300).all())
+    del om, d_Y
+    torch.cuda.empty_cache()
+
+
+def test_full_source_term_step_cfg4_sampled(mechs):
+    """configs[4]: 256^3 flame-front field, (rho, e, Y, T_guess) -> T -> omega on one stream."""
+    mech, gm, orc = mechs(4)
+    n = inputs.CONFIG_POINTS[4]
+    st = inputs.config_states(4)
+    d_Y = dev(st["Y"])
+    d_rho = dev(st["rho"])
+    bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T = gm.get_temperature(dev(st["e"]), d_Y, dev(st["T_guess"]), rho=d_rho, n_not_converged=bad)
+    om = gm.get_net_production_rates(d_rho, T, d_Y)
+    torch.cuda.synchronize()
+    assert int(bad.item()) == 0
+    # sample: random points plus four full x-lines through the flame front
+    lines = np.concatenate([np.arange(256) + 256 * (y + 256 * z) for y, z in ((0, 0), (17, 200), (128, 128), (255, 255))])
+    idx = np.unique(np.concatenate([_sample(n, 3000), lines]))
+    T_ref, it, conv = orc.get_temperature(st["e"][idx], st["Y"][:, idx], st["T_guess"][idx])
+    T_s = T[torch.from_numpy(idx).cuda()].cpu().numpy()
+    parity.assert_T_parity(T_s, T_ref)
+    assert conv.all() and it.max() <= 10
+    # rates parity on the temperature the GPU solve produced (the two T agree to ~1e-15; feeding the
+    # oracle the same T keeps the two tolerances independent)
+    om_ref, bound = orc.get_net_production_rates(st["rho"][idx], T_s, st["Y"][:, idx])
+    parity.assert_omega_parity(om[:, torch.from_numpy(idx).cuda()].cpu().numpy(), om_ref, bound)
+    assert bool(torch.isfinite(om).all()) and bool(torch.isfinite(T).all())
+    # T everywhere recovers the field that generated e (double-precision e at this size: 1e-10)
+    assert float(((T - dev(st["T"])).abs() / dev(st["T"])).max()) < 1e-10
+
+
+# ------------------------------------------------------------------ edge cases
+def test_empty_single_ragged_and_padded_leading_dimension(mechs):
+    mech, gm, orc = mechs(0)
+    ns = mech.n_species
+    # n = 0 launches nothing
+    z = torch.empty(0, dtype=torch.float64, device="cuda")
+    zY = torch.empty((ns, 0), dtype=torch.float64, device="cuda")
+    assert gm.get_net_production_rates(z, z, zY).shape == (ns, 0)
+    assert gm.get_temperature(z, zY, z).shape == (0,)
+    st = inputs.config_states(0, n=1000)
+    om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+    T_ref, _, _ = orc.get_temperature(st["e"], st["Y"], st["T_guess"])
+    for n in (1, 31, 33, 129, 1000):
+        # ld > n: fields are windows into wider buffers, padding filled with NaN that must not be read
+        ld = n + 7
+        Ybuf = torch.full((ns, ld), float("nan"), dtype=torch.float64, device="cuda")
+        Ybuf[:, :n] = dev(st["Y"][:, :n])
+        out = torch.full((ns, ld), -7.0, dtype=torch.float64, device="cuda")
+        gm.get_net_production_rates(dev(st["rho"][:n]), dev(st["T"][:n]), Ybuf[:, :n], out=out[:, :n])
+        Tout = gm.get_temperature(dev(st["e"][:n]), Ybuf[:, :n], dev(st["T_guess"][:n]))
+        torch.cuda.synchronize()
+        parity.assert_omega_parity(out[:, :n].cpu().numpy(), om_ref[:, :n], bound[:, :n])
+        assert bool((out[:, n:] == -7.0).all())   # nothing written beyond n
+        parity.assert_T_parity(Tout.cpu().numpy(), T_ref[:n])
+
+
+def test_temperature_in_place_and_iteration_cap(mechs):
+    mech, gm, orc = mechs(0)
+    st = inputs.config_states(0, n=2048)
+    # T may alias T_guess
+    Tg = dev(st["T_guess"])
+    gm.get_temperature(dev(st["e"]), dev(st["Y"]), Tg, out=Tg)
+    torch.cuda.synchronize()
+    T_ref, _, _ = orc.get_temperature(st["e"], st["Y"], st["T_guess"])
+    parity.assert_T_parity(Tg.cpu().numpy(), T_ref)
+    # cap: non-converged points are counted, the last iterate is returned
+    gm2 = binding.Mechanism(mech)
+    gm2.set_newton(abs_tol_K=1e-6, max_iter=2)
+    bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T2 = gm2.get_temperature(dev(st["e"]), dev(st["Y"]), dev(st["T_guess"]), n_not_converged=bad)
+    torch.cuda.synchronize()
+    T_ref2, it2, conv2 = orc.get_temperature(st["e"], st["Y"], st["T_guess"], tol=1e-6, max_iter=2)
+    parity.assert_T_parity(T2.cpu().numpy(), T_ref2)
+    assert int(bad.item()) == int((conv2 == 0).sum()) > 0
+
+
+def test_abi_error_codes_on_device(mechs):
+    mech, gm, _ = mechs(0)
+    lib = binding.load_library()
+    st = inputs.config_states(0, n=64)
+    rho, T, Y = dev(st["rho"]), dev(st["T"]), dev(st["Y"])
+    om = torch.empty_like(Y)
+    h = gm._h
+    f = lib.pyro_get_net_production_rates
+    assert f(None, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), om.data_ptr(), None) == 1
+    assert f(h, 64, 64, None, T.data_ptr(), Y.data_ptr(), om.data_ptr(), None) == 1
+    assert f(h, -1, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), om.data_ptr(), None) == 2
+    assert f(h, 64, 63, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), om.data_ptr(), None) == 2
+    assert f(h, 64, 64, rho.data_ptr() + 4, T.data_ptr(), Y.data_ptr(), om.data_ptr(), None) == 5
+    assert f(h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), Y.data_ptr(), None) == 2   # omega aliases Y
+    g = lib.pyro_get_temperature
+    assert g(h, 64, 64, None, None, Y.data_ptr(), T.data_ptr(), T.data_ptr(), None, None) == 1
+    assert g(h, 64, 10, None, rho.data_ptr(), Y.data_ptr(), T.data_ptr(), T.data_ptr(), None, None) == 2
+    assert lib.pyro_mech_set_newton(h, -1.0, 10) == 2 and lib.pyro_mech_set_newton(h, 1e-6, 0) == 2
+    assert lib.pyro_last_error_string()
+    out = C.c_void_p()
+    assert lib.pyro_mech_create(None, 0, C.byref(out)) == 1
+    desc, keep = binding.make_desc(mech)
+    assert lib.pyro_mech_create(C.byref(desc), 99, C.byref(out)) == 2 and not out.value
+
+
+def test_two_mechanisms_share_the_constant_bank_across_streams(mechs):
+    """Alternating launches of two mechanisms on two streams: the table bank is re-uploaded in order."""
+    m0, g0, o0 = mechs(0)
+    m2, g2, o2 = mechs(2)
+    assert g0.info()["tables_in_constant"] == 1 and g2.info()["tables_in_constant"] == 1
+    s0 = inputs.config_states(0, n=3000)
+    s2 = inputs.config_states(2, n=1500)
+    ref0, b0 = o0.get_net_production_rates(s0["rho"], s0["T"], s0["Y"])
+    ref2, b2 = o2.get_net_production_rates(s2["rho"], s2["T"], s2["Y"])
+    a0 = [dev(s0[k]) for k in ("rho", "T", "Y")]
+    a2 = [dev(s2[k]) for k in ("rho", "T", "Y")]
+    torch.cuda.synchronize()
+    sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for rep in range(6):
+        outs.append((0, g0.get_net_production_rates(*a0, stream=sa if rep % 2 else sb)))
+        outs.append((2, g2.get_net_production_rates(*a2, stream=sb if rep % 2 else sa)))
+    torch.cuda.synchronize()
+    for which, om in outs:
+        parity.assert_omega_parity(om.cpu().numpy(), ref0 if which == 0 else ref2, b0 if which == 0 else b2)
+
+
+def test_tables_in_global_memory_path(mechs, monkeypatch):
+    """Mechanisms too large for the 64 KB constant bank read their tables from global memory
+    (configs[3] does so by size; here the path is forced for configs[2] as well)."""
+    mech3, g3, _ = mechs(3)
+    assert g3.info()["tables_in_constant"] == 0
+    monkeypatch.setenv("PYRO_TABLES", "global")
+    mech, _, orc = mechs(2)
+    gm = binding.Mechanism(mech)
+    assert gm.info()["tables_in_constant"] == 0
+    st = inputs.config_states(2, n=1111)
+    om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+    parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
+
+
+@pytest.mark.parametrize("block", [32, 64, 128])
+def test_every_block_size_variant(mechs, monkeypatch, block):
+    monkeypatch.setenv("PYRO_RATES_BLOCK", str(block))
+    mech, _, orc = mechs(2)
+    gm = binding.Mechanism(mech)
+    assert gm.info()["block_threads"] == block
+    st = inputs.config_states(2, n=777)
+    om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+    parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
+
+
+def test_host_buffer_pipeline_matches_oracle(mechs, monkeypatch):
+    """pyro_source_terms_host: slabbed H2D -> T -> omega -> D2H with a slab size that leaves a ragged tail."""
+    monkeypatch.setenv("PYRO_HOST_SLAB", "4096")
+    mech, _, orc = mechs(0)
+    gm = binding.Mechanism(mech)
+    n = 4096 * 5 + 123
+    st = inputs.config_states(0, n=n)
+    pin = lambda x: torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
+    T = torch.empty(n, dtype=torch.float64).pin_memory()
+    om = torch.empty((mech.n_species, n), dtype=torch.float64).pin_memory()
+    bad = gm.source_terms_host(pin(st["rho"]), pin(st["e"]), pin(st["Y"]), pin(st["T_guess"]), T, om)
+    assert bad == 0
+    T_ref, _, _ = orc.get_temperature(st["e"], st["Y"], st["T_guess"])
+    parity.assert_T_parity(T.numpy(), T_ref)
+    om_ref, bound = orc.get_net_production_rates(st["rho"], T.numpy(), st["Y"])
+    parity.assert_omega_parity(om.numpy(), om_ref, bound)
+    # pageable numpy buffers work too
+    T2 = np.empty(n)
+    om2 = np.empty((mech.n_species, n))
+    gm.source_terms_host(st["rho"], st["e"], st["Y"], st["T_guess"], T2, om2)
+    assert np.array_equal(T2, T.numpy()) and np.array_equal(om2, om.numpy())

@@ -1,0 +1,222 @@
+"""Host logic without a GPU: the C-ABI library loads and exports what include/pyro.h declares;
+the packer's validation; and the packer + per-point device arithmetic (compiled for the host by
+tests/hostemu, a test-only build) against the oracle."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import mpmath as mp
+import numpy as np
+import pytest
+
+import hand_cases
+import parity
+from oracle import oracle
+from paper_2503_24286_b200 import binding, build, inputs
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+# ------------------------------------------------------------------ boundary
+def test_library_builds_loads_and_exports_every_declared_symbol():
+    build.build_libpyro()
+    lib = C.CDLL(binding.LIB_PATH)
+    header = open(os.path.join(ROOT, "include", "pyro.h")).read()
+    declared = set(re.findall(r"^(?:int|const char \*)\s*(pyro_[a-z0-9_]+)\s*\(", header, flags=re.M))
+    assert declared == set(binding.EXPORTS), declared ^ set(binding.EXPORTS)
+    for name in declared:
+        assert hasattr(lib, name), name
+    # extern "C", plain pointers and sizes: no C++ or torch types in the signatures
+    nm = subprocess.run(["nm", "-D", "--defined-only", binding.LIB_PATH], capture_output=True, text=True).stdout
+    for name in declared:
+        assert re.search(rf"\bT {name}\b", nm), name
+    assert "torch" not in header and "at::" not in header
+
+
+def test_status_strings_and_no_cpu_fallback():
+    lib = binding.load_library()
+    for st, name in binding.STATUS_NAMES.items():
+        assert lib.pyro_status_string(st).decode().startswith(name)
+    import torch
+    if not torch.cuda.is_available():
+        # the product path must fail loudly without a CUDA device
+        with pytest.raises(binding.PyroError) as ei:
+            binding.Mechanism(inputs.config_mechanism(0))
+        assert ei.value.status == 6 and "no CPU fallback" in str(ei.value)
+    assert lib.pyro_mech_destroy(None) == 0
+
+
+# ------------------------------------------------------------------ host emulation helpers
+@pytest.fixture(scope="module")
+def emu():
+    src = os.path.join(ROOT, "tests", "hostemu", "hostemu.cpp")
+    lib = os.path.join(ROOT, "tests", "hostemu", "libhostemu.so")
+    deps = [src] + [os.path.join(ROOT, "paper_2503_24286_b200", "csrc", f)
+                    for f in ("pyro_pack.cpp", "pyro_pack.h", "pyro_point.cuh", "pyro_math.cuh", "pyro_tables.h")]
+    if not os.path.exists(lib) or any(os.path.getmtime(d) > os.path.getmtime(lib) for d in deps):
+        subprocess.run(["g++", "-std=c++17", "-O2", "-mfma", "-shared", "-fPIC", "-o", lib, src,
+                        os.path.join(ROOT, "paper_2503_24286_b200", "csrc", "pyro_pack.cpp")], check=True)
+    L = C.CDLL(lib)
+    L.emu_last_error.restype = C.c_char_p
+    L.emu_exp2.restype = C.c_double
+    L.emu_exp2.argtypes = [C.c_double]
+    vp, i64 = C.c_void_p, C.c_int64
+    L.emu_pack_status.argtypes = [vp, vp]
+    L.emu_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp]
+    L.emu_temperature.argtypes = [vp, i64, i64, vp, vp, vp, C.c_double, C.c_int, vp, vp]
+    return L
+
+
+def emu_rates(emu, mech, rho, T, Y):
+    desc, keep = binding.make_desc(mech)
+    rho, T, Y = (np.ascontiguousarray(x, dtype=np.float64) for x in (rho, T, Y))
+    om = np.empty_like(Y)
+    st = emu.emu_rates(C.byref(desc), rho.shape[0], rho.shape[0], rho.ctypes.data, T.ctypes.data, Y.ctypes.data,
+                       om.ctypes.data)
+    assert st == 0, emu.emu_last_error()
+    return om
+
+
+def emu_temperature(emu, mech, e, Y, Tg, tol=1e-6, max_iter=10):
+    desc, keep = binding.make_desc(mech)
+    e, Y, Tg = (np.ascontiguousarray(x, dtype=np.float64) for x in (e, Y, Tg))
+    T = np.empty_like(e)
+    bad = C.c_int64(0)
+    st = emu.emu_temperature(C.byref(desc), e.shape[0], e.shape[0], e.ctypes.data, Y.ctypes.data, Tg.ctypes.data,
+                             tol, max_iter, T.ctypes.data, C.byref(bad))
+    assert st == 0, emu.emu_last_error()
+    return T, int(bad.value)
+
+
+def pack_status(emu, mech, mutate=None):
+    desc, keep = binding.make_desc(mech)
+    if mutate:
+        mutate(desc, keep)
+    info = (C.c_int64 * 4)()
+    st = emu.emu_pack_status(C.byref(desc), info)
+    return st, list(info), emu.emu_last_error().decode()
+
+
+# ------------------------------------------------------------------ exp2
+def test_exp2_poly_accuracy_and_edges(emu):
+    mp.mp.dps = 40
+    rng = np.random.default_rng(1)
+    ys = np.concatenate([rng.uniform(-1000, 1000, 4000), rng.uniform(-1, 1, 1000),
+                         np.arange(-20, 21) * 0.5, [1e-300, -1e-300, 0.0]])
+    worst = 0.0
+    for y in ys:
+        got = emu.emu_exp2(float(y))
+        ref = mp.mpf(2) ** mp.mpf(float(y))
+        worst = max(worst, float(abs(mp.mpf(got) / ref - 1)))
+    assert worst < 2e-15, worst
+    assert emu.emu_exp2(0.0) == 1.0 and emu.emu_exp2(10.0) == 1024.0 and emu.emu_exp2(-3.0) == 0.125
+    assert emu.emu_exp2(-1100.0) < 1e-307 and emu.emu_exp2(-1e9) < 1e-307       # flushed, never negative or NaN
+    assert emu.emu_exp2(-1100.0) >= 0.0
+    assert np.isnan(emu.emu_exp2(float("nan")))
+    assert not np.isfinite(emu.emu_exp2(1100.0)) or emu.emu_exp2(1100.0) > 1e307
+
+
+# ------------------------------------------------------------------ packer validation (row a0)
+def test_packer_classes_and_table_size(emu):
+    st, info, _ = pack_status(emu, inputs.config_mechanism(0))
+    assert st == 0 and info[0] == 17 and info[1] == 4 and info[3] == 12
+    st, info, _ = pack_status(emu, inputs.config_mechanism(2))
+    assert st == 0 and info[0] == 268 and info[1] == 57 and info[2] <= 63 * 1024
+    st, info, _ = pack_status(emu, hand_cases.all_paths_mechanism())
+    assert st == 0 and info[0] == 5 and info[1] == 6   # 5 plain; 5 special + 1 with a species on both sides
+
+
+def test_packer_error_codes(emu):
+    m = hand_cases.all_paths_mechanism()
+
+    def set_arr(name, idx, val):
+        def f(desc, keep):
+            for a in list(keep):
+                if a.ctypes.data == getattr(desc, name):
+                    c = a.copy()          # never touch the cached mechanism's own arrays
+                    c.flat[idx] = val
+                    keep.append(c)
+                    setattr(desc, name, c.ctypes.data)
+                    break
+        return f
+
+    def null(name):
+        return lambda desc, keep: setattr(desc, name, None)
+
+    assert emu.emu_pack_status(None, None) == 1
+    cases = [
+        (null("mol_weight"), 1), (null("reac_ptr"), 1), (null("A"), 1), (null("troe"), 1), (null("A0"), 1),
+        (lambda d, k: setattr(d, "n_species", 0), 2), (lambda d, k: setattr(d, "n_reactions", -1), 2),
+        (set_arr("mol_weight", 1, -2.0), 3), (set_arr("nasa_lo", 3, np.nan), 3), (set_arr("t_mid", 0, 0.0), 3),
+        (set_arr("A", 2, 0.0), 3), (set_arr("A", 2, -1.0), 3), (set_arr("theta", 0, np.inf), 3),
+        (set_arr("reac_species", 0, 99), 3), (set_arr("prod_species", 1, -1), 3), (set_arr("reac_coeff", 0, 0), 3),
+        (set_arr("reac_coeff", 0, 4), 3),            # more than 3 molecules on a side
+        (set_arr("reac_ptr", 2, 0), 3),              # CSR not monotone
+        (set_arr("type", 0, 9), 3), (set_arr("troe", 4 * 8 + 1, -5.0), 3), (set_arr("troe", 4 * 8 + 2, 0.0), 3),
+        (set_arr("A0", 7, 0.0), 3), (set_arr("eff_species", 0, 77), 3),
+        (set_arr("t_mid", 1, 1200.0), 7),            # two different T_mid: no kernel in this build
+        (lambda d, k: setattr(d, "n_species", 100000), 4),
+    ]
+    for mutate, expected in cases:
+        st, _, msg = pack_status(emu, m, mutate)
+        assert st == expected, (expected, st, msg)
+        assert msg
+    # element balance is checked when a composition is given
+    mech = inputs.config_mechanism(0)
+    assert pack_status(emu, mech)[0] == 0
+    st, _, msg = pack_status(emu, mech, set_arr("elem_comp", 0, 5))
+    assert st == 3 and "balance" in msg
+
+
+# ------------------------------------------------------------------ packer + device arithmetic vs oracle
+def test_emu_rates_hand_mechanism_all_paths(emu):
+    mech = hand_cases.all_paths_mechanism()
+    rho, T, Y = hand_cases.random_states(mech, 512)
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+    om = emu_rates(emu, mech, rho, T, Y)
+    parity.assert_omega_parity(om, om_ref, bound)
+    # one reaction at a time, so that no path hides behind another
+    for j in range(mech.n_reactions):
+        sub = hand_cases.simple_mechanism(hand_cases.species5(), [])   # placeholder to fetch builder
+        rx = _reaction_dict(mech, j)
+        one = hand_cases.simple_mechanism(hand_cases.species5(), [rx])
+        om_ref, bound = oracle.Oracle(one).get_net_production_rates(rho[:64], T[:64], Y[:, :64])
+        parity.assert_omega_parity(emu_rates(emu, one, rho[:64], T[:64], Y[:, :64]), om_ref, bound)
+
+
+def _reaction_dict(mech, j):
+    d = dict(
+        reac={int(mech.reac_species[q]): int(mech.reac_coeff[q]) for q in range(mech.reac_ptr[j], mech.reac_ptr[j + 1])},
+        prod={int(mech.prod_species[q]): int(mech.prod_coeff[q]) for q in range(mech.prod_ptr[j], mech.prod_ptr[j + 1])},
+        A=mech.A[j], b=mech.b[j], theta=mech.theta[j], type=int(mech.rtype[j]), reversible=int(mech.reversible[j]),
+        eff_default=mech.eff_default[j], A0=mech.A0[j], b0=mech.b0[j], theta0=mech.theta0[j],
+        eff={int(mech.eff_species[q]): float(mech.eff_value[q]) for q in range(mech.eff_ptr[j], mech.eff_ptr[j + 1])},
+    )
+    if mech.rtype[j] == 3:
+        d["troe"] = tuple(mech.troe[j])
+    return d
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 4096), (1, 2048), (2, 1024), (3, 256)])
+def test_emu_rates_config_mechanisms(emu, cfg, n):
+    mech = inputs.config_mechanism(cfg)
+    st = inputs.config_states(cfg, n=n)
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
+    r = parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"]), om_ref, bound)
+    assert r < 1e-12   # typical residual is a few 1e-15; 1e-11 is the bar
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 4096), (2, 1024), (3, 256), (4, 512)])
+def test_emu_temperature_config_mechanisms(emu, cfg, n):
+    mech = inputs.config_mechanism(cfg)
+    st = inputs.config_states(cfg, n=n)
+    T_ref, it, conv = oracle.Oracle(mech).get_temperature(st["e"], st["Y"], st["T_guess"])
+    T, bad = emu_temperature(emu, mech, st["e"], st["Y"], st["T_guess"])
+    parity.assert_T_parity(T, T_ref)
+    assert bad == int((conv == 0).sum()) == 0
+    # capped iteration: both stop at the same iterate
+    T_ref3, _, conv3 = oracle.Oracle(mech).get_temperature(st["e"], st["Y"], st["T_guess"], max_iter=2)
+    T3, bad3 = emu_temperature(emu, mech, st["e"], st["Y"], st["T_guess"], max_iter=2)
+    parity.assert_T_parity(T3, T_ref3)
+    assert bad3 == int((conv3 == 0).sum())
