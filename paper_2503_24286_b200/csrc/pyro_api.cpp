@@ -243,7 +243,10 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         const size_t smem = (size_t)2 * lay.n_species * sizeof(double) * bd;
         if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
         const void *fn = pyro::rates_kernel_ptr(bd, m->in_const);
-        if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
+        // the limit is a property of the function, shared by every mechanism: always raise it to the
+        // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
+        if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                       (int)prop.sharedMemPerBlockOptin)) != cudaSuccess)
             return bail(ce, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
         int nblk = 0;
         if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, bd, smem)) != cudaSuccess)
