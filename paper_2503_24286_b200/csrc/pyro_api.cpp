@@ -159,9 +159,14 @@ pyro::RatesArgs rates_args(const pyro_mech *m, int64_t n, int64_t ld, const doub
     pyro::RatesArgs a{};
     a.n = n; a.ld = ld; a.rho = rho; a.T = T; a.Y = Y; a.omega = omega;
     a.gtab = m->d_blob;
-    a.off_inv_w = l.off_inv_w; a.off_rxn_e = l.off_rxn_e; a.off_rxn_x = l.off_rxn_x;
+    a.off_inv_w = l.off_inv_w; a.off_rxn_e = l.off_rxn_e; a.off_rxn_x = l.off_rxn_x; a.off_fall = l.off_fall;
     a.off_eff_delta = l.off_eff_delta; a.off_eff_species = l.off_eff_species;
     a.n_species = l.n_species; a.n_e = l.n_e; a.n_x = l.n_x;
+    for (int s = 0; s < 9; ++s) {
+        a.shape_pairs[s] = l.shape_pairs[s];
+        a.shape_singles[s] = l.shape_singles[s];
+    }
+    for (int k = 0; k < 4; ++k) a.ext_count[k] = l.ext_count[k];
     a.t_mid = l.t_mid;
     return a;
 }
@@ -237,10 +242,10 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     int forced = 0;
     if (const char *env = std::getenv("PYRO_RATES_BLOCK")) forced = std::atoi(env);
     int best_threads = -1;
-    const int candidates[3] = {64, 128, 32};
+    const int candidates[3] = {64, 32, 128};
     for (int bd : candidates) {
         if (forced && bd != forced) continue;
-        const size_t smem = (size_t)2 * lay.n_species * sizeof(double) * bd;
+        const size_t smem = (size_t)2 * (lay.n_species + 1) * sizeof(double) * pyro::kPointsPerThread * bd;
         if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
         const void *fn = pyro::rates_kernel_ptr(bd, m->in_const);
         // the limit is a property of the function, shared by every mechanism: always raise it to the

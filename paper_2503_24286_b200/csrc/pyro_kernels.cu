@@ -17,7 +17,7 @@ __constant__ __align__(16) unsigned char c_tab[kConstBankBytes];
 
 template <bool kConst> struct DevTab {
     const unsigned char *base;   // global-memory copy of the blob (used when !kConst)
-    uint32_t off_inv_w, off_rxn_e, off_rxn_x, off_eff_delta, off_eff_species;
+    uint32_t off_inv_w, off_rxn_e, off_rxn_x, off_fall, off_eff_delta, off_eff_species;
 
     __device__ __forceinline__ const unsigned char *at(uint32_t off) const {
         if constexpr (kConst)
@@ -28,39 +28,99 @@ template <bool kConst> struct DevTab {
     __device__ __forceinline__ double inv_w(int k) const { return reinterpret_cast<const double *>(at(off_inv_w))[k]; }
     __device__ __forceinline__ const RxnE &rxn_e(int j) const { return reinterpret_cast<const RxnE *>(at(off_rxn_e))[j]; }
     __device__ __forceinline__ const RxnX &rxn_x(int j) const { return reinterpret_cast<const RxnX *>(at(off_rxn_x))[j]; }
+    __device__ __forceinline__ const RxnFall &rxn_fall(int j) const { return reinterpret_cast<const RxnFall *>(at(off_fall))[j]; }
     __device__ __forceinline__ double eff_delta(int q) const { return reinterpret_cast<const double *>(at(off_eff_delta))[q]; }
     __device__ __forceinline__ int eff_species(int q) const { return reinterpret_cast<const uint16_t *>(at(off_eff_species))[q]; }
 };
 
 // ---------------------------------------------------------------------------------------
 // omega[k][p] from rho[p], T[p], Y[k][p]   (rows a1-a3, a5-a9)
+// Thread t of a block owns the P = 2 adjacent points 2t, 2t+1 of the block's tile, so a warp
+// reads 512 contiguous bytes of every species plane (128-bit loads when the planes are
+// 16-byte aligned) and every shared-memory access is a conflict-free 128-bit one.
 // ---------------------------------------------------------------------------------------
 template <int BD, bool kConst>
 __global__ void __launch_bounds__(BD) rates_kernel(const RatesArgs a) {
-    extern __shared__ double smem[];
+    constexpr int P = kPointsPerThread;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
     const int tid = threadIdx.x;
-    const int64_t p = (int64_t)blockIdx.x * BD + tid;
-    if (p >= a.n) return;
+    const int64_t p0 = ((int64_t)blockIdx.x * BD + tid) * P;
+    if (p0 >= a.n) return;
     const int ns = a.n_species;
-    double *sC = smem + tid;
-    double *sW = smem + (size_t)ns * BD + tid;
-    DevTab<kConst> tab{a.gtab, a.off_inv_w, a.off_rxn_e, a.off_rxn_x, a.off_eff_delta, a.off_eff_species};
+    Vec<P> *sC = reinterpret_cast<Vec<P> *>(smem_raw) + tid;
+    Vec<P> *sW = sC + (size_t)(ns + 1) * BD;   // + 1: the dummy species (C = 1, omega = sink)
+    DevTab<kConst> tab{a.gtab, a.off_inv_w, a.off_rxn_e, a.off_rxn_x, a.off_fall, a.off_eff_delta, a.off_eff_species};
 
-    const double rho = a.rho[p];
-    const double T = a.T[p];
-    const double *Yp = a.Y + p;
-    double ctot = 0.0;
-#pragma unroll 4
-    for (int k = 0; k < ns; ++k) {
-        const double c = rho * Yp[(int64_t)k * a.ld] * tab.inv_w(k);   // (A.8) PAPER.md:921
-        sC[k * BD] = c;
-        sW[k * BD] = 0.0;
-        ctot += c;
+    const bool full = p0 + P <= a.n;   // the last thread of an odd n owns one point only
+    const bool vec = full && ((a.ld & 1) == 0) && ((reinterpret_cast<uintptr_t>(a.Y) & 15) == 0) &&
+                     ((reinterpret_cast<uintptr_t>(a.omega) & 15) == 0);
+    int64_t pi[P];
+#pragma unroll
+    for (int i = 0; i < P; ++i) pi[i] = (p0 + i < a.n) ? p0 + i : a.n - 1;
+    double rho[P], T[P], ctot[P];
+#pragma unroll
+    for (int i = 0; i < P; ++i) {
+        rho[i] = a.rho[pi[i]];
+        T[i] = a.T[pi[i]];
+        ctot[i] = 0.0;
     }
-    accumulate_reactions(tab, a.n_e, a.n_x, a.t_mid, T, ctot, sC, sW, BD);
-    double *Wp = a.omega + p;
+    if (vec) {
+        const Vec<P> *Yv = reinterpret_cast<const Vec<P> *>(a.Y + p0);
+        const int64_t ldv = a.ld / P;
 #pragma unroll 4
-    for (int k = 0; k < ns; ++k) Wp[(int64_t)k * a.ld] = sW[k * BD];
+        for (int k = 0; k < ns; ++k) {
+            const Vec<P> y = Yv[(int64_t)k * ldv];
+            const double iw = tab.inv_w(k);
+            Vec<P> c, z;
+#pragma unroll
+            for (int i = 0; i < P; ++i) {
+                c.v[i] = rho[i] * y.v[i] * iw;   // (A.8) PAPER.md:921
+                z.v[i] = 0.0;
+                ctot[i] += c.v[i];
+            }
+            sC[k * BD] = c;
+            sW[k * BD] = z;
+        }
+    } else {
+#pragma unroll 2
+        for (int k = 0; k < ns; ++k) {
+            const double iw = tab.inv_w(k);
+            Vec<P> c, z;
+#pragma unroll
+            for (int i = 0; i < P; ++i) {
+                c.v[i] = rho[i] * a.Y[(int64_t)k * a.ld + pi[i]] * iw;
+                z.v[i] = 0.0;
+                ctot[i] += c.v[i];
+            }
+            sC[k * BD] = c;
+            sW[k * BD] = z;
+        }
+    }
+    {
+        Vec<P> one, z;
+#pragma unroll
+        for (int i = 0; i < P; ++i) {
+            one.v[i] = 1.0;
+            z.v[i] = 0.0;
+        }
+        sC[ns * BD] = one;
+        sW[ns * BD] = z;
+    }
+    const PointT<P> pt = make_point<P>(T, a.t_mid);
+    accumulate_reactions<P>(tab, a.shape_pairs, a.shape_singles, a.ext_count, pt, ctot, sC, sW, BD);
+    if (vec) {
+        Vec<P> *Wv = reinterpret_cast<Vec<P> *>(a.omega + p0);
+        const int64_t ldv = a.ld / P;
+#pragma unroll 4
+        for (int k = 0; k < ns; ++k) Wv[(int64_t)k * ldv] = sW[k * BD];
+    } else {
+        for (int k = 0; k < ns; ++k) {
+            const Vec<P> w = sW[k * BD];
+#pragma unroll
+            for (int i = 0; i < P; ++i)
+                if (p0 + i < a.n) a.omega[(int64_t)k * a.ld + p0 + i] = w.v[i];
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -160,7 +220,8 @@ cudaError_t upload_const_table(const void *src_device, size_t bytes, cudaStream_
 cudaError_t launch_rates(const RatesArgs &a, int bd, bool in_const, size_t smem_bytes, cudaStream_t stream) {
     const void *fn = rates_kernel_ptr(bd, in_const);
     if (!fn) return cudaErrorInvalidValue;
-    const int64_t blocks = (a.n + bd - 1) / bd;
+    const int64_t per_block = (int64_t)bd * kPointsPerThread;
+    const int64_t blocks = (a.n + per_block - 1) / per_block;
     RatesArgs copy = a;
     void *params[] = {&copy};
     return cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)bd), params, smem_bytes, stream);

@@ -14,10 +14,13 @@ struct RatesArgs {
     const double *rho, *T, *Y;
     double *omega;
     const unsigned char *gtab;   // device copy of the table blob in global memory
-    uint32_t off_inv_w, off_rxn_e, off_rxn_x, off_eff_delta, off_eff_species;
+    uint32_t off_inv_w, off_rxn_e, off_rxn_x, off_fall, off_eff_delta, off_eff_species;
     int32_t n_species, n_e, n_x;
+    int32_t shape_pairs[9], shape_singles[9], ext_count[4];
     double t_mid;
 };
+
+constexpr int kPointsPerThread = 2;   // grid points owned by one thread of the rates kernel
 
 struct TempArgs {
     int64_t n, ld;

@@ -5,6 +5,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <algorithm>
 #include <map>
 
 namespace pyro {
@@ -161,35 +162,40 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         // ---- reactions: records
         std::vector<RxnE> recE;
         std::vector<RxnX> recX;
+        std::vector<RxnFall> recFall;
         std::vector<double> eff_delta;
         std::vector<uint16_t> eff_species;
         out.order.clear();
-        std::vector<int> orderX;
+        std::vector<int> orderX, orderE, shapeE;
+        std::vector<std::vector<int>> speciesE;
         bool needs_ctot = false;
         for (int j = 0; j < nr; ++j) {
             RxnE e;
             std::memset(&e, 0, sizeof e);
-            for (int s = 0; s < 6; ++s) e.slot[s] = kNoSpecies;
+            uint16_t slot[6];
+            for (int s = 0; s < 6; ++s) slot[s] = (uint16_t)ns;   // dummy species: C = 1, omega = sink
             std::map<int, int> net;
-            bool both_sides = false;
+            bool repeated = false;   // a coefficient above 1 or a species on both sides
             int nreac = 0, nprod = 0;
             for (int q = d->reac_ptr[j]; q < d->reac_ptr[j + 1]; ++q) {
-                for (int r = 0; r < d->reac_coeff[q]; ++r) e.slot[nreac++] = (uint16_t)d->reac_species[q];
+                for (int r = 0; r < d->reac_coeff[q]; ++r) slot[nreac++] = (uint16_t)d->reac_species[q];
+                if (d->reac_coeff[q] > 1) repeated = true;
                 net[d->reac_species[q]] -= d->reac_coeff[q];
             }
             for (int q = d->prod_ptr[j]; q < d->prod_ptr[j + 1]; ++q) {
-                for (int r = 0; r < d->prod_coeff[q]; ++r) e.slot[3 + nprod++] = (uint16_t)d->prod_species[q];
-                if (net.count(d->prod_species[q])) both_sides = true;
+                for (int r = 0; r < d->prod_coeff[q]; ++r) slot[3 + nprod++] = (uint16_t)d->prod_species[q];
+                if (d->prod_coeff[q] > 1 || net.count(d->prod_species[q])) repeated = true;
                 net[d->prod_species[q]] += d->prod_coeff[q];
             }
-            e.nreac = (uint8_t)nreac;
-            e.nprod = (uint8_t)nprod;
-            e.reversible = d->reversible[j] ? 1 : 0;
+            const bool reversible = d->reversible[j] != 0;
+            e.sw[0] = (uint64_t)slot[0] | ((uint64_t)slot[1] << 16) | ((uint64_t)slot[2] << 32) | ((uint64_t)slot[3] << 48);
+            e.sw[1] = (uint64_t)slot[4] | ((uint64_t)slot[5] << 16) | ((uint64_t)nreac << 32) | ((uint64_t)nprod << 40) |
+                      ((uint64_t)(reversible ? 1 : 0) << 48);
             // (A.9): log2 k_f = log2 A + b log2 T - theta log2e / T
             e.f[0] = (double)(std::log((long double)d->A[j]) * kLog2e);
             e.f[1] = d->b[j];
             e.f[2] = (double)(-(long double)d->theta[j] * kLog2e);
-            if (e.reversible) {
+            if (reversible) {
                 // (A.10), G1: ln K_c = dnu ln(p0/(R T)) - sum_i nu_i g_i/(RT);  ln k_r = ln k_f - ln K_c
                 const int dnu = nprod - nreac;
                 for (int range = 0; range < 2; ++range) {
@@ -205,24 +211,27 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                 }
             }
             const int type = d->type[j];
-            if (type == PYRO_ELEMENTARY && !both_sides) {
+            if (type == PYRO_ELEMENTARY && !repeated && reversible) {
                 recE.push_back(e);
-                out.order.push_back(j);
+                shapeE.push_back(3 * (nreac - 1) + (nprod - 1));
+                orderE.push_back(j);
+                std::vector<int> sp;
+                for (auto &kv : net) sp.push_back(kv.first);
+                speciesE.push_back(sp);
                 continue;
             }
             RxnX x;
             std::memset(&x, 0, sizeof x);
             x.e = e;
             x.type = (uint8_t)type;
-            for (int s = 0; s < 6; ++s) x.sc_species[s] = kNoSpecies;
+            for (int s = 0; s < 6; ++s) x.sc_species[s] = (uint16_t)ns;
             int nsc = 0;
             for (auto &kv : net)
                 if (kv.second != 0) {
                     x.sc_species[nsc] = (uint16_t)kv.first;
-                    x.sc_coef[nsc] = (double)kv.second;
+                    x.sc_nu[nsc] = (int8_t)kv.second;
                     ++nsc;
                 }
-            x.n_scatter = (uint8_t)nsc;
             x.eff_default = 1.0;
             if (type != PYRO_ELEMENTARY) {
                 needs_ctot = true;
@@ -237,22 +246,67 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                 }
             }
             if (type >= PYRO_FALLOFF_LINDEMANN) {
-                x.l[0] = (double)(std::log((long double)d->A0[j]) * kLog2e);
-                x.l[1] = d->b0[j];
-                x.l[2] = (double)(-(long double)d->theta0[j] * kLog2e);
-            }
-            if (type == PYRO_FALLOFF_TROE) {
-                const double *t = d->troe + 4 * j;
-                x.troe_alpha = t[0];
-                x.troe_t3 = (double)(-kLog2e / (long double)t[1]);
-                x.troe_t1 = std::isinf(t[2]) ? 0.0 : (double)(-kLog2e / (long double)t[2]);
-                x.troe_has_t2 = std::isinf(t[3]) ? 0 : 1;
-                x.troe_t2 = x.troe_has_t2 ? (double)(-kLog2e * (long double)t[3]) : 0.0;
+                RxnFall fl;
+                std::memset(&fl, 0, sizeof fl);
+                fl.l[0] = (double)(std::log((long double)d->A0[j]) * kLog2e);
+                fl.l[1] = d->b0[j];
+                fl.l[2] = (double)(-(long double)d->theta0[j] * kLog2e);
+                if (type == PYRO_FALLOFF_TROE) {
+                    const double *t = d->troe + 4 * j;
+                    fl.troe_alpha = t[0];
+                    fl.troe_t3 = (double)(-kLog2e / (long double)t[1]);
+                    fl.troe_t1 = std::isinf(t[2]) ? 0.0 : (double)(-kLog2e / (long double)t[2]);
+                    fl.troe_has_t2 = std::isinf(t[3]) ? 0.0 : 1.0;
+                    fl.troe_t2 = std::isinf(t[3]) ? 0.0 : (double)(-kLog2e * (long double)t[3]);
+                }
+                PYRO_REQUIRE(recFall.size() < 65535, PYRO_ERR_TOO_LARGE, "too many falloff reactions");
+                x.fall_index = (uint16_t)recFall.size();
+                recFall.push_back(fl);
             }
             recX.push_back(x);
             orderX.push_back(j);
         }
-        out.order.insert(out.order.end(), orderX.begin(), orderX.end());
+        // plain class: by shape; within a shape greedy coupling of species-disjoint reactions, so
+        // that the kernel can run two reactions in lockstep with all their shared-memory
+        // read-modify-writes independent
+        std::vector<RxnE> sortedE;
+        int shape_pairs[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, shape_singles[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+        for (int shape = 0; shape < 9; ++shape) {
+            std::vector<int> open, couples;
+            for (size_t i = 0; i < recE.size(); ++i) {
+                if (shapeE[i] != shape) continue;
+                int partner = -1;
+                for (size_t o = 0; o < open.size() && partner < 0; ++o) {
+                    bool disjoint = true;
+                    for (int a : speciesE[open[o]])
+                        for (int b : speciesE[i]) disjoint = disjoint && a != b;
+                    if (disjoint) partner = (int)o;
+                }
+                if (partner >= 0) {
+                    couples.push_back(open[partner]);
+                    couples.push_back((int)i);
+                    open.erase(open.begin() + partner);
+                } else {
+                    open.push_back((int)i);
+                }
+            }
+            shape_pairs[shape] = (int)couples.size();
+            shape_singles[shape] = (int)open.size();
+            for (int i : couples) { sortedE.push_back(recE[i]); out.order.push_back(orderE[i]); }
+            for (int i : open) { sortedE.push_back(recE[i]); out.order.push_back(orderE[i]); }
+        }
+        recE.swap(sortedE);
+        // extended class: by kind
+        std::vector<RxnX> sortedX;
+        int ext_count[4] = {0, 0, 0, 0};
+        for (int kind = 0; kind < 4; ++kind)
+            for (size_t i = 0; i < recX.size(); ++i)
+                if ((int)recX[i].type == kind) {
+                    sortedX.push_back(recX[i]);
+                    out.order.push_back(orderX[i]);
+                    ext_count[kind]++;
+                }
+        recX.swap(sortedX);
 
         // ---- blob
         TableLayout &lay = out.lay;
@@ -261,8 +315,14 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         lay.n_e = (int)recE.size();
         lay.n_x = (int)recX.size();
         lay.n_eff = (int)eff_delta.size();
+        lay.n_fall = (int)recFall.size();
         lay.needs_ctot = needs_ctot ? 1 : 0;
         lay.t_mid = d->t_mid[0];
+        for (int s = 0; s < 9; ++s) {
+            lay.shape_pairs[s] = shape_pairs[s];
+            lay.shape_singles[s] = shape_singles[s];
+        }
+        for (int k = 0; k < 4; ++k) lay.ext_count[k] = ext_count[k];
         uint32_t off = 0;
         lay.off_inv_w = off;
         off = align8(off + (uint32_t)(ns * sizeof(double)));
@@ -270,6 +330,8 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         off = align8(off + (uint32_t)(recE.size() * sizeof(RxnE)));
         lay.off_rxn_x = off;
         off = align8(off + (uint32_t)(recX.size() * sizeof(RxnX)));
+        lay.off_fall = off;
+        off = align8(off + (uint32_t)(recFall.size() * sizeof(RxnFall)));
         lay.off_eff_delta = off;
         off = align8(off + (uint32_t)(eff_delta.size() * sizeof(double)));
         lay.off_eff_species = off;
@@ -281,6 +343,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         put(out.blob, lay.off_inv_w, inv_w.data(), inv_w.size());
         put(out.blob, lay.off_rxn_e, recE.data(), recE.size());
         put(out.blob, lay.off_rxn_x, recX.data(), recX.size());
+        put(out.blob, lay.off_fall, recFall.data(), recFall.size());
         put(out.blob, lay.off_eff_delta, eff_delta.data(), eff_delta.size());
         put(out.blob, lay.off_eff_species, eff_species.data(), eff_species.size());
 

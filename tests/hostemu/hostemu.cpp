@@ -19,6 +19,7 @@ struct HostTab {
     pyro::TableLayout lay;
     const pyro::RxnE &rxn_e(int j) const { return reinterpret_cast<const pyro::RxnE *>(base + lay.off_rxn_e)[j]; }
     const pyro::RxnX &rxn_x(int j) const { return reinterpret_cast<const pyro::RxnX *>(base + lay.off_rxn_x)[j]; }
+    const pyro::RxnFall &rxn_fall(int j) const { return reinterpret_cast<const pyro::RxnFall *>(base + lay.off_fall)[j]; }
     double inv_w(int k) const { return reinterpret_cast<const double *>(base + lay.off_inv_w)[k]; }
     double eff_delta(int q) const { return reinterpret_cast<const double *>(base + lay.off_eff_delta)[q]; }
     int eff_species(int q) const { return reinterpret_cast<const uint16_t *>(base + lay.off_eff_species)[q]; }
@@ -44,21 +45,37 @@ int emu_pack_status(const pyro_mech_desc *d, int64_t *info4) {
 
 int emu_rates(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
               double *omega) {
+    constexpr int P = 2;   // as the kernel: one "thread" owns two adjacent points
     pyro::PackedMech pm;
     int st = pyro::pack_mechanism(d, pm, g_err);
     if (st != PYRO_OK) return st;
     HostTab tab{pm.blob.data(), pm.lay};
     const int ns = pm.n_species;
-    std::vector<double> C(ns), W(ns);
-    for (int64_t p = 0; p < n; ++p) {
-        double ctot = 0;
-        for (int k = 0; k < ns; ++k) {
-            C[k] = rho[p] * Y[k * ld + p] * tab.inv_w(k);
-            W[k] = 0;
-            ctot += C[k];
+    std::vector<pyro::Vec<P>> C(ns + 1), W(ns + 1);   // + the dummy species
+    for (int64_t p0 = 0; p0 < n; p0 += P) {
+        double ctot[P], Tp[P];
+        int64_t pi[P];
+        for (int i = 0; i < P; ++i) {
+            pi[i] = p0 + i < n ? p0 + i : n - 1;
+            Tp[i] = T[pi[i]];
+            ctot[i] = 0;
         }
-        pyro::accumulate_reactions(tab, pm.lay.n_e, pm.lay.n_x, pm.lay.t_mid, T[p], ctot, C.data(), W.data(), 1);
-        for (int k = 0; k < ns; ++k) omega[k * ld + p] = W[k];
+        for (int k = 0; k < ns; ++k)
+            for (int i = 0; i < P; ++i) {
+                C[k].v[i] = rho[pi[i]] * Y[k * ld + pi[i]] * tab.inv_w(k);
+                W[k].v[i] = 0;
+                ctot[i] += C[k].v[i];
+            }
+        for (int i = 0; i < P; ++i) {
+            C[ns].v[i] = 1.0;
+            W[ns].v[i] = 0.0;
+        }
+        const pyro::PointT<P> pt = pyro::make_point<P>(Tp, pm.lay.t_mid);
+        pyro::accumulate_reactions<P>(tab, pm.lay.shape_pairs, pm.lay.shape_singles, pm.lay.ext_count, pt, ctot,
+                                      C.data(), W.data(), 1);
+        for (int k = 0; k < ns; ++k)
+            for (int i = 0; i < P; ++i)
+                if (p0 + i < n) omega[k * ld + p0 + i] = W[k].v[i];
     }
     return PYRO_OK;
 }

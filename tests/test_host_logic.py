@@ -118,13 +118,28 @@ def test_exp2_poly_accuracy_and_edges(emu):
 
 
 # ------------------------------------------------------------------ packer validation (row a0)
+def _expected_plain(mech):
+    """Plain class = elementary, reversible, every coefficient 1, no species on both sides."""
+    n = 0
+    for j in range(mech.n_reactions):
+        rc = mech.reac_coeff[mech.reac_ptr[j]:mech.reac_ptr[j + 1]]
+        pc = mech.prod_coeff[mech.prod_ptr[j]:mech.prod_ptr[j + 1]]
+        rs = set(mech.reac_species[mech.reac_ptr[j]:mech.reac_ptr[j + 1]])
+        ps = set(mech.prod_species[mech.prod_ptr[j]:mech.prod_ptr[j + 1]])
+        if mech.rtype[j] == 0 and mech.reversible[j] and (rc == 1).all() and (pc == 1).all() and not (rs & ps):
+            n += 1
+    return n
+
+
 def test_packer_classes_and_table_size(emu):
-    st, info, _ = pack_status(emu, inputs.config_mechanism(0))
-    assert st == 0 and info[0] == 17 and info[1] == 4 and info[3] == 12
+    for mech in (inputs.config_mechanism(0), inputs.config_mechanism(2), hand_cases.all_paths_mechanism()):
+        st, info, _ = pack_status(emu, mech)
+        n_plain = _expected_plain(mech)
+        assert st == 0 and info[0] == n_plain and info[1] == mech.n_reactions - n_plain
+        assert info[3] == len(mech.eff_species)
     st, info, _ = pack_status(emu, inputs.config_mechanism(2))
-    assert st == 0 and info[0] == 268 and info[1] == 57 and info[2] <= 63 * 1024
-    st, info, _ = pack_status(emu, hand_cases.all_paths_mechanism())
-    assert st == 0 and info[0] == 5 and info[1] == 6   # 5 plain; 5 special + 1 with a species on both sides
+    assert info[2] <= 63 * 1024          # configs[2] tables fit the constant bank
+    assert info[0] > 200                 # and most reactions are in the plain class
 
 
 def test_packer_error_codes(emu):
