@@ -74,8 +74,8 @@ typedef struct {
                            T* or T** = +inf drops that term (3-parameter form when T** = +inf)     */
 } pyro_mech_desc;
 
-/* Validate `desc`, flatten it into device tables (packed rate and equilibrium coefficients,
- * fixed-width species slots, efficiency lists, falloff parameters, NASA energy tables) and
+/* Validate `desc`, flatten it into device tables (per-species Gibbs rows, packed Arrhenius
+ * coefficients, fixed-width species slots, efficiency lists, falloff parameters, NASA energy tables) and
  * upload them to CUDA device `device`.  *out receives the handle.  On error *out = NULL. */
 int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out);
 
@@ -123,6 +123,7 @@ int pyro_source_terms_host(pyro_mech *mech, int64_t n, int64_t ld, const double 
  *   [6] threads per block of the rates kernel  [7] dynamic shared memory per block (bytes)
  *   [8] resident blocks per SM (occupancy query)  [9] registers per thread of the rates kernel
  *   [10] local (spill) bytes per thread  [11] SM count of the device
+ *   [12] grid points per thread of the rates kernel
  * returns the number of values written (negative pyro_status on error). */
 int pyro_mech_info(const pyro_mech *mech, int64_t *out, int cap);
 

@@ -110,7 +110,8 @@ def make_desc(mech):
 
 
 _INFO_KEYS = ("n_species", "n_reactions", "n_plain", "n_extended", "table_bytes", "tables_in_constant",
-              "block_threads", "smem_bytes", "blocks_per_sm", "registers", "local_bytes", "sm_count")
+              "block_threads", "smem_bytes", "blocks_per_sm", "registers", "local_bytes", "sm_count",
+              "points_per_thread")
 
 
 def _ptr(t):
@@ -150,8 +151,8 @@ class Mechanism:
             pass
 
     def info(self):
-        out = (C.c_int64 * 12)()
-        n = self._lib.pyro_mech_info(self._h, out, 12)
+        out = (C.c_int64 * 13)()
+        n = self._lib.pyro_mech_info(self._h, out, 13)
         if n < 0:
             _check(-n)
         return dict(zip(_INFO_KEYS, [int(v) for v in out[:n]]))

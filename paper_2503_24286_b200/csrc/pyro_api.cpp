@@ -79,7 +79,8 @@ struct pyro_mech {
     unsigned char *d_blob = nullptr;
     pyro::EnergyRow *d_energy = nullptr;
     bool in_const = false;
-    int block_threads = 64;
+    int block_threads = 32;
+    int points_per_thread = 1;
     size_t smem_bytes = 0;
     int blocks_per_sm = 0;
     int sm_count = 0;
@@ -117,7 +118,7 @@ bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0
 // Enqueue the rates kernel of `m` on `stream`, making its tables resident first.
 int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t stream) {
     if (!m->in_const) {
-        PYRO_CUDA(pyro::launch_rates(a, m->block_threads, false, m->smem_bytes, stream));
+        PYRO_CUDA(pyro::launch_rates(a, m->block_threads, m->points_per_thread, false, m->smem_bytes, stream));
         return PYRO_OK;
     }
     ConstBank &bank = g_bank[m->device];
@@ -136,7 +137,7 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     } else if (stream != bank.upload_stream) {
         PYRO_CUDA(cudaStreamWaitEvent(stream, bank.upload_done, 0));
     }
-    PYRO_CUDA(pyro::launch_rates(a, m->block_threads, true, m->smem_bytes, stream));
+    PYRO_CUDA(pyro::launch_rates(a, m->block_threads, m->points_per_thread, true, m->smem_bytes, stream));
     cudaEvent_t ev = nullptr;
     for (auto &r : bank.readers)
         if (r.first == stream) ev = r.second;
@@ -159,15 +160,15 @@ pyro::RatesArgs rates_args(const pyro_mech *m, int64_t n, int64_t ld, const doub
     pyro::RatesArgs a{};
     a.n = n; a.ld = ld; a.rho = rho; a.T = T; a.Y = Y; a.omega = omega;
     a.gtab = m->d_blob;
-    a.off_inv_w = l.off_inv_w; a.off_rxn_e = l.off_rxn_e; a.off_rxn_x = l.off_rxn_x; a.off_fall = l.off_fall;
+    a.off_spec = l.off_spec; a.off_rxn_p = l.off_rxn_p; a.off_rxn_x = l.off_rxn_x; a.off_fall = l.off_fall;
     a.off_eff_delta = l.off_eff_delta; a.off_eff_species = l.off_eff_species;
-    a.n_species = l.n_species; a.n_e = l.n_e; a.n_x = l.n_x;
+    a.n_species = l.n_species; a.n_p = l.n_p; a.n_x = l.n_x;
     for (int s = 0; s < 9; ++s) {
+        a.shape_quads[s] = l.shape_quads[s];
         a.shape_pairs[s] = l.shape_pairs[s];
         a.shape_singles[s] = l.shape_singles[s];
     }
     for (int k = 0; k < 4; ++k) a.ext_count[k] = l.ext_count[k];
-    a.t_mid = l.t_mid;
     return a;
 }
 
@@ -238,32 +239,38 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     cudaDeviceProp prop;
     if ((ce = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) return bail(ce, "cudaGetDeviceProperties");
     m->sm_count = prop.multiProcessorCount;
-    // launch shape: the block size that keeps the most threads resident per SM
-    int forced = 0;
-    if (const char *env = std::getenv("PYRO_RATES_BLOCK")) forced = std::atoi(env);
-    int best_threads = -1;
-    const int candidates[3] = {64, 32, 128};
-    for (int bd : candidates) {
-        if (forced && bd != forced) continue;
-        const size_t smem = (size_t)2 * (lay.n_species + 1) * sizeof(double) * pyro::kPointsPerThread * bd;
-        if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
-        const void *fn = pyro::rates_kernel_ptr(bd, m->in_const);
-        // the limit is a property of the function, shared by every mechanism: always raise it to the
-        // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
-        if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                       (int)prop.sharedMemPerBlockOptin)) != cudaSuccess)
-            return bail(ce, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
-        int nblk = 0;
-        if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, bd, smem)) != cudaSuccess)
-            return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
-        if (nblk * bd > best_threads) {
-            best_threads = nblk * bd;
-            m->block_threads = bd;
-            m->smem_bytes = smem;
-            m->blocks_per_sm = nblk;
+    // launch shape (threads per block, points per thread): with the three planes of n_species + 1
+    // doubles per point in shared memory, take the variant that keeps at least two warps per
+    // scheduler resident with the most points in flight; below that, the most warps.
+    int forced_bd = 0, forced_p = 0;
+    if (const char *env = std::getenv("PYRO_RATES_BLOCK")) forced_bd = std::atoi(env);
+    if (const char *env = std::getenv("PYRO_RATES_POINTS")) forced_p = std::atoi(env);
+    long best_score = -1;
+    for (int p = 1; p <= 2; ++p)
+        for (int bd = 32; bd <= 128; bd *= 2) {
+            if ((forced_bd && bd != forced_bd) || (forced_p && p != forced_p)) continue;
+            const size_t smem = (size_t)pyro::kPlanes * (lay.n_species + 1) * sizeof(double) * p * bd;
+            if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
+            const void *fn = pyro::rates_kernel_ptr(bd, p, m->in_const);
+            // the limit is a property of the function, shared by every mechanism: always raise it to the
+            // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
+            if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)prop.sharedMemPerBlockOptin)) != cudaSuccess)
+                return bail(ce, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
+            int nblk = 0;
+            if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, bd, smem)) != cudaSuccess)
+                return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+            const long warps = (long)nblk * bd / 32, points = (long)nblk * bd * p;
+            const long score = (warps < 8 ? warps : 8) * 100000 + points;
+            if (nblk > 0 && score > best_score) {
+                best_score = score;
+                m->block_threads = bd;
+                m->points_per_thread = p;
+                m->smem_bytes = smem;
+                m->blocks_per_sm = nblk;
+            }
         }
-    }
-    if (best_threads <= 0) {
+    if (best_score < 0) {
         cudaFree(m->d_blob);
         cudaFree(m->d_energy);
         delete m;
@@ -305,6 +312,10 @@ int pyro_get_temperature(const pyro_mech *m, int64_t n, int64_t ld, const double
     if (!aligned8(e) || !aligned8(Y) || !aligned8(T_guess) || !aligned8(T) ||
         (reinterpret_cast<uintptr_t>(n_not_converged) & 3u))
         return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
+    if (!m->packed.lay.single_t_mid)
+        return fail(PYRO_ERR_UNSUPPORTED,
+                    "species with different T_mid: the temperature solve of this build sums the energy "
+                    "polynomials per NASA range and needs one T_mid per mechanism");
     DeviceGuard guard(m->device);
     PYRO_CUDA(pyro::launch_temperature(temp_args(m, n, ld, e, Y, T_guess, T, n_not_converged),
                                        static_cast<cudaStream_t>(cuda_stream)));
@@ -396,12 +407,12 @@ int pyro_mech_info(const pyro_mech *m, int64_t *out, int cap) {
     if (!m || !out) return -fail(PYRO_ERR_NULL, "NULL argument");
     DeviceGuard guard(m->device);
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->block_threads, m->in_const));
-    const int64_t v[12] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_e, m->packed.lay.n_x,
+    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->block_threads, m->points_per_thread, m->in_const));
+    const int64_t v[13] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
                            (int64_t)m->packed.lay.bytes, m->in_const ? 1 : 0, m->block_threads,
                            (int64_t)m->smem_bytes, m->blocks_per_sm, fa.numRegs, (int64_t)fa.localSizeBytes,
-                           m->sm_count};
-    int cnt = cap < 12 ? cap : 12;
+                           m->sm_count, m->points_per_thread};
+    int cnt = cap < 13 ? cap : 13;
     for (int i = 0; i < cnt; ++i) out[i] = v[i];
     return cnt;
 }

@@ -35,20 +35,22 @@ template <class T> void put(std::vector<unsigned char> &blob, uint32_t off, cons
     if (count) std::memcpy(blob.data() + off, src, count * sizeof(T));
 }
 
-uint32_t align8(uint32_t x) { return (x + 7u) & ~7u; }
-
-// coefficients of  sum_i nu_i g_i/(RT)  on the features (1, ln T, 1/T, T, T^2, T^3, T^4):
+// log2 E_k on the features (1, log2 T, 1/T, T, T^2, T^3, T^4), E_k = exp(g_k/RT) RT/p0 with
 //   g/RT = a1 (1 - ln T) - a2/2 T - a3/6 T^2 - a4/12 T^3 - a5/20 T^4 + a6/T - a7
-// which is h/RT - s/R of (A.12), (A.13) with the readings G2, G3.
-void add_gibbs(long double c[7], long double nu, const double *a) {
-    c[0] += nu * ((long double)a[0] - (long double)a[6]);
-    c[1] += nu * (-(long double)a[0]);
-    c[2] += nu * (long double)a[5];
-    c[3] += nu * (-(long double)a[1] / 2);
-    c[4] += nu * (-(long double)a[2] / 6);
-    c[5] += nu * (-(long double)a[3] / 12);
-    c[6] += nu * (-(long double)a[4] / 20);
+// which is h/RT - s/R of (A.12), (A.13) with the readings G2, G3.  The coefficient of log2 T
+// needs no log2e factor (a ln T = a log2 T / log2e).
+void species_row(const double *a, double dst[7]) {
+    const long double c0 = (long double)a[0] - (long double)a[6] + std::log(kR / kP0);
+    dst[0] = (double)(c0 * kLog2e);
+    dst[1] = (double)(1.0L - (long double)a[0]);
+    dst[2] = (double)((long double)a[5] * kLog2e);
+    dst[3] = (double)(-(long double)a[1] / 2 * kLog2e);
+    dst[4] = (double)(-(long double)a[2] / 6 * kLog2e);
+    dst[5] = (double)(-(long double)a[3] / 12 * kLog2e);
+    dst[6] = (double)(-(long double)a[4] / 20 * kLog2e);
 }
+
+uint32_t align16(uint32_t x) { return (x + 15u) & ~15u; }
 
 }   // namespace
 
@@ -82,9 +84,6 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         }
         bool single_tmid = true;
         for (int k = 1; k < ns; ++k) single_tmid = single_tmid && d->t_mid[k] == d->t_mid[0];
-        PYRO_REQUIRE(single_tmid, PYRO_ERR_UNSUPPORTED,
-                     "species with different T_mid: this build folds the Gibbs sums per reaction and needs one "
-                     "T_mid per mechanism");
 
         // ---- reactions: validation
         bool any_special = false;
@@ -160,76 +159,65 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         }
 
         // ---- reactions: records
-        std::vector<RxnE> recE;
+        std::vector<RxnP> recP;
         std::vector<RxnX> recX;
         std::vector<RxnFall> recFall;
         std::vector<double> eff_delta;
-        std::vector<uint16_t> eff_species;
+        std::vector<uint32_t> eff_species;
         out.order.clear();
-        std::vector<int> orderX, orderE, shapeE;
-        std::vector<std::vector<int>> speciesE;
+        std::vector<int> orderX, orderP, shapeP;
+        std::vector<std::vector<int>> speciesP;
         bool needs_ctot = false;
         for (int j = 0; j < nr; ++j) {
-            RxnE e;
-            std::memset(&e, 0, sizeof e);
-            uint16_t slot[6];
-            for (int s = 0; s < 6; ++s) slot[s] = (uint16_t)ns;   // dummy species: C = 1, omega = sink
+            uint32_t slot[6];
+            for (int s = 0; s < 6; ++s) slot[s] = (uint32_t)ns;   // dummy species: A = B = 1, omega = sink
             std::map<int, int> net;
             bool repeated = false;   // a coefficient above 1 or a species on both sides
             int nreac = 0, nprod = 0;
             for (int q = d->reac_ptr[j]; q < d->reac_ptr[j + 1]; ++q) {
-                for (int r = 0; r < d->reac_coeff[q]; ++r) slot[nreac++] = (uint16_t)d->reac_species[q];
+                for (int r = 0; r < d->reac_coeff[q]; ++r) slot[nreac++] = (uint32_t)d->reac_species[q];
                 if (d->reac_coeff[q] > 1) repeated = true;
                 net[d->reac_species[q]] -= d->reac_coeff[q];
             }
             for (int q = d->prod_ptr[j]; q < d->prod_ptr[j + 1]; ++q) {
-                for (int r = 0; r < d->prod_coeff[q]; ++r) slot[3 + nprod++] = (uint16_t)d->prod_species[q];
+                for (int r = 0; r < d->prod_coeff[q]; ++r) slot[3 + nprod++] = (uint32_t)d->prod_species[q];
                 if (d->prod_coeff[q] > 1 || net.count(d->prod_species[q])) repeated = true;
                 net[d->prod_species[q]] += d->prod_coeff[q];
             }
             const bool reversible = d->reversible[j] != 0;
-            e.sw[0] = (uint64_t)slot[0] | ((uint64_t)slot[1] << 16) | ((uint64_t)slot[2] << 32) | ((uint64_t)slot[3] << 48);
-            e.sw[1] = (uint64_t)slot[4] | ((uint64_t)slot[5] << 16) | ((uint64_t)nreac << 32) | ((uint64_t)nprod << 40) |
-                      ((uint64_t)(reversible ? 1 : 0) << 48);
             // (A.9): log2 k_f = log2 A + b log2 T - theta log2e / T
-            e.f[0] = (double)(std::log((long double)d->A[j]) * kLog2e);
-            e.f[1] = d->b[j];
-            e.f[2] = (double)(-(long double)d->theta[j] * kLog2e);
-            if (reversible) {
-                // (A.10), G1: ln K_c = dnu ln(p0/(R T)) - sum_i nu_i g_i/(RT);  ln k_r = ln k_f - ln K_c
-                const int dnu = nprod - nreac;
-                for (int range = 0; range < 2; ++range) {
-                    long double c[7] = {0, 0, 0, 0, 0, 0, 0};
-                    const double *nasa = range ? d->nasa_hi : d->nasa_lo;
-                    for (auto &kv : net) add_gibbs(c, (long double)kv.second, nasa + 7 * kv.first);
-                    // ln k_r on (1, ln T, 1/T, T..T^4)
-                    c[0] += std::log((long double)d->A[j]) - dnu * std::log(kP0 / kR);
-                    c[1] += (long double)d->b[j] + dnu;
-                    c[2] += -(long double)d->theta[j];
-                    double *dst = range ? e.rhi : e.rlo;
-                    for (int m = 0; m < 7; ++m) dst[m] = (double)(m == 1 ? c[m] : c[m] * kLog2e);
-                }
-            }
+            double f[3];
+            f[0] = (double)(std::log((long double)d->A[j]) * kLog2e);
+            f[1] = d->b[j];
+            f[2] = (double)(-(long double)d->theta[j] * kLog2e);
             const int type = d->type[j];
             if (type == PYRO_ELEMENTARY && !repeated && reversible) {
-                recE.push_back(e);
-                shapeE.push_back(3 * (nreac - 1) + (nprod - 1));
-                orderE.push_back(j);
+                RxnP p;
+                std::memset(&p, 0, sizeof p);
+                for (int m = 0; m < 3; ++m) p.f[m] = f[m];
+                for (int m = 0; m < nreac; ++m) p.slot[m] = slot[m];
+                for (int m = 0; m < nprod; ++m) p.slot[nreac + m] = slot[3 + m];
+                for (int m = nreac + nprod; m < 6; ++m) p.slot[m] = (uint32_t)ns;
+                recP.push_back(p);
+                shapeP.push_back(3 * (nreac - 1) + (nprod - 1));
+                orderP.push_back(j);
                 std::vector<int> sp;
                 for (auto &kv : net) sp.push_back(kv.first);
-                speciesE.push_back(sp);
+                speciesP.push_back(sp);
                 continue;
             }
             RxnX x;
             std::memset(&x, 0, sizeof x);
-            x.e = e;
-            x.type = (uint8_t)type;
-            for (int s = 0; s < 6; ++s) x.sc_species[s] = (uint16_t)ns;
+            for (int m = 0; m < 3; ++m) x.f[m] = f[m];
+            for (int m = 0; m < 6; ++m) x.slot[m] = slot[m];
+            x.rev = reversible ? 1.0 : 0.0;
+            x.type = (uint32_t)type;
+            for (int s = 0; s < 6; ++s) x.sc_species[s] = (uint32_t)ns;
             int nsc = 0;
             for (auto &kv : net)
                 if (kv.second != 0) {
-                    x.sc_species[nsc] = (uint16_t)kv.first;
-                    x.sc_nu[nsc] = (int8_t)kv.second;
+                    x.sc_species[nsc] = (uint32_t)kv.first;
+                    x.sc_nu[nsc] = (double)kv.second;
                     ++nsc;
                 }
             x.eff_default = 1.0;
@@ -237,12 +225,10 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                 needs_ctot = true;
                 x.eff_default = d->eff_default[j];
                 x.eff_begin = (uint32_t)eff_delta.size();
-                const int cnt = d->eff_ptr[j + 1] - d->eff_ptr[j];
-                PYRO_REQUIRE(cnt <= 65535, PYRO_ERR_TOO_LARGE, "too many efficiencies in reaction %d", j);
-                x.eff_count = (uint16_t)cnt;
+                x.eff_count = (uint32_t)(d->eff_ptr[j + 1] - d->eff_ptr[j]);
                 for (int q = d->eff_ptr[j]; q < d->eff_ptr[j + 1]; ++q) {
                     eff_delta.push_back(d->eff_value[q] - d->eff_default[j]);
-                    eff_species.push_back((uint16_t)d->eff_species[q]);
+                    eff_species.push_back((uint32_t)d->eff_species[q]);
                 }
             }
             if (type >= PYRO_FALLOFF_LINDEMANN) {
@@ -259,43 +245,75 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                     fl.troe_has_t2 = std::isinf(t[3]) ? 0.0 : 1.0;
                     fl.troe_t2 = std::isinf(t[3]) ? 0.0 : (double)(-kLog2e * (long double)t[3]);
                 }
-                PYRO_REQUIRE(recFall.size() < 65535, PYRO_ERR_TOO_LARGE, "too many falloff reactions");
-                x.fall_index = (uint16_t)recFall.size();
+                x.fall_index = (uint32_t)recFall.size();
                 recFall.push_back(fl);
             }
             recX.push_back(x);
             orderX.push_back(j);
         }
-        // plain class: by shape; within a shape greedy coupling of species-disjoint reactions, so
-        // that the kernel can run two reactions in lockstep with all their shared-memory
-        // read-modify-writes independent
-        std::vector<RxnE> sortedE;
-        int shape_pairs[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, shape_singles[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+        // plain class: by shape; within a shape greedy grouping of mutually species-disjoint
+        // reactions (fours, then couples, then the rest), so that the kernel can run a group in
+        // lockstep with all its shared-memory read-modify-writes independent
+        std::vector<RxnP> sortedP;
+        int shape_quads[9] = {0}, shape_pairs[9] = {0}, shape_singles[9] = {0};
+        auto disjoint = [&](int a, int b) {
+            for (int x : speciesP[a])
+                for (int y : speciesP[b])
+                    if (x == y) return false;
+            return true;
+        };
         for (int shape = 0; shape < 9; ++shape) {
-            std::vector<int> open, couples;
-            for (size_t i = 0; i < recE.size(); ++i) {
-                if (shapeE[i] != shape) continue;
-                int partner = -1;
-                for (size_t o = 0; o < open.size() && partner < 0; ++o) {
-                    bool disjoint = true;
-                    for (int a : speciesE[open[o]])
-                        for (int b : speciesE[i]) disjoint = disjoint && a != b;
-                    if (disjoint) partner = (int)o;
+            std::vector<std::vector<int>> open;
+            std::vector<int> fours, twos, ones;
+            for (size_t i = 0; i < recP.size(); ++i) {
+                if (shapeP[i] != shape) continue;
+                int home = -1;
+                for (size_t g = 0; g < open.size() && home < 0; ++g) {
+                    bool ok = true;
+                    for (int member : open[g]) ok = ok && disjoint(member, (int)i);
+                    if (ok) home = (int)g;
                 }
-                if (partner >= 0) {
-                    couples.push_back(open[partner]);
-                    couples.push_back((int)i);
-                    open.erase(open.begin() + partner);
-                } else {
-                    open.push_back((int)i);
+                if (home < 0) {
+                    open.push_back({(int)i});
+                    continue;
+                }
+                open[home].push_back((int)i);
+                if (open[home].size() == 4) {
+                    fours.insert(fours.end(), open[home].begin(), open[home].end());
+                    open.erase(open.begin() + home);
                 }
             }
-            shape_pairs[shape] = (int)couples.size();
-            shape_singles[shape] = (int)open.size();
-            for (int i : couples) { sortedE.push_back(recE[i]); out.order.push_back(orderE[i]); }
-            for (int i : open) { sortedE.push_back(recE[i]); out.order.push_back(orderE[i]); }
+            for (auto &g : open) {
+                size_t at = 0;
+                if (g.size() >= 2) {
+                    twos.push_back(g[0]);
+                    twos.push_back(g[1]);
+                    at = 2;
+                }
+                for (; at < g.size(); ++at) ones.push_back(g[at]);
+            }
+            // leftover singles of different groups may still pair up
+            std::vector<int> rest;
+            for (int i : ones) {
+                int partner = -1;
+                for (size_t o = 0; o < rest.size() && partner < 0; ++o)
+                    if (disjoint(rest[o], i)) partner = (int)o;
+                if (partner >= 0) {
+                    twos.push_back(rest[partner]);
+                    twos.push_back(i);
+                    rest.erase(rest.begin() + partner);
+                } else {
+                    rest.push_back(i);
+                }
+            }
+            shape_quads[shape] = (int)fours.size();
+            shape_pairs[shape] = (int)twos.size();
+            shape_singles[shape] = (int)rest.size();
+            for (int i : fours) { sortedP.push_back(recP[i]); out.order.push_back(orderP[i]); }
+            for (int i : twos) { sortedP.push_back(recP[i]); out.order.push_back(orderP[i]); }
+            for (int i : rest) { sortedP.push_back(recP[i]); out.order.push_back(orderP[i]); }
         }
-        recE.swap(sortedE);
+        recP.swap(sortedP);
         // extended class: by kind
         std::vector<RxnX> sortedX;
         int ext_count[4] = {0, 0, 0, 0};
@@ -308,40 +326,49 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                 }
         recX.swap(sortedX);
 
+        // ---- species rows
+        std::vector<SpecRow> spec(ns);
+        for (int k = 0; k < ns; ++k) {
+            spec[k].inv_w = (double)(1.0L / (long double)d->mol_weight[k]);
+            spec[k].t_mid = d->t_mid[k];
+            species_row(d->nasa_lo + 7 * k, spec[k].lo);
+            species_row(d->nasa_hi + 7 * k, spec[k].hi);
+        }
+
         // ---- blob
         TableLayout &lay = out.lay;
         std::memset(&lay, 0, sizeof lay);
         lay.n_species = ns;
-        lay.n_e = (int)recE.size();
+        lay.n_p = (int)recP.size();
         lay.n_x = (int)recX.size();
         lay.n_eff = (int)eff_delta.size();
         lay.n_fall = (int)recFall.size();
         lay.needs_ctot = needs_ctot ? 1 : 0;
+        lay.single_t_mid = single_tmid ? 1 : 0;
         lay.t_mid = d->t_mid[0];
         for (int s = 0; s < 9; ++s) {
+            lay.shape_quads[s] = shape_quads[s];
             lay.shape_pairs[s] = shape_pairs[s];
             lay.shape_singles[s] = shape_singles[s];
         }
         for (int k = 0; k < 4; ++k) lay.ext_count[k] = ext_count[k];
         uint32_t off = 0;
-        lay.off_inv_w = off;
-        off = align8(off + (uint32_t)(ns * sizeof(double)));
-        lay.off_rxn_e = off;
-        off = align8(off + (uint32_t)(recE.size() * sizeof(RxnE)));
+        lay.off_spec = off;
+        off = align16(off + (uint32_t)(spec.size() * sizeof(SpecRow)));
+        lay.off_rxn_p = off;
+        off = align16(off + (uint32_t)(recP.size() * sizeof(RxnP)));
         lay.off_rxn_x = off;
-        off = align8(off + (uint32_t)(recX.size() * sizeof(RxnX)));
+        off = align16(off + (uint32_t)(recX.size() * sizeof(RxnX)));
         lay.off_fall = off;
-        off = align8(off + (uint32_t)(recFall.size() * sizeof(RxnFall)));
+        off = align16(off + (uint32_t)(recFall.size() * sizeof(RxnFall)));
         lay.off_eff_delta = off;
-        off = align8(off + (uint32_t)(eff_delta.size() * sizeof(double)));
+        off = align16(off + (uint32_t)(eff_delta.size() * sizeof(double)));
         lay.off_eff_species = off;
-        off = align8(off + (uint32_t)(eff_species.size() * sizeof(uint16_t)));
+        off = align16(off + (uint32_t)(eff_species.size() * sizeof(uint32_t)));
         lay.bytes = off;
         out.blob.assign(off, 0);
-        std::vector<double> inv_w(ns);
-        for (int k = 0; k < ns; ++k) inv_w[k] = (double)(1.0L / (long double)d->mol_weight[k]);
-        put(out.blob, lay.off_inv_w, inv_w.data(), inv_w.size());
-        put(out.blob, lay.off_rxn_e, recE.data(), recE.size());
+        put(out.blob, lay.off_spec, spec.data(), spec.size());
+        put(out.blob, lay.off_rxn_p, recP.data(), recP.size());
         put(out.blob, lay.off_rxn_x, recX.data(), recX.size());
         put(out.blob, lay.off_fall, recFall.data(), recFall.size());
         put(out.blob, lay.off_eff_delta, eff_delta.data(), eff_delta.size());

@@ -8,9 +8,9 @@
 
 namespace pyro {
 
-// Limits of the on-chip staging: two FP64 arrays of n_species per thread in shared memory,
-// 32 threads per block at least, 227 KB per block at most.
-constexpr int kMaxSpecies = 440;
+// Limits of the on-chip staging: three FP64 planes of n_species + 1 per point in shared memory,
+// 32 points per block at least, 227 KB per block at most.
+constexpr int kMaxSpecies = 300;
 constexpr int kMaxReactions = 1 << 20;
 
 struct PackedMech {

@@ -238,15 +238,35 @@ def test_tables_in_global_memory_path(mechs, monkeypatch):
     parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
 
 
-@pytest.mark.parametrize("block", [32, 64, 128])
-def test_every_block_size_variant(mechs, monkeypatch, block):
+@pytest.mark.parametrize("cfg,block,points", [(2, 32, 1), (2, 64, 1), (2, 128, 1), (2, 32, 2), (2, 64, 2),
+                                              (0, 32, 2), (0, 64, 2), (0, 128, 2), (0, 128, 1)])
+def test_every_kernel_variant(mechs, monkeypatch, cfg, block, points):
+    """Every compiled (threads per block, points per thread) variant of the rates kernel, forced."""
     monkeypatch.setenv("PYRO_RATES_BLOCK", str(block))
-    mech, _, orc = mechs(2)
+    monkeypatch.setenv("PYRO_RATES_POINTS", str(points))
+    mech, _, orc = mechs(cfg)
     gm = binding.Mechanism(mech)
-    assert gm.info()["block_threads"] == block
-    st = inputs.config_states(2, n=777)
-    om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+    assert gm.info()["block_threads"] == block and gm.info()["points_per_thread"] == points
+    for n in (777, 2 * block * points + 1):
+        st = inputs.config_states(cfg, n=n)
+        om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+        parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
+
+
+def test_species_with_different_t_mid(mechs):
+    """The rates path switches NASA range per species; the temperature solve of this build refuses."""
+    import copy
+    mech = copy.deepcopy(inputs.config_mechanism(0))
+    mech.t_mid = mech.t_mid.copy()
+    mech.t_mid[::2] = 1400.0
+    mech.t_mid[1::3] = 800.0
+    gm = binding.Mechanism(mech)
+    st = inputs.config_states(0, n=3000)
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
     parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
+    with pytest.raises(binding.PyroError) as ei:
+        gm.get_temperature(dev(st["e"]), dev(st["Y"]), dev(st["T_guess"]))
+    assert ei.value.status == 7
 
 
 def test_host_buffer_pipeline_matches_oracle(mechs, monkeypatch):

@@ -63,17 +63,19 @@ def emu():
     L.emu_exp2.argtypes = [C.c_double]
     vp, i64 = C.c_void_p, C.c_int64
     L.emu_pack_status.argtypes = [vp, vp]
-    L.emu_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp]
+    L.emu_rates.argtypes = [vp, C.c_int, i64, i64, vp, vp, vp, vp]
+    L.emu_pack_order.argtypes = [vp, vp]
+    L.emu_exp2_pair.argtypes = [C.c_double, vp, vp]
     L.emu_temperature.argtypes = [vp, i64, i64, vp, vp, vp, C.c_double, C.c_int, vp, vp]
     return L
 
 
-def emu_rates(emu, mech, rho, T, Y):
+def emu_rates(emu, mech, rho, T, Y, points_per_thread=1):
     desc, keep = binding.make_desc(mech)
     rho, T, Y = (np.ascontiguousarray(x, dtype=np.float64) for x in (rho, T, Y))
     om = np.empty_like(Y)
-    st = emu.emu_rates(C.byref(desc), rho.shape[0], rho.shape[0], rho.ctypes.data, T.ctypes.data, Y.ctypes.data,
-                       om.ctypes.data)
+    st = emu.emu_rates(C.byref(desc), points_per_thread, rho.shape[0], rho.shape[0], rho.ctypes.data, T.ctypes.data,
+                       Y.ctypes.data, om.ctypes.data)
     assert st == 0, emu.emu_last_error()
     return om
 
@@ -93,7 +95,7 @@ def pack_status(emu, mech, mutate=None):
     desc, keep = binding.make_desc(mech)
     if mutate:
         mutate(desc, keep)
-    info = (C.c_int64 * 4)()
+    info = (C.c_int64 * 34)()
     st = emu.emu_pack_status(C.byref(desc), info)
     return st, list(info), emu.emu_last_error().decode()
 
@@ -115,6 +117,24 @@ def test_exp2_poly_accuracy_and_edges(emu):
     assert emu.emu_exp2(-1100.0) >= 0.0
     assert np.isnan(emu.emu_exp2(float("nan")))
     assert not np.isfinite(emu.emu_exp2(1100.0)) or emu.emu_exp2(1100.0) > 1e307
+
+
+def test_exp2_pair_is_exp2_and_its_reciprocal(emu):
+    """(2^y, 2^-y) from one range reduction: each as accurate as exp2_poly, product 1 to a few ulp."""
+    mp.mp.dps = 40
+    rng = np.random.default_rng(2)
+    ys = np.concatenate([rng.uniform(-1000, 1000, 3000), rng.uniform(-1, 1, 1000), np.arange(-20, 21) * 0.5, [0.0]])
+    worst = worst_prod = 0.0
+    e, b = C.c_double(), C.c_double()
+    for y in ys:
+        emu.emu_exp2_pair(float(y), C.byref(e), C.byref(b))
+        ref = mp.mpf(2) ** mp.mpf(float(y))
+        worst = max(worst, float(abs(mp.mpf(e.value) / ref - 1)), float(abs(mp.mpf(b.value) * ref - 1)))
+        worst_prod = max(worst_prod, abs(e.value * b.value - 1.0))
+    assert worst < 2e-15, worst
+    assert worst_prod < 1e-15, worst_prod
+    emu.emu_exp2_pair(10.0, C.byref(e), C.byref(b))
+    assert e.value == 1024.0 and b.value == 1.0 / 1024.0
 
 
 # ------------------------------------------------------------------ packer validation (row a0)
@@ -140,6 +160,34 @@ def test_packer_classes_and_table_size(emu):
     st, info, _ = pack_status(emu, inputs.config_mechanism(2))
     assert info[2] <= 63 * 1024          # configs[2] tables fit the constant bank
     assert info[0] > 200                 # and most reactions are in the plain class
+    assert info[4] > 0.7 * info[0]       # mostly stored as lockstep groups of four
+    assert info[6] == 1
+
+
+def test_packer_groups_are_species_disjoint_and_order_is_a_permutation(emu):
+    """The lockstep groups of the plain class batch their omega read-modify-writes: the members of
+    a group must not share a species.  `order` maps packed positions back to the description."""
+    for cfg in (0, 2, 3):
+        mech = inputs.config_mechanism(cfg)
+        desc, keep = binding.make_desc(mech)
+        order = np.empty(mech.n_reactions, dtype=np.int32)
+        assert emu.emu_pack_order(C.byref(desc), order.ctypes.data) == 0
+        assert sorted(order.tolist()) == list(range(mech.n_reactions))
+        st, info, _ = pack_status(emu, mech)
+        species = lambda j: set(mech.reac_species[mech.reac_ptr[j]:mech.reac_ptr[j + 1]]) | \
+            set(mech.prod_species[mech.prod_ptr[j]:mech.prod_ptr[j + 1]])
+        shape = lambda j: 3 * (int(mech.reac_coeff[mech.reac_ptr[j]:mech.reac_ptr[j + 1]].sum()) - 1) + \
+            int(mech.prod_coeff[mech.prod_ptr[j]:mech.prod_ptr[j + 1]].sum()) - 1
+        pos = 0
+        for sh in range(9):
+            for size, count in ((4, info[7 + sh]), (2, info[16 + sh]), (1, info[25 + sh])):
+                assert count % size == 0
+                for g0 in range(pos, pos + count, size):
+                    group = order[g0:g0 + size]
+                    assert all(shape(j) == sh for j in group)
+                    assert len(set().union(*[species(j) for j in group])) == sum(len(species(j)) for j in group)
+                pos += count
+        assert pos == info[0]
 
 
 def test_packer_error_codes(emu):
@@ -170,13 +218,15 @@ def test_packer_error_codes(emu):
         (set_arr("reac_ptr", 2, 0), 3),              # CSR not monotone
         (set_arr("type", 0, 9), 3), (set_arr("troe", 4 * 8 + 1, -5.0), 3), (set_arr("troe", 4 * 8 + 2, 0.0), 3),
         (set_arr("A0", 7, 0.0), 3), (set_arr("eff_species", 0, 77), 3),
-        (set_arr("t_mid", 1, 1200.0), 7),            # two different T_mid: no kernel in this build
         (lambda d, k: setattr(d, "n_species", 100000), 4),
     ]
     for mutate, expected in cases:
         st, _, msg = pack_status(emu, m, mutate)
         assert st == expected, (expected, st, msg)
         assert msg
+    # species with different T_mid pack (the rates path takes the range per species) ...
+    st, info, _ = pack_status(emu, m, set_arr("t_mid", 1, 1200.0))
+    assert st == 0 and info[6] == 0
     # element balance is checked when a composition is given
     mech = inputs.config_mechanism(0)
     assert pack_status(emu, mech)[0] == 0
@@ -219,7 +269,28 @@ def test_emu_rates_config_mechanisms(emu, cfg, n):
     st = inputs.config_states(cfg, n=n)
     om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
     r = parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"]), om_ref, bound)
-    assert r < 1e-12   # typical residual is a few 1e-15; 1e-11 is the bar
+    assert r < 1e-12   # typical residual is a few 1e-14; 1e-11 is the bar
+    r2 = parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"], points_per_thread=2),
+                                    om_ref, bound)
+    assert r2 < 1e-12
+
+
+def test_emu_rates_species_with_different_t_mid(emu):
+    """Each species switches NASA range at its own T_mid (G10); states straddle both."""
+    import copy
+    mech = copy.deepcopy(inputs.config_mechanism(0))
+    mech.t_mid = mech.t_mid.copy()
+    mech.t_mid[::2] = 1400.0
+    mech.t_mid[1::3] = 800.0
+    st = inputs.config_states(0, n=2048)
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
+    parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"]), om_ref, bound)
+    # the temperature solve of this build needs one T_mid
+    desc, keep = binding.make_desc(mech)
+    e = np.ascontiguousarray(st["e"], dtype=np.float64)
+    T = np.empty_like(e)
+    assert emu.emu_temperature(C.byref(desc), e.shape[0], e.shape[0], e.ctypes.data, st["Y"].ctypes.data,
+                               st["T_guess"].ctypes.data, 1e-6, 10, T.ctypes.data, None) == 7
 
 
 @pytest.mark.parametrize("cfg,n", [(0, 4096), (2, 1024), (3, 256), (4, 512)])
