@@ -306,7 +306,7 @@ def main():
                 "step": "pyro_get_temperature then pyro_get_net_production_rates on one stream",
                 "l2": "inputs (%.2f GB per step) are larger than the 126 MB L2; no flush needed" % (8e-9 * n * (ns + 3)),
                 "block_threads": info["block_threads"], "blocks_per_sm": info["blocks_per_sm"],
-                "smem_bytes_per_block": info["smem_bytes"], "tables_in_constant": info["tables_in_constant"],
+                "smem_bytes_per_block": info["smem_bytes"], "tables_in_shared": info["tables_in_shared"], "tmem_columns": info["tmem_columns"],
                 "registers": info["registers"], "spill_bytes": info["local_bytes"],
                 "newton_not_converged": not_converged,
             },

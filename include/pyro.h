@@ -16,9 +16,7 @@
  *          device; "host" pointers are ordinary (preferably pinned) host memory.
  *   Every function returns a pyro_status (0 = PYRO_OK); nothing throws or aborts across the ABI.
  *   Device calls enqueue on `cuda_stream` (a cudaStream_t passed as void*, NULL = default
- *   stream) and return without synchronising; they allocate nothing and copy nothing
- *   (exception: the first launch after a *different* mechanism used the constant-memory
- *   table bank re-uploads <= 64 KB on that stream, ordered after earlier launches by events).
+ *   stream) and return without synchronising; they allocate nothing and copy nothing.
  *   Concurrent calls on one handle from several host threads are allowed.
  *   There is no CPU fallback: without a CUDA device pyro_mech_create fails with PYRO_ERR_CUDA.
  */
@@ -38,7 +36,7 @@ typedef enum {
     PYRO_ERR_BAD_MECH = 3,    /* index out of range, A <= 0, W <= 0, bad Troe temperature,
                                  coefficient <= 0, more than 3 molecules on a side, CSR not monotone,
                                  unknown reaction type                                              */
-    PYRO_ERR_TOO_LARGE = 4,   /* species / reactions beyond what the on-chip staging can hold        */
+    PYRO_ERR_TOO_LARGE = 4,   /* species / reactions beyond what the on-chip staging can hold (255 species) */
     PYRO_ERR_ALIGN = 5,       /* a field pointer is not 8-byte aligned                               */
     PYRO_ERR_CUDA = 6,        /* CUDA runtime error (text via pyro_last_error_string)                */
     PYRO_ERR_UNSUPPORTED = 7  /* valid input that this build has no kernel for                      */
@@ -119,11 +117,12 @@ int pyro_source_terms_host(pyro_mech *mech, int64_t n, int64_t ld, const double 
 
 /* Facts about a packed mechanism, for reports: fills up to `cap` int64 values
  *   [0] n_species  [1] n_reactions  [2] reactions in the plain class  [3] in the extended class
- *   [4] table bytes  [5] 1 if tables live in __constant__ memory, 0 if in global memory
- *   [6] threads per block of the rates kernel  [7] dynamic shared memory per block (bytes)
- *   [8] resident blocks per SM (occupancy query)  [9] registers per thread of the rates kernel
- *   [10] local (spill) bytes per thread  [11] SM count of the device
- *   [12] grid points per thread of the rates kernel
+ *   [4] table bytes  [5] 1 if the rates kernel stages the tables in shared memory, 0 if it reads
+ *   them from global memory  [6] threads (= points) per block of the rates kernel
+ *   [7] dynamic shared memory per block (bytes)  [8] resident (persistent) blocks per SM
+ *   [9] registers per thread of the rates kernel  [10] local (spill) bytes per thread
+ *   [11] SM count of the device  [12] grid points per thread of the rates kernel (1)
+ *   [13] tensor-memory columns a block allocates
  * returns the number of values written (negative pyro_status on error). */
 int pyro_mech_info(const pyro_mech *mech, int64_t *out, int cap);
 

@@ -109,9 +109,9 @@ def make_desc(mech):
     return d, keep
 
 
-_INFO_KEYS = ("n_species", "n_reactions", "n_plain", "n_extended", "table_bytes", "tables_in_constant",
+_INFO_KEYS = ("n_species", "n_reactions", "n_plain", "n_extended", "table_bytes", "tables_in_shared",
               "block_threads", "smem_bytes", "blocks_per_sm", "registers", "local_bytes", "sm_count",
-              "points_per_thread")
+              "points_per_thread", "tmem_columns")
 
 
 def _ptr(t):
@@ -151,8 +151,8 @@ class Mechanism:
             pass
 
     def info(self):
-        out = (C.c_int64 * 13)()
-        n = self._lib.pyro_mech_info(self._h, out, 13)
+        out = (C.c_int64 * 14)()
+        n = self._lib.pyro_mech_info(self._h, out, 14)
         if n < 0:
             _check(-n)
         return dict(zip(_INFO_KEYS, [int(v) for v in out[:n]]))

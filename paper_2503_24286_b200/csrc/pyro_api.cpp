@@ -1,5 +1,5 @@
 // C-ABI layer of libpyro (include/pyro.h): handle management, argument checks, the
-// constant-bank residency protocol, launches, and the pipelined host-buffer entry point.
+// launch configuration, launches, and the pipelined host-buffer entry point.
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -47,18 +47,7 @@ struct DeviceGuard {
     }
 };
 
-// Who owns the __constant__ table bank of a device, and which streams may still be reading it.
-struct ConstBank {
-    std::mutex mu;
-    uint64_t resident = 0;   // id of the mechanism whose tables are in the bank (0 = none)
-    cudaStream_t upload_stream = nullptr;
-    cudaEvent_t upload_done = nullptr;
-    std::vector<std::pair<cudaStream_t, cudaEvent_t>> readers;
-};
-
 constexpr int kMaxDevices = 64;
-ConstBank g_bank[kMaxDevices];
-std::atomic<uint64_t> g_next_id{1};
 
 struct HostPipe {   // staging of pyro_source_terms_host
     static constexpr int kBuf = 3;
@@ -73,15 +62,15 @@ struct HostPipe {   // staging of pyro_source_terms_host
 }   // namespace
 
 struct pyro_mech {
-    uint64_t id = 0;
     int device = 0;
     pyro::PackedMech packed;
     unsigned char *d_blob = nullptr;
     pyro::EnergyRow *d_energy = nullptr;
-    bool in_const = false;
-    int block_threads = 32;
-    int points_per_thread = 1;
-    size_t smem_bytes = 0;
+    bool tab_smem = false;     // tables staged in shared memory (else read from global memory)
+    int block_threads = 32;    // = points per block
+    size_t smem_bytes = 0;     // dynamic shared memory: tables (if staged) + the A/B planes
+    uint32_t planes_off = 0;
+    uint32_t tmem_cols = 32;
     int blocks_per_sm = 0;
     int sm_count = 0;
     double newton_tol = 1e-6;
@@ -115,42 +104,11 @@ int check_fields(const pyro_mech *m, int64_t n, int64_t ld) {
 
 bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
 
-// Enqueue the rates kernel of `m` on `stream`, making its tables resident first.
+// Enqueue the rates kernel of `m` on `stream`: persistent blocks, blocks_per_sm per SM at most.
 int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t stream) {
-    if (!m->in_const) {
-        PYRO_CUDA(pyro::launch_rates(a, m->block_threads, m->points_per_thread, false, m->smem_bytes, stream));
-        return PYRO_OK;
-    }
-    ConstBank &bank = g_bank[m->device];
-    std::lock_guard<std::mutex> lock(bank.mu);
-    if (!bank.upload_done) PYRO_CUDA(cudaEventCreateWithFlags(&bank.upload_done, cudaEventDisableTiming));
-    if (bank.resident != m->id) {
-        // order the overwrite after every launch that may still read the old tables
-        for (auto &r : bank.readers)
-            if (r.first != stream) PYRO_CUDA(cudaStreamWaitEvent(stream, r.second, 0));
-        PYRO_CUDA(pyro::upload_const_table(m->d_blob, m->packed.lay.bytes, stream));
-        PYRO_CUDA(cudaEventRecord(bank.upload_done, stream));
-        bank.upload_stream = stream;
-        bank.resident = m->id;
-        for (auto &r : bank.readers) cudaEventDestroy(r.second);
-        bank.readers.clear();
-    } else if (stream != bank.upload_stream) {
-        PYRO_CUDA(cudaStreamWaitEvent(stream, bank.upload_done, 0));
-    }
-    PYRO_CUDA(pyro::launch_rates(a, m->block_threads, m->points_per_thread, true, m->smem_bytes, stream));
-    cudaEvent_t ev = nullptr;
-    for (auto &r : bank.readers)
-        if (r.first == stream) ev = r.second;
-    if (!ev) {
-        if (bank.readers.size() >= 64) {   // too many distinct streams: fall back to a device-wide fence
-            PYRO_CUDA(cudaDeviceSynchronize());
-            for (auto &r : bank.readers) cudaEventDestroy(r.second);
-            bank.readers.clear();
-        }
-        PYRO_CUDA(cudaEventCreateWithFlags(&ev, cudaEventDisableTiming));
-        bank.readers.emplace_back(stream, ev);
-    }
-    PYRO_CUDA(cudaEventRecord(ev, stream));
+    int64_t blocks = (int64_t)m->sm_count * m->blocks_per_sm;
+    if (blocks > a.n_tiles) blocks = a.n_tiles;
+    PYRO_CUDA(pyro::launch_rates(a, m->block_threads, (int)blocks, m->tab_smem, m->smem_bytes, stream));
     return PYRO_OK;
 }
 
@@ -159,16 +117,23 @@ pyro::RatesArgs rates_args(const pyro_mech *m, int64_t n, int64_t ld, const doub
     const pyro::TableLayout &l = m->packed.lay;
     pyro::RatesArgs a{};
     a.n = n; a.ld = ld; a.rho = rho; a.T = T; a.Y = Y; a.omega = omega;
+    a.n_tiles = (n + m->block_threads - 1) / m->block_threads;
     a.gtab = m->d_blob;
+    a.tab_bytes = l.bytes;
+    a.planes_off = m->planes_off;
+    a.tmem_cols = m->tmem_cols;
     a.off_spec = l.off_spec; a.off_rxn_p = l.off_rxn_p; a.off_rxn_x = l.off_rxn_x; a.off_fall = l.off_fall;
-    a.off_eff_delta = l.off_eff_delta; a.off_eff_species = l.off_eff_species;
-    a.n_species = l.n_species; a.n_p = l.n_p; a.n_x = l.n_x;
+    a.off_eff = l.off_eff;
+    a.n_species = l.n_species;
     for (int s = 0; s < 9; ++s) {
-        a.shape_quads[s] = l.shape_quads[s];
-        a.shape_pairs[s] = l.shape_pairs[s];
-        a.shape_singles[s] = l.shape_singles[s];
+        a.groups.shape_g8[s] = l.shape_g8[s];
+        a.groups.shape_g4[s] = l.shape_g4[s];
+        a.groups.shape_g2[s] = l.shape_g2[s];
     }
-    for (int k = 0; k < 4; ++k) a.ext_count[k] = l.ext_count[k];
+    for (int k = 0; k < 4; ++k) {
+        a.groups.ext_g4[k] = l.ext_g4[k];
+        a.groups.ext_g2[k] = l.ext_g2[k];
+    }
     return a;
 }
 
@@ -216,7 +181,6 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         return fail(PYRO_ERR_CUDA, "cudaSetDevice failed");
     }
     m->device = device;
-    m->id = g_next_id.fetch_add(1);
     const pyro::TableLayout &lay = m->packed.lay;
     auto bail = [&](cudaError_t e, const char *what) {
         cudaFree(m->d_blob);
@@ -232,50 +196,72 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if ((ce = cudaMemcpy(m->d_energy, m->packed.energy.data(), ebytes, cudaMemcpyHostToDevice)) != cudaSuccess)
         return bail(ce, "cudaMemcpy(energy table)");
 
-    m->in_const = lay.bytes <= (uint32_t)pyro::kConstBankBytes;
-    if (const char *env = std::getenv("PYRO_TABLES")) {
-        if (!std::strcmp(env, "global")) m->in_const = false;
-    }
     cudaDeviceProp prop;
     if ((ce = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) return bail(ce, "cudaGetDeviceProperties");
     m->sm_count = prop.multiProcessorCount;
-    // launch shape (threads per block, points per thread): with the three planes of n_species + 1
-    // doubles per point in shared memory, take the variant that keeps at least two warps per
-    // scheduler resident with the most points in flight; below that, the most warps.
-    int forced_bd = 0, forced_p = 0;
-    if (const char *env = std::getenv("PYRO_RATES_BLOCK")) forced_bd = std::atoi(env);
-    if (const char *env = std::getenv("PYRO_RATES_POINTS")) forced_p = std::atoi(env);
-    long best_score = -1;
-    for (int p = 1; p <= 2; ++p)
-        for (int bd = 32; bd <= 128; bd *= 2) {
-            if ((forced_bd && bd != forced_bd) || (forced_p && p != forced_p)) continue;
-            const size_t smem = (size_t)pyro::kPlanes * (lay.n_species + 1) * sizeof(double) * p * bd;
-            if (smem > (size_t)prop.sharedMemPerBlockOptin) continue;
-            const void *fn = pyro::rates_kernel_ptr(bd, p, m->in_const);
-            // the limit is a property of the function, shared by every mechanism: always raise it to the
-            // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
-            if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)prop.sharedMemPerBlockOptin)) != cudaSuccess)
-                return bail(ce, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
-            int nblk = 0;
-            if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, bd, smem)) != cudaSuccess)
-                return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
-            const long warps = (long)nblk * bd / 32, points = (long)nblk * bd * p;
-            const long score = (warps < 8 ? warps : 8) * 100000 + points;
-            if (nblk > 0 && score > best_score) {
-                best_score = score;
-                m->block_threads = bd;
-                m->points_per_thread = p;
-                m->smem_bytes = smem;
-                m->blocks_per_sm = nblk;
-            }
-        }
-    if (best_score < 0) {
+    // Launch shape.  A point needs two doubles per species row in shared memory (planes A, B) and
+    // two 32-bit tensor-memory columns per row (plane W); warps share the 128 tensor-memory lanes
+    // four at a time, so a block of w warps takes ceil(w/4) column groups of 2 rows columns out of
+    // 512.  Take the most threads (a multiple of 32, at most kRatesMaxThreads) that fit, with the
+    // tables staged in shared memory unless that costs more than 40 % of the points.
+    const size_t rows = (size_t)lay.n_species + 1;
+    size_t static_smem = 0;   // the kernels keep the tensor-memory base address in static shared memory
+    for (int v = 0; v < 2; ++v) {
+        cudaFuncAttributes fa{};
+        if ((ce = cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(v != 0))) != cudaSuccess)
+            return bail(ce, "cudaFuncGetAttributes");
+        if (fa.sharedSizeBytes > static_smem) static_smem = fa.sharedSizeBytes;
+    }
+    const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin - static_smem;
+    const size_t tab_room = ((size_t)lay.bytes + 15) & ~(size_t)15;
+    auto threads_for = [&](size_t table_bytes) {
+        if (smem_max < table_bytes + 16 * rows * 32) return 0;
+        size_t t = (smem_max - table_bytes) / (16 * rows);
+        t = (t / 32) * 32;
+        const size_t groups_max = 512 / (2 * rows);
+        if (t > 128 * groups_max) t = 128 * groups_max;
+        if (t > (size_t)pyro::kRatesMaxThreads) t = pyro::kRatesMaxThreads;
+        return (int)t;
+    };
+    int t_smem = threads_for(tab_room), t_glob = threads_for(0);
+    if (const char *env = std::getenv("PYRO_TABLES")) {
+        if (!std::strcmp(env, "global")) t_smem = 0;
+        if (!std::strcmp(env, "shared")) t_glob = 0;
+    }
+    m->tab_smem = t_smem > 0 && 10 * t_smem >= 6 * t_glob;
+    int threads = m->tab_smem ? t_smem : t_glob;
+    if (const char *env = std::getenv("PYRO_RATES_BLOCK")) {
+        const int forced = std::atoi(env);
+        if (forced >= 32 && forced % 32 == 0 && forced <= threads) threads = forced;
+    }
+    if (threads < 32) {
         cudaFree(m->d_blob);
         cudaFree(m->d_energy);
         delete m;
-        return fail(PYRO_ERR_TOO_LARGE, "species arrays do not fit the shared memory of one block");
+        return fail(PYRO_ERR_TOO_LARGE, "species arrays do not fit the on-chip memory of one block");
     }
+    m->block_threads = threads;
+    m->planes_off = m->tab_smem ? (uint32_t)tab_room : 0u;
+    m->smem_bytes = m->planes_off + 16 * rows * (size_t)threads;
+    const uint32_t cols_needed = (uint32_t)(((threads / 32 + 3) / 4) * 2 * rows);
+    m->tmem_cols = 32;
+    while (m->tmem_cols < cols_needed) m->tmem_cols *= 2;
+    const void *fn = pyro::rates_kernel_ptr(m->tab_smem);
+    // the limit is a property of the function, shared by every mechanism: always raise it to the
+    // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
+    if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
+        return bail(ce, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
+    int nblk = 0;
+    if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, threads, m->smem_bytes)) != cudaSuccess)
+        return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (nblk > (int)(512 / m->tmem_cols)) nblk = (int)(512 / m->tmem_cols);   // resident blocks share 512 columns
+    if (nblk < 1) {
+        cudaFree(m->d_blob);
+        cudaFree(m->d_energy);
+        delete m;
+        return fail(PYRO_ERR_TOO_LARGE, "the rates kernel does not fit one SM for this mechanism");
+    }
+    m->blocks_per_sm = nblk;
     *out = m;
     return PYRO_OK;
 }
@@ -407,12 +393,12 @@ int pyro_mech_info(const pyro_mech *m, int64_t *out, int cap) {
     if (!m || !out) return -fail(PYRO_ERR_NULL, "NULL argument");
     DeviceGuard guard(m->device);
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->block_threads, m->points_per_thread, m->in_const));
-    const int64_t v[13] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
-                           (int64_t)m->packed.lay.bytes, m->in_const ? 1 : 0, m->block_threads,
+    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem));
+    const int64_t v[14] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
+                           (int64_t)m->packed.lay.bytes, m->tab_smem ? 1 : 0, m->block_threads,
                            (int64_t)m->smem_bytes, m->blocks_per_sm, fa.numRegs, (int64_t)fa.localSizeBytes,
-                           m->sm_count, m->points_per_thread};
-    int cnt = cap < 13 ? cap : 13;
+                           m->sm_count, 1, (int64_t)m->tmem_cols};
+    int cnt = cap < 14 ? cap : 14;
     for (int i = 0; i < cnt; ++i) out[i] = v[i];
     return cnt;
 }

@@ -2,10 +2,17 @@
 //
 // Thread mapping: one thread per grid point, a warp reads 256
 // contiguous bytes of every species plane of the SoA fields.  Per-point arrays that are
-// indexed by a run-time species number (A_k = C_k E_k, B_k = 1/E_k, omega_k; pyro_tables.h)
-// live in shared memory as [k][plane][tid] columns (conflict-free: lane l touches its own banks);
-// mechanism tables are read at warp-uniform addresses from the __constant__ bank (or from
-// global memory when a mechanism does not fit the 64 KB bank).
+// indexed by a run-time species number live on chip (pyro_tables.h, pyro_point.cuh):
+//   A_k = C_k E_k and B_k = 1/E_k in shared memory as [k][plane][thread] columns (conflict-free:
+//   lane l touches its own banks), read-only while the reactions run;
+//   omega_k in TENSOR MEMORY: thread t of a warp owns lane 32 (warp % 4) + t, species k is the
+//   pair of 32-bit columns 2k, 2k+1 of that warp's column group.  The stoichiometric
+//   accumulation is tcgen05.ld / add / tcgen05.st on warp-uniform column addresses, which
+//   takes the read-modify-write traffic (8 of the 14 indexed accesses of a reaction) off the
+//   shared-memory pipe and doubles the points resident per SM.
+// The mechanism tables are staged once per block into shared memory and read with 128-bit
+// loads at warp-uniform addresses; blocks are persistent (one per SM for the 53-species
+// mechanism) and walk the tiles of points.
 #include <cuda_runtime.h>
 
 #include "pyro_kernels.h"
@@ -13,112 +20,132 @@
 
 namespace pyro {
 
-__constant__ __align__(16) unsigned char c_tab[kConstBankBytes];
+struct DevTab {
+    const unsigned char *base;   // shared-memory copy of the blob, or the global one
+    uint32_t off_spec, off_rxn_p, off_rxn_x, off_fall, off_eff;
 
-template <bool kConst> struct DevTab {
-    const unsigned char *base;   // global-memory copy of the blob (used when !kConst)
-    uint32_t off_spec, off_rxn_p, off_rxn_x, off_fall, off_eff_delta, off_eff_species;
-
-    __device__ __forceinline__ const unsigned char *at(uint32_t off) const {
-        if constexpr (kConst)
-            return c_tab + off;
-        else
-            return base + off;
-    }
-    __device__ __forceinline__ const SpecRow &spec(int k) const { return reinterpret_cast<const SpecRow *>(at(off_spec))[k]; }
-    __device__ __forceinline__ const RxnP &rxn_p(int j) const { return reinterpret_cast<const RxnP *>(at(off_rxn_p))[j]; }
-    __device__ __forceinline__ const RxnX &rxn_x(int j) const { return reinterpret_cast<const RxnX *>(at(off_rxn_x))[j]; }
-    __device__ __forceinline__ const RxnFall &rxn_fall(int j) const { return reinterpret_cast<const RxnFall *>(at(off_fall))[j]; }
-    __device__ __forceinline__ double eff_delta(int q) const { return reinterpret_cast<const double *>(at(off_eff_delta))[q]; }
-    __device__ __forceinline__ int eff_species(int q) const { return (int)reinterpret_cast<const uint32_t *>(at(off_eff_species))[q]; }
+    __device__ __forceinline__ const SpecRow &spec(int k) const { return reinterpret_cast<const SpecRow *>(base + off_spec)[k]; }
+    __device__ __forceinline__ const RxnP &rxn_p(int j) const { return reinterpret_cast<const RxnP *>(base + off_rxn_p)[j]; }
+    __device__ __forceinline__ const RxnX &rxn_x(int j) const { return reinterpret_cast<const RxnX *>(base + off_rxn_x)[j]; }
+    __device__ __forceinline__ const RxnFall &rxn_fall(int j) const { return reinterpret_cast<const RxnFall *>(base + off_fall)[j]; }
+    __device__ __forceinline__ const EffEntry &eff(int q) const { return reinterpret_cast<const EffEntry *>(base + off_eff)[q]; }
 };
 
-// Shared-memory planes of one thread: species k, plane Q of its P points is the P-vector at
-// base + (k kPlanes + Q) BD sizeof(Vec<P>), base = the thread's own column.  Explicit
-// ld/st.shared on 32-bit window addresses: a handle costs one integer multiply-add and the
-// planes are immediate offsets from it.  The accesses are volatile asm, so they keep their
-// program order (the omega read-modify-writes of consecutive groups may touch one address).
-template <int BD, int P> struct SmemPlanes {
-    static constexpr uint32_t kPlaneBytes = BD * 8 * P, kSpeciesBytes = kPlanes * kPlaneBytes;
-    uint32_t base;
+// On-chip planes of one thread.  Shared memory: species k of plane A is the double at
+// baseA + k stride (stride = 16 bytes x threads per block), plane B the one at baseB + k stride.
+// Tensor memory: species k is the column pair tw + 2k of the thread's lane.  All accesses are
+// volatile asm, so they keep their program order.
+struct DevMem {
+    struct WRaw {
+        uint32_t lo, hi;
+    };
+    uint32_t baseA, baseB, stride, tw;
 
-    __device__ __forceinline__ uint32_t at(uint32_t k) const { return base + k * kSpeciesBytes; }
-    template <int Q> __device__ __forceinline__ Vec<P> ld(uint32_t h) const {
-        Vec<P> v;
-        if constexpr (P == 1)
-            asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v.v[0]) : "r"(h), "n"(Q * kPlaneBytes));
-        else
-            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(v.v[0]), "=d"(v.v[1]) : "r"(h), "n"(Q * kPlaneBytes));
+    __device__ __forceinline__ uint32_t atA(uint32_t k) const { return baseA + k * stride; }
+    __device__ __forceinline__ uint32_t atB(uint32_t k) const { return baseB + k * stride; }
+    __device__ __forceinline__ uint32_t atW(uint32_t k) const { return tw + 2u * k; }
+    __device__ __forceinline__ double ldA(uint32_t h) const {
+        double v;
+        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(h));
         return v;
     }
-    template <int Q> __device__ __forceinline__ void st(uint32_t h, const Vec<P> &v) const {
-        if constexpr (P == 1)
-            asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(h), "n"(Q * kPlaneBytes), "d"(v.v[0]));
-        else
-            asm volatile("st.shared.v2.f64 [%0+%1], {%2, %3};" ::"r"(h), "n"(Q * kPlaneBytes), "d"(v.v[0]), "d"(v.v[1]));
+    __device__ __forceinline__ double ldB(uint32_t h) const { return ldA(h); }
+    __device__ __forceinline__ void stA(uint32_t h, double v) const { asm volatile("st.shared.f64 [%0], %1;" ::"r"(h), "d"(v)); }
+    __device__ __forceinline__ void stB(uint32_t h, double v) const { stA(h, v); }
+    __device__ __forceinline__ WRaw ldW(uint32_t h) const {
+        WRaw r;
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r.lo), "=r"(r.hi) : "r"(h));
+        return r;
     }
+    __device__ __forceinline__ void stW(uint32_t h, double v) const {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(h), "r"(__double2loint(v)), "r"(__double2hiint(v)));
+    }
+    // the loaded registers are defined only after the wait: tie them to it
+    template <int N> __device__ __forceinline__ void fence_ldW(WRaw (&r)[N]) const {
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int i = 0; i < N; ++i) asm volatile("" : "+r"(r[i].lo), "+r"(r[i].hi));
+    }
+    __device__ __forceinline__ void fence_stW() const { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+    __device__ __forceinline__ double value(const WRaw &r) const { return __hiloint2double((int)r.hi, (int)r.lo); }
 };
 
 // ---------------------------------------------------------------------------------------
 // omega[k][p] from rho[p], T[p], Y[k][p]   (rows a1-a3, a5-a9)
-// Thread t of a block owns the P adjacent points P t .. P t + P - 1 of the block's tile, so a
-// warp reads 256 P contiguous bytes of every species plane (128-bit loads for P = 2 when the
-// planes are 16-byte aligned) and every shared-memory access is conflict-free.  Tail threads
-// recompute the last point and store nothing: control flow stays warp-uniform throughout.
+// Thread t of a block owns point t of the block's current tile.  Tail threads recompute the
+// last point and store nothing: control flow stays warp-uniform throughout (the tensor-memory
+// instructions are warp-collective).
 // ---------------------------------------------------------------------------------------
-template <int BD, int P, bool kConst>
-__global__ void __launch_bounds__(BD) rates_kernel(const RatesArgs a) {
-    static_assert(P == 1 || P == 2, "one or two points per thread");
+template <bool kTabSmem>
+__global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int tid = threadIdx.x;
-    const int64_t p0 = ((int64_t)blockIdx.x * BD + tid) * P;
+    __shared__ uint32_t s_tmem_base;
+    const int tid = threadIdx.x, warp = tid >> 5, nthreads = blockDim.x;
     const int ns = a.n_species;
-    const SmemPlanes<BD, P> mem{(uint32_t)__cvta_generic_to_shared(smem_raw) + (uint32_t)tid * (8 * P)};
-    DevTab<kConst> tab{a.gtab, a.off_spec, a.off_rxn_p, a.off_rxn_x, a.off_fall, a.off_eff_delta, a.off_eff_species};
 
-    const bool full = p0 + P <= a.n;   // the last thread of a ragged tile owns fewer points
-    const bool vec = P > 1 && full && (a.ld % P == 0) && ((reinterpret_cast<uintptr_t>(a.Y) % (8 * P)) == 0) &&
-                     ((reinterpret_cast<uintptr_t>(a.omega) % (8 * P)) == 0);
-    int64_t pi[P];
-#pragma unroll
-    for (int i = 0; i < P; ++i) pi[i] = (p0 + i < a.n) ? p0 + i : a.n - 1;
-    double rho[P], T[P], ctot[P];
-#pragma unroll
-    for (int i = 0; i < P; ++i) {
-        rho[i] = a.rho[pi[i]];
-        T[i] = a.T[pi[i]];
-        ctot[i] = 0.0;
+    if (kTabSmem) {
+        const uint4 *src = reinterpret_cast<const uint4 *>(a.gtab);
+        uint4 *dst = reinterpret_cast<uint4 *>(smem_raw);
+        for (uint32_t i = tid; i < a.tab_bytes / 16u; i += nthreads) dst[i] = src[i];
     }
-    const PointT<P> pt = make_point<P>(T);
-    if (vec) {
-        const Vec<P> *Yv = reinterpret_cast<const Vec<P> *>(a.Y + p0);
-        const int64_t ldv = a.ld / P;
-        fill_planes<P>(tab, ns, pt, rho, ctot, mem, [&](int k, double(&y)[P]) {
-            const Vec<P> v = Yv[(int64_t)k * ldv];
-#pragma unroll
-            for (int i = 0; i < P; ++i) y[i] = v.v[i];
-        });
-    } else {
-        fill_planes<P>(tab, ns, pt, rho, ctot, mem, [&](int k, double(&y)[P]) {
-#pragma unroll
-            for (int i = 0; i < P; ++i) y[i] = a.Y[(int64_t)k * a.ld + pi[i]];
-        });
+    if (warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(
+                         (uint32_t)__cvta_generic_to_shared(&s_tmem_base)),
+                     "r"(a.tmem_cols));
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
     }
-    accumulate_reactions<P>(tab, a.shape_quads, a.shape_pairs, a.shape_singles, a.ext_count, pt, ctot, mem);
-    if (vec) {
-        Vec<P> *Wv = reinterpret_cast<Vec<P> *>(a.omega + p0);
-        const int64_t ldv = a.ld / P;
-#pragma unroll 4
-        for (int k = 0; k < ns; ++k) Wv[(int64_t)k * ldv] = mem.template ld<kW>(mem.at((uint32_t)k));
-    } else {
-#pragma unroll 2
-        for (int k = 0; k < ns; ++k) {
-            const Vec<P> w = mem.template ld<kW>(mem.at((uint32_t)k));
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;");
+    const uint32_t tmem_base = s_tmem_base;
+
+    DevTab tab{kTabSmem ? smem_raw : a.gtab, a.off_spec, a.off_rxn_p, a.off_rxn_x, a.off_fall, a.off_eff};
+    const uint32_t planes = (uint32_t)__cvta_generic_to_shared(smem_raw) + a.planes_off;
+    const uint32_t rows = (uint32_t)ns + 1u;
+    DevMem mem;
+    mem.stride = 16u * (uint32_t)nthreads;
+    mem.baseA = planes + 8u * (uint32_t)tid;
+    mem.baseB = mem.baseA + 8u * (uint32_t)nthreads;
+    mem.tw = tmem_base + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * 2u * rows;
+
+    for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
+        const int64_t p = tile * nthreads + tid;
+        const int64_t pc = p < a.n ? p : a.n - 1;
+        const double rho = a.rho[pc];
+        const PointT pt = make_point(a.T[pc]);
+        const double *Yp = a.Y + pc;
+        const double ctot = fill_planes(tab, ns, pt, rho, mem, [&](int k) { return __ldg(Yp + (int64_t)k * a.ld); });
+        {   // bring the next tile's mass fractions into L2 while the reactions run
+            const int64_t pn = p + (int64_t)gridDim.x * nthreads;
+            if (pn < a.n && (tid & 15) == 0)
+                for (int k = 0; k < ns; ++k) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)k * a.ld + pn));
+        }
+        accumulate_reactions(tab, a.groups, pt, ctot, mem);
+        double *Wp = a.omega + p;
+        int k = 0;
+#pragma unroll 1
+        for (; k + 4 <= ns; k += 4) {
+            DevMem::WRaw r[4];
 #pragma unroll
-            for (int i = 0; i < P; ++i)
-                if (p0 + i < a.n) a.omega[(int64_t)k * a.ld + p0 + i] = w.v[i];
+            for (int i = 0; i < 4; ++i) r[i] = mem.ldW(mem.atW((uint32_t)(k + i)));
+            mem.fence_ldW<4>(r);
+            if (p < a.n) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) Wp[(int64_t)(k + i) * a.ld] = mem.value(r[i]);
+            }
+        }
+#pragma unroll 1
+        for (; k < ns; ++k) {
+            DevMem::WRaw r[1];
+            r[0] = mem.ldW(mem.atW((uint32_t)k));
+            mem.fence_ldW<1>(r);
+            if (p < a.n) Wp[(int64_t)k * a.ld] = mem.value(r[0]);
         }
     }
+    asm volatile("tcgen05.fence::before_thread_sync;");
+    __syncthreads();
+    if (warp == 0)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(a.tmem_cols));
 }
 
 // ---------------------------------------------------------------------------------------
@@ -200,43 +227,16 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double *out, int iters,
 // ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
-template <int BD, int P> static const void *rates_fn(bool in_const) {
-    return in_const ? (const void *)rates_kernel<BD, P, true> : (const void *)rates_kernel<BD, P, false>;
+const void *rates_kernel_ptr(bool tables_in_shared) {
+    return tables_in_shared ? (const void *)rates_kernel<true> : (const void *)rates_kernel<false>;
 }
 
-const void *rates_kernel_ptr(int bd, int points_per_thread, bool in_const) {
-    if (points_per_thread == 1) {
-        switch (bd) {
-            case 32: return rates_fn<32, 1>(in_const);
-            case 64: return rates_fn<64, 1>(in_const);
-            case 128: return rates_fn<128, 1>(in_const);
-            default: return nullptr;
-        }
-    }
-    if (points_per_thread == 2) {
-        switch (bd) {
-            case 32: return rates_fn<32, 2>(in_const);
-            case 64: return rates_fn<64, 2>(in_const);
-            case 128: return rates_fn<128, 2>(in_const);
-            default: return nullptr;
-        }
-    }
-    return nullptr;
-}
-
-cudaError_t upload_const_table(const void *src_device, size_t bytes, cudaStream_t stream) {
-    return cudaMemcpyToSymbolAsync(c_tab, src_device, bytes, 0, cudaMemcpyDeviceToDevice, stream);
-}
-
-cudaError_t launch_rates(const RatesArgs &a, int bd, int points_per_thread, bool in_const, size_t smem_bytes,
+cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, size_t smem_bytes,
                          cudaStream_t stream) {
-    const void *fn = rates_kernel_ptr(bd, points_per_thread, in_const);
-    if (!fn) return cudaErrorInvalidValue;
-    const int64_t per_block = (int64_t)bd * points_per_thread;
-    const int64_t blocks = (a.n + per_block - 1) / per_block;
+    const void *fn = rates_kernel_ptr(tables_in_shared);
     RatesArgs copy = a;
     void *params[] = {&copy};
-    return cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)bd), params, smem_bytes, stream);
+    return cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)threads), params, smem_bytes, stream);
 }
 
 constexpr int kTempBD = 128, kTempPPT = 4;

@@ -9,14 +9,19 @@
 
 namespace pyro {
 
+constexpr int kRatesMaxThreads = 256;   // threads (= points) per block of the rates kernel, a multiple of 32
+
 struct RatesArgs {
-    int64_t n, ld;
+    int64_t n, ld, n_tiles;      // n_tiles = ceil(n / threads per block)
     const double *rho, *T, *Y;
     double *omega;
     const unsigned char *gtab;   // device copy of the table blob in global memory
-    uint32_t off_spec, off_rxn_p, off_rxn_x, off_fall, off_eff_delta, off_eff_species;
-    int32_t n_species, n_p, n_x;
-    int32_t shape_quads[9], shape_pairs[9], shape_singles[9], ext_count[4];
+    uint32_t tab_bytes;          // blob size (a multiple of 16)
+    uint32_t planes_off;         // byte offset of the A/B planes in dynamic shared memory
+    uint32_t tmem_cols;          // tensor-memory columns the block allocates (a power of two >= 32)
+    uint32_t off_spec, off_rxn_p, off_rxn_x, off_fall, off_eff;
+    int32_t n_species;
+    GroupCounts groups;
 };
 
 struct TempArgs {
@@ -29,12 +34,10 @@ struct TempArgs {
     double t_mid, tol;
 };
 
-// variants: block_threads in {32, 64, 128}, points_per_thread in {1, 2}
-const void *rates_kernel_ptr(int block_threads, int points_per_thread, bool tables_in_constant);
+const void *rates_kernel_ptr(bool tables_in_shared);
 const void *temperature_kernel_ptr();
-cudaError_t upload_const_table(const void *src_device, size_t bytes, cudaStream_t stream);
-cudaError_t launch_rates(const RatesArgs &a, int block_threads, int points_per_thread, bool tables_in_constant,
-                         size_t smem_bytes, cudaStream_t stream);
+cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, size_t smem_bytes,
+                         cudaStream_t stream);
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream);
 cudaError_t launch_dfma_probe(double *out, int iters, int blocks, cudaStream_t stream);
 

@@ -162,11 +162,10 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         std::vector<RxnP> recP;
         std::vector<RxnX> recX;
         std::vector<RxnFall> recFall;
-        std::vector<double> eff_delta;
-        std::vector<uint32_t> eff_species;
+        std::vector<std::vector<EffEntry>> effX;   // listed efficiencies of each extended record
         out.order.clear();
         std::vector<int> orderX, orderP, shapeP;
-        std::vector<std::vector<int>> speciesP;
+        std::vector<std::vector<int>> speciesP, speciesX;
         bool needs_ctot = false;
         for (int j = 0; j < nr; ++j) {
             uint32_t slot[6];
@@ -210,26 +209,25 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
             std::memset(&x, 0, sizeof x);
             for (int m = 0; m < 3; ++m) x.f[m] = f[m];
             for (int m = 0; m < 6; ++m) x.slot[m] = slot[m];
-            x.rev = reversible ? 1.0 : 0.0;
+            x.rev = reversible ? 1.0f : 0.0f;
             x.type = (uint32_t)type;
             for (int s = 0; s < 6; ++s) x.sc_species[s] = (uint32_t)ns;
             int nsc = 0;
+            std::vector<int> scs;
             for (auto &kv : net)
                 if (kv.second != 0) {
                     x.sc_species[nsc] = (uint32_t)kv.first;
-                    x.sc_nu[nsc] = (double)kv.second;
+                    x.sc_nu[nsc] = (float)kv.second;
+                    scs.push_back(kv.first);
                     ++nsc;
                 }
             x.eff_default = 1.0;
+            std::vector<EffEntry> effs;
             if (type != PYRO_ELEMENTARY) {
                 needs_ctot = true;
                 x.eff_default = d->eff_default[j];
-                x.eff_begin = (uint32_t)eff_delta.size();
-                x.eff_count = (uint32_t)(d->eff_ptr[j + 1] - d->eff_ptr[j]);
-                for (int q = d->eff_ptr[j]; q < d->eff_ptr[j + 1]; ++q) {
-                    eff_delta.push_back(d->eff_value[q] - d->eff_default[j]);
-                    eff_species.push_back((uint32_t)d->eff_species[q]);
-                }
+                for (int q = d->eff_ptr[j]; q < d->eff_ptr[j + 1]; ++q)
+                    effs.push_back(EffEntry{d->eff_value[q] - d->eff_default[j], (uint32_t)d->eff_species[q], 0u});
             }
             if (type >= PYRO_FALLOFF_LINDEMANN) {
                 RxnFall fl;
@@ -250,80 +248,136 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
             }
             recX.push_back(x);
             orderX.push_back(j);
+            effX.push_back(effs);
+            speciesX.push_back(scs);
         }
-        // plain class: by shape; within a shape greedy grouping of mutually species-disjoint
-        // reactions (fours, then couples, then the rest), so that the kernel can run a group in
-        // lockstep with all its shared-memory read-modify-writes independent
-        std::vector<RxnP> sortedP;
-        int shape_quads[9] = {0}, shape_pairs[9] = {0}, shape_singles[9] = {0};
-        auto disjoint = [&](int a, int b) {
-            for (int x : speciesP[a])
-                for (int y : speciesP[b])
-                    if (x == y) return false;
-            return true;
-        };
-        for (int shape = 0; shape < 9; ++shape) {
+        // Lockstep groups.  The kernels run the reactions of a group side by side (their
+        // exponentials interleaved, their omega read-modify-writes batched), which needs the
+        // scatter lists of a group to be mutually disjoint.  Greedy: every reaction joins the first
+        // open group it is disjoint from; a full group (eight) is closed.  What is left open is cut
+        // into fours and couples; reactions left alone are re-coupled where possible and otherwise
+        // coupled with a null record (index -1).
+        auto make_groups = [&](const std::vector<int> &members, const std::vector<std::vector<int>> &species,
+                               int largest, std::vector<int> &g8, std::vector<int> &g4, std::vector<int> &g2) {
+            auto disjoint = [&](int a, int b) {
+                for (int x : species[a])
+                    for (int y : species[b])
+                        if (x == y) return false;
+                return true;
+            };
             std::vector<std::vector<int>> open;
-            std::vector<int> fours, twos, ones;
-            for (size_t i = 0; i < recP.size(); ++i) {
-                if (shapeP[i] != shape) continue;
+            for (int i : members) {
                 int home = -1;
                 for (size_t g = 0; g < open.size() && home < 0; ++g) {
                     bool ok = true;
-                    for (int member : open[g]) ok = ok && disjoint(member, (int)i);
+                    for (int member : open[g]) ok = ok && disjoint(member, i);
                     if (ok) home = (int)g;
                 }
                 if (home < 0) {
-                    open.push_back({(int)i});
+                    open.push_back({i});
                     continue;
                 }
-                open[home].push_back((int)i);
-                if (open[home].size() == 4) {
-                    fours.insert(fours.end(), open[home].begin(), open[home].end());
+                open[home].push_back(i);
+                if ((int)open[home].size() == largest) {
+                    std::vector<int> &dst = largest == 8 ? g8 : g4;
+                    dst.insert(dst.end(), open[home].begin(), open[home].end());
                     open.erase(open.begin() + home);
                 }
             }
+            std::vector<int> ones;
             for (auto &g : open) {
                 size_t at = 0;
-                if (g.size() >= 2) {
-                    twos.push_back(g[0]);
-                    twos.push_back(g[1]);
-                    at = 2;
+                if (g.size() - at >= 4) {
+                    g4.insert(g4.end(), g.begin() + at, g.begin() + at + 4);
+                    at += 4;
+                }
+                while (g.size() - at >= 2) {
+                    g2.push_back(g[at]);
+                    g2.push_back(g[at + 1]);
+                    at += 2;
                 }
                 for (; at < g.size(); ++at) ones.push_back(g[at]);
             }
-            // leftover singles of different groups may still pair up
             std::vector<int> rest;
             for (int i : ones) {
                 int partner = -1;
                 for (size_t o = 0; o < rest.size() && partner < 0; ++o)
                     if (disjoint(rest[o], i)) partner = (int)o;
                 if (partner >= 0) {
-                    twos.push_back(rest[partner]);
-                    twos.push_back(i);
+                    g2.push_back(rest[partner]);
+                    g2.push_back(i);
                     rest.erase(rest.begin() + partner);
                 } else {
                     rest.push_back(i);
                 }
             }
-            shape_quads[shape] = (int)fours.size();
-            shape_pairs[shape] = (int)twos.size();
-            shape_singles[shape] = (int)rest.size();
-            for (int i : fours) { sortedP.push_back(recP[i]); out.order.push_back(orderP[i]); }
-            for (int i : twos) { sortedP.push_back(recP[i]); out.order.push_back(orderP[i]); }
-            for (int i : rest) { sortedP.push_back(recP[i]); out.order.push_back(orderP[i]); }
+            for (int i : rest) {
+                g2.push_back(i);
+                g2.push_back(-1);
+            }
+        };
+        // plain class: by shape
+        RxnP nullP;
+        std::memset(&nullP, 0, sizeof nullP);
+        for (int m = 0; m < 6; ++m) nullP.slot[m] = (uint32_t)ns;
+        std::vector<RxnP> sortedP;
+        int shape_g8[9] = {0}, shape_g4[9] = {0}, shape_g2[9] = {0};
+        for (int shape = 0; shape < 9; ++shape) {
+            std::vector<int> members, g8, g4, g2;
+            for (size_t i = 0; i < recP.size(); ++i)
+                if (shapeP[i] == shape) members.push_back((int)i);
+            make_groups(members, speciesP, 4, g8, g4, g2);   // (groups of eight: kept in the format, not formed yet)
+            shape_g8[shape] = (int)g8.size();
+            shape_g4[shape] = (int)g4.size();
+            shape_g2[shape] = (int)g2.size();
+            for (const std::vector<int> *g : {&g8, &g4, &g2})
+                for (int i : *g) {
+                    sortedP.push_back(i < 0 ? nullP : recP[i]);
+                    out.order.push_back(i < 0 ? -1 : orderP[i]);
+                }
         }
         recP.swap(sortedP);
-        // extended class: by kind
+        // extended class: by kind; the efficiency lists of a group are padded to one length
+        RxnX nullX;
+        std::memset(&nullX, 0, sizeof nullX);
+        for (int m = 0; m < 6; ++m) nullX.slot[m] = nullX.sc_species[m] = (uint32_t)ns;
+        nullX.rev = 1.0f;
+        nullX.eff_default = 1.0;
         std::vector<RxnX> sortedX;
-        int ext_count[4] = {0, 0, 0, 0};
-        for (int kind = 0; kind < 4; ++kind)
+        std::vector<EffEntry> effs;
+        int ext_g4[4] = {0, 0, 0, 0}, ext_g2[4] = {0, 0, 0, 0};
+        for (int kind = 0; kind < 4; ++kind) {
+            std::vector<int> members, g8, g4, g2;
             for (size_t i = 0; i < recX.size(); ++i)
-                if ((int)recX[i].type == kind) {
-                    sortedX.push_back(recX[i]);
-                    out.order.push_back(orderX[i]);
-                    ext_count[kind]++;
+                if ((int)recX[i].type == kind) members.push_back((int)i);
+            make_groups(members, speciesX, 4, g8, g4, g2);
+            ext_g4[kind] = (int)g4.size();
+            ext_g2[kind] = (int)g2.size();
+            auto emit = [&](const std::vector<int> &g, size_t width) {
+                for (size_t at = 0; at < g.size(); at += width) {
+                    size_t longest = 0;
+                    for (size_t m = 0; m < width; ++m)
+                        if (g[at + m] >= 0) longest = std::max(longest, effX[g[at + m]].size());
+                    for (size_t m = 0; m < width; ++m) {
+                        const int i = g[at + m];
+                        RxnX x = i < 0 ? nullX : recX[i];
+                        if (i < 0) {   // a null record next to a falloff reaction reads that reaction's falloff row
+                            x.type = (uint32_t)kind;
+                            for (size_t m2 = 0; m2 < width; ++m2)
+                                if (g[at + m2] >= 0) x.fall_index = recX[g[at + m2]].fall_index;
+                        }
+                        x.eff_begin = (uint32_t)effs.size();
+                        x.eff_count = (uint32_t)longest;
+                        if (i >= 0) effs.insert(effs.end(), effX[i].begin(), effX[i].end());
+                        while (effs.size() < x.eff_begin + longest) effs.push_back(EffEntry{0.0, (uint32_t)ns, 0u});
+                        sortedX.push_back(x);
+                        out.order.push_back(i < 0 ? -1 : orderX[i]);
+                    }
                 }
+            };
+            emit(g4, 4);
+            emit(g2, 2);
+        }
         recX.swap(sortedX);
 
         // ---- species rows
@@ -331,6 +385,8 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         for (int k = 0; k < ns; ++k) {
             spec[k].inv_w = (double)(1.0L / (long double)d->mol_weight[k]);
             spec[k].t_mid = d->t_mid[k];
+            std::memset(spec[k].lo, 0, sizeof spec[k].lo);
+            std::memset(spec[k].hi, 0, sizeof spec[k].hi);
             species_row(d->nasa_lo + 7 * k, spec[k].lo);
             species_row(d->nasa_hi + 7 * k, spec[k].hi);
         }
@@ -341,17 +397,20 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         lay.n_species = ns;
         lay.n_p = (int)recP.size();
         lay.n_x = (int)recX.size();
-        lay.n_eff = (int)eff_delta.size();
+        lay.n_eff = (int)effs.size();
         lay.n_fall = (int)recFall.size();
         lay.needs_ctot = needs_ctot ? 1 : 0;
         lay.single_t_mid = single_tmid ? 1 : 0;
         lay.t_mid = d->t_mid[0];
         for (int s = 0; s < 9; ++s) {
-            lay.shape_quads[s] = shape_quads[s];
-            lay.shape_pairs[s] = shape_pairs[s];
-            lay.shape_singles[s] = shape_singles[s];
+            lay.shape_g8[s] = shape_g8[s];
+            lay.shape_g4[s] = shape_g4[s];
+            lay.shape_g2[s] = shape_g2[s];
         }
-        for (int k = 0; k < 4; ++k) lay.ext_count[k] = ext_count[k];
+        for (int k = 0; k < 4; ++k) {
+            lay.ext_g4[k] = ext_g4[k];
+            lay.ext_g2[k] = ext_g2[k];
+        }
         uint32_t off = 0;
         lay.off_spec = off;
         off = align16(off + (uint32_t)(spec.size() * sizeof(SpecRow)));
@@ -361,18 +420,15 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         off = align16(off + (uint32_t)(recX.size() * sizeof(RxnX)));
         lay.off_fall = off;
         off = align16(off + (uint32_t)(recFall.size() * sizeof(RxnFall)));
-        lay.off_eff_delta = off;
-        off = align16(off + (uint32_t)(eff_delta.size() * sizeof(double)));
-        lay.off_eff_species = off;
-        off = align16(off + (uint32_t)(eff_species.size() * sizeof(uint32_t)));
+        lay.off_eff = off;
+        off = align16(off + (uint32_t)(effs.size() * sizeof(EffEntry)));
         lay.bytes = off;
         out.blob.assign(off, 0);
         put(out.blob, lay.off_spec, spec.data(), spec.size());
         put(out.blob, lay.off_rxn_p, recP.data(), recP.size());
         put(out.blob, lay.off_rxn_x, recX.data(), recX.size());
         put(out.blob, lay.off_fall, recFall.data(), recFall.size());
-        put(out.blob, lay.off_eff_delta, eff_delta.data(), eff_delta.size());
-        put(out.blob, lay.off_eff_species, eff_species.data(), eff_species.size());
+        put(out.blob, lay.off_eff, effs.data(), effs.size());
 
         // ---- energy table of the temperature solve
         out.energy.assign(ns, EnergyRow{});

@@ -8,16 +8,16 @@
 
 namespace pyro {
 
-// Limits of the on-chip staging: three FP64 planes of n_species + 1 per point in shared memory,
-// 32 points per block at least, 227 KB per block at most.
-constexpr int kMaxSpecies = 300;
+// Limits of the on-chip staging: two FP64 planes of n_species + 1 values per point in shared
+// memory and one in tensor memory (512 32-bit columns per thread at most).
+constexpr int kMaxSpecies = 255;
 constexpr int kMaxReactions = 1 << 20;
 
 struct PackedMech {
     TableLayout lay;
     std::vector<unsigned char> blob;   // rates tables, laid out by `lay`
     std::vector<EnergyRow> energy;     // temperature-solve table [n_species]
-    std::vector<int> order;            // packed position -> reaction index of the description
+    std::vector<int> order;            // packed record -> reaction index of the description (-1: null record)
     int n_species = 0, n_reactions = 0;
 };
 

@@ -1,13 +1,16 @@
-// Per-point arithmetic of the hot path, shared by every kernel variant.
+// Per-point arithmetic of the hot path, shared by the kernels and the host test build.
 //
-// One thread owns P grid points.  Per-point arrays indexed by a run-time species number live
-// on chip as three planes per species, each a column of P-vectors:
-//     plane kA  A_k = C_k E_k      plane kB  B_k = 1/E_k      plane kW  omega_k
+// One thread owns one grid point.  Per-point arrays indexed by a run-time species number live
+// on chip as three planes per species:
+//     plane A  A_k = C_k E_k      plane B  B_k = 1/E_k      plane W  omega_k
 // with E_k = exp(g_k/RT) RT/p0 (pyro_tables.h).  The functions below reach them through a
-// `Mem` accessor (shared memory in the kernels, a plain array in the host build):
-//     h = mem.at(k)                  handle of species k for this thread
-//     mem.template ld<Q>(h)          the thread's P-vector of plane Q
-//     mem.template st<Q>(h, v)
+// `Mem` accessor (A and B in shared memory and W in tensor memory in the kernels, plain arrays
+// in the host build):
+//     h = mem.atA(k), mem.atB(k), mem.atW(k)     handle of species k for this thread
+//     mem.ldA(h), mem.ldB(h), mem.stA(h, v), mem.stB(h, v)
+//     r = mem.ldW(h)            raw omega value; becomes readable by mem.value(r) only after
+//     mem.fence_ldW(raws)       (tensor-memory loads are asynchronous)
+//     mem.stW(h, v); mem.fence_stW() before a later ldW may see the stored value
 #pragma once
 #include "../../include/pyro.h"
 #include "pyro_math.cuh"
@@ -16,25 +19,17 @@
 namespace pyro {
 
 constexpr double kLog10of2 = 0.30102999566398119521;   // log10(2)
-enum { kA = 0, kB = 1, kW = 2 };
 
-template <int P> struct alignas(8 * P) Vec {
-    double v[P];
+// Per-thread temperature features of its point.
+struct PointT {
+    double T, invT, L2T;
 };
 
-// Per-thread temperature features of its P points.
-template <int P> struct PointT {
-    double T[P], invT[P], L2T[P];
-};
-
-template <int P> PYRO_HD PointT<P> make_point(const double (&T)[P]) {
-    PointT<P> pt;
-#pragma unroll
-    for (int i = 0; i < P; ++i) {
-        pt.T[i] = T[i];
-        pt.invT[i] = 1.0 / T[i];
-        pt.L2T[i] = log2(T[i]);
-    }
+PYRO_HD PointT make_point(double T) {
+    PointT pt;
+    pt.T = T;
+    pt.invT = 1.0 / T;
+    pt.L2T = log2(T);
     return pt;
 }
 
@@ -44,7 +39,7 @@ PYRO_HD double arrhenius_log2(double c0, double c1, double c2, double L2T, doubl
 }
 
 // log2 E_k = c0 + c1 log2T + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4     (A.11)-(A.13) folded
-PYRO_HD double species_log2E(const double (&c)[7], double T, double L2T, double invT) {
+PYRO_HD double species_log2E(const double *c, double T, double L2T, double invT) {
     double h = fma(c[6], T, c[5]);
     h = fma(h, T, c[4]);
     h = fma(h, T, c[3]);
@@ -53,28 +48,28 @@ PYRO_HD double species_log2E(const double (&c)[7], double T, double L2T, double 
     return fma(c[2], invT, y);
 }
 
-// Rows a2, a3 of SURVEY.md 8(a) for one species: C_k = rho Y_k / W_k (A.8) PAPER.md:921,
-// the NASA range chosen per point (T < T_mid,k: low; G10), E_k and 1/E_k by one paired
-// exponential.  Returns A_k = C_k E_k, B_k = 1/E_k and adds C_k to ctot.
-template <int P>
-PYRO_HD void species_planes(const SpecRow &row, const PointT<P> &pt, const double (&rho)[P], const double (&Y)[P],
-                            double (&ctot)[P], Vec<P> &A, Vec<P> &B) {
-    double y[P], e[P], b[P];
+// Rows a2, a3 of SURVEY.md 8(a) for NK species in lockstep: C_k = rho Y_k / W_k (A.8)
+// PAPER.md:921, the NASA range chosen per point (T < T_mid,k: low; G10) by fetching only that
+// coefficient set, E_k and 1/E_k by one paired exponential.  Writes A_k = C_k E_k, B_k = 1/E_k,
+// omega_k = 0 and adds C_k to ctot.
+template <int NK, class Tab, class Mem>
+PYRO_HD void species_planes(const Tab &tab, int k0, const PointT &pt, double rho, const double (&Y)[NK], double &ctot,
+                            const Mem &mem) {
+    double y[NK], e[NK], b[NK], C[NK];
 #pragma unroll
-    for (int i = 0; i < P; ++i) {
-        const bool low = pt.T[i] < row.t_mid;
-        double c[7];
-#pragma unroll
-        for (int m = 0; m < 7; ++m) c[m] = low ? row.lo[m] : row.hi[m];
-        y[i] = species_log2E(c, pt.T[i], pt.L2T[i], pt.invT[i]);
+    for (int i = 0; i < NK; ++i) {
+        const SpecRow &row = tab.spec(k0 + i);
+        const double *c = pt.T < row.t_mid ? row.lo : row.hi;
+        y[i] = species_log2E(c, pt.T, pt.L2T, pt.invT);
+        C[i] = rho * Y[i] * row.inv_w;
     }
-    exp2_pair_n<P>(y, e, b);
+    exp2_pair_n<NK>(y, e, b);
 #pragma unroll
-    for (int i = 0; i < P; ++i) {
-        const double C = rho[i] * Y[i] * row.inv_w;
-        ctot[i] += C;
-        A.v[i] = C * e[i];
-        B.v[i] = b[i];
+    for (int i = 0; i < NK; ++i) {
+        ctot += C[i];
+        mem.stA(mem.atA((uint32_t)(k0 + i)), C[i] * e[i]);
+        mem.stB(mem.atB((uint32_t)(k0 + i)), b[i]);
+        mem.stW(mem.atW((uint32_t)(k0 + i)), 0.0);
     }
 }
 
@@ -88,252 +83,269 @@ template <int N> PYRO_HD void load_slots(const uint32_t (&src)[6], uint32_t (&ds
     }
 }
 
-template <int P> PYRO_HD Vec<P> splat(double x) {
-    Vec<P> v;
-#pragma unroll
-    for (int i = 0; i < P; ++i) v.v[i] = x;
-    return v;
-}
-
 // Plain-class reactions of one shape (NR reactant molecules, NP product molecules), NB in
-// lockstep (the packer stores groups of NB mutually species-disjoint reactions):
+// lockstep (the packer stores groups of mutually species-disjoint reactions):
 //   R = k_f prod_reac B_k [prod_reac A_k - prod_prod A_k]    (A.7), (A.10) as in pyro_tables.h
 //   omega -= R on reactants, += R on products                (A.5)
-// Branch-free.  The NB P exponentials run as interleaved Horner chains; all species touched in
+// Branch-free.  The NB exponentials run as interleaved Horner chains; all species touched in
 // one iteration are distinct, so the omega read-modify-writes are one batch of loads, the
 // adds, one batch of stores.
-template <int P, int NR, int NP, int NB, class Tab, class Mem>
-PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT<P> &pt, const Mem &mem) {
+template <int NR, int NP, int NB, class Tab, class Mem>
+PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT &pt, const Mem &mem) {
     constexpr int NS = NR + NP;
 #pragma unroll 1
     for (int j = j0; j < j0 + count; j += NB) {
-        uint32_t h[NB][NS];
-        double y[NB * P];
+        uint32_t hA[NB][NS], hB[NB][NR], hW[NB][NS];
+        double y[NB];
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             const RxnP &r = tab.rxn_p(j + b);
             uint32_t slot[6];
             load_slots<NS>(r.slot, slot);
 #pragma unroll
-            for (int m = 0; m < NS; ++m) h[b][m] = mem.at(slot[m]);
-            const double f0 = r.f[0], f1 = r.f[1], f2 = r.f[2];
-#pragma unroll
-            for (int i = 0; i < P; ++i) y[b * P + i] = arrhenius_log2(f0, f1, f2, pt.L2T[i], pt.invT[i]);
+            for (int m = 0; m < NS; ++m) {
+                hA[b][m] = mem.atA(slot[m]);
+                if (m < NR) hB[b][m] = mem.atB(slot[m]);
+                hW[b][m] = mem.atW(slot[m]);
+            }
+            y[b] = arrhenius_log2(r.f[0], r.f[1], r.f[2], pt.L2T, pt.invT);
         }
-        Vec<P> a[NB][NS], bb[NB][NR], w[NB][NS];
+        mem.fence_stW();
+        typename Mem::WRaw wr[NB * NS];
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+            for (int m = 0; m < NS; ++m) wr[b * NS + m] = mem.ldW(hW[b][m]);
+        double a[NB][NS], bb[NB][NR];
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
             for (int m = 0; m < NS; ++m) {
-                a[b][m] = mem.template ld<kA>(h[b][m]);
-                if (m < NR) bb[b][m] = mem.template ld<kB>(h[b][m]);
-                w[b][m] = mem.template ld<kW>(h[b][m]);
+                a[b][m] = mem.ldA(hA[b][m]);
+                if (m < NR) bb[b][m] = mem.ldB(hB[b][m]);
             }
-        exp2_poly_n<NB * P>(y);
+        exp2_poly_n<NB>(y);
+        double R[NB];
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            double R[P];
+            double pf = a[b][0], pb = bb[b][0], pr = a[b][NR];
 #pragma unroll
-            for (int i = 0; i < P; ++i) {
-                double pf = a[b][0].v[i], pb = bb[b][0].v[i], pr = a[b][NR].v[i];
-#pragma unroll
-                for (int m = 1; m < NR; ++m) {
-                    pf *= a[b][m].v[i];
-                    pb *= bb[b][m].v[i];
-                }
-#pragma unroll
-                for (int m = 1; m < NP; ++m) pr *= a[b][NR + m].v[i];
-                R[i] = (y[b * P + i] * pb) * (pf - pr);
+            for (int m = 1; m < NR; ++m) {
+                pf *= a[b][m];
+                pb *= bb[b][m];
             }
 #pragma unroll
-            for (int m = 0; m < NS; ++m)
-#pragma unroll
-                for (int i = 0; i < P; ++i) w[b][m].v[i] = m < NR ? w[b][m].v[i] - R[i] : w[b][m].v[i] + R[i];
+            for (int m = 1; m < NP; ++m) pr *= a[b][NR + m];
+            R[b] = (y[b] * pb) * (pf - pr);
         }
+        mem.template fence_ldW<NB * NS>(wr);
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
-            for (int m = 0; m < NS; ++m) mem.template st<kW>(h[b][m], w[b][m]);
+            for (int m = 0; m < NS; ++m) {
+                const double w = mem.value(wr[b * NS + m]);
+                mem.stW(hW[b][m], m < NR ? w - R[b] : w + R[b]);
+            }
     }
 }
 
-template <int P, int NR, int NP, class Tab, class Mem>
-PYRO_HD int plain_shape(const Tab &tab, int j, int quads, int pairs, int singles, const PointT<P> &pt,
-                        const Mem &mem) {
-    plain_reactions<P, NR, NP, 4>(tab, j, quads, pt, mem);
-    plain_reactions<P, NR, NP, 2>(tab, j + quads, pairs, pt, mem);
-    plain_reactions<P, NR, NP, 1>(tab, j + quads + pairs, singles, pt, mem);
-    return j + quads + pairs + singles;
+// One shape of the plain class: its groups of eight and of four run four in lockstep, its
+// couples two in lockstep.
+template <int NR, int NP, class Tab, class Mem>
+PYRO_HD int plain_shape(const Tab &tab, int j, int g8, int g4, int g2, const PointT &pt, const Mem &mem) {
+    plain_reactions<NR, NP, 4>(tab, j, g8 + g4, pt, mem);
+    plain_reactions<NR, NP, 2>(tab, j + g8 + g4, g2, pt, mem);
+    return j + g8 + g4 + g2;
 }
 
-// Extended-class reactions of one kind: third body, falloff (Lindemann / Troe), and general
-// elementary reactions (irreversible, repeated species).  Forms per reading G6-G8
-// (PAPER.md:928 only cites them).  One reaction per iteration, its exponentials batched;
-// slots and scatter entries are padded with the dummy species so there are no branches.
-template <int P, int KIND, class Tab, class Mem>
-PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT<P> &pt, const double (&ctot)[P],
-                                const Mem &mem) {
-    constexpr int NE = KIND == kExtTroe ? 5 : (KIND == kExtLindemann ? 2 : 1);   // exponentials per point
+// Extended-class reactions of one kind, NB in lockstep: third body, falloff (Lindemann /
+// Troe), and general elementary reactions (irreversible, repeated species).  Forms per
+// reading G6-G8 (PAPER.md:928 only cites them).  Slots and scatter entries are padded with the
+// dummy species and the efficiency lists of a group have one length, so there are no
+// data-dependent branches; logarithms and divisions are the branch-free log2_pos and
+// rcp_newton of pyro_math.cuh.
+template <int KIND, int NB, class Tab, class Mem>
+PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT &pt, double ctot, const Mem &mem) {
+    constexpr int NE = KIND == kExtTroe ? 5 : (KIND == kExtLindemann ? 2 : 1);   // exponentials per reaction
 #pragma unroll 1
-    for (int j = j0; j < j0 + count; ++j) {
-        const RxnX &x = tab.rxn_x(j);
-        uint32_t h[6], hsc[6], slot[6], sc[6];
-        double nu[6];
-        load_slots<6>(x.slot, slot);
-        load_slots<6>(x.sc_species, sc);
+    for (int j = j0; j < j0 + count; j += NB) {
+        uint32_t hA[NB][6], hB[NB][3], hW[NB][6];
+        double nu[NB][6], rev[NB], M[NB], alpha[NB], has_t2[NB];
+        double y[NB * NE];
+        uint32_t q0[NB], nq = 0;
 #pragma unroll
-        for (int m = 0; m < 6; ++m) {
-            h[m] = mem.at(slot[m]);
-            hsc[m] = mem.at(sc[m]);
-            nu[m] = x.sc_nu[m];
-        }
-        const bool reversible = x.rev != 0.0;
-        double y[NE * P];
+        for (int b = 0; b < NB; ++b) {
+            const RxnX &x = tab.rxn_x(j + b);
+            uint32_t slot[6], sc[6];
+            load_slots<6>(x.slot, slot);
+            load_slots<6>(x.sc_species, sc);
 #pragma unroll
-        for (int i = 0; i < P; ++i) y[i] = arrhenius_log2(x.f[0], x.f[1], x.f[2], pt.L2T[i], pt.invT[i]);
-        double M[P];
-#pragma unroll
-        for (int i = 0; i < P; ++i) M[i] = 1.0;
-        if (KIND != kExtGeneral) {
-            // [M] = sum_k eff_k C_k = eff_default C_tot + sum_listed (eff_k - eff_default) C_k,  C_k = A_k B_k
-#pragma unroll
-            for (int i = 0; i < P; ++i) M[i] = x.eff_default * ctot[i];
-            const int q0 = (int)x.eff_begin, q1 = q0 + (int)x.eff_count;
-            for (int q = q0; q < q1; ++q) {
-                const double d = tab.eff_delta(q);
-                const uint32_t he = mem.at((uint32_t)tab.eff_species(q));
-                const Vec<P> ak = mem.template ld<kA>(he), bk = mem.template ld<kB>(he);
-#pragma unroll
-                for (int i = 0; i < P; ++i) M[i] = fma(d, ak.v[i] * bk.v[i], M[i]);
+            for (int m = 0; m < 6; ++m) {
+                hA[b][m] = mem.atA(slot[m]);
+                if (m < 3) hB[b][m] = mem.atB(slot[m]);
+                hW[b][m] = mem.atW(sc[m]);
+                nu[b][m] = (double)x.sc_nu[m];
             }
-        }
-        double alpha = 0.0, has_t2 = 0.0;
-        if (KIND >= kExtLindemann) {
-            const RxnFall &fl = tab.rxn_fall((int)x.fall_index);
-#pragma unroll
-            for (int i = 0; i < P; ++i)   // log2(k0 / k_inf)
-                y[P + i] = arrhenius_log2(fl.l[0], fl.l[1], fl.l[2], pt.L2T[i], pt.invT[i]) - y[i];
-            if (KIND == kExtTroe) {
-                alpha = fl.troe_alpha;
-                has_t2 = fl.troe_has_t2;
-#pragma unroll
-                for (int i = 0; i < P; ++i) {
-                    y[2 * P + i] = fl.troe_t3 * pt.T[i];
-                    y[3 * P + i] = fl.troe_t1 * pt.T[i];
-                    y[4 * P + i] = fl.troe_t2 * pt.invT[i];
+            rev[b] = (double)x.rev;
+            y[b * NE] = arrhenius_log2(x.f[0], x.f[1], x.f[2], pt.L2T, pt.invT);
+            M[b] = x.eff_default * ctot;
+            q0[b] = x.eff_begin;
+            nq = x.eff_count;   // one length per group
+            if (KIND >= kExtLindemann) {
+                const RxnFall &fl = tab.rxn_fall((int)x.fall_index);
+                y[b * NE + 1] = arrhenius_log2(fl.l[0], fl.l[1], fl.l[2], pt.L2T, pt.invT) - y[b * NE];   // log2(k0/k_inf)
+                if (KIND == kExtTroe) {
+                    alpha[b] = fl.troe_alpha;
+                    has_t2[b] = fl.troe_has_t2;
+                    y[b * NE + 2] = fl.troe_t3 * pt.T;
+                    y[b * NE + 3] = fl.troe_t1 * pt.T;
+                    y[b * NE + 4] = fl.troe_t2 * pt.invT;
                 }
             }
         }
-        Vec<P> a[6], bb[3], w[6];
+        mem.fence_stW();
+        typename Mem::WRaw wr[NB * 6];
 #pragma unroll
-        for (int m = 0; m < 6; ++m) {
-            a[m] = mem.template ld<kA>(h[m]);
-            if (m < 3) bb[m] = mem.template ld<kB>(h[m]);
-            w[m] = mem.template ld<kW>(hsc[m]);
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+            for (int m = 0; m < 6; ++m) wr[b * 6 + m] = mem.ldW(hW[b][m]);
+        double a[NB][6], bb[NB][3];
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+            for (int m = 0; m < 6; ++m) {
+                a[b][m] = mem.ldA(hA[b][m]);
+                if (m < 3) bb[b][m] = mem.ldB(hB[b][m]);
+            }
+        if (KIND != kExtGeneral) {
+            // [M] = sum_k eff_k C_k = eff_default C_tot + sum_listed (eff_k - eff_default) C_k,  C_k = A_k B_k
+#pragma unroll 2
+            for (uint32_t q = 0; q < nq; ++q) {
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    const EffEntry &en = tab.eff((int)(q0[b] + q));
+                    const double ak = mem.ldA(mem.atA(en.species)), bk = mem.ldB(mem.atB(en.species));
+                    M[b] = fma(en.delta, ak * bk, M[b]);
+                }
+            }
         }
-        exp2_poly_n<NE * P>(y);
-        double fall[P];
+        exp2_poly_n<NB * NE>(y);
+        double fall[NB];
 #pragma unroll
-        for (int i = 0; i < P; ++i) fall[i] = 1.0;
+        for (int b = 0; b < NB; ++b) fall[b] = 1.0;
         if (KIND >= kExtLindemann) {
-            double Pr[P];
+            double Pr[NB];
 #pragma unroll
-            for (int i = 0; i < P; ++i) {
-                Pr[i] = y[P + i] * M[i];              // Pr = k0 [M] / k_inf
-                fall[i] = Pr[i] / (1.0 + Pr[i]);      // k = k_inf Pr/(1+Pr) F
+            for (int b = 0; b < NB; ++b) {
+                Pr[b] = y[b * NE + 1] * M[b];                    // Pr = k0 [M] / k_inf
+                fall[b] = Pr[b] * rcp_newton(1.0 + Pr[b]);       // k = k_inf Pr/(1+Pr) F
             }
             if (KIND == kExtTroe) {
-                double z[P];
+                double z[NB];
 #pragma unroll
-                for (int i = 0; i < P; ++i) {
-                    const double Fc = fma(1.0 - alpha, y[2 * P + i], fma(alpha, y[3 * P + i], has_t2 * y[4 * P + i]));
-                    const double l2Fc = log2(Fc);
+                for (int b = 0; b < NB; ++b) {
+                    const double Fc = fma(1.0 - alpha[b], y[b * NE + 2], fma(alpha[b], y[b * NE + 3], has_t2[b] * y[b * NE + 4]));
+                    const double l2Fc = log2_pos(Fc);
                     const double lFc = l2Fc * kLog10of2;
                     const double cc = -0.4 - 0.67 * lFc;
                     const double n = 0.75 - 1.27 * lFc;
-                    const double lPr = log2(Pr[i]) * kLog10of2 + cc;
+                    const double lPr = log2_pos(Pr[b]) * kLog10of2 + cc;
                     // F = Fcent^(1/(1+f1^2)), f1 = lPr/d, d = n - 0.14 lPr:  1/(1+f1^2) = d^2/(d^2 + lPr^2)
                     const double d = n - 0.14 * lPr;
                     const double d2 = d * d;
-                    z[i] = l2Fc * (d2 / fma(lPr, lPr, d2));
+                    z[b] = l2Fc * (d2 * rcp_newton(fma(lPr, lPr, d2)));
                 }
-                exp2_poly_n<P>(z);
+                exp2_poly_n<NB>(z);
 #pragma unroll
-                for (int i = 0; i < P; ++i) fall[i] *= z[i];
+                for (int b = 0; b < NB; ++b) fall[b] *= z[b];
             }
         }
-        double R[P];
+        double R[NB];
 #pragma unroll
-        for (int i = 0; i < P; ++i) {
-            const double pf = a[0].v[i] * a[1].v[i] * a[2].v[i];
-            const double pr = reversible ? a[3].v[i] * a[4].v[i] * a[5].v[i] : 0.0;
-            const double pb = bb[0].v[i] * bb[1].v[i] * bb[2].v[i];
-            R[i] = (y[i] * pb) * (pf - pr) * fall[i];
-            if (KIND == kExtThreeBody) R[i] *= M[i];   // R = [M](q_f - q_r), reading G8
+        for (int b = 0; b < NB; ++b) {
+            const double pf = a[b][0] * a[b][1] * a[b][2];
+            const double pr = rev[b] != 0.0 ? a[b][3] * a[b][4] * a[b][5] : 0.0;   // irreversible: r_r = 0 (G19)
+            const double pb = bb[b][0] * bb[b][1] * bb[b][2];
+            R[b] = (y[b * NE] * pb) * (pf - pr) * fall[b];
+            if (KIND == kExtThreeBody) R[b] *= M[b];   // R = [M](q_f - q_r), reading G8
         }
+        mem.template fence_ldW<NB * 6>(wr);
 #pragma unroll
-        for (int m = 0; m < 6; ++m) {
+        for (int b = 0; b < NB; ++b)
 #pragma unroll
-            for (int i = 0; i < P; ++i) w[m].v[i] = fma(nu[m], R[i], w[m].v[i]);
-            mem.template st<kW>(hsc[m], w[m]);
-        }
+            for (int m = 0; m < 6; ++m) mem.stW(hW[b][m], fma(nu[b][m], R[b], mem.value(wr[b * 6 + m])));
     }
+}
+
+template <int KIND, class Tab, class Mem>
+PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, const PointT &pt, double ctot, const Mem &mem) {
+    extended_reactions<KIND, 2>(tab, j, g4, pt, ctot, mem);
+    extended_reactions<KIND, 1>(tab, j + g4, g2, pt, ctot, mem);
+    return j + g4 + g2;
 }
 
 // Rows a5-a9 of SURVEY.md 8(a): rates of progress of every reaction and their stoichiometric
-// accumulation into plane kW, (A.5)-(A.10) PAPER.md:908-934.  The planes hold n_species + 1
+// accumulation into plane W, (A.5)-(A.10) PAPER.md:908-934.  The planes hold n_species + 1
 // entries: the last one is the dummy species (A = B = 1, omega = sink) that pads the
-// extended records.
-template <int P, class Tab, class Mem>
-PYRO_HD void accumulate_reactions(const Tab &tab, const int (&quads)[9], const int (&pairs)[9],
-                                  const int (&singles)[9], const int (&ext)[4], const PointT<P> &pt,
-                                  const double (&ctot)[P], const Mem &mem) {
+// extended records and the null records.
+template <class Tab, class Mem>
+PYRO_HD void accumulate_reactions(const Tab &tab, const GroupCounts &g, const PointT &pt, double ctot, const Mem &mem) {
     int j = 0;
-    j = plain_shape<P, 1, 1>(tab, j, quads[0], pairs[0], singles[0], pt, mem);
-    j = plain_shape<P, 1, 2>(tab, j, quads[1], pairs[1], singles[1], pt, mem);
-    j = plain_shape<P, 1, 3>(tab, j, quads[2], pairs[2], singles[2], pt, mem);
-    j = plain_shape<P, 2, 1>(tab, j, quads[3], pairs[3], singles[3], pt, mem);
-    j = plain_shape<P, 2, 2>(tab, j, quads[4], pairs[4], singles[4], pt, mem);
-    j = plain_shape<P, 2, 3>(tab, j, quads[5], pairs[5], singles[5], pt, mem);
-    j = plain_shape<P, 3, 1>(tab, j, quads[6], pairs[6], singles[6], pt, mem);
-    j = plain_shape<P, 3, 2>(tab, j, quads[7], pairs[7], singles[7], pt, mem);
-    j = plain_shape<P, 3, 3>(tab, j, quads[8], pairs[8], singles[8], pt, mem);
+    j = plain_shape<1, 1>(tab, j, g.shape_g8[0], g.shape_g4[0], g.shape_g2[0], pt, mem);
+    j = plain_shape<1, 2>(tab, j, g.shape_g8[1], g.shape_g4[1], g.shape_g2[1], pt, mem);
+    j = plain_shape<1, 3>(tab, j, g.shape_g8[2], g.shape_g4[2], g.shape_g2[2], pt, mem);
+    j = plain_shape<2, 1>(tab, j, g.shape_g8[3], g.shape_g4[3], g.shape_g2[3], pt, mem);
+    j = plain_shape<2, 2>(tab, j, g.shape_g8[4], g.shape_g4[4], g.shape_g2[4], pt, mem);
+    j = plain_shape<2, 3>(tab, j, g.shape_g8[5], g.shape_g4[5], g.shape_g2[5], pt, mem);
+    j = plain_shape<3, 1>(tab, j, g.shape_g8[6], g.shape_g4[6], g.shape_g2[6], pt, mem);
+    j = plain_shape<3, 2>(tab, j, g.shape_g8[7], g.shape_g4[7], g.shape_g2[7], pt, mem);
+    j = plain_shape<3, 3>(tab, j, g.shape_g8[8], g.shape_g4[8], g.shape_g2[8], pt, mem);
     int x = 0;
-    extended_reactions<P, kExtGeneral>(tab, x, ext[0], pt, ctot, mem); x += ext[0];
-    extended_reactions<P, kExtThreeBody>(tab, x, ext[1], pt, ctot, mem); x += ext[1];
-    extended_reactions<P, kExtLindemann>(tab, x, ext[2], pt, ctot, mem); x += ext[2];
-    extended_reactions<P, kExtTroe>(tab, x, ext[3], pt, ctot, mem);
+    x = extended_kind<kExtGeneral>(tab, x, g.ext_g4[0], g.ext_g2[0], pt, ctot, mem);
+    x = extended_kind<kExtThreeBody>(tab, x, g.ext_g4[1], g.ext_g2[1], pt, ctot, mem);
+    x = extended_kind<kExtLindemann>(tab, x, g.ext_g4[2], g.ext_g2[2], pt, ctot, mem);
+    x = extended_kind<kExtTroe>(tab, x, g.ext_g4[3], g.ext_g2[3], pt, ctot, mem);
+    mem.fence_stW();
 }
 
 // Rows a2, a3 for every species, then the dummy species (A = B = 1, omega = sink): fills the
-// three planes.  `load_y(k, y)` fetches the thread's mass fractions of species k.
-template <int P, class Tab, class Mem, class LoadY>
-PYRO_HD void fill_planes(const Tab &tab, int ns, const PointT<P> &pt, const double (&rho)[P], double (&ctot)[P],
-                         const Mem &mem, const LoadY &load_y) {
-    const Vec<P> zero = splat<P>(0.0);
-#pragma unroll 2
-    for (int k = 0; k < ns; ++k) {
-        double y[P];
-        load_y(k, y);
-        Vec<P> A, B;
-        species_planes<P>(tab.spec(k), pt, rho, y, ctot, A, B);
-        const uint32_t h = mem.at((uint32_t)k);
-        mem.template st<kA>(h, A);
-        mem.template st<kB>(h, B);
-        mem.template st<kW>(h, zero);
+// three planes.  `load_y(k)` fetches the thread's mass fraction of species k.  Returns C_tot.
+template <class Tab, class Mem, class LoadY>
+PYRO_HD double fill_planes(const Tab &tab, int ns, const PointT &pt, double rho, const Mem &mem, const LoadY &load_y) {
+    double ctot = 0.0;
+    int k = 0;
+#pragma unroll 1
+    for (; k + 4 <= ns; k += 4) {
+        const double y[4] = {load_y(k), load_y(k + 1), load_y(k + 2), load_y(k + 3)};
+        species_planes<4>(tab, k, pt, rho, y, ctot, mem);
     }
-    const uint32_t h = mem.at((uint32_t)ns);
-    mem.template st<kA>(h, splat<P>(1.0));
-    mem.template st<kB>(h, splat<P>(1.0));
-    mem.template st<kW>(h, zero);
+#pragma unroll 1
+    for (; k < ns; ++k) {
+        const double y[1] = {load_y(k)};
+        species_planes<1>(tab, k, pt, rho, y, ctot, mem);
+    }
+    mem.stA(mem.atA((uint32_t)ns), 1.0);
+    mem.stB(mem.atB((uint32_t)ns), 1.0);
+    mem.stW(mem.atW((uint32_t)ns), 0.0);
+    return ctot;
 }
 
-// Plain array of kPlanes * (n_species + 1) P-vectors (host build, tests).
-template <int P> struct ArrayMem {
-    Vec<P> *s;
-    PYRO_HD uint32_t at(uint32_t k) const { return k * kPlanes; }
-    template <int Q> PYRO_HD Vec<P> ld(uint32_t h) const { return s[h + Q]; }
-    template <int Q> PYRO_HD void st(uint32_t h, const Vec<P> &v) const { s[h + Q] = v; }
+// Plain arrays of n_species + 1 entries per plane (host build, tests).
+struct ArrayMem {
+    typedef double WRaw;
+    double *A, *B, *W;
+    PYRO_HD uint32_t atA(uint32_t k) const { return k; }
+    PYRO_HD uint32_t atB(uint32_t k) const { return k; }
+    PYRO_HD uint32_t atW(uint32_t k) const { return k; }
+    PYRO_HD double ldA(uint32_t h) const { return A[h]; }
+    PYRO_HD double ldB(uint32_t h) const { return B[h]; }
+    PYRO_HD void stA(uint32_t h, double v) const { A[h] = v; }
+    PYRO_HD void stB(uint32_t h, double v) const { B[h] = v; }
+    PYRO_HD WRaw ldW(uint32_t h) const { return W[h]; }
+    PYRO_HD void stW(uint32_t h, double v) const { W[h] = v; }
+    template <int N> PYRO_HD void fence_ldW(WRaw (&)[N]) const {}
+    PYRO_HD void fence_stW() const {}
+    PYRO_HD double value(WRaw r) const { return r; }
 };
 
 // Newton iteration on the mixture energy polynomial (row a4): (A.27)-(A.28) PAPER.md:1017-1021,

@@ -12,6 +12,9 @@
 // reaction costs ONE exponential (k_f), three coefficients and its species slots.
 // All exponents are stored in log2 units on the per-point features
 //     (1, log2 T, 1/T, T, T^2, T^3, T^4).
+//
+// Every record is a multiple of 16 bytes and 16-byte aligned: the kernels read the tables
+// from shared memory with 128-bit loads at warp-uniform addresses (one wavefront each).
 #pragma once
 #include <cstdint>
 
@@ -23,49 +26,53 @@
 
 namespace pyro {
 
-constexpr int kMaxSide = 3;                  // molecules per reaction side held in fixed-width slots
-constexpr int kConstBankBytes = 63 * 1024;   // of the 64 KB __constant__ bank; the rest is left to the compiler
-constexpr int kPlanes = 3;                   // on-chip planes per species: A_k, B_k, omega_k
+constexpr int kMaxSide = 3;   // molecules per reaction side held in fixed-width slots
 
 // Per species: 1/W_k, T_mid,k and log2 E_k = c0 + c1 log2T + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4
-// for each NASA range (T < T_mid: lo, else hi; reading G10).  128 bytes.
+// for each NASA range (T < T_mid: lo, else hi; reading G10).  Both coefficient sets start on
+// a 16-byte boundary so that a thread fetches only the set of its own range.  144 bytes.
 struct alignas(16) SpecRow {
     double inv_w, t_mid;
-    double lo[7], hi[7];
+    double lo[8];   // [7] unused
+    double hi[8];   // [7] unused
 };
 
 // Plain class: reversible elementary reactions whose species are all distinct with unit
 // coefficients (so the scatter list is the slot list and the slots of one reaction never
 // collide).  Stored by shape (molecules per side), shape s = 3 (nreac-1) + (nprod-1); within a
-// shape first the groups of four mutually species-disjoint reactions, then the disjoint
-// couples, then the rest.  48 bytes.
+// shape first the groups of eight mutually species-disjoint reactions, then the groups of
+// four, then the couples (a reaction left alone is coupled with a null record: every slot
+// names the dummy species, so its rate is exactly zero).  48 bytes.
 struct alignas(16) RxnP {
     double f[3];        // log2 k_f = f0 + f1 log2T + f2/T          (A.9) PAPER.md:925
     uint32_t slot[6];   // species: reactants 0..nreac-1, then products nreac..nreac+nprod-1
 };
 
 // Extended class: three-body and falloff reactions, irreversible reactions, and reactions
-// with a repeated species (coefficient 2 or 3, or a species on both sides).  Stored by kind.
-// The six slots list every molecule (a coefficient 2 repeats the species), reactants in
-// 0..2 and products in 3..5; unused slots and unused scatter entries name the dummy species
-// n_species (A = B = 1, omega = sink), so that the code is branch-free.  The scatter list
-// holds each species once, with its net coefficient.
+// with a repeated species (coefficient 2 or 3, or a species on both sides).  Stored by kind,
+// within a kind first the groups of four reactions with mutually disjoint scatter lists, then
+// the couples (null-padded like the plain class).  The six slots list every molecule (a
+// coefficient 2 repeats the species), reactants in 0..2 and products in 3..5; unused slots and
+// unused scatter entries name the dummy species n_species (A = B = 1, omega = sink), so that
+// the code is branch-free.  The scatter list holds each species once, with its net
+// coefficient.  128 bytes.
 enum { kExtGeneral = 0, kExtThreeBody = 1, kExtLindemann = 2, kExtTroe = 3 };
 
 struct alignas(16) RxnX {
     double f[3];             // log2 k_f (high-pressure limit for falloff kinds)
     uint32_t slot[6];
     uint32_t sc_species[6];  // omega[sc_species] += sc_nu * R
-    double sc_nu[6];
+    float sc_nu[6];          // small integers, exact in binary32
     double eff_default;      // [M] = eff_default * C_tot + sum_listed eff_delta * C_k
-    double rev;              // 1.0 reversible, 0.0 irreversible (r_r = 0)
-    uint32_t eff_begin;      // range in the efficiency arrays
-    uint32_t eff_count;
+    float rev;               // 1 reversible, 0 irreversible (r_r = 0)
+    uint32_t eff_begin;      // first entry of the efficiency list
+    uint32_t eff_count;      // entries, padded to the maximum of the lockstep group with (0, dummy)
     uint32_t fall_index;     // row of the falloff table (kinds kExtLindemann, kExtTroe)
     uint32_t type;           // PYRO_ELEMENTARY .. PYRO_FALLOFF_TROE
+    uint32_t pad;
 };
 
-// Falloff parameters of an extended reaction.
+// Falloff parameters of an extended reaction.  64 bytes.
 struct alignas(16) RxnFall {
     double l[3];             // log2 k_0 (low-pressure limit)
     double troe_alpha;       // Troe: Fcent = (1-alpha) 2^(t3 T) + alpha 2^(t1 T) + has_t2 2^(t2/T)
@@ -73,23 +80,36 @@ struct alignas(16) RxnFall {
     double troe_has_t2;      // 1.0 or 0.0
 };
 
-// Byte offsets into the table blob (all 16-byte aligned).
+// One listed third-body efficiency: delta = eff - eff_default of the reaction.  16 bytes.
+struct alignas(16) EffEntry {
+    double delta;
+    uint32_t species;
+    uint32_t pad;
+};
+
+// Byte offsets into the table blob (all 16-byte aligned) and the loop counts of the kernels.
 struct TableLayout {
     uint32_t off_spec;       // SpecRow[n_species]
     uint32_t off_rxn_p;      // RxnP[n_p]
     uint32_t off_rxn_x;      // RxnX[n_x]
     uint32_t off_fall;       // RxnFall[n_fall]
-    uint32_t off_eff_delta;  // double[n_eff]       eff - eff_default
-    uint32_t off_eff_species;// uint32[n_eff]
+    uint32_t off_eff;        // EffEntry[n_eff]
     uint32_t bytes;
-    int32_t n_species, n_p, n_x, n_eff, n_fall;
-    int32_t shape_quads[9];    // plain class, per shape: reactions stored as disjoint groups of four
-    int32_t shape_pairs[9];    // ... as disjoint couples
-    int32_t shape_singles[9];  // ... unpaired
-    int32_t ext_count[4];      // extended class, per kind
-    int32_t needs_ctot;        // any extended reaction uses [M]
-    int32_t single_t_mid;      // 1 if every species has the same T_mid (needed by the temperature solve)
-    double t_mid;              // that T_mid
+    int32_t n_species;
+    int32_t n_p, n_x, n_eff, n_fall;   // stored records (null padding included)
+    int32_t shape_g8[9];     // plain class, per shape: records stored as disjoint groups of eight
+    int32_t shape_g4[9];     // ... of four
+    int32_t shape_g2[9];     // ... as couples
+    int32_t ext_g4[4];       // extended class, per kind: records stored as disjoint groups of four
+    int32_t ext_g2[4];       // ... as couples
+    int32_t needs_ctot;      // any extended reaction uses [M]
+    int32_t single_t_mid;    // 1 if every species has the same T_mid (needed by the temperature solve)
+    double t_mid;            // that T_mid
+};
+
+// Loop counts of one mechanism, as the kernels take them (copied from TableLayout).
+struct GroupCounts {
+    int32_t shape_g8[9], shape_g4[9], shape_g2[9], ext_g4[4], ext_g2[4];
 };
 
 // Energy table of the temperature solve: per species and NASA range the six coefficients

@@ -21,41 +21,22 @@ struct HostTab {
     const pyro::RxnP &rxn_p(int j) const { return reinterpret_cast<const pyro::RxnP *>(base + lay.off_rxn_p)[j]; }
     const pyro::RxnX &rxn_x(int j) const { return reinterpret_cast<const pyro::RxnX *>(base + lay.off_rxn_x)[j]; }
     const pyro::RxnFall &rxn_fall(int j) const { return reinterpret_cast<const pyro::RxnFall *>(base + lay.off_fall)[j]; }
-    double eff_delta(int q) const { return reinterpret_cast<const double *>(base + lay.off_eff_delta)[q]; }
-    int eff_species(int q) const { return (int)reinterpret_cast<const uint32_t *>(base + lay.off_eff_species)[q]; }
+    const pyro::EffEntry &eff(int q) const { return reinterpret_cast<const pyro::EffEntry *>(base + lay.off_eff)[q]; }
 };
 thread_local std::string g_err;
 
-template <int P>
-int emu_rates_p(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
-                double *omega) {
-    pyro::PackedMech pm;
-    int st = pyro::pack_mechanism(d, pm, g_err);
-    if (st != PYRO_OK) return st;
-    HostTab tab{pm.blob.data(), pm.lay};
-    const int ns = pm.n_species;
-    std::vector<pyro::Vec<P>> s((size_t)pyro::kPlanes * (ns + 1));   // + the dummy species
-    for (int64_t p0 = 0; p0 < n; p0 += P) {
-        double ctot[P], Tp[P], rh[P];
-        int64_t pi[P];
-        for (int i = 0; i < P; ++i) {
-            pi[i] = p0 + i < n ? p0 + i : n - 1;
-            Tp[i] = T[pi[i]];
-            rh[i] = rho[pi[i]];
-            ctot[i] = 0;
-        }
-        const pyro::PointT<P> pt = pyro::make_point<P>(Tp);
-        const pyro::ArrayMem<P> mem{s.data()};
-        pyro::fill_planes<P>(tab, ns, pt, rh, ctot, mem, [&](int k, double (&y)[P]) {
-            for (int i = 0; i < P; ++i) y[i] = Y[k * ld + pi[i]];
-        });
-        pyro::accumulate_reactions<P>(tab, pm.lay.shape_quads, pm.lay.shape_pairs, pm.lay.shape_singles,
-                                      pm.lay.ext_count, pt, ctot, mem);
-        for (int k = 0; k < ns; ++k)
-            for (int i = 0; i < P; ++i)
-                if (p0 + i < n) omega[k * ld + p0 + i] = s[k * pyro::kPlanes + 2].v[i];
+pyro::GroupCounts group_counts(const pyro::TableLayout &l) {
+    pyro::GroupCounts g;
+    for (int s = 0; s < 9; ++s) {
+        g.shape_g8[s] = l.shape_g8[s];
+        g.shape_g4[s] = l.shape_g4[s];
+        g.shape_g2[s] = l.shape_g2[s];
     }
-    return PYRO_OK;
+    for (int k = 0; k < 4; ++k) {
+        g.ext_g4[k] = l.ext_g4[k];
+        g.ext_g2[k] = l.ext_g2[k];
+    }
+    return g;
 }
 }   // namespace
 
@@ -63,9 +44,10 @@ extern "C" {
 
 const char *emu_last_error() { return g_err.c_str(); }
 
-// info: [0] plain reactions [1] extended [2] table bytes [3] efficiencies
-//       [4] plain reactions stored in groups of four [5] in couples [6] single T_mid
-//       [7..15] per shape: reactions in fours, [16..24] in couples, [25..33] single
+// info: [0] plain records [1] extended records [2] table bytes [3] efficiency entries
+//       [4] plain records stored in groups of eight [5] of four [6] single T_mid
+//       [7..15] per shape: records in eights, [16..24] in fours, [25..33] in couples
+//       [34..37] extended records per kind in fours, [38..41] in couples
 int emu_pack_status(const pyro_mech_desc *d, int64_t *info) {
     pyro::PackedMech pm;
     int st = pyro::pack_mechanism(d, pm, g_err);
@@ -76,31 +58,48 @@ int emu_pack_status(const pyro_mech_desc *d, int64_t *info) {
         info[3] = pm.lay.n_eff;
         info[4] = info[5] = 0;
         for (int s = 0; s < 9; ++s) {
-            info[4] += pm.lay.shape_quads[s];
-            info[5] += pm.lay.shape_pairs[s];
-            info[7 + s] = pm.lay.shape_quads[s];
-            info[16 + s] = pm.lay.shape_pairs[s];
-            info[25 + s] = pm.lay.shape_singles[s];
+            info[4] += pm.lay.shape_g8[s];
+            info[5] += pm.lay.shape_g4[s];
+            info[7 + s] = pm.lay.shape_g8[s];
+            info[16 + s] = pm.lay.shape_g4[s];
+            info[25 + s] = pm.lay.shape_g2[s];
+        }
+        for (int k = 0; k < 4; ++k) {
+            info[34 + k] = pm.lay.ext_g4[k];
+            info[38 + k] = pm.lay.ext_g2[k];
         }
         info[6] = pm.lay.single_t_mid;
     }
     return st;
 }
 
-// packed position -> reaction index of the description (order[n_reactions])
-int emu_pack_order(const pyro_mech_desc *d, int32_t *order) {
+// packed record -> reaction index of the description, -1 for a null record; order[cap]
+int emu_pack_order(const pyro_mech_desc *d, int32_t *order, int32_t cap) {
     pyro::PackedMech pm;
     int st = pyro::pack_mechanism(d, pm, g_err);
     if (st == PYRO_OK)
-        for (size_t i = 0; i < pm.order.size(); ++i) order[i] = pm.order[i];
+        for (size_t i = 0; i < pm.order.size() && (int32_t)i < cap; ++i) order[i] = pm.order[i];
     return st;
 }
 
-// points_per_thread selects the kernel variant that is emulated (1 or 2 points per "thread")
-int emu_rates(const pyro_mech_desc *d, int points_per_thread, int64_t n, int64_t ld, const double *rho,
-              const double *T, const double *Y, double *omega) {
-    return points_per_thread == 2 ? emu_rates_p<2>(d, n, ld, rho, T, Y, omega)
-                                  : emu_rates_p<1>(d, n, ld, rho, T, Y, omega);
+// the per-point functions of the rates kernel, one point after the other
+int emu_rates(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
+              double *omega) {
+    pyro::PackedMech pm;
+    int st = pyro::pack_mechanism(d, pm, g_err);
+    if (st != PYRO_OK) return st;
+    HostTab tab{pm.blob.data(), pm.lay};
+    const pyro::GroupCounts g = group_counts(pm.lay);
+    const int ns = pm.n_species;
+    std::vector<double> A(ns + 1), B(ns + 1), W(ns + 1);   // + the dummy species
+    for (int64_t p = 0; p < n; ++p) {
+        const pyro::PointT pt = pyro::make_point(T[p]);
+        const pyro::ArrayMem mem{A.data(), B.data(), W.data()};
+        const double ctot = pyro::fill_planes(tab, ns, pt, rho[p], mem, [&](int k) { return Y[k * ld + p]; });
+        pyro::accumulate_reactions(tab, g, pt, ctot, mem);
+        for (int k = 0; k < ns; ++k) omega[k * ld + p] = W[k];
+    }
+    return PYRO_OK;
 }
 
 int emu_temperature(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *e, const double *Y,
@@ -127,6 +126,8 @@ int emu_temperature(const pyro_mech_desc *d, int64_t n, int64_t ld, const double
 }
 
 double emu_exp2(double y) { return pyro::exp2_poly(y); }
+
+double emu_log2(double x) { return pyro::log2_pos(x); }
 
 void emu_exp2_pair(double y, double *e, double *b) {
     const double yy[1] = {y};

@@ -202,11 +202,12 @@ def test_abi_error_codes_on_device(mechs):
     assert lib.pyro_mech_create(C.byref(desc), 99, C.byref(out)) == 2 and not out.value
 
 
-def test_two_mechanisms_share_the_constant_bank_across_streams(mechs):
-    """Alternating launches of two mechanisms on two streams: the table bank is re-uploaded in order."""
+def test_two_mechanisms_alternate_across_streams(mechs):
+    """Alternating launches of two mechanisms on two streams: every launch stages its own tables and
+    allocates its own tensor-memory columns, so concurrent kernels of different mechanisms coexist."""
     m0, g0, o0 = mechs(0)
     m2, g2, o2 = mechs(2)
-    assert g0.info()["tables_in_constant"] == 1 and g2.info()["tables_in_constant"] == 1
+    assert g0.info()["tables_in_shared"] == 1 and g2.info()["tables_in_shared"] == 1
     s0 = inputs.config_states(0, n=3000)
     s2 = inputs.config_states(2, n=1500)
     ref0, b0 = o0.get_net_production_rates(s0["rho"], s0["T"], s0["Y"])
@@ -225,29 +226,32 @@ def test_two_mechanisms_share_the_constant_bank_across_streams(mechs):
 
 
 def test_tables_in_global_memory_path(mechs, monkeypatch):
-    """Mechanisms too large for the 64 KB constant bank read their tables from global memory
-    (configs[3] does so by size; here the path is forced for configs[2] as well)."""
-    mech3, g3, _ = mechs(3)
-    assert g3.info()["tables_in_constant"] == 0
+    """Mechanisms whose tables would crowd the planes out of shared memory read them from global
+    memory; here that path is forced for configs[2] and configs[3]."""
     monkeypatch.setenv("PYRO_TABLES", "global")
-    mech, _, orc = mechs(2)
-    gm = binding.Mechanism(mech)
-    assert gm.info()["tables_in_constant"] == 0
-    st = inputs.config_states(2, n=1111)
-    om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
-    parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
+    for cfg, n in ((2, 1111), (3, 300)):
+        mech, _, orc = mechs(cfg)
+        gm = binding.Mechanism(mech)
+        assert gm.info()["tables_in_shared"] == 0
+        st = inputs.config_states(cfg, n=n)
+        om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+        parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
 
 
-@pytest.mark.parametrize("cfg,block,points", [(2, 32, 1), (2, 64, 1), (2, 128, 1), (2, 32, 2), (2, 64, 2),
-                                              (0, 32, 2), (0, 64, 2), (0, 128, 2), (0, 128, 1)])
-def test_every_kernel_variant(mechs, monkeypatch, cfg, block, points):
-    """Every compiled (threads per block, points per thread) variant of the rates kernel, forced."""
+@pytest.mark.parametrize("cfg,block", [(2, 32), (2, 64), (2, 96), (2, 160), (2, 192), (0, 32), (0, 128), (0, 256),
+                                       (3, 32), (3, 64)])
+def test_every_block_size(mechs, monkeypatch, cfg, block):
+    """Threads (= points) per block of the rates kernel, forced: 1 to 8 warps, i.e. one and two
+    tensor-memory column groups, with a ragged last tile and more tiles than resident blocks."""
     monkeypatch.setenv("PYRO_RATES_BLOCK", str(block))
-    monkeypatch.setenv("PYRO_RATES_POINTS", str(points))
     mech, _, orc = mechs(cfg)
     gm = binding.Mechanism(mech)
-    assert gm.info()["block_threads"] == block and gm.info()["points_per_thread"] == points
-    for n in (777, 2 * block * points + 1):
+    info = gm.info()
+    assert info["block_threads"] == block
+    assert info["tmem_columns"] >= ((block // 32 + 3) // 4) * 2 * (mech.n_species + 1)
+    for n in (777, 2 * block + 1, info["sm_count"] * info["blocks_per_sm"] * block + 5 * block + 3):
+        if cfg == 3 and n > 3000:
+            n = 3001
         st = inputs.config_states(cfg, n=n)
         om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
         parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)

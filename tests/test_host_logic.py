@@ -63,18 +63,20 @@ def emu():
     L.emu_exp2.argtypes = [C.c_double]
     vp, i64 = C.c_void_p, C.c_int64
     L.emu_pack_status.argtypes = [vp, vp]
-    L.emu_rates.argtypes = [vp, C.c_int, i64, i64, vp, vp, vp, vp]
-    L.emu_pack_order.argtypes = [vp, vp]
+    L.emu_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp]
+    L.emu_pack_order.argtypes = [vp, vp, C.c_int32]
+    L.emu_log2.restype = C.c_double
+    L.emu_log2.argtypes = [C.c_double]
     L.emu_exp2_pair.argtypes = [C.c_double, vp, vp]
     L.emu_temperature.argtypes = [vp, i64, i64, vp, vp, vp, C.c_double, C.c_int, vp, vp]
     return L
 
 
-def emu_rates(emu, mech, rho, T, Y, points_per_thread=1):
+def emu_rates(emu, mech, rho, T, Y):
     desc, keep = binding.make_desc(mech)
     rho, T, Y = (np.ascontiguousarray(x, dtype=np.float64) for x in (rho, T, Y))
     om = np.empty_like(Y)
-    st = emu.emu_rates(C.byref(desc), points_per_thread, rho.shape[0], rho.shape[0], rho.ctypes.data, T.ctypes.data,
+    st = emu.emu_rates(C.byref(desc), rho.shape[0], rho.shape[0], rho.ctypes.data, T.ctypes.data,
                        Y.ctypes.data, om.ctypes.data)
     assert st == 0, emu.emu_last_error()
     return om
@@ -95,7 +97,7 @@ def pack_status(emu, mech, mutate=None):
     desc, keep = binding.make_desc(mech)
     if mutate:
         mutate(desc, keep)
-    info = (C.c_int64 * 34)()
+    info = (C.c_int64 * 42)()
     st = emu.emu_pack_status(C.byref(desc), info)
     return st, list(info), emu.emu_last_error().decode()
 
@@ -137,6 +139,21 @@ def test_exp2_pair_is_exp2_and_its_reciprocal(emu):
     assert e.value == 1024.0 and b.value == 1.0 / 1024.0
 
 
+def test_log2_pos_accuracy(emu):
+    """Branch-free log2 of the falloff path: absolute error a few 1e-16 near 1, 1 ulp-ish beyond."""
+    mp.mp.dps = 40
+    rng = np.random.default_rng(3)
+    xs = np.concatenate([10.0 ** rng.uniform(-300, 300, 3000), rng.uniform(0.5, 2.0, 3000),
+                         2.0 ** np.arange(-40, 41), [np.sqrt(2.0), np.sqrt(0.5), 1.0, 1.0 + 2.0 ** -52, 1.0 - 2.0 ** -53]])
+    worst = 0.0
+    for x in xs:
+        got = emu.emu_log2(float(x))
+        ref = mp.log(mp.mpf(float(x)), 2)
+        worst = max(worst, float(abs(mp.mpf(got) - ref) / max(1, abs(ref))))
+    assert worst < 4e-16, worst
+    assert emu.emu_log2(1.0) == 0.0 and emu.emu_log2(8.0) == 3.0 and emu.emu_log2(0.25) == -2.0
+
+
 # ------------------------------------------------------------------ packer validation (row a0)
 def _expected_plain(mech):
     """Plain class = elementary, reversible, every coefficient 1, no species on both sides."""
@@ -155,39 +172,66 @@ def test_packer_classes_and_table_size(emu):
     for mech in (inputs.config_mechanism(0), inputs.config_mechanism(2), hand_cases.all_paths_mechanism()):
         st, info, _ = pack_status(emu, mech)
         n_plain = _expected_plain(mech)
-        assert st == 0 and info[0] == n_plain and info[1] == mech.n_reactions - n_plain
-        assert info[3] == len(mech.eff_species)
+        order = pack_order(emu, mech, info[0] + info[1])
+        assert st == 0
+        # records = reactions + null records that complete a couple
+        assert (order[:info[0]] >= 0).sum() == n_plain and (order[info[0]:] >= 0).sum() == mech.n_reactions - n_plain
+        assert info[0] % 2 == 0 and info[1] % 2 == 0
+        assert info[3] >= len(mech.eff_species)      # efficiency lists padded to one length per lockstep group
     st, info, _ = pack_status(emu, inputs.config_mechanism(2))
-    assert info[2] <= 63 * 1024          # configs[2] tables fit the constant bank
+    assert info[2] <= 40 * 1024          # configs[2] tables are staged in shared memory beside the planes
     assert info[0] > 200                 # and most reactions are in the plain class
-    assert info[4] > 0.7 * info[0]       # mostly stored as lockstep groups of four
+    assert info[4] + info[5] > 0.7 * info[0]       # mostly stored as lockstep groups of eight or four
+    assert info[3] <= 1.25 * len(inputs.config_mechanism(2).eff_species)
     assert info[6] == 1
 
 
+def pack_order(emu, mech, n_records):
+    desc, keep = binding.make_desc(mech)
+    order = np.full(n_records, -7, dtype=np.int32)
+    assert emu.emu_pack_order(C.byref(desc), order.ctypes.data, n_records) == 0
+    return order
+
+
 def test_packer_groups_are_species_disjoint_and_order_is_a_permutation(emu):
-    """The lockstep groups of the plain class batch their omega read-modify-writes: the members of
-    a group must not share a species.  `order` maps packed positions back to the description."""
-    for cfg in (0, 2, 3):
-        mech = inputs.config_mechanism(cfg)
-        desc, keep = binding.make_desc(mech)
-        order = np.empty(mech.n_reactions, dtype=np.int32)
-        assert emu.emu_pack_order(C.byref(desc), order.ctypes.data) == 0
-        assert sorted(order.tolist()) == list(range(mech.n_reactions))
+    """The lockstep groups batch their omega read-modify-writes: the members of a group must not
+    share a species that they update.  `order` maps packed records back to the description
+    (-1 for the null records that complete a couple)."""
+    for mech in (inputs.config_mechanism(0), inputs.config_mechanism(2), inputs.config_mechanism(3),
+                 hand_cases.all_paths_mechanism()):
         st, info, _ = pack_status(emu, mech)
-        species = lambda j: set(mech.reac_species[mech.reac_ptr[j]:mech.reac_ptr[j + 1]]) | \
-            set(mech.prod_species[mech.prod_ptr[j]:mech.prod_ptr[j + 1]])
+        order = pack_order(emu, mech, info[0] + info[1])
+        assert sorted(j for j in order.tolist() if j >= 0) == list(range(mech.n_reactions))
+        assert set(order.tolist()) <= set(range(-1, mech.n_reactions))
+
+        def net(j):
+            nu = {}
+            for q in range(mech.reac_ptr[j], mech.reac_ptr[j + 1]):
+                nu[int(mech.reac_species[q])] = nu.get(int(mech.reac_species[q]), 0) - int(mech.reac_coeff[q])
+            for q in range(mech.prod_ptr[j], mech.prod_ptr[j + 1]):
+                nu[int(mech.prod_species[q])] = nu.get(int(mech.prod_species[q]), 0) + int(mech.prod_coeff[q])
+            return {k for k, v in nu.items() if v != 0}
         shape = lambda j: 3 * (int(mech.reac_coeff[mech.reac_ptr[j]:mech.reac_ptr[j + 1]].sum()) - 1) + \
             int(mech.prod_coeff[mech.prod_ptr[j]:mech.prod_ptr[j + 1]].sum()) - 1
+        kind = lambda j: int(mech.rtype[j])
+
+        def check(pos, size, count, same):
+            assert count % size == 0
+            for g0 in range(pos, pos + count, size):
+                group = [j for j in order[g0:g0 + size] if j >= 0]
+                assert group and all(same(j) for j in group)
+                assert len(set().union(*[net(j) for j in group])) == sum(len(net(j)) for j in group)
+                assert size == 2 or len(group) == size          # null records only complete couples
+            return pos + count
         pos = 0
         for sh in range(9):
-            for size, count in ((4, info[7 + sh]), (2, info[16 + sh]), (1, info[25 + sh])):
-                assert count % size == 0
-                for g0 in range(pos, pos + count, size):
-                    group = order[g0:g0 + size]
-                    assert all(shape(j) == sh for j in group)
-                    assert len(set().union(*[species(j) for j in group])) == sum(len(species(j)) for j in group)
-                pos += count
+            for size, count in ((8, info[7 + sh]), (4, info[16 + sh]), (2, info[25 + sh])):
+                pos = check(pos, size, count, lambda j: shape(j) == sh)
         assert pos == info[0]
+        for k in range(4):
+            for size, count in ((4, info[34 + k]), (2, info[38 + k])):
+                pos = check(pos, size, count, lambda j: kind(j) == k)
+        assert pos == info[0] + info[1]
 
 
 def test_packer_error_codes(emu):
@@ -270,9 +314,6 @@ def test_emu_rates_config_mechanisms(emu, cfg, n):
     om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
     r = parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"]), om_ref, bound)
     assert r < 1e-12   # typical residual is a few 1e-14; 1e-11 is the bar
-    r2 = parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"], points_per_thread=2),
-                                    om_ref, bound)
-    assert r2 < 1e-12
 
 
 def test_emu_rates_species_with_different_t_mid(emu):
