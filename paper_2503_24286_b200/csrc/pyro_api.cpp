@@ -48,6 +48,7 @@ struct DeviceGuard {
 };
 
 constexpr int kMaxDevices = 64;
+constexpr uint32_t kWorkSlots = 4096;   // launches of one mechanism that may be in flight at once
 
 struct HostPipe {   // staging of pyro_source_terms_host
     static constexpr int kBuf = 3;
@@ -66,6 +67,8 @@ struct pyro_mech {
     pyro::PackedMech packed;
     unsigned char *d_blob = nullptr;
     pyro::EnergyRow *d_energy = nullptr;
+    unsigned long long *d_work = nullptr;      // ring of chunk counters, one per launch in flight
+    mutable std::atomic<uint32_t> next_work{0};
     bool tab_smem = false;     // tables staged in shared memory (else read from global memory)
     int block_threads = 32;    // = points per block
     size_t smem_bytes = 0;     // dynamic shared memory: tables (if staged) + the A/B planes
@@ -106,9 +109,13 @@ bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0
 
 // Enqueue the rates kernel of `m` on `stream`: persistent blocks, blocks_per_sm per SM at most.
 int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t stream) {
+    const int warps = m->block_threads / 32;
     int64_t blocks = (int64_t)m->sm_count * m->blocks_per_sm;
-    if (blocks > a.n_tiles) blocks = a.n_tiles;
-    PYRO_CUDA(pyro::launch_rates(a, m->block_threads, (int)blocks, m->tab_smem, m->smem_bytes, stream));
+    if (blocks > (a.n_chunks + warps - 1) / warps) blocks = (a.n_chunks + warps - 1) / warps;
+    pyro::RatesArgs args = a;
+    args.work = m->d_work + (m->next_work.fetch_add(1) % kWorkSlots);
+    PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
+    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->smem_bytes, stream));
     return PYRO_OK;
 }
 
@@ -117,7 +124,7 @@ pyro::RatesArgs rates_args(const pyro_mech *m, int64_t n, int64_t ld, const doub
     const pyro::TableLayout &l = m->packed.lay;
     pyro::RatesArgs a{};
     a.n = n; a.ld = ld; a.rho = rho; a.T = T; a.Y = Y; a.omega = omega;
-    a.n_tiles = (n + m->block_threads - 1) / m->block_threads;
+    a.n_chunks = (n + 31) / 32;
     a.gtab = m->d_blob;
     a.tab_bytes = l.bytes;
     a.planes_off = m->planes_off;
@@ -185,12 +192,15 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     auto bail = [&](cudaError_t e, const char *what) {
         cudaFree(m->d_blob);
         cudaFree(m->d_energy);
+        cudaFree(m->d_work);
         delete m;
         return cuda_fail(e, what);
     };
     if ((ce = cudaMalloc(&m->d_blob, lay.bytes > 0 ? lay.bytes : 8)) != cudaSuccess) return bail(ce, "cudaMalloc(tables)");
     if ((ce = cudaMemcpy(m->d_blob, m->packed.blob.data(), lay.bytes, cudaMemcpyHostToDevice)) != cudaSuccess)
         return bail(ce, "cudaMemcpy(tables)");
+    if ((ce = cudaMalloc(&m->d_work, kWorkSlots * sizeof(unsigned long long))) != cudaSuccess)
+        return bail(ce, "cudaMalloc(work counters)");
     const size_t ebytes = m->packed.energy.size() * sizeof(pyro::EnergyRow);
     if ((ce = cudaMalloc(&m->d_energy, ebytes)) != cudaSuccess) return bail(ce, "cudaMalloc(energy table)");
     if ((ce = cudaMemcpy(m->d_energy, m->packed.energy.data(), ebytes, cudaMemcpyHostToDevice)) != cudaSuccess)
@@ -237,6 +247,7 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (threads < 32) {
         cudaFree(m->d_blob);
         cudaFree(m->d_energy);
+        cudaFree(m->d_work);
         delete m;
         return fail(PYRO_ERR_TOO_LARGE, "species arrays do not fit the on-chip memory of one block");
     }
@@ -258,6 +269,7 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (nblk < 1) {
         cudaFree(m->d_blob);
         cudaFree(m->d_energy);
+        cudaFree(m->d_work);
         delete m;
         return fail(PYRO_ERR_TOO_LARGE, "the rates kernel does not fit one SM for this mechanism");
     }
@@ -275,6 +287,7 @@ int pyro_mech_destroy(pyro_mech *m) {
     }
     cudaFree(m->d_blob);
     cudaFree(m->d_energy);
+    cudaFree(m->d_work);
     delete m;
     return PYRO_OK;
 }

@@ -72,7 +72,7 @@ struct DevMem {
 
 // ---------------------------------------------------------------------------------------
 // omega[k][p] from rho[p], T[p], Y[k][p]   (rows a1-a3, a5-a9)
-// Thread t of a block owns point t of the block's current tile.  Tail threads recompute the
+// Lane l of a warp owns point l of the warp's current chunk.  Tail lanes recompute the
 // last point and store nothing: control flow stays warp-uniform throughout (the tensor-memory
 // instructions are warp-collective).
 // ---------------------------------------------------------------------------------------
@@ -108,17 +108,29 @@ __global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesA
     mem.baseB = mem.baseA + 8u * (uint32_t)nthreads;
     mem.tw = tmem_base + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * 2u * rows;
 
-    for (int64_t tile = blockIdx.x; tile < a.n_tiles; tile += gridDim.x) {
-        const int64_t p = tile * nthreads + tid;
+    // Warps are independent (own shared-memory columns, own tensor-memory lanes): each takes the
+    // next chunk of 32 consecutive points from a device-wide counter until none is left, which
+    // balances warps that share a scheduler against warps that have one to themselves.
+    const int lane = tid & 31;
+    auto grab = [&]() -> int64_t {
+        unsigned long long c = 0;
+        if (lane == 0) c = atomicAdd(a.work, 1ull);
+        return (int64_t)__shfl_sync(0xffffffffu, c, 0);
+    };
+    int64_t chunk = grab();
+    while (chunk < a.n_chunks) {
+        const int64_t p = chunk * 32 + lane;
         const int64_t pc = p < a.n ? p : a.n - 1;
         const double rho = a.rho[pc];
         const PointT pt = make_point(a.T[pc]);
         const double *Yp = a.Y + pc;
         const double ctot = fill_planes(tab, ns, pt, rho, mem, [&](int k) { return __ldg(Yp + (int64_t)k * a.ld); });
-        {   // bring the next tile's mass fractions into L2 while the reactions run
-            const int64_t pn = p + (int64_t)gridDim.x * nthreads;
-            if (pn < a.n && (tid & 15) == 0)
-                for (int k = 0; k < ns; ++k) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)k * a.ld + pn));
+        const int64_t next = grab();
+        if (next < a.n_chunks && (lane & 15) == 0) {   // bring the next chunk's inputs into L2 while the reactions run
+            const int64_t pn = next * 32 + lane;
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.rho + pn));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.T + pn));
+            for (int k = 0; k < ns; ++k) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)k * a.ld + pn));
         }
         accumulate_reactions(tab, a.groups, pt, ctot, mem);
         double *Wp = a.omega + p;
@@ -141,6 +153,7 @@ __global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesA
             mem.fence_ldW<1>(r);
             if (p < a.n) Wp[(int64_t)k * a.ld] = mem.value(r[0]);
         }
+        chunk = next;
     }
     asm volatile("tcgen05.fence::before_thread_sync;");
     __syncthreads();

@@ -12,7 +12,8 @@ namespace pyro {
 constexpr int kRatesMaxThreads = 256;   // threads (= points) per block of the rates kernel, a multiple of 32
 
 struct RatesArgs {
-    int64_t n, ld, n_tiles;      // n_tiles = ceil(n / threads per block)
+    int64_t n, ld, n_chunks;     // n_chunks = ceil(n / 32): a warp takes 32 consecutive points at a time
+    unsigned long long *work;    // device counter of the chunks handed out, zero at launch
     const double *rho, *T, *Y;
     double *omega;
     const unsigned char *gtab;   // device copy of the table blob in global memory

@@ -209,15 +209,15 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
             std::memset(&x, 0, sizeof x);
             for (int m = 0; m < 3; ++m) x.f[m] = f[m];
             for (int m = 0; m < 6; ++m) x.slot[m] = slot[m];
-            x.rev = reversible ? 1.0f : 0.0f;
-            x.type = (uint32_t)type;
+            x.rev = reversible ? 1 : 0;
+            x.type = (int8_t)type;
             for (int s = 0; s < 6; ++s) x.sc_species[s] = (uint32_t)ns;
             int nsc = 0;
             std::vector<int> scs;
             for (auto &kv : net)
                 if (kv.second != 0) {
                     x.sc_species[nsc] = (uint32_t)kv.first;
-                    x.sc_nu[nsc] = (float)kv.second;
+                    x.sc_nu[nsc] = (int8_t)kv.second;
                     scs.push_back(kv.first);
                     ++nsc;
                 }
@@ -341,7 +341,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         RxnX nullX;
         std::memset(&nullX, 0, sizeof nullX);
         for (int m = 0; m < 6; ++m) nullX.slot[m] = nullX.sc_species[m] = (uint32_t)ns;
-        nullX.rev = 1.0f;
+        nullX.rev = 1;
         nullX.eff_default = 1.0;
         std::vector<RxnX> sortedX;
         std::vector<EffEntry> effs;
@@ -362,7 +362,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                         const int i = g[at + m];
                         RxnX x = i < 0 ? nullX : recX[i];
                         if (i < 0) {   // a null record next to a falloff reaction reads that reaction's falloff row
-                            x.type = (uint32_t)kind;
+                            x.type = (int8_t)kind;
                             for (size_t m2 = 0; m2 < width; ++m2)
                                 if (g[at + m2] >= 0) x.fall_index = recX[g[at + m2]].fall_index;
                         }
@@ -385,8 +385,6 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         for (int k = 0; k < ns; ++k) {
             spec[k].inv_w = (double)(1.0L / (long double)d->mol_weight[k]);
             spec[k].t_mid = d->t_mid[k];
-            std::memset(spec[k].lo, 0, sizeof spec[k].lo);
-            std::memset(spec[k].hi, 0, sizeof spec[k].hi);
             species_row(d->nasa_lo + 7 * k, spec[k].lo);
             species_row(d->nasa_hi + 7 * k, spec[k].hi);
         }

@@ -30,11 +30,12 @@ constexpr int kMaxSide = 3;   // molecules per reaction side held in fixed-width
 
 // Per species: 1/W_k, T_mid,k and log2 E_k = c0 + c1 log2T + c2/T + c3 T + c4 T^2 + c5 T^3 + c6 T^4
 // for each NASA range (T < T_mid: lo, else hi; reading G10).  Both coefficient sets start on
-// a 16-byte boundary so that a thread fetches only the set of its own range.  144 bytes.
+// a 16-byte boundary so that a thread fetches only the set of its own range.  128 bytes.
 struct alignas(16) SpecRow {
-    double inv_w, t_mid;
-    double lo[8];   // [7] unused
-    double hi[8];   // [7] unused
+    double lo[7];
+    double inv_w;
+    double hi[7];
+    double t_mid;
 };
 
 // Plain class: reversible elementary reactions whose species are all distinct with unit
@@ -55,21 +56,21 @@ struct alignas(16) RxnP {
 // coefficient 2 repeats the species), reactants in 0..2 and products in 3..5; unused slots and
 // unused scatter entries name the dummy species n_species (A = B = 1, omega = sink), so that
 // the code is branch-free.  The scatter list holds each species once, with its net
-// coefficient.  128 bytes.
+// coefficient.  112 bytes.
 enum { kExtGeneral = 0, kExtThreeBody = 1, kExtLindemann = 2, kExtTroe = 3 };
 
 struct alignas(16) RxnX {
     double f[3];             // log2 k_f (high-pressure limit for falloff kinds)
     uint32_t slot[6];
     uint32_t sc_species[6];  // omega[sc_species] += sc_nu * R
-    float sc_nu[6];          // small integers, exact in binary32
     double eff_default;      // [M] = eff_default * C_tot + sum_listed eff_delta * C_k
-    float rev;               // 1 reversible, 0 irreversible (r_r = 0)
+    int8_t sc_nu[6];         // net stoichiometric coefficients of the scatter list
+    int8_t rev;              // 1 reversible, 0 irreversible (r_r = 0)
+    int8_t type;             // PYRO_ELEMENTARY .. PYRO_FALLOFF_TROE
     uint32_t eff_begin;      // first entry of the efficiency list
     uint32_t eff_count;      // entries, padded to the maximum of the lockstep group with (0, dummy)
     uint32_t fall_index;     // row of the falloff table (kinds kExtLindemann, kExtTroe)
-    uint32_t type;           // PYRO_ELEMENTARY .. PYRO_FALLOFF_TROE
-    uint32_t pad;
+    uint32_t pad[3];
 };
 
 // Falloff parameters of an extended reaction.  64 bytes.
@@ -106,6 +107,10 @@ struct TableLayout {
     int32_t single_t_mid;    // 1 if every species has the same T_mid (needed by the temperature solve)
     double t_mid;            // that T_mid
 };
+
+static_assert(sizeof(SpecRow) == 128 && sizeof(RxnP) == 48 && sizeof(RxnX) == 112 && sizeof(RxnFall) == 64 &&
+                  sizeof(EffEntry) == 16,
+              "table records are read with 128-bit loads");
 
 // Loop counts of one mechanism, as the kernels take them (copied from TableLayout).
 struct GroupCounts {
