@@ -111,7 +111,7 @@ def make_desc(mech):
 
 _INFO_KEYS = ("n_species", "n_reactions", "n_plain", "n_extended", "table_bytes", "tables_in_shared",
               "block_threads", "smem_bytes", "blocks_per_sm", "registers", "local_bytes", "sm_count",
-              "points_per_thread", "tmem_columns")
+              "points_per_thread", "tmem_columns", "c_in_tmem")
 
 
 def _ptr(t):
@@ -151,8 +151,8 @@ class Mechanism:
             pass
 
     def info(self):
-        out = (C.c_int64 * 14)()
-        n = self._lib.pyro_mech_info(self._h, out, 14)
+        out = (C.c_int64 * 15)()
+        n = self._lib.pyro_mech_info(self._h, out, 15)
         if n < 0:
             _check(-n)
         return dict(zip(_INFO_KEYS, [int(v) for v in out[:n]]))

@@ -70,6 +70,7 @@ struct pyro_mech {
     unsigned long long *d_work = nullptr;      // ring of chunk counters, one per launch in flight
     mutable std::atomic<uint32_t> next_work{0};
     bool tab_smem = false;     // tables staged in shared memory (else read from global memory)
+    bool c_tmem = false;       // concentrations C_k kept in tensor memory beside omega_k
     int block_threads = 32;    // = points per block
     size_t smem_bytes = 0;     // dynamic shared memory: tables (if staged) + the A/B planes
     uint32_t planes_off = 0;
@@ -115,7 +116,7 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     pyro::RatesArgs args = a;
     args.work = m->d_work + (m->next_work.fetch_add(1) % kWorkSlots);
     PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
-    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->smem_bytes, stream));
+    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->c_tmem, m->smem_bytes, stream));
     return PYRO_OK;
 }
 
@@ -216,9 +217,9 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     // tables staged in shared memory unless that costs more than 40 % of the points.
     const size_t rows = (size_t)lay.n_species + 1;
     size_t static_smem = 0;   // the kernels keep the tensor-memory base address in static shared memory
-    for (int v = 0; v < 2; ++v) {
+    for (int v = 0; v < 4; ++v) {
         cudaFuncAttributes fa{};
-        if ((ce = cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(v != 0))) != cudaSuccess)
+        if ((ce = cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr((v & 1) != 0, (v & 2) != 0))) != cudaSuccess)
             return bail(ce, "cudaFuncGetAttributes");
         if (fa.sharedSizeBytes > static_smem) static_smem = fa.sharedSizeBytes;
     }
@@ -254,10 +255,15 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     m->block_threads = threads;
     m->planes_off = m->tab_smem ? (uint32_t)tab_room : 0u;
     m->smem_bytes = m->planes_off + 16 * rows * (size_t)threads;
-    const uint32_t cols_needed = (uint32_t)(((threads / 32 + 3) / 4) * 2 * rows);
+    const uint32_t groups = (uint32_t)((threads / 32 + 3) / 4);
+    m->c_tmem = lay.needs_ctot && groups * 4 * rows <= 512;
+    if (const char *env = std::getenv("PYRO_C_PLANE")) {
+        if (!std::strcmp(env, "shared")) m->c_tmem = false;
+    }
+    const uint32_t cols_needed = (uint32_t)(groups * (m->c_tmem ? 4 : 2) * rows);
     m->tmem_cols = 32;
     while (m->tmem_cols < cols_needed) m->tmem_cols *= 2;
-    const void *fn = pyro::rates_kernel_ptr(m->tab_smem);
+    const void *fn = pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem);
     // the limit is a property of the function, shared by every mechanism: always raise it to the
     // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
@@ -406,12 +412,12 @@ int pyro_mech_info(const pyro_mech *m, int64_t *out, int cap) {
     if (!m || !out) return -fail(PYRO_ERR_NULL, "NULL argument");
     DeviceGuard guard(m->device);
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem));
-    const int64_t v[14] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
+    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem));
+    const int64_t v[15] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
                            (int64_t)m->packed.lay.bytes, m->tab_smem ? 1 : 0, m->block_threads,
                            (int64_t)m->smem_bytes, m->blocks_per_sm, fa.numRegs, (int64_t)fa.localSizeBytes,
-                           m->sm_count, 1, (int64_t)m->tmem_cols};
-    int cnt = cap < 14 ? cap : 14;
+                           m->sm_count, 1, (int64_t)m->tmem_cols, m->c_tmem ? 1 : 0};
+    int cnt = cap < 15 ? cap : 15;
     for (int i = 0; i < cnt; ++i) out[i] = v[i];
     return cnt;
 }

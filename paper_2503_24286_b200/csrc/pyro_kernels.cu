@@ -6,7 +6,8 @@
 //   A_k = C_k E_k and B_k = 1/E_k in shared memory as [k][plane][thread] columns (conflict-free:
 //   lane l touches its own banks), read-only while the reactions run;
 //   omega_k in TENSOR MEMORY: thread t of a warp owns lane 32 (warp % 4) + t, species k is the
-//   pair of 32-bit columns 2k, 2k+1 of that warp's column group.  The stoichiometric
+//   pair of 32-bit columns 2k, 2k+1 of that warp's column group; C_k (read by the third-body
+//   sums only) in a second set of columns when they fit.  The stoichiometric
 //   accumulation is tcgen05.ld / add / tcgen05.st on warp-uniform column addresses, which
 //   takes the read-modify-write traffic (8 of the 14 indexed accesses of a reaction) off the
 //   shared-memory pipe and doubles the points resident per SM.
@@ -35,11 +36,11 @@ struct DevTab {
 // baseA + k stride (stride = 16 bytes x threads per block), plane B the one at baseB + k stride.
 // Tensor memory: species k is the column pair tw + 2k of the thread's lane.  All accesses are
 // volatile asm, so they keep their program order.
-struct DevMem {
+template <bool kCTmem> struct DevMem {
     struct WRaw {
         uint32_t lo, hi;
     };
-    uint32_t baseA, baseB, stride, tw;
+    uint32_t baseA, baseB, stride, tw, tc;
 
     __device__ __forceinline__ uint32_t atA(uint32_t k) const { return baseA + k * stride; }
     __device__ __forceinline__ uint32_t atB(uint32_t k) const { return baseB + k * stride; }
@@ -56,6 +57,16 @@ struct DevMem {
         WRaw r;
         asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r.lo), "=r"(r.hi) : "r"(h));
         return r;
+    }
+    // plane C: tensor memory when its columns fit beside plane W, else recomputed as A_k B_k
+    __device__ __forceinline__ uint32_t atC(uint32_t k) const { return kCTmem ? tc + 2u * k : k; }
+    __device__ __forceinline__ WRaw ldC(uint32_t h) const {
+        if (kCTmem) return ldW(h);
+        const double c = ldA(atA(h)) * ldB(atB(h));
+        return WRaw{(uint32_t)__double2loint(c), (uint32_t)__double2hiint(c)};
+    }
+    __device__ __forceinline__ void stC(uint32_t h, double v) const {
+        if (kCTmem) stW(h, v);
     }
     __device__ __forceinline__ void stW(uint32_t h, double v) const {
         asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(h), "r"(__double2loint(v)), "r"(__double2hiint(v)));
@@ -76,7 +87,7 @@ struct DevMem {
 // last point and store nothing: control flow stays warp-uniform throughout (the tensor-memory
 // instructions are warp-collective).
 // ---------------------------------------------------------------------------------------
-template <bool kTabSmem>
+template <bool kTabSmem, bool kCTmem>
 __global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_tmem_base;
@@ -102,11 +113,12 @@ __global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesA
     DevTab tab{kTabSmem ? smem_raw : a.gtab, a.off_spec, a.off_rxn_p, a.off_rxn_x, a.off_fall, a.off_eff};
     const uint32_t planes = (uint32_t)__cvta_generic_to_shared(smem_raw) + a.planes_off;
     const uint32_t rows = (uint32_t)ns + 1u;
-    DevMem mem;
+    DevMem<kCTmem> mem;
     mem.stride = 16u * (uint32_t)nthreads;
     mem.baseA = planes + 8u * (uint32_t)tid;
     mem.baseB = mem.baseA + 8u * (uint32_t)nthreads;
-    mem.tw = tmem_base + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * 2u * rows;
+    mem.tw = tmem_base + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * (kCTmem ? 4u : 2u) * rows;
+    mem.tc = mem.tw + 2u * rows;
 
     // Warps are independent (own shared-memory columns, own tensor-memory lanes): each takes the
     // next chunk of 32 consecutive points from a device-wide counter until none is left, which
@@ -137,10 +149,10 @@ __global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesA
         int k = 0;
 #pragma unroll 1
         for (; k + 4 <= ns; k += 4) {
-            DevMem::WRaw r[4];
+            typename DevMem<kCTmem>::WRaw r[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) r[i] = mem.ldW(mem.atW((uint32_t)(k + i)));
-            mem.fence_ldW<4>(r);
+            mem.template fence_ldW<4>(r);
             if (p < a.n) {
 #pragma unroll
                 for (int i = 0; i < 4; ++i) Wp[(int64_t)(k + i) * a.ld] = mem.value(r[i]);
@@ -148,9 +160,9 @@ __global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesA
         }
 #pragma unroll 1
         for (; k < ns; ++k) {
-            DevMem::WRaw r[1];
+            typename DevMem<kCTmem>::WRaw r[1];
             r[0] = mem.ldW(mem.atW((uint32_t)k));
-            mem.fence_ldW<1>(r);
+            mem.template fence_ldW<1>(r);
             if (p < a.n) Wp[(int64_t)k * a.ld] = mem.value(r[0]);
         }
         chunk = next;
@@ -240,13 +252,14 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double *out, int iters,
 // ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
-const void *rates_kernel_ptr(bool tables_in_shared) {
-    return tables_in_shared ? (const void *)rates_kernel<true> : (const void *)rates_kernel<false>;
+const void *rates_kernel_ptr(bool tables_in_shared, bool c_in_tmem) {
+    if (tables_in_shared) return c_in_tmem ? (const void *)rates_kernel<true, true> : (const void *)rates_kernel<true, false>;
+    return c_in_tmem ? (const void *)rates_kernel<false, true> : (const void *)rates_kernel<false, false>;
 }
 
-cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, size_t smem_bytes,
-                         cudaStream_t stream) {
-    const void *fn = rates_kernel_ptr(tables_in_shared);
+cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool c_in_tmem,
+                         size_t smem_bytes, cudaStream_t stream) {
+    const void *fn = rates_kernel_ptr(tables_in_shared, c_in_tmem);
     RatesArgs copy = a;
     void *params[] = {&copy};
     return cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)threads), params, smem_bytes, stream);

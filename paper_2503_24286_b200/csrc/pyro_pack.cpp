@@ -358,6 +358,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                     size_t longest = 0;
                     for (size_t m = 0; m < width; ++m)
                         if (g[at + m] >= 0) longest = std::max(longest, effX[g[at + m]].size());
+                    longest = (longest + 3) / 4 * 4;   // the kernels read the lists four entries at a time
                     for (size_t m = 0; m < width; ++m) {
                         const int i = g[at + m];
                         RxnX x = i < 0 ? nullX : recX[i];

@@ -2,15 +2,15 @@
 //
 // One thread owns one grid point.  Per-point arrays indexed by a run-time species number live
 // on chip as three planes per species:
-//     plane A  A_k = C_k E_k      plane B  B_k = 1/E_k      plane W  omega_k
-// with E_k = exp(g_k/RT) RT/p0 (pyro_tables.h).  The functions below reach them through a
-// `Mem` accessor (A and B in shared memory and W in tensor memory in the kernels, plain arrays
-// in the host build):
-//     h = mem.atA(k), mem.atB(k), mem.atW(k)     handle of species k for this thread
+//     plane A  A_k = C_k E_k      plane B  B_k = 1/E_k      plane W  omega_k      plane C  C_k
+// with E_k = exp(g_k/RT) RT/p0 (pyro_tables.h); C_k is read by the third-body sums only.  The
+// functions below reach them through a `Mem` accessor (A and B in shared memory, W and C in
+// tensor memory in the kernels, plain arrays in the host build):
+//     h = mem.atA(k), mem.atB(k), mem.atW(k), mem.atC(k)   handle of species k for this thread
 //     mem.ldA(h), mem.ldB(h), mem.stA(h, v), mem.stB(h, v)
-//     r = mem.ldW(h)            raw omega value; becomes readable by mem.value(r) only after
-//     mem.fence_ldW(raws)       (tensor-memory loads are asynchronous)
-//     mem.stW(h, v); mem.fence_stW() before a later ldW may see the stored value
+//     r = mem.ldW(h), mem.ldC(h)   raw value; becomes readable by mem.value(r) only after
+//     mem.fence_ldW(raws)          (tensor-memory loads are asynchronous)
+//     mem.stW(h, v), mem.stC(h, v); mem.fence_stW() before a later load may see the stored value
 #pragma once
 #include "../../include/pyro.h"
 #include "pyro_math.cuh"
@@ -70,6 +70,7 @@ PYRO_HD void species_planes(const Tab &tab, int k0, const PointT &pt, double rho
         mem.stA(mem.atA((uint32_t)(k0 + i)), C[i] * e[i]);
         mem.stB(mem.atB((uint32_t)(k0 + i)), b[i]);
         mem.stW(mem.atW((uint32_t)(k0 + i)), 0.0);
+        mem.stC(mem.atC((uint32_t)(k0 + i)), C[i]);
     }
 }
 
@@ -218,15 +219,25 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
                 if (m < 3) bb[b][m] = mem.ldB(hB[b][m]);
             }
         if (KIND != kExtGeneral) {
-            // [M] = sum_k eff_k C_k = eff_default C_tot + sum_listed (eff_k - eff_default) C_k,  C_k = A_k B_k
-#pragma unroll 2
-            for (uint32_t q = 0; q < nq; ++q) {
+            // [M] = sum_k eff_k C_k = eff_default C_tot + sum_listed (eff_k - eff_default) C_k; the lists of
+            // a group are padded to one length, a multiple of four
+#pragma unroll 1
+            for (uint32_t q = 0; q < nq; q += 4) {
+                typename Mem::WRaw cr[NB * 4];
+                double dl[NB * 4];
 #pragma unroll
-                for (int b = 0; b < NB; ++b) {
-                    const EffEntry &en = tab.eff((int)(q0[b] + q));
-                    const double ak = mem.ldA(mem.atA(en.species)), bk = mem.ldB(mem.atB(en.species));
-                    M[b] = fma(en.delta, ak * bk, M[b]);
-                }
+                for (int b = 0; b < NB; ++b)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const EffEntry &en = tab.eff((int)(q0[b] + q) + u);
+                        cr[b * 4 + u] = mem.ldC(mem.atC(en.species));
+                        dl[b * 4 + u] = en.delta;
+                    }
+                mem.template fence_ldW<NB * 4>(cr);
+#pragma unroll
+                for (int b = 0; b < NB; ++b)
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) M[b] = fma(dl[b * 4 + u], mem.value(cr[b * 4 + u]), M[b]);
             }
         }
         exp2_poly_n<NB * NE>(y);
@@ -279,8 +290,10 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
 
 template <int KIND, class Tab, class Mem>
 PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, const PointT &pt, double ctot, const Mem &mem) {
-    extended_reactions<KIND, 2>(tab, j, g4, pt, ctot, mem);
-    extended_reactions<KIND, 1>(tab, j + g4, g2, pt, ctot, mem);
+    // a group of four runs four in lockstep (Troe: two and two, its five exponentials per reaction
+    // already fill the pipe), a couple two
+    extended_reactions<KIND, KIND == kExtTroe ? 2 : 4>(tab, j, g4, pt, ctot, mem);
+    extended_reactions<KIND, 2>(tab, j + g4, g2, pt, ctot, mem);
     return j + g4 + g2;
 }
 
@@ -327,14 +340,18 @@ PYRO_HD double fill_planes(const Tab &tab, int ns, const PointT &pt, double rho,
     mem.stA(mem.atA((uint32_t)ns), 1.0);
     mem.stB(mem.atB((uint32_t)ns), 1.0);
     mem.stW(mem.atW((uint32_t)ns), 0.0);
+    mem.stC(mem.atC((uint32_t)ns), 0.0);
     return ctot;
 }
 
 // Plain arrays of n_species + 1 entries per plane (host build, tests).
 struct ArrayMem {
     typedef double WRaw;
-    double *A, *B, *W;
+    double *A, *B, *W, *C;
     PYRO_HD uint32_t atA(uint32_t k) const { return k; }
+    PYRO_HD uint32_t atC(uint32_t k) const { return k; }
+    PYRO_HD WRaw ldC(uint32_t h) const { return C[h]; }
+    PYRO_HD void stC(uint32_t h, double v) const { C[h] = v; }
     PYRO_HD uint32_t atB(uint32_t k) const { return k; }
     PYRO_HD uint32_t atW(uint32_t k) const { return k; }
     PYRO_HD double ldA(uint32_t h) const { return A[h]; }

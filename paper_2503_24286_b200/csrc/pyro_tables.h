@@ -68,7 +68,7 @@ struct alignas(16) RxnX {
     int8_t rev;              // 1 reversible, 0 irreversible (r_r = 0)
     int8_t type;             // PYRO_ELEMENTARY .. PYRO_FALLOFF_TROE
     uint32_t eff_begin;      // first entry of the efficiency list
-    uint32_t eff_count;      // entries, padded to the maximum of the lockstep group with (0, dummy)
+    uint32_t eff_count;      // entries, padded with (0, dummy) to the maximum of the lockstep group, a multiple of 4
     uint32_t fall_index;     // row of the falloff table (kinds kExtLindemann, kExtTroe)
     uint32_t pad[3];
 };
