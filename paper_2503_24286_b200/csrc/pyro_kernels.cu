@@ -71,11 +71,10 @@ template <bool kCTmem> struct DevMem {
     __device__ __forceinline__ void stW(uint32_t h, double v) const {
         asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(h), "r"(__double2loint(v)), "r"(__double2hiint(v)));
     }
-    // the loaded registers are defined only after the wait: tie them to it
-    template <int N> __device__ __forceinline__ void fence_ldW(WRaw (&r)[N]) const {
+    // the loaded registers are defined only after the wait (ptxas turns it into the scoreboard wait of
+    // the LDTMs); value() is only called after the fence
+    template <int N> __device__ __forceinline__ void fence_ldW(WRaw (&)[N]) const {
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-        for (int i = 0; i < N; ++i) asm volatile("" : "+r"(r[i].lo), "+r"(r[i].hi));
     }
     __device__ __forceinline__ void fence_stW() const { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
     __device__ __forceinline__ double value(const WRaw &r) const { return __hiloint2double((int)r.hi, (int)r.lo); }

@@ -210,14 +210,14 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
             for (int m = 0; m < 3; ++m) x.f[m] = f[m];
             for (int m = 0; m < 6; ++m) x.slot[m] = slot[m];
             x.rev = reversible ? 1 : 0;
-            x.type = (int8_t)type;
+            x.type = (int16_t)type;
             for (int s = 0; s < 6; ++s) x.sc_species[s] = (uint32_t)ns;
             int nsc = 0;
             std::vector<int> scs;
             for (auto &kv : net)
                 if (kv.second != 0) {
                     x.sc_species[nsc] = (uint32_t)kv.first;
-                    x.sc_nu[nsc] = (int8_t)kv.second;
+                    x.sc_nu[nsc] = (int16_t)kv.second;
                     scs.push_back(kv.first);
                     ++nsc;
                 }
@@ -363,7 +363,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                         const int i = g[at + m];
                         RxnX x = i < 0 ? nullX : recX[i];
                         if (i < 0) {   // a null record next to a falloff reaction reads that reaction's falloff row
-                            x.type = (int8_t)kind;
+                            x.type = (int16_t)kind;
                             for (size_t m2 = 0; m2 < width; ++m2)
                                 if (g[at + m2] >= 0) x.fall_index = recX[g[at + m2]].fall_index;
                         }

@@ -64,13 +64,13 @@ struct alignas(16) RxnX {
     uint32_t slot[6];
     uint32_t sc_species[6];  // omega[sc_species] += sc_nu * R
     double eff_default;      // [M] = eff_default * C_tot + sum_listed eff_delta * C_k
-    int8_t sc_nu[6];         // net stoichiometric coefficients of the scatter list
-    int8_t rev;              // 1 reversible, 0 irreversible (r_r = 0)
-    int8_t type;             // PYRO_ELEMENTARY .. PYRO_FALLOFF_TROE
+    int16_t sc_nu[6];        // net stoichiometric coefficients of the scatter list (one I2F each)
+    int16_t rev;             // 1 reversible, 0 irreversible (r_r = 0)
+    int16_t type;            // PYRO_ELEMENTARY .. PYRO_FALLOFF_TROE
     uint32_t eff_begin;      // first entry of the efficiency list
     uint32_t eff_count;      // entries, padded with (0, dummy) to the maximum of the lockstep group, a multiple of 4
     uint32_t fall_index;     // row of the falloff table (kinds kExtLindemann, kExtTroe)
-    uint32_t pad[3];
+    uint32_t pad;
 };
 
 // Falloff parameters of an extended reaction.  64 bytes.
