@@ -27,13 +27,18 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2503_24286_b200 import inputs  # noqa: E402
+from paper_2503_24286_b200 import inputs, sharding  # noqa: E402
 
 METRIC = "source-term points/sec (FP64, 53 sp/325 rxn) and % of B200 FP64/HBM roofline"
 
 # FP64 cost of the transcendental functions, counted in SASS of nvcc 12.9 -O3 for sm_100a
 # (DADD + DMUL + 2 DFMA on the fast path of CUDA's exp / log / division).
 FLOPS_EXP, FLOPS_LOG, FLOPS_DIV = 30, 46, 15
+
+# DRAM traffic of the rates kernel measured once with `ncu --set full` (dram__bytes_read.sum +
+# dram__bytes_write.sum = 867.2 MB for 2^20 points of configs[2]; profiles/r01_v5_rates_kernel.md).
+# Reported as `traffic` for the configs[2]/[4] mechanism only, scaled to the points of one launch.
+NCU_RATES_DRAM_BYTES_PER_POINT_53SP = 867.2e6 / 1048576
 
 # FP64 roof of one B200: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
@@ -208,7 +213,7 @@ def main():
     ns = mech.n_species
     n = args.points or inputs.CONFIG_POINTS[cfg]
     # weak scaling: every rank owns a full-size batch of independent points (own seed), no collective
-    st = inputs.config_states(cfg, n=n, seed=2000 + cfg + 100 * rank, e_dtype=np.float64)
+    st = inputs.config_states(cfg, n=n, seed=sharding.rank_state_seed(cfg, rank), e_dtype=np.float64)
     gm = binding.Mechanism(mech, device=local_rank)
     info = gm.info()
 
@@ -249,12 +254,9 @@ def main():
     total_ms = t_begin.elapsed_time(t_end)
     temp_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
     rates_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = sharding.max_over_ranks(total_ms, device="cuda")
     ms_per_step = total_ms / args.steps
-    value = world * n / (ms_per_step * 1e-3)
+    value = sharding.job_throughput(n, world, ms_per_step)
     not_converged = int(bad.item())
 
     # end to end through the host-buffer entry point (pinned host memory, copies inside the timed region)
@@ -270,10 +272,7 @@ def main():
             gm.source_terms_host(h["rho"], h["e"], h["Y"], h["T_guess"], T_h, om_h)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt = sharding.max_over_ranks(dt, device="cuda")
         e2e = {"value": world * n * e2e_steps / dt, "unit": "points/s",
                "h2d_bytes_per_step": int(8 * n * (ns + 3)), "d2h_bytes_per_step": int(8 * n * (ns + 1)),
                "steps": e2e_steps, "ms_per_step": 1e3 * dt / e2e_steps,
@@ -313,7 +312,10 @@ def main():
             "kernels_ms": {"temperature": temp_ms, "rates": rates_ms},
             "roofline": {
                 "bound": "alu", "kernel": "rates_kernel", "achieved": achieved_tflops, "peak": FP64_PEAK_TFLOPS,
-                "unit": "TFLOP/s", "frac": achieved_tflops / FP64_PEAK_TFLOPS, "traffic": None,
+                "unit": "TFLOP/s", "frac": achieved_tflops / FP64_PEAK_TFLOPS,
+                "traffic": NCU_RATES_DRAM_BYTES_PER_POINT_53SP * n if ns == 53 else None,
+                "traffic_note": "bytes per launch, ncu dram read + write of one profiled launch scaled by points; "
+                                "algorithmic bytes per launch = %.4g" % (bytes_pt["rates"] * n),
                 "flops_per_point": flops_pt,
                 "peak_source": "148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md); measured DFMA probe alongside",
                 "measured_dfma_tflops": measured_peak,

@@ -193,7 +193,13 @@ __global__ void __launch_bounds__(BD) temperature_kernel(const TempArgs a) {
         pt[i] = p < a.n ? p : a.n - 1;   // tail lanes recompute the last point and store nothing
     }
     const int ns = a.n_species;
+    constexpr int kAhead = 8;   // species planes prefetched into L2 ahead of the loads (the loop is latency-bound)
     for (int k = 0; k < ns; ++k) {
+        if (k + kAhead < ns && (threadIdx.x & 15) == 0) {
+#pragma unroll
+            for (int i = 0; i < PPT; ++i)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)(k + kAhead) * a.ld + pt[i]));
+        }
         double y[PPT];
 #pragma unroll
         for (int i = 0; i < PPT; ++i) y[i] = a.Y[(int64_t)k * a.ld + pt[i]];
