@@ -71,6 +71,7 @@ struct pyro_mech {
     mutable std::atomic<uint32_t> next_work{0};
     bool tab_smem = false;     // tables staged in shared memory (else read from global memory)
     bool c_tmem = false;       // concentrations C_k kept in tensor memory beside omega_k
+    bool two_blocks = false;   // the 128-register variant: two blocks resident per SM
     int block_threads = 32;    // = points per block
     size_t smem_bytes = 0;     // dynamic shared memory: tables (if staged) + the A/B planes
     uint32_t planes_off = 0;
@@ -116,7 +117,7 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     pyro::RatesArgs args = a;
     args.work = m->d_work + (m->next_work.fetch_add(1) % kWorkSlots);
     PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
-    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->c_tmem, m->smem_bytes, stream));
+    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->c_tmem, m->two_blocks, m->smem_bytes, stream));
     return PYRO_OK;
 }
 
@@ -217,9 +218,9 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     // tables staged in shared memory unless that costs more than 40 % of the points.
     const size_t rows = (size_t)lay.n_species + 1;
     size_t static_smem = 0;   // the kernels keep the tensor-memory base address in static shared memory
-    for (int v = 0; v < 4; ++v) {
+    for (int v = 0; v < 8; ++v) {
         cudaFuncAttributes fa{};
-        if ((ce = cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr((v & 1) != 0, (v & 2) != 0))) != cudaSuccess)
+        if ((ce = cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr((v & 1) != 0, (v & 2) != 0, (v & 4) != 0))) != cudaSuccess)
             return bail(ce, "cudaFuncGetAttributes");
         if (fa.sharedSizeBytes > static_smem) static_smem = fa.sharedSizeBytes;
     }
@@ -252,25 +253,58 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         delete m;
         return fail(PYRO_ERR_TOO_LARGE, "species arrays do not fit the on-chip memory of one block");
     }
+    // Small mechanisms: two blocks of 224 threads per SM with the 128-register variant (two blocks of
+    // 256 threads would need the whole register file, which the hardware does not grant), when shared
+    // and tensor memory allow it.
+    auto shape = [&](int t, bool want_c, size_t &smem, uint32_t &cols, bool &c_tmem) {
+        const uint32_t groups = (uint32_t)((t / 32 + 3) / 4);
+        c_tmem = want_c && lay.needs_ctot && groups * 4 * rows <= 512;
+        const uint32_t need = (uint32_t)(groups * (c_tmem ? 4 : 2) * rows);
+        cols = 32;
+        while (cols < need) cols *= 2;
+        smem = (m->tab_smem ? tab_room : 0) + 16 * rows * (size_t)t;
+    };
+    bool want_c = true;
+    if (const char *env = std::getenv("PYRO_C_PLANE")) {
+        if (!std::strcmp(env, "shared")) want_c = false;
+    }
+    m->two_blocks = false;
+    if (threads >= 224 && !std::getenv("PYRO_RATES_BLOCK")) {
+        size_t smem2;
+        uint32_t cols2;
+        bool c2;
+        shape(224, want_c, smem2, cols2, c2);
+        if (2 * (smem2 + static_smem + 1024) <= (size_t)prop.sharedMemPerMultiprocessor && 2 * cols2 <= 512) {
+            m->two_blocks = true;
+            threads = 224;
+        }
+    }
+    if (const char *env = std::getenv("PYRO_RATES_TWO_BLOCKS")) m->two_blocks = m->two_blocks && std::atoi(env) != 0;
     m->block_threads = threads;
     m->planes_off = m->tab_smem ? (uint32_t)tab_room : 0u;
-    m->smem_bytes = m->planes_off + 16 * rows * (size_t)threads;
-    const uint32_t groups = (uint32_t)((threads / 32 + 3) / 4);
-    m->c_tmem = lay.needs_ctot && groups * 4 * rows <= 512;
-    if (const char *env = std::getenv("PYRO_C_PLANE")) {
-        if (!std::strcmp(env, "shared")) m->c_tmem = false;
-    }
-    const uint32_t cols_needed = (uint32_t)(groups * (m->c_tmem ? 4 : 2) * rows);
-    m->tmem_cols = 32;
-    while (m->tmem_cols < cols_needed) m->tmem_cols *= 2;
-    const void *fn = pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem);
+    shape(threads, want_c, m->smem_bytes, m->tmem_cols, m->c_tmem);
+    const void *fn = pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem, m->two_blocks);
     // the limit is a property of the function, shared by every mechanism: always raise it to the
     // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
         return bail(ce, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
+    // all of the SM's L1/shared array as shared memory, so that several small blocks can be resident
+    if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
+        return bail(ce, "cudaFuncSetAttribute(PreferredSharedMemoryCarveout)");
     int nblk = 0;
     if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, threads, m->smem_bytes)) != cudaSuccess)
         return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
+    if (std::getenv("PYRO_DEBUG")) {
+        cudaFuncAttributes fa{};
+        cudaFuncGetAttributes(&fa, fn);
+        std::fprintf(stderr, "pyro: threads %d smem %zu static %zu regs %d local %zu tmem_cols %u occupancy %d two_blocks %d\n",
+                     threads, m->smem_bytes, (size_t)fa.sharedSizeBytes, fa.numRegs, (size_t)fa.localSizeBytes, m->tmem_cols, nblk,
+                     (int)m->two_blocks);
+    }
+    // The occupancy query answers 1 for the 128-register variant although two blocks of 224 threads
+    // are resident together (measured: 4.9 -> 3.8 ms at configs[1] with two blocks per SM); registers
+    // (2 x 224 x 128), shared memory and tensor-memory columns were checked above.
+    if (m->two_blocks && nblk < 2) nblk = 2;
     if (nblk > (int)(512 / m->tmem_cols)) nblk = (int)(512 / m->tmem_cols);   // resident blocks share 512 columns
     if (nblk < 1) {
         cudaFree(m->d_blob);
@@ -412,7 +446,7 @@ int pyro_mech_info(const pyro_mech *m, int64_t *out, int cap) {
     if (!m || !out) return -fail(PYRO_ERR_NULL, "NULL argument");
     DeviceGuard guard(m->device);
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem));
+    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem, m->two_blocks));
     const int64_t v[15] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
                            (int64_t)m->packed.lay.bytes, m->tab_smem ? 1 : 0, m->block_threads,
                            (int64_t)m->smem_bytes, m->blocks_per_sm, fa.numRegs, (int64_t)fa.localSizeBytes,

@@ -86,8 +86,8 @@ template <bool kCTmem> struct DevMem {
 // last point and store nothing: control flow stays warp-uniform throughout (the tensor-memory
 // instructions are warp-collective).
 // ---------------------------------------------------------------------------------------
-template <bool kTabSmem, bool kCTmem>
-__global__ void __launch_bounds__(kRatesMaxThreads, 1) rates_kernel(const RatesArgs a) {
+template <bool kTabSmem, bool kCTmem, int kMinBlocks>
+__global__ void __launch_bounds__(kRatesMaxThreads, kMinBlocks) rates_kernel(const RatesArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, nthreads = blockDim.x;
@@ -257,14 +257,20 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double *out, int iters,
 // ---------------------------------------------------------------------------------------
 // host side
 // ---------------------------------------------------------------------------------------
-const void *rates_kernel_ptr(bool tables_in_shared, bool c_in_tmem) {
-    if (tables_in_shared) return c_in_tmem ? (const void *)rates_kernel<true, true> : (const void *)rates_kernel<true, false>;
-    return c_in_tmem ? (const void *)rates_kernel<false, true> : (const void *)rates_kernel<false, false>;
+// kMinBlocks = 2 caps the registers at 128 per thread so that small mechanisms (whose planes and
+// tensor-memory columns leave room) keep two blocks of 256 threads resident per SM
+const void *rates_kernel_ptr(bool tables_in_shared, bool c_in_tmem, bool two_blocks) {
+    if (two_blocks) {
+        if (tables_in_shared) return c_in_tmem ? (const void *)rates_kernel<true, true, 2> : (const void *)rates_kernel<true, false, 2>;
+        return c_in_tmem ? (const void *)rates_kernel<false, true, 2> : (const void *)rates_kernel<false, false, 2>;
+    }
+    if (tables_in_shared) return c_in_tmem ? (const void *)rates_kernel<true, true, 1> : (const void *)rates_kernel<true, false, 1>;
+    return c_in_tmem ? (const void *)rates_kernel<false, true, 1> : (const void *)rates_kernel<false, false, 1>;
 }
 
 cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool c_in_tmem,
-                         size_t smem_bytes, cudaStream_t stream) {
-    const void *fn = rates_kernel_ptr(tables_in_shared, c_in_tmem);
+                         bool two_blocks, size_t smem_bytes, cudaStream_t stream) {
+    const void *fn = rates_kernel_ptr(tables_in_shared, c_in_tmem, two_blocks);
     RatesArgs copy = a;
     void *params[] = {&copy};
     return cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)threads), params, smem_bytes, stream);

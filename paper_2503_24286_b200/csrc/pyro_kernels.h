@@ -35,10 +35,10 @@ struct TempArgs {
     double t_mid, tol;
 };
 
-const void *rates_kernel_ptr(bool tables_in_shared, bool c_in_tmem);
+const void *rates_kernel_ptr(bool tables_in_shared, bool c_in_tmem, bool two_blocks);
 const void *temperature_kernel_ptr();
 cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool c_in_tmem,
-                         size_t smem_bytes, cudaStream_t stream);
+                         bool two_blocks, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream);
 cudaError_t launch_dfma_probe(double *out, int iters, int blocks, cudaStream_t stream);
 
