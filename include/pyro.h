@@ -122,8 +122,8 @@ int pyro_source_terms_host(pyro_mech *mech, int64_t n, int64_t ld, const double 
  *   [7] dynamic shared memory per block (bytes)  [8] resident (persistent) blocks per SM
  *   [9] registers per thread of the rates kernel  [10] local (spill) bytes per thread
  *   [11] SM count of the device  [12] grid points per thread of the rates kernel (1)
- *   [13] tensor-memory columns a block allocates  [14] 1 if the concentrations C_k are kept in
- *   tensor memory beside omega_k (else recomputed from shared memory)
+ *   [13] tensor-memory columns a block allocates  [14] 1 if B_k = 1/E_k is kept in tensor memory
+ *   beside omega_k (else in a second shared-memory plane)
  * returns the number of values written (negative pyro_status on error). */
 int pyro_mech_info(const pyro_mech *mech, int64_t *out, int cap);
 

@@ -111,7 +111,7 @@ def make_desc(mech):
 
 _INFO_KEYS = ("n_species", "n_reactions", "n_plain", "n_extended", "table_bytes", "tables_in_shared",
               "block_threads", "smem_bytes", "blocks_per_sm", "registers", "local_bytes", "sm_count",
-              "points_per_thread", "tmem_columns", "c_in_tmem")
+              "points_per_thread", "tmem_columns", "b_in_tmem")
 
 
 def _ptr(t):

@@ -70,7 +70,7 @@ struct pyro_mech {
     unsigned long long *d_work = nullptr;      // ring of chunk counters, one per launch in flight
     mutable std::atomic<uint32_t> next_work{0};
     bool tab_smem = false;     // tables staged in shared memory (else read from global memory)
-    bool c_tmem = false;       // concentrations C_k kept in tensor memory beside omega_k
+    bool b_tmem = false;       // plane B in tensor memory beside omega (else in shared memory)
     bool two_blocks = false;   // the 128-register variant: two blocks resident per SM
     int block_threads = 32;    // = points per block
     size_t smem_bytes = 0;     // dynamic shared memory: tables (if staged) + the A/B planes
@@ -117,7 +117,7 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     pyro::RatesArgs args = a;
     args.work = m->d_work + (m->next_work.fetch_add(1) % kWorkSlots);
     PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
-    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->c_tmem, m->two_blocks, m->smem_bytes, stream));
+    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->smem_bytes, stream));
     return PYRO_OK;
 }
 
@@ -211,10 +211,11 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     cudaDeviceProp prop;
     if ((ce = cudaGetDeviceProperties(&prop, device)) != cudaSuccess) return bail(ce, "cudaGetDeviceProperties");
     m->sm_count = prop.multiProcessorCount;
-    // Launch shape.  A point needs two doubles per species row in shared memory (planes A, B) and
-    // two 32-bit tensor-memory columns per row (plane W); warps share the 128 tensor-memory lanes
-    // four at a time, so a block of w warps takes ceil(w/4) column groups of 2 rows columns out of
-    // 512.  Take the most threads (a multiple of 32, at most kRatesMaxThreads) that fit, with the
+    // Launch shape.  A point needs, per species row, one double in shared memory (plane A) and four
+    // 32-bit tensor-memory columns (planes W and B); warps share the 128 tensor-memory lanes four at a
+    // time, so a block of w warps takes ceil(w/4) column groups of 4 rows columns out of 512.
+    // Mechanisms of more than 127 species keep B in a second shared-memory plane (2 columns per
+    // row).  Take the most threads (a multiple of 32, at most kRatesMaxThreads) that fit, with the
     // tables staged in shared memory unless that costs more than 40 % of the points.
     const size_t rows = (size_t)lay.n_species + 1;
     size_t static_smem = 0;   // the kernels keep the tensor-memory base address in static shared memory
@@ -226,11 +227,16 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     }
     const size_t smem_max = (size_t)prop.sharedMemPerBlockOptin - static_smem;
     const size_t tab_room = ((size_t)lay.bytes + 15) & ~(size_t)15;
+    m->b_tmem = 4 * rows <= 512;
+    if (const char *env = std::getenv("PYRO_B_PLANE")) {
+        if (!std::strcmp(env, "shared")) m->b_tmem = false;
+    }
+    const size_t smem_row = m->b_tmem ? 8 : 16, cols_row = m->b_tmem ? 4 : 2;
     auto threads_for = [&](size_t table_bytes) {
-        if (smem_max < table_bytes + 16 * rows * 32) return 0;
-        size_t t = (smem_max - table_bytes) / (16 * rows);
+        if (smem_max < table_bytes + smem_row * rows * 32) return 0;
+        size_t t = (smem_max - table_bytes) / (smem_row * rows);
         t = (t / 32) * 32;
-        const size_t groups_max = 512 / (2 * rows);
+        const size_t groups_max = 512 / (cols_row * rows);
         if (t > 128 * groups_max) t = 128 * groups_max;
         if (t > (size_t)pyro::kRatesMaxThreads) t = pyro::kRatesMaxThreads;
         return (int)t;
@@ -253,27 +259,21 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         delete m;
         return fail(PYRO_ERR_TOO_LARGE, "species arrays do not fit the on-chip memory of one block");
     }
+    auto shape = [&](int t, size_t &smem, uint32_t &cols) {
+        const uint32_t groups = (uint32_t)((t / 32 + 3) / 4);
+        const uint32_t need = (uint32_t)(groups * cols_row * rows);
+        cols = 32;
+        while (cols < need) cols *= 2;
+        smem = (m->tab_smem ? tab_room : 0) + smem_row * rows * (size_t)t;
+    };
     // Small mechanisms: two blocks of 224 threads per SM with the 128-register variant (two blocks of
     // 256 threads would need the whole register file, which the hardware does not grant), when shared
     // and tensor memory allow it.
-    auto shape = [&](int t, bool want_c, size_t &smem, uint32_t &cols, bool &c_tmem) {
-        const uint32_t groups = (uint32_t)((t / 32 + 3) / 4);
-        c_tmem = want_c && lay.needs_ctot && groups * 4 * rows <= 512;
-        const uint32_t need = (uint32_t)(groups * (c_tmem ? 4 : 2) * rows);
-        cols = 32;
-        while (cols < need) cols *= 2;
-        smem = (m->tab_smem ? tab_room : 0) + 16 * rows * (size_t)t;
-    };
-    bool want_c = true;
-    if (const char *env = std::getenv("PYRO_C_PLANE")) {
-        if (!std::strcmp(env, "shared")) want_c = false;
-    }
     m->two_blocks = false;
     if (threads >= 224 && !std::getenv("PYRO_RATES_BLOCK")) {
         size_t smem2;
         uint32_t cols2;
-        bool c2;
-        shape(224, want_c, smem2, cols2, c2);
+        shape(224, smem2, cols2);
         if (2 * (smem2 + static_smem + 1024) <= (size_t)prop.sharedMemPerMultiprocessor && 2 * cols2 <= 512) {
             m->two_blocks = true;
             threads = 224;
@@ -282,8 +282,8 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (const char *env = std::getenv("PYRO_RATES_TWO_BLOCKS")) m->two_blocks = m->two_blocks && std::atoi(env) != 0;
     m->block_threads = threads;
     m->planes_off = m->tab_smem ? (uint32_t)tab_room : 0u;
-    shape(threads, want_c, m->smem_bytes, m->tmem_cols, m->c_tmem);
-    const void *fn = pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem, m->two_blocks);
+    shape(threads, m->smem_bytes, m->tmem_cols);
+    const void *fn = pyro::rates_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks);
     // the limit is a property of the function, shared by every mechanism: always raise it to the
     // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
@@ -446,11 +446,11 @@ int pyro_mech_info(const pyro_mech *m, int64_t *out, int cap) {
     if (!m || !out) return -fail(PYRO_ERR_NULL, "NULL argument");
     DeviceGuard guard(m->device);
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem, m->c_tmem, m->two_blocks));
+    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks));
     const int64_t v[15] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
                            (int64_t)m->packed.lay.bytes, m->tab_smem ? 1 : 0, m->block_threads,
                            (int64_t)m->smem_bytes, m->blocks_per_sm, fa.numRegs, (int64_t)fa.localSizeBytes,
-                           m->sm_count, 1, (int64_t)m->tmem_cols, m->c_tmem ? 1 : 0};
+                           m->sm_count, 1, (int64_t)m->tmem_cols, m->b_tmem ? 1 : 0};
     int cnt = cap < 15 ? cap : 15;
     for (int i = 0; i < cnt; ++i) out[i] = v[i];
     return cnt;

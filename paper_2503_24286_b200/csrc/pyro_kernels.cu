@@ -3,14 +3,14 @@
 // Thread mapping: one thread per grid point, a warp reads 256
 // contiguous bytes of every species plane of the SoA fields.  Per-point arrays that are
 // indexed by a run-time species number live on chip (pyro_tables.h, pyro_point.cuh):
-//   A_k = C_k E_k and B_k = 1/E_k in shared memory as [k][plane][thread] columns (conflict-free:
-//   lane l touches its own banks), read-only while the reactions run;
-//   omega_k in TENSOR MEMORY: thread t of a warp owns lane 32 (warp % 4) + t, species k is the
-//   pair of 32-bit columns 2k, 2k+1 of that warp's column group; C_k (read by the third-body
-//   sums only) in a second set of columns when they fit.  The stoichiometric
-//   accumulation is tcgen05.ld / add / tcgen05.st on warp-uniform column addresses, which
-//   takes the read-modify-write traffic (8 of the 14 indexed accesses of a reaction) off the
-//   shared-memory pipe and doubles the points resident per SM.
+//   A_k = C_k E_k in shared memory as [k][thread] columns (conflict-free: lane l touches its own
+//   banks), read-only while the reactions run;
+//   omega_k and B_k = 1/E_k in TENSOR MEMORY: thread t of a warp owns lane 32 (warp % 4) + t,
+//   species k is the four 32-bit columns 4k .. 4k+3 of that warp's column group (omega_k, B_k).
+//   The stoichiometric accumulation is tcgen05.ld / add / tcgen05.st on warp-uniform column
+//   addresses, which takes the read-modify-write traffic and the B loads (10 of the 14 indexed
+//   accesses of a reaction) off the shared-memory pipe and lets 256 points (8 warps) be
+//   resident per SM for the 53-species mechanism.
 // The mechanism tables are staged once per block into shared memory and read with 128-bit
 // loads at warp-uniform addresses; blocks are persistent (one per SM for the 53-species
 // mechanism) and walk the tiles of points.
@@ -32,52 +32,77 @@ struct DevTab {
     __device__ __forceinline__ const EffEntry &eff(int q) const { return reinterpret_cast<const EffEntry *>(base + off_eff)[q]; }
 };
 
-// On-chip planes of one thread.  Shared memory: species k of plane A is the double at
-// baseA + k stride (stride = 16 bytes x threads per block), plane B the one at baseB + k stride.
-// Tensor memory: species k is the column pair tw + 2k of the thread's lane.  All accesses are
-// volatile asm, so they keep their program order.
-template <bool kCTmem> struct DevMem {
+// On-chip planes of one thread.
+//   Shared memory: species k of plane A is the double at baseA + k strideA (strideA = 8 bytes x
+//   threads per block).
+//   Tensor memory, kBTmem: species k is the four 32-bit columns tw + 4k .. 4k+3 of the thread's
+//   lane, omega_k in the first pair and B_k in the second, so a reactant slot fetches both with
+//   one LDTM.x4.  Very large mechanisms (!kBTmem: more than 127 species) keep B in a second
+//   shared-memory plane and omega alone in tensor memory (columns tw + 2k).
+// All accesses are volatile asm, so they keep their program order.
+template <bool kBTmem> struct DevMem {
     struct WRaw {
         uint32_t lo, hi;
     };
-    uint32_t baseA, baseB, stride, tw, tc;
+    struct WBRaw {
+        uint32_t wlo, whi, blo, bhi;
+    };
+    uint32_t baseA, baseB, strideA, tw;
 
-    __device__ __forceinline__ uint32_t atA(uint32_t k) const { return baseA + k * stride; }
-    __device__ __forceinline__ uint32_t atB(uint32_t k) const { return baseB + k * stride; }
-    __device__ __forceinline__ uint32_t atW(uint32_t k) const { return tw + 2u * k; }
-    __device__ __forceinline__ double ldA(uint32_t h) const {
+    __device__ __forceinline__ uint32_t atA(uint32_t k) const { return baseA + k * strideA; }
+    __device__ __forceinline__ uint32_t atB(uint32_t k) const { return kBTmem ? 0u : baseB + k * strideA; }
+    __device__ __forceinline__ uint32_t atW(uint32_t k) const { return tw + (kBTmem ? 4u : 2u) * k; }
+    __device__ __forceinline__ double lds(uint32_t h) const {
         double v;
         asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(h));
         return v;
     }
-    __device__ __forceinline__ double ldB(uint32_t h) const { return ldA(h); }
-    __device__ __forceinline__ void stA(uint32_t h, double v) const { asm volatile("st.shared.f64 [%0], %1;" ::"r"(h), "d"(v)); }
-    __device__ __forceinline__ void stB(uint32_t h, double v) const { stA(h, v); }
-    __device__ __forceinline__ WRaw ldW(uint32_t h) const {
+    __device__ __forceinline__ void sts(uint32_t h, double v) const { asm volatile("st.shared.f64 [%0], %1;" ::"r"(h), "d"(v)); }
+    __device__ __forceinline__ double ldA(uint32_t h) const { return lds(h); }
+    __device__ __forceinline__ WRaw ldtm2(uint32_t t) const {
         WRaw r;
-        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r.lo), "=r"(r.hi) : "r"(h));
+        asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r.lo), "=r"(r.hi) : "r"(t));
         return r;
     }
-    // plane C: tensor memory when its columns fit beside plane W, else recomputed as A_k B_k
-    __device__ __forceinline__ uint32_t atC(uint32_t k) const { return kCTmem ? tc + 2u * k : k; }
-    __device__ __forceinline__ WRaw ldC(uint32_t h) const {
-        if (kCTmem) return ldW(h);
-        const double c = ldA(atA(h)) * ldB(atB(h));
-        return WRaw{(uint32_t)__double2loint(c), (uint32_t)__double2hiint(c)};
+    __device__ __forceinline__ WRaw ldW(uint32_t hW) const { return ldtm2(hW); }
+    __device__ __forceinline__ WRaw ldB(uint32_t hW, uint32_t hB) const {
+        if (kBTmem) return ldtm2(hW + 2u);
+        const double b = lds(hB);
+        return WRaw{(uint32_t)__double2loint(b), (uint32_t)__double2hiint(b)};
     }
-    __device__ __forceinline__ void stC(uint32_t h, double v) const {
-        if (kCTmem) stW(h, v);
+    __device__ __forceinline__ WBRaw ldWB(uint32_t hW, uint32_t hB) const {
+        WBRaw r;
+        if (kBTmem) {
+            asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0, %1, %2, %3}, [%4];"
+                         : "=r"(r.wlo), "=r"(r.whi), "=r"(r.blo), "=r"(r.bhi)
+                         : "r"(hW));
+        } else {
+            const WRaw w = ldtm2(hW);
+            const double b = lds(hB);
+            r = WBRaw{w.lo, w.hi, (uint32_t)__double2loint(b), (uint32_t)__double2hiint(b)};
+        }
+        return r;
     }
-    __device__ __forceinline__ void stW(uint32_t h, double v) const {
-        asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(h), "r"(__double2loint(v)), "r"(__double2hiint(v)));
+    __device__ __forceinline__ void stW(uint32_t hW, double v) const {
+        asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1, %2};" ::"r"(hW), "r"(__double2loint(v)), "r"(__double2hiint(v)));
     }
-    // the loaded registers are defined only after the wait (ptxas turns it into the scoreboard wait of
-    // the LDTMs); value() is only called after the fence
-    template <int N> __device__ __forceinline__ void fence_ldW(WRaw (&)[N]) const {
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+    __device__ __forceinline__ void st_species(uint32_t k, double a, double b) const {
+        sts(atA(k), a);
+        if (kBTmem) {
+            asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1, %2, %3, %4};" ::"r"(atW(k)), "r"(0), "r"(0),
+                         "r"(__double2loint(b)), "r"(__double2hiint(b)));
+        } else {
+            sts(atB(k), b);
+            stW(atW(k), 0.0);
+        }
     }
-    __device__ __forceinline__ void fence_stW() const { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+    // the registers of a tensor-memory load are defined only after the wait (ptxas turns it into the
+    // scoreboard wait of the LDTMs); the value functions are only called after it
+    __device__ __forceinline__ void fence_ld() const { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+    __device__ __forceinline__ void fence_st() const { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
     __device__ __forceinline__ double value(const WRaw &r) const { return __hiloint2double((int)r.hi, (int)r.lo); }
+    __device__ __forceinline__ double value_w(const WBRaw &r) const { return __hiloint2double((int)r.whi, (int)r.wlo); }
+    __device__ __forceinline__ double value_b(const WBRaw &r) const { return __hiloint2double((int)r.bhi, (int)r.blo); }
 };
 
 // ---------------------------------------------------------------------------------------
@@ -86,7 +111,7 @@ template <bool kCTmem> struct DevMem {
 // last point and store nothing: control flow stays warp-uniform throughout (the tensor-memory
 // instructions are warp-collective).
 // ---------------------------------------------------------------------------------------
-template <bool kTabSmem, bool kCTmem, int kMinBlocks>
+template <bool kTabSmem, bool kBTmem, int kMinBlocks>
 __global__ void __launch_bounds__(kRatesMaxThreads, kMinBlocks) rates_kernel(const RatesArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_tmem_base;
@@ -112,12 +137,11 @@ __global__ void __launch_bounds__(kRatesMaxThreads, kMinBlocks) rates_kernel(con
     DevTab tab{kTabSmem ? smem_raw : a.gtab, a.off_spec, a.off_rxn_p, a.off_rxn_x, a.off_fall, a.off_eff};
     const uint32_t planes = (uint32_t)__cvta_generic_to_shared(smem_raw) + a.planes_off;
     const uint32_t rows = (uint32_t)ns + 1u;
-    DevMem<kCTmem> mem;
-    mem.stride = 16u * (uint32_t)nthreads;
+    DevMem<kBTmem> mem;
+    mem.strideA = 8u * (uint32_t)nthreads;
     mem.baseA = planes + 8u * (uint32_t)tid;
-    mem.baseB = mem.baseA + 8u * (uint32_t)nthreads;
-    mem.tw = tmem_base + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * (kCTmem ? 4u : 2u) * rows;
-    mem.tc = mem.tw + 2u * rows;
+    mem.baseB = mem.baseA + rows * mem.strideA;   // second plane, used when B is not in tensor memory
+    mem.tw = tmem_base + (((uint32_t)(warp & 3) * 32u) << 16) + (uint32_t)(warp >> 2) * (kBTmem ? 4u : 2u) * rows;
 
     // Warps are independent (own shared-memory columns, own tensor-memory lanes): each takes the
     // next chunk of 32 consecutive points from a device-wide counter until none is left, which
@@ -148,10 +172,10 @@ __global__ void __launch_bounds__(kRatesMaxThreads, kMinBlocks) rates_kernel(con
         int k = 0;
 #pragma unroll 1
         for (; k + 4 <= ns; k += 4) {
-            typename DevMem<kCTmem>::WRaw r[4];
+            typename DevMem<kBTmem>::WRaw r[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) r[i] = mem.ldW(mem.atW((uint32_t)(k + i)));
-            mem.template fence_ldW<4>(r);
+            mem.fence_ld();
             if (p < a.n) {
 #pragma unroll
                 for (int i = 0; i < 4; ++i) Wp[(int64_t)(k + i) * a.ld] = mem.value(r[i]);
@@ -159,9 +183,9 @@ __global__ void __launch_bounds__(kRatesMaxThreads, kMinBlocks) rates_kernel(con
         }
 #pragma unroll 1
         for (; k < ns; ++k) {
-            typename DevMem<kCTmem>::WRaw r[1];
+            typename DevMem<kBTmem>::WRaw r[1];
             r[0] = mem.ldW(mem.atW((uint32_t)k));
-            mem.template fence_ldW<1>(r);
+            mem.fence_ld();
             if (p < a.n) Wp[(int64_t)k * a.ld] = mem.value(r[0]);
         }
         chunk = next;
@@ -259,18 +283,18 @@ __global__ void __launch_bounds__(256) dfma_probe_kernel(double *out, int iters,
 // ---------------------------------------------------------------------------------------
 // kMinBlocks = 2 caps the registers at 128 per thread so that small mechanisms (whose planes and
 // tensor-memory columns leave room) keep two blocks of 256 threads resident per SM
-const void *rates_kernel_ptr(bool tables_in_shared, bool c_in_tmem, bool two_blocks) {
+const void *rates_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks) {
     if (two_blocks) {
-        if (tables_in_shared) return c_in_tmem ? (const void *)rates_kernel<true, true, 2> : (const void *)rates_kernel<true, false, 2>;
-        return c_in_tmem ? (const void *)rates_kernel<false, true, 2> : (const void *)rates_kernel<false, false, 2>;
+        if (tables_in_shared) return b_in_tmem ? (const void *)rates_kernel<true, true, 2> : (const void *)rates_kernel<true, false, 2>;
+        return b_in_tmem ? (const void *)rates_kernel<false, true, 2> : (const void *)rates_kernel<false, false, 2>;
     }
-    if (tables_in_shared) return c_in_tmem ? (const void *)rates_kernel<true, true, 1> : (const void *)rates_kernel<true, false, 1>;
-    return c_in_tmem ? (const void *)rates_kernel<false, true, 1> : (const void *)rates_kernel<false, false, 1>;
+    if (tables_in_shared) return b_in_tmem ? (const void *)rates_kernel<true, true, 1> : (const void *)rates_kernel<true, false, 1>;
+    return b_in_tmem ? (const void *)rates_kernel<false, true, 1> : (const void *)rates_kernel<false, false, 1>;
 }
 
-cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool c_in_tmem,
+cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem,
                          bool two_blocks, size_t smem_bytes, cudaStream_t stream) {
-    const void *fn = rates_kernel_ptr(tables_in_shared, c_in_tmem, two_blocks);
+    const void *fn = rates_kernel_ptr(tables_in_shared, b_in_tmem, two_blocks);
     RatesArgs copy = a;
     void *params[] = {&copy};
     return cudaLaunchKernel(fn, dim3((unsigned)blocks), dim3((unsigned)threads), params, smem_bytes, stream);

@@ -18,7 +18,7 @@ struct RatesArgs {
     double *omega;
     const unsigned char *gtab;   // device copy of the table blob in global memory
     uint32_t tab_bytes;          // blob size (a multiple of 16)
-    uint32_t planes_off;         // byte offset of the A/B planes in dynamic shared memory
+    uint32_t planes_off;         // byte offset of the A (and B) planes in dynamic shared memory
     uint32_t tmem_cols;          // tensor-memory columns the block allocates (a power of two >= 32)
     uint32_t off_spec, off_rxn_p, off_rxn_x, off_fall, off_eff;
     int32_t n_species;
@@ -35,9 +35,9 @@ struct TempArgs {
     double t_mid, tol;
 };
 
-const void *rates_kernel_ptr(bool tables_in_shared, bool c_in_tmem, bool two_blocks);
+const void *rates_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks);
 const void *temperature_kernel_ptr();
-cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool c_in_tmem,
+cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem,
                          bool two_blocks, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream);
 cudaError_t launch_dfma_probe(double *out, int iters, int blocks, cudaStream_t stream);

@@ -8,8 +8,8 @@
 
 namespace pyro {
 
-// Limits of the on-chip staging: two FP64 planes of n_species + 1 values per point in shared
-// memory and one in tensor memory (512 32-bit columns per thread at most).
+// Limits of the on-chip staging: per point n_species + 1 values of plane W in tensor memory (512
+// 32-bit columns per thread at most) and of planes A, B in shared / tensor memory.
 constexpr int kMaxSpecies = 255;
 constexpr int kMaxReactions = 1 << 20;
 

@@ -2,15 +2,16 @@
 //
 // One thread owns one grid point.  Per-point arrays indexed by a run-time species number live
 // on chip as three planes per species:
-//     plane A  A_k = C_k E_k      plane B  B_k = 1/E_k      plane W  omega_k      plane C  C_k
-// with E_k = exp(g_k/RT) RT/p0 (pyro_tables.h); C_k is read by the third-body sums only.  The
-// functions below reach them through a `Mem` accessor (A and B in shared memory, W and C in
-// tensor memory in the kernels, plain arrays in the host build):
-//     h = mem.atA(k), mem.atB(k), mem.atW(k), mem.atC(k)   handle of species k for this thread
-//     mem.ldA(h), mem.ldB(h), mem.stA(h, v), mem.stB(h, v)
-//     r = mem.ldW(h), mem.ldC(h)   raw value; becomes readable by mem.value(r) only after
-//     mem.fence_ldW(raws)          (tensor-memory loads are asynchronous)
-//     mem.stW(h, v), mem.stC(h, v); mem.fence_stW() before a later load may see the stored value
+//     plane A  A_k = C_k E_k      plane B  B_k = 1/E_k      plane W  omega_k
+// with E_k = exp(g_k/RT) RT/p0 (pyro_tables.h).  The functions below reach them through a
+// `Mem` accessor (A in shared memory, W and B side by side in tensor memory in the kernels --
+// or B in shared memory for very large mechanisms -- plain arrays in the host build):
+//     hA = mem.atA(k), hW = mem.atW(k), hB = mem.atB(k)    handles of species k for this thread
+//     mem.ldA(hA)
+//     r = mem.ldW(hW), mem.ldB(hW, hB), mem.ldWB(hW, hB)   raw values; readable by mem.value(r),
+//         mem.value_w(r), mem.value_b(r) only after mem.fence_ld()   (tensor-memory loads are asynchronous)
+//     mem.stW(hW, v); mem.fence_st() before a later load may see the stored value
+//     mem.st_species(k, a, b)                              fill: A_k = a, B_k = b, omega_k = 0
 #pragma once
 #include "../../include/pyro.h"
 #include "pyro_math.cuh"
@@ -67,10 +68,7 @@ PYRO_HD void species_planes(const Tab &tab, int k0, const PointT &pt, double rho
 #pragma unroll
     for (int i = 0; i < NK; ++i) {
         ctot += C[i];
-        mem.stA(mem.atA((uint32_t)(k0 + i)), C[i] * e[i]);
-        mem.stB(mem.atB((uint32_t)(k0 + i)), b[i]);
-        mem.stW(mem.atW((uint32_t)(k0 + i)), 0.0);
-        mem.stC(mem.atC((uint32_t)(k0 + i)), C[i]);
+        mem.st_species((uint32_t)(k0 + i), C[i] * e[i], b[i]);
     }
 }
 
@@ -111,42 +109,44 @@ PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT &pt
             }
             y[b] = arrhenius_log2(r.f[0], r.f[1], r.f[2], pt.L2T, pt.invT);
         }
-        mem.fence_stW();
-        typename Mem::WRaw wr[NB * NS];
-#pragma unroll
-        for (int b = 0; b < NB; ++b)
-#pragma unroll
-            for (int m = 0; m < NS; ++m) wr[b * NS + m] = mem.ldW(hW[b][m]);
-        double a[NB][NS], bb[NB][NR];
-#pragma unroll
-        for (int b = 0; b < NB; ++b)
-#pragma unroll
-            for (int m = 0; m < NS; ++m) {
-                a[b][m] = mem.ldA(hA[b][m]);
-                if (m < NR) bb[b][m] = mem.ldB(hB[b][m]);
-            }
-        exp2_poly_n<NB>(y);
-        double R[NB];
+        mem.fence_st();
+        typename Mem::WBRaw wbr[NB][NR];   // reactants: omega and B together
+        typename Mem::WRaw wr[NB][NP];     // products: omega
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            double pf = a[b][0], pb = bb[b][0], pr = a[b][NR];
 #pragma unroll
-            for (int m = 1; m < NR; ++m) {
-                pf *= a[b][m];
-                pb *= bb[b][m];
-            }
+            for (int m = 0; m < NR; ++m) wbr[b][m] = mem.ldWB(hW[b][m], hB[b][m]);
 #pragma unroll
-            for (int m = 1; m < NP; ++m) pr *= a[b][NR + m];
-            R[b] = (y[b] * pb) * (pf - pr);
+            for (int m = 0; m < NP; ++m) wr[b][m] = mem.ldW(hW[b][NR + m]);
         }
-        mem.template fence_ldW<NB * NS>(wr);
+        double a[NB][NS];
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
-            for (int m = 0; m < NS; ++m) {
-                const double w = mem.value(wr[b * NS + m]);
-                mem.stW(hW[b][m], m < NR ? w - R[b] : w + R[b]);
-            }
+            for (int m = 0; m < NS; ++m) a[b][m] = mem.ldA(hA[b][m]);
+        exp2_poly_n<NB>(y);
+        double pd[NB];   // k_f (prod_reac A - prod_prod A)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            double pf = a[b][0], pr = a[b][NR];
+#pragma unroll
+            for (int m = 1; m < NR; ++m) pf *= a[b][m];
+#pragma unroll
+            for (int m = 1; m < NP; ++m) pr *= a[b][NR + m];
+            pd[b] = y[b] * (pf - pr);
+        }
+        mem.fence_ld();
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            double pb = mem.value_b(wbr[b][0]);
+#pragma unroll
+            for (int m = 1; m < NR; ++m) pb *= mem.value_b(wbr[b][m]);
+            const double R = pb * pd[b];
+#pragma unroll
+            for (int m = 0; m < NR; ++m) mem.stW(hW[b][m], mem.value_w(wbr[b][m]) - R);
+#pragma unroll
+            for (int m = 0; m < NP; ++m) mem.stW(hW[b][NR + m], mem.value(wr[b][m]) + R);
+        }
     }
 }
 
@@ -170,7 +170,7 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
     constexpr int NE = KIND == kExtTroe ? 5 : (KIND == kExtLindemann ? 2 : 1);   // exponentials per reaction
 #pragma unroll 1
     for (int j = j0; j < j0 + count; j += NB) {
-        uint32_t hA[NB][6], hB[NB][3], hW[NB][6];
+        uint32_t hA[NB][6], hB[NB][3], hWs[NB][3], hW[NB][6];   // hWs: tensor-memory handle of a reactant slot (its B)
         double nu[NB][6], rev[NB], M[NB], alpha[NB], has_t2[NB];
         double y[NB * NE];
         uint32_t q0[NB], nq = 0;
@@ -183,7 +183,10 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
 #pragma unroll
             for (int m = 0; m < 6; ++m) {
                 hA[b][m] = mem.atA(slot[m]);
-                if (m < 3) hB[b][m] = mem.atB(slot[m]);
+                if (m < 3) {
+                    hB[b][m] = mem.atB(slot[m]);
+                    hWs[b][m] = mem.atW(slot[m]);
+                }
                 hW[b][m] = mem.atW(sc[m]);
                 nu[b][m] = (double)x.sc_nu[m];
             }
@@ -204,40 +207,41 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
                 }
             }
         }
-        mem.fence_stW();
-        typename Mem::WRaw wr[NB * 6];
-#pragma unroll
-        for (int b = 0; b < NB; ++b)
-#pragma unroll
-            for (int m = 0; m < 6; ++m) wr[b * 6 + m] = mem.ldW(hW[b][m]);
-        double a[NB][6], bb[NB][3];
+        mem.fence_st();
+        typename Mem::WRaw wr[NB][6], br[NB][3];
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
             for (int m = 0; m < 6; ++m) {
-                a[b][m] = mem.ldA(hA[b][m]);
-                if (m < 3) bb[b][m] = mem.ldB(hB[b][m]);
+                wr[b][m] = mem.ldW(hW[b][m]);
+                if (m < 3) br[b][m] = mem.ldB(hWs[b][m], hB[b][m]);
             }
+        double a[NB][6];
+#pragma unroll
+        for (int b = 0; b < NB; ++b)
+#pragma unroll
+            for (int m = 0; m < 6; ++m) a[b][m] = mem.ldA(hA[b][m]);
         if (KIND != kExtGeneral) {
-            // [M] = sum_k eff_k C_k = eff_default C_tot + sum_listed (eff_k - eff_default) C_k; the lists of
-            // a group are padded to one length, a multiple of four
+            // [M] = sum_k eff_k C_k = eff_default C_tot + sum_listed (eff_k - eff_default) C_k with
+            // C_k = A_k B_k; the lists of a group are padded to one length, a multiple of four
 #pragma unroll 1
             for (uint32_t q = 0; q < nq; q += 4) {
-                typename Mem::WRaw cr[NB * 4];
-                double dl[NB * 4];
+                typename Mem::WRaw cb[NB * 4];
+                double dl[NB * 4], ca[NB * 4];
 #pragma unroll
                 for (int b = 0; b < NB; ++b)
 #pragma unroll
                     for (int u = 0; u < 4; ++u) {
                         const EffEntry &en = tab.eff((int)(q0[b] + q) + u);
-                        cr[b * 4 + u] = mem.ldC(mem.atC(en.species));
+                        cb[b * 4 + u] = mem.ldB(mem.atW(en.species), mem.atB(en.species));
+                        ca[b * 4 + u] = mem.ldA(mem.atA(en.species));
                         dl[b * 4 + u] = en.delta;
                     }
-                mem.template fence_ldW<NB * 4>(cr);
+                mem.fence_ld();
 #pragma unroll
                 for (int b = 0; b < NB; ++b)
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) M[b] = fma(dl[b * 4 + u], mem.value(cr[b * 4 + u]), M[b]);
+                    for (int u = 0; u < 4; ++u) M[b] = fma(dl[b * 4 + u], ca[b * 4 + u] * mem.value(cb[b * 4 + u]), M[b]);
             }
         }
         exp2_poly_n<NB * NE>(y);
@@ -271,20 +275,17 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
                 for (int b = 0; b < NB; ++b) fall[b] *= z[b];
             }
         }
-        double R[NB];
+        mem.fence_ld();
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             const double pf = a[b][0] * a[b][1] * a[b][2];
             const double pr = rev[b] != 0.0 ? a[b][3] * a[b][4] * a[b][5] : 0.0;   // irreversible: r_r = 0 (G19)
-            const double pb = bb[b][0] * bb[b][1] * bb[b][2];
-            R[b] = (y[b * NE] * pb) * (pf - pr) * fall[b];
-            if (KIND == kExtThreeBody) R[b] *= M[b];   // R = [M](q_f - q_r), reading G8
+            const double pb = mem.value(br[b][0]) * mem.value(br[b][1]) * mem.value(br[b][2]);
+            double R = (y[b * NE] * pb) * (pf - pr) * fall[b];
+            if (KIND == kExtThreeBody) R *= M[b];   // R = [M](q_f - q_r), reading G8
+#pragma unroll
+            for (int m = 0; m < 6; ++m) mem.stW(hW[b][m], fma(nu[b][m], R, mem.value(wr[b][m])));
         }
-        mem.template fence_ldW<NB * 6>(wr);
-#pragma unroll
-        for (int b = 0; b < NB; ++b)
-#pragma unroll
-            for (int m = 0; m < 6; ++m) mem.stW(hW[b][m], fma(nu[b][m], R[b], mem.value(wr[b * 6 + m])));
     }
 }
 
@@ -318,7 +319,7 @@ PYRO_HD void accumulate_reactions(const Tab &tab, const GroupCounts &g, const Po
     x = extended_kind<kExtThreeBody>(tab, x, g.ext_g4[1], g.ext_g2[1], pt, ctot, mem);
     x = extended_kind<kExtLindemann>(tab, x, g.ext_g4[2], g.ext_g2[2], pt, ctot, mem);
     x = extended_kind<kExtTroe>(tab, x, g.ext_g4[3], g.ext_g2[3], pt, ctot, mem);
-    mem.fence_stW();
+    mem.fence_st();
 }
 
 // Rows a2, a3 for every species, then the dummy species (A = B = 1, omega = sink): fills the
@@ -337,32 +338,35 @@ PYRO_HD double fill_planes(const Tab &tab, int ns, const PointT &pt, double rho,
         const double y[1] = {load_y(k)};
         species_planes<1>(tab, k, pt, rho, y, ctot, mem);
     }
-    mem.stA(mem.atA((uint32_t)ns), 1.0);
-    mem.stB(mem.atB((uint32_t)ns), 1.0);
-    mem.stW(mem.atW((uint32_t)ns), 0.0);
-    mem.stC(mem.atC((uint32_t)ns), 0.0);
+    mem.st_species((uint32_t)ns, 1.0, 1.0);
     return ctot;
 }
 
 // Plain arrays of n_species + 1 entries per plane (host build, tests).
 struct ArrayMem {
     typedef double WRaw;
-    double *A, *B, *W, *C;
+    struct WBRaw {
+        double w, b;
+    };
+    double *A, *B, *W;
     PYRO_HD uint32_t atA(uint32_t k) const { return k; }
-    PYRO_HD uint32_t atC(uint32_t k) const { return k; }
-    PYRO_HD WRaw ldC(uint32_t h) const { return C[h]; }
-    PYRO_HD void stC(uint32_t h, double v) const { C[h] = v; }
     PYRO_HD uint32_t atB(uint32_t k) const { return k; }
     PYRO_HD uint32_t atW(uint32_t k) const { return k; }
     PYRO_HD double ldA(uint32_t h) const { return A[h]; }
-    PYRO_HD double ldB(uint32_t h) const { return B[h]; }
-    PYRO_HD void stA(uint32_t h, double v) const { A[h] = v; }
-    PYRO_HD void stB(uint32_t h, double v) const { B[h] = v; }
     PYRO_HD WRaw ldW(uint32_t h) const { return W[h]; }
+    PYRO_HD WRaw ldB(uint32_t, uint32_t hB) const { return B[hB]; }
+    PYRO_HD WBRaw ldWB(uint32_t hW, uint32_t hB) const { return WBRaw{W[hW], B[hB]}; }
     PYRO_HD void stW(uint32_t h, double v) const { W[h] = v; }
-    template <int N> PYRO_HD void fence_ldW(WRaw (&)[N]) const {}
-    PYRO_HD void fence_stW() const {}
+    PYRO_HD void st_species(uint32_t k, double a, double b) const {
+        A[k] = a;
+        B[k] = b;
+        W[k] = 0.0;
+    }
+    PYRO_HD void fence_ld() const {}
+    PYRO_HD void fence_st() const {}
     PYRO_HD double value(WRaw r) const { return r; }
+    PYRO_HD double value_w(const WBRaw &r) const { return r.w; }
+    PYRO_HD double value_b(const WBRaw &r) const { return r.b; }
 };
 
 // Newton iteration on the mixture energy polynomial (row a4): (A.27)-(A.28) PAPER.md:1017-1021,

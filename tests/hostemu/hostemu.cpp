@@ -91,10 +91,10 @@ int emu_rates(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho,
     HostTab tab{pm.blob.data(), pm.lay};
     const pyro::GroupCounts g = group_counts(pm.lay);
     const int ns = pm.n_species;
-    std::vector<double> A(ns + 1), B(ns + 1), W(ns + 1), Cc(ns + 1);   // + the dummy species
+    std::vector<double> A(ns + 1), B(ns + 1), W(ns + 1);   // + the dummy species
     for (int64_t p = 0; p < n; ++p) {
         const pyro::PointT pt = pyro::make_point(T[p]);
-        const pyro::ArrayMem mem{A.data(), B.data(), W.data(), Cc.data()};
+        const pyro::ArrayMem mem{A.data(), B.data(), W.data()};
         const double ctot = pyro::fill_planes(tab, ns, pt, rho[p], mem, [&](int k) { return Y[k * ld + p]; });
         pyro::accumulate_reactions(tab, g, pt, ctot, mem);
         for (int k = 0; k < ns; ++k) omega[k * ld + p] = W[k];

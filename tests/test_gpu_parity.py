@@ -238,7 +238,7 @@ def test_tables_in_global_memory_path(mechs, monkeypatch):
         parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
 
 
-@pytest.mark.parametrize("cfg,block", [(2, 32), (2, 64), (2, 96), (2, 160), (2, 192), (0, 32), (0, 128), (0, 256),
+@pytest.mark.parametrize("cfg,block", [(2, 32), (2, 64), (2, 96), (2, 160), (2, 256), (0, 32), (0, 128), (0, 256),
                                        (3, 32), (3, 64)])
 def test_every_block_size(mechs, monkeypatch, cfg, block):
     """Threads (= points) per block of the rates kernel, forced: 1 to 8 warps, i.e. one and two
@@ -248,10 +248,23 @@ def test_every_block_size(mechs, monkeypatch, cfg, block):
     gm = binding.Mechanism(mech)
     info = gm.info()
     assert info["block_threads"] == block
-    assert info["tmem_columns"] >= ((block // 32 + 3) // 4) * 2 * (mech.n_species + 1)
+    assert info["tmem_columns"] >= ((block // 32 + 3) // 4) * (4 if info["b_in_tmem"] else 2) * (mech.n_species + 1)
     for n in (777, 2 * block + 1, info["sm_count"] * info["blocks_per_sm"] * block + 5 * block + 3):
         if cfg == 3 and n > 3000:
             n = 3001
+        st = inputs.config_states(cfg, n=n)
+        om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
+        parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
+
+
+def test_plane_b_in_shared_memory_path(mechs, monkeypatch):
+    """Mechanisms of more than 127 species keep plane B in shared memory (two tensor-memory columns
+    per species instead of four); here that variant is forced for configs[0], [2] and [3]."""
+    monkeypatch.setenv("PYRO_B_PLANE", "shared")
+    for cfg, n in ((0, 3000), (2, 1111), (3, 300)):
+        mech, _, orc = mechs(cfg)
+        gm = binding.Mechanism(mech)
+        assert gm.info()["b_in_tmem"] == 0
         st = inputs.config_states(cfg, n=n)
         om_ref, bound = orc.get_net_production_rates(st["rho"], st["T"], st["Y"])
         parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
