@@ -53,6 +53,15 @@ def _load():
         for sfx, real in (("f64", C.c_double), ("f80", C.c_longdouble)):
             getattr(_lib, f"oracle_mixture_e_{sfx}").restype = real
             getattr(_lib, f"oracle_mixture_cv_{sfx}").restype = real
+            for nm in ("mixture_h", "mixture_cp"):
+                getattr(_lib, f"oracle_{nm}_{sfx}").restype = real
+                getattr(_lib, f"oracle_{nm}_{sfx}").argtypes = [C.c_void_p, real, C.c_void_p]
+            getattr(_lib, f"oracle_get_temperature_h_{sfx}").argtypes = [
+                C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, real, C.c_int,
+                C.c_void_p, C.c_void_p, C.c_void_p]
+            for nm in ("get_density", "get_pressure"):
+                getattr(_lib, f"oracle_{nm}_{sfx}").argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p,
+                                                                C.c_void_p, C.c_void_p, C.c_void_p]
             getattr(_lib, f"oracle_mixture_e_{sfx}").argtypes = [C.c_void_p, real, C.c_void_p]
             getattr(_lib, f"oracle_mixture_cv_{sfx}").argtypes = [C.c_void_p, real, C.c_void_p]
             getattr(_lib, f"oracle_species_thermo_{sfx}").argtypes = [C.c_void_p, C.c_int, real, C.c_void_p]
@@ -131,6 +140,15 @@ class Oracle:
         Y = self._vec(Y)
         return self._fn("mixture_cv")(C.byref(self._m), self._creal(T), Y.ctypes.data)
 
+    def mixture_h(self, T, Y):
+        """Mixture enthalpy per unit mass (enthalpy form of the inversion)."""
+        Y = self._vec(Y)
+        return self._fn("mixture_h")(C.byref(self._m), self._creal(T), Y.ctypes.data)
+
+    def mixture_cp(self, T, Y):
+        Y = self._vec(Y)
+        return self._fn("mixture_cp")(C.byref(self._m), self._creal(T), Y.ctypes.data)
+
     def reaction_detail(self, j, rho, T, Y):
         Y = self._vec(Y)
         out = np.zeros(9, dtype=self.dtype)
@@ -152,6 +170,37 @@ class Oracle:
                                     self._creal(tol), int(max_iter), T.ctypes.data, iters.ctypes.data,
                                     conv.ctypes.data)
         return T, iters, conv
+
+    def get_temperature_from_enthalpy(self, h, Y, T_guess, tol=1e-6, max_iter=10):
+        h = self._vec(h)
+        Y = self._vec(Y)
+        Tg = self._vec(T_guess)
+        n = h.shape[0]
+        assert Y.shape == (self.n_species, n)
+        T = np.empty(n, dtype=self.dtype)
+        iters = np.empty(n, dtype=np.int32)
+        conv = np.empty(n, dtype=np.int32)
+        self._fn("get_temperature_h")(C.byref(self._m), n, n, h.ctypes.data, Y.ctypes.data, Tg.ctypes.data,
+                                      self._creal(tol), int(max_iter), T.ctypes.data, iters.ctypes.data,
+                                      conv.ctypes.data)
+        return T, iters, conv
+
+    def _eos(self, name, a, T, Y):
+        a = self._vec(a)
+        T = self._vec(T)
+        Y = self._vec(Y)
+        n = a.shape[0]
+        assert Y.shape == (self.n_species, n)
+        out = np.empty(n, dtype=self.dtype)
+        self._fn(name)(C.byref(self._m), n, n, a.ctypes.data, T.ctypes.data, Y.ctypes.data, out.ctypes.data)
+        return out
+
+    def get_density(self, p, T, Y):
+        """rho = p W / (R T), W = 1 / sum_k Y_k/W_k   (A.2), (A.3) PAPER.md:892-899."""
+        return self._eos("get_density", p, T, Y)
+
+    def get_pressure(self, rho, T, Y):
+        return self._eos("get_pressure", rho, T, Y)
 
     def get_net_production_rates(self, rho, T, Y, want_rates=False, want_bound=True):
         rho = self._vec(rho)

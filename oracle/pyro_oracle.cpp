@@ -20,6 +20,9 @@
 //   equilibrium const   W2 hand computation, P7 K_c(fwd) K_c(bwd) = 1, P6 detailed balance
 //   third body/falloff  W3 hand computation, P9 [M] = p/RT, P10 Lindemann limits, P11 Troe -> Lindemann
 //   production rates    P5 mass + element conservation, P12 scaling, P15 dense nu brute force, P16
+//   mixture_h / cp      N1 h - e = R T sum_k Y_k/W_k, N2 c_p = dh/dT, N3 c_p - c_v = R sum_k Y_k/W_k
+//   get_temperature_h   N4 recovers generating T, closed form for a constant-c_p species
+//   density / pressure  N5 single species rho = p W/(R T), N6 p(rho(p)) = p, N7 sum_k C_k = p/(R T)
 //   No function is "parity unpinned".
 //
 // Readings of garbled / silent passages are
@@ -102,16 +105,60 @@ Real mixture_cv(const oracle_mech &m, Real T, const Real *Y, int64_t ld) {
     return cv;
 }
 
+// Enthalpy form ("minor modifications"; `do_energy=False` of listing 22, :674):
+//   h = sum_k Y_k h_k,  h_k = h_RT_k R T / W_k  (J/kg; A.12 with PAPER.md:939),  c_p = sum_k Y_k c_p,k  (A.30)
+template <class Real>
+Real mixture_h(const oracle_mech &m, Real T, const Real *Y, int64_t ld) {
+    Real h = 0;
+    for (int k = 0; k < m.n_species; ++k) {
+        Real cp_R, h_RT, s_R, g_RT;
+        species_thermo<Real>(m, k, T, cp_R, h_RT, s_R, g_RT);
+        h += Y[k * ld] * h_RT * Const<Real>::R * T / Real(m.mol_weight[k]);
+    }
+    return h;
+}
+
+template <class Real>
+Real mixture_cp(const oracle_mech &m, Real T, const Real *Y, int64_t ld) {
+    Real cp = 0;
+    for (int k = 0; k < m.n_species; ++k) {
+        Real cp_R, h_RT, s_R, g_RT;
+        species_thermo<Real>(m, k, T, cp_R, h_RT, s_R, g_RT);
+        cp += Y[k * ld] * cp_R * Const<Real>::R / Real(m.mol_weight[k]);
+    }
+    return cp;
+}
+
+// Ideal-gas equation of state (A.2), (A.3) PAPER.md:892-899:  p = rho R T / W,  W = (sum_k Y_k/W_k)^-1
+template <class Real>
+Real mean_molecular_weight(const oracle_mech &m, const Real *Y, int64_t ld) {
+    Real s = 0;
+    for (int k = 0; k < m.n_species; ++k) s += Y[k * ld] / Real(m.mol_weight[k]);
+    return Real(1) / s;
+}
+
+template <class Real>
+Real density_point(const oracle_mech &m, Real p, Real T, const Real *Y, int64_t ld) {
+    return p * mean_molecular_weight<Real>(m, Y, ld) / (Const<Real>::R * T);
+}
+
+template <class Real>
+Real pressure_point(const oracle_mech &m, Real rho, Real T, const Real *Y, int64_t ld) {
+    return rho * Const<Real>::R * T / mean_molecular_weight<Real>(m, Y, ld);
+}
+
 // (A.27), (A.28); listing 22; per-point stop rule (G11):
 // apply the update, then test |dT| < tol; cap max_iter; last iterate returned.
+// `enthalpy`: the same iteration on h(T) = h with c_p in place of c_v.
 template <class Real>
 void get_temperature_point(const oracle_mech &m, Real e, const Real *Y, int64_t ld, Real T_guess, Real tol,
-                           int max_iter, Real &T_out, int &iters, int &converged) {
+                           int max_iter, Real &T_out, int &iters, int &converged, bool enthalpy = false) {
     Real T = T_guess;
     iters = 0;
     converged = 0;
     for (int it = 1; it <= max_iter; ++it) {
-        const Real dT = -(mixture_e<Real>(m, T, Y, ld) - e) / mixture_cv<Real>(m, T, Y, ld);
+        const Real dT = enthalpy ? -(mixture_h<Real>(m, T, Y, ld) - e) / mixture_cp<Real>(m, T, Y, ld)
+                                 : -(mixture_e<Real>(m, T, Y, ld) - e) / mixture_cv<Real>(m, T, Y, ld);
         T = T + dT;
         iters = it;
         if (std::fabs(dT) < tol) {
@@ -259,11 +306,12 @@ void get_net_production_rates(const oracle_mech &m, int64_t n, int64_t ld, const
 
 template <class Real>
 void get_temperature(const oracle_mech &m, int64_t n, int64_t ld, const Real *e, const Real *Y,
-                     const Real *T_guess, Real tol, int max_iter, Real *T, int32_t *iters, int32_t *conv) {
+                     const Real *T_guess, Real tol, int max_iter, Real *T, int32_t *iters, int32_t *conv,
+                     bool enthalpy = false) {
 #pragma omp parallel for schedule(static)
     for (int64_t p = 0; p < n; ++p) {
         int it, cv;
-        get_temperature_point<Real>(m, e[p], Y + p, ld, T_guess[p], tol, max_iter, T[p], it, cv);
+        get_temperature_point<Real>(m, e[p], Y + p, ld, T_guess[p], tol, max_iter, T[p], it, cv, enthalpy);
         if (iters) iters[p] = it;
         if (conv) conv[p] = cv;
     }
@@ -321,6 +369,25 @@ int oracle_sizeof_real80() { return (int)sizeof(long double); }
                                          const Real *Y, const Real *T_guess, Real tol, int max_iter, Real *T, \
                                          int32_t *iters, int32_t *converged) {                                \
         get_temperature<Real>(*m, n, ld, e, Y, T_guess, tol, max_iter, T, iters, converged);                  \
+    }                                                                                                         \
+    Real oracle_mixture_h_##SUFFIX(const oracle_mech *m, Real T, const Real *Y) {                             \
+        return mixture_h<Real>(*m, T, Y, 1);                                                                  \
+    }                                                                                                         \
+    Real oracle_mixture_cp_##SUFFIX(const oracle_mech *m, Real T, const Real *Y) {                            \
+        return mixture_cp<Real>(*m, T, Y, 1);                                                                 \
+    }                                                                                                         \
+    void oracle_get_temperature_h_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *h,        \
+                                           const Real *Y, const Real *T_guess, Real tol, int max_iter,       \
+                                           Real *T, int32_t *iters, int32_t *converged) {                    \
+        get_temperature<Real>(*m, n, ld, h, Y, T_guess, tol, max_iter, T, iters, converged, true);            \
+    }                                                                                                         \
+    void oracle_get_density_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *p,              \
+                                     const Real *T, const Real *Y, Real *rho) {                               \
+        for (int64_t i = 0; i < n; ++i) rho[i] = density_point<Real>(*m, p[i], T[i], Y + i, ld);              \
+    }                                                                                                         \
+    void oracle_get_pressure_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *rho,           \
+                                      const Real *T, const Real *Y, Real *p) {                                \
+        for (int64_t i = 0; i < n; ++i) p[i] = pressure_point<Real>(*m, rho[i], T[i], Y + i, ld);             \
     }                                                                                                         \
     void oracle_get_net_production_rates_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld,                \
                                                   const Real *rho, const Real *T, const Real *Y, Real *omega, \

@@ -421,3 +421,62 @@ def test_paper_toy_inputs_forward_rate_closed_form():
         dp = o.reaction_detail(0, rho, L(T) + h, Y)["qf"]
         dm = o.reaction_detail(0, rho, L(T) - h, Y)["qf"]
         assert abs((dp - dm) / (2 * h) / (d["qf"] * (L(W1["b"]) / L(T) + L(W1["theta"]) / L(T) ** 2)) - 1) < 1e-9
+
+
+# ---------------------------------------------------------------- N1-N7: SURVEY.md 8(f) NEXT-1 (EOS, enthalpy form)
+def test_n1_n2_n3_enthalpy_identities(cfg0):
+    """h - e = R T sum_k Y_k/W_k (h_k = e_k + R T/W_k, A.26); c_p = dh/dT; c_p - c_v = R sum_k Y_k/W_k (A.29, G4)."""
+    mech, o, o80 = cfg0
+    st = inputs.config_states(0, n=16)
+    L = np.longdouble
+    for p in range(16):
+        T, Y = float(st["T"][p]), st["Y"][:, p]
+        rw = R_UNIVERSAL * float((Y / mech.mol_weight).sum())
+        assert abs((o.mixture_h(T, Y) - o.mixture_e(T, Y)) / (rw * T) - 1) < 1e-11   # h, e are ~1e3 x R T/W here
+        assert abs((o.mixture_cp(T, Y) - o.mixture_cv(T, Y)) / rw - 1) < 1e-12
+        if abs(T - 1000.0) < 1.0:
+            continue
+        dT = L(T) * L(1e-5)
+        dh = (o80.mixture_h(L(T) + dT, Y) - o80.mixture_h(L(T) - dT, Y)) / (2 * dT)
+        assert abs(dh / o80.mixture_cp(L(T), Y) - 1) < 1e-8
+
+
+def test_n4_newton_on_enthalpy_recovers_temperature_and_closed_form():
+    """Enthalpy form of the inversion: constant-c_p species h = (a1 T + a6) R/W gives T in
+    one step; on configs[0] the solve recovers the T that generated h."""
+    mech1 = simple_mechanism([dict(W=28.014, lo=[3.5, 0, 0, 0, 0, -1000.0, 0.0])], [])
+    o1 = oracle.Oracle(mech1)
+    h = (3.5 * 1234.5 - 1000.0) * R_UNIVERSAL / 28.014
+    assert abs(o1.mixture_h(1234.5, [1.0]) / h - 1) < 1e-15
+    assert abs(o1.mixture_cp(1234.5, [1.0]) / (3.5 * R_UNIVERSAL / 28.014) - 1) < 1e-15
+    for Tg in (300.0, 1111.0, 2999.0):
+        T, it, cv = o1.get_temperature_from_enthalpy([h], np.array([[1.0]]), [Tg])
+        assert abs(T[0] / 1234.5 - 1) < 1e-14 and it[0] <= 2 and cv[0] == 1
+    mech = inputs.config_mechanism(0)
+    o = oracle.Oracle(mech)
+    st = inputs.config_states(0, n=256)
+    hh = np.array([o.mixture_h(float(st["T"][p]), st["Y"][:, p]) for p in range(256)])
+    T, it, conv = o.get_temperature_from_enthalpy(hh, st["Y"], st["T_guess"])
+    assert conv.all() and it.max() <= 6
+    assert np.max(np.abs(T - st["T"]) / st["T"]) < 1e-12
+    # it is a different equation from the energy form: feeding e instead of h lands elsewhere
+    T_e, _, _ = o.get_temperature_from_enthalpy(st["e"][:256], st["Y"], st["T_guess"])
+    assert np.min(np.abs(T_e - st["T"]) / st["T"]) > 1e-3
+
+
+def test_n5_n6_n7_equation_of_state():
+    """(A.2), (A.3): single species rho = p W/(R T); p(rho(p)) = p; sum_k C_k = p/(R T) with C_k of (A.8)."""
+    mech1 = simple_mechanism([dict(W=28.014, lo=[3.5, 0, 0, 0, 0, -1000.0, 0.0])], [])
+    o1 = oracle.Oracle(mech1)
+    rho = o1.get_density([2 * P_ATM], [750.0], np.array([[1.0]]))
+    assert abs(rho[0] / (2 * P_ATM * 28.014 / (R_UNIVERSAL * 750.0)) - 1) < 1e-15
+    mech = inputs.config_mechanism(2)
+    o = oracle.Oracle(mech)
+    st = inputs.config_states(2, n=64)
+    p = np.full(64, P_ATM) * np.linspace(0.1, 50.0, 64)
+    rho = o.get_density(p, st["T"], st["Y"])
+    assert np.max(np.abs(o.get_pressure(rho, st["T"], st["Y"]) / p - 1)) < 1e-14
+    C = rho[None, :] * st["Y"] / mech.mol_weight[:, None]
+    assert np.max(np.abs(C.sum(axis=0) / (p / (R_UNIVERSAL * st["T"])) - 1)) < 1e-13
+    # the generator's own density (ideal gas at 1 atm, H7) is the same function
+    assert np.max(np.abs(o.get_density(np.full(64, P_ATM), st["T"], st["Y"]) / st["rho"] - 1)) < 1e-13
