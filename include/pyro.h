@@ -99,6 +99,21 @@ int pyro_get_temperature(const pyro_mech *mech, int64_t n, int64_t ld, const dou
                          const double *Y, const double *T_guess, double *T, int32_t *n_not_converged,
                          void *cuda_stream);
 
+/* Enthalpy form of the inversion ("minor modifications"; `do_energy=False` of listing
+ * 22): solves  sum_k Y_k h_k(T) = h  per point, T <- T - (Y.h(T) - h)/c_p(T,Y).
+ * Arguments, stop rule and non-convergence report as pyro_get_temperature, with h [n] in J/kg. */
+int pyro_get_temperature_from_enthalpy(const pyro_mech *mech, int64_t n, int64_t ld, const double *h,
+                                       const double *Y, const double *T_guess, double *T,
+                                       int32_t *n_not_converged, void *cuda_stream);
+
+/* Ideal-gas equation of state (A.2)-(A.3) PAPER.md:892-899:  p = rho R T / W,  W = (sum_k Y_k/W_k)^-1.
+ *   pyro_get_density :  rho[p] = p[p] W / (R T[p])      pyro_get_pressure :  p[p] = rho[p] R T[p] / W
+ * All pointers device; p / rho / T [n], Y [n_species][ld]; the output may alias its scalar input. */
+int pyro_get_density(const pyro_mech *mech, int64_t n, int64_t ld, const double *p, const double *T,
+                     const double *Y, double *rho, void *cuda_stream);
+int pyro_get_pressure(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *T,
+                      const double *Y, double *p, void *cuda_stream);
+
 /* Net molar production rates omega[k*ld+p] = sum_j nu_kj R_j  (A.5)-(A.10) PAPER.md:908-934 from
  *   rho [n], T [n], Y [n_species][ld]   (device; T > 0, rho > 0, Y >= 0 are preconditions)
  *   omega [n_species][ld]               (device, out; must not alias Y) */

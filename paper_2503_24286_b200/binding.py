@@ -16,6 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libpyro.so")
 
 EXPORTS = (
     "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
+    "pyro_get_temperature_from_enthalpy", "pyro_get_density", "pyro_get_pressure",
     "pyro_get_net_production_rates", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
     "pyro_status_string", "pyro_last_error_string",
 )
@@ -64,6 +65,9 @@ def load_library():
     lib.pyro_mech_destroy.argtypes = [vp]
     lib.pyro_mech_set_newton.argtypes = [vp, dbl, C.c_int]
     lib.pyro_get_temperature.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp]
+    lib.pyro_get_temperature_from_enthalpy.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
+    lib.pyro_get_density.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+    lib.pyro_get_pressure.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_get_net_production_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_source_terms_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]
     lib.pyro_mech_info.argtypes = [vp, C.POINTER(i64), C.c_int]
@@ -170,6 +174,34 @@ class Mechanism:
         _check(self._lib.pyro_get_temperature(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T_guess),
                                               _ptr(out), _ptr(n_not_converged), _stream(stream)))
         return out
+
+    def get_temperature_from_enthalpy(self, h, Y, T_guess, out=None, n_not_converged=None, stream=None):
+        """pyro_get_temperature_from_enthalpy: T from (h, Y, T_guess); returns T."""
+        import torch
+        n = h.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        if out is None:
+            out = torch.empty_like(h)
+        _check(self._lib.pyro_get_temperature_from_enthalpy(self._h, n, ld, _ptr(h), _ptr(Y), _ptr(T_guess),
+                                                            _ptr(out), _ptr(n_not_converged), _stream(stream)))
+        return out
+
+    def _eos(self, fn, a, T, Y, out, stream):
+        import torch
+        n = a.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        if out is None:
+            out = torch.empty_like(a)
+        _check(fn(self._h, n, ld, _ptr(a), _ptr(T), _ptr(Y), _ptr(out), _stream(stream)))
+        return out
+
+    def get_density(self, p, T, Y, out=None, stream=None):
+        """pyro_get_density: rho from (p, T, Y); returns rho."""
+        return self._eos(self._lib.pyro_get_density, p, T, Y, out, stream)
+
+    def get_pressure(self, rho, T, Y, out=None, stream=None):
+        """pyro_get_pressure: p from (rho, T, Y); returns p."""
+        return self._eos(self._lib.pyro_get_pressure, rho, T, Y, out, stream)
 
     def get_net_production_rates(self, rho, T, Y, out=None, stream=None):
         """pyro_get_net_production_rates: omega from (rho, T, Y); returns omega."""

@@ -155,6 +155,7 @@ pyro::TempArgs temp_args(const pyro_mech *m, int64_t n, int64_t ld, const double
     a.max_iter = m->newton_max_iter;
     a.t_mid = m->packed.lay.t_mid;
     a.tol = m->newton_tol;
+    a.enthalpy = 0;
     return a;
 }
 
@@ -340,10 +341,9 @@ int pyro_mech_set_newton(pyro_mech *m, double abs_tol_K, int max_iter) {
     return PYRO_OK;
 }
 
-int pyro_get_temperature(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e,
-                         const double *Y, const double *T_guess, double *T, int32_t *n_not_converged,
-                         void *cuda_stream) {
-    (void)rho;   // the ideal-gas caloric equation of state does not depend on density (G23)
+namespace {
+int temperature_call(const pyro_mech *m, int64_t n, int64_t ld, const double *e, const double *Y, const double *T_guess,
+                     double *T, int32_t *n_not_converged, void *cuda_stream, bool enthalpy) {
     int st = check_fields(m, n, ld);
     if (st != PYRO_OK) return st;
     if (n == 0) return PYRO_OK;
@@ -356,9 +356,52 @@ int pyro_get_temperature(const pyro_mech *m, int64_t n, int64_t ld, const double
                     "species with different T_mid: the temperature solve of this build sums the energy "
                     "polynomials per NASA range and needs one T_mid per mechanism");
     DeviceGuard guard(m->device);
-    PYRO_CUDA(pyro::launch_temperature(temp_args(m, n, ld, e, Y, T_guess, T, n_not_converged),
-                                       static_cast<cudaStream_t>(cuda_stream)));
+    pyro::TempArgs a = temp_args(m, n, ld, e, Y, T_guess, T, n_not_converged);
+    a.enthalpy = enthalpy ? 1 : 0;
+    PYRO_CUDA(pyro::launch_temperature(a, static_cast<cudaStream_t>(cuda_stream)));
     return PYRO_OK;
+}
+
+int eos_call(const pyro_mech *m, int64_t n, int64_t ld, const double *in, const double *T, const double *Y,
+             double *out, void *cuda_stream, bool to_density) {
+    int st = check_fields(m, n, ld);
+    if (st != PYRO_OK) return st;
+    if (n == 0) return PYRO_OK;
+    if (!in || !T || !Y || !out) return fail(PYRO_ERR_NULL, "a field pointer is NULL");
+    if (!aligned8(in) || !aligned8(T) || !aligned8(Y) || !aligned8(out))
+        return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
+    DeviceGuard guard(m->device);
+    pyro::EosArgs a{};
+    a.n = n; a.ld = ld; a.in = in; a.T = T; a.Y = Y; a.out = out;
+    a.energy = m->d_energy;
+    a.n_species = m->packed.n_species;
+    a.to_density = to_density ? 1 : 0;
+    PYRO_CUDA(pyro::launch_eos(a, static_cast<cudaStream_t>(cuda_stream)));
+    return PYRO_OK;
+}
+}   // namespace
+
+int pyro_get_temperature(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e,
+                         const double *Y, const double *T_guess, double *T, int32_t *n_not_converged,
+                         void *cuda_stream) {
+    (void)rho;   // the ideal-gas caloric equation of state does not depend on density (G23)
+    return temperature_call(m, n, ld, e, Y, T_guess, T, n_not_converged, cuda_stream, false);
+}
+
+int pyro_get_temperature_from_enthalpy(const pyro_mech *m, int64_t n, int64_t ld, const double *h, const double *Y,
+                                       const double *T_guess, double *T, int32_t *n_not_converged,
+                                       void *cuda_stream) {
+    return temperature_call(m, n, ld, h, Y, T_guess, T, n_not_converged, cuda_stream, true);
+}
+
+int pyro_get_density(const pyro_mech *m, int64_t n, int64_t ld, const double *p, const double *T, const double *Y,
+                     double *rho, void *cuda_stream) {
+    return eos_call(m, n, ld, p, T, Y, rho, cuda_stream, true);
+}
+
+int pyro_get_pressure(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
+                      double *p, void *cuda_stream) {
+    return eos_call(m, n, ld, rho, T, Y, p, cuda_stream, false);
 }
 
 int pyro_get_net_production_rates(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T,

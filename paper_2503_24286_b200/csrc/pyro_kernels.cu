@@ -205,11 +205,13 @@ __global__ void __launch_bounds__(kRatesMaxThreads, kMinBlocks) rates_kernel(con
 template <int BD, int PPT>
 __global__ void __launch_bounds__(BD) temperature_kernel(const TempArgs a) {
     const int64_t base = (int64_t)blockIdx.x * (BD * PPT) + threadIdx.x;
-    double Slo[PPT][6], Shi[PPT][6];
+    double Slo[PPT][6], Shi[PPT][6], Rm[PPT];
 #pragma unroll
-    for (int i = 0; i < PPT; ++i)
+    for (int i = 0; i < PPT; ++i) {
+        Rm[i] = 0.0;
 #pragma unroll
         for (int m = 0; m < 6; ++m) Slo[i][m] = Shi[i][m] = 0.0;
+    }
     int64_t pt[PPT];
 #pragma unroll
     for (int i = 0; i < PPT; ++i) {
@@ -242,6 +244,18 @@ __global__ void __launch_bounds__(BD) temperature_kernel(const TempArgs a) {
                 Slo[i][m] = fma(y[i], c[m], Slo[i][m]);
                 Shi[i][m] = fma(y[i], c[6 + m], Shi[i][m]);
             }
+        if (a.enthalpy) {   // h(T) = e(T) + T sum_k Y_k R/W_k
+            const double rw = __ldg(&a.energy[k].rw);
+#pragma unroll
+            for (int i = 0; i < PPT; ++i) Rm[i] = fma(y[i], rw, Rm[i]);
+        }
+    }
+    if (a.enthalpy) {
+#pragma unroll
+        for (int i = 0; i < PPT; ++i) {
+            Slo[i][1] += Rm[i];
+            Shi[i][1] += Rm[i];
+        }
     }
     int bad = 0;
 #pragma unroll
@@ -256,6 +270,43 @@ __global__ void __launch_bounds__(BD) temperature_kernel(const TempArgs a) {
         }
     }
     if (a.n_not_converged != nullptr && bad) atomicAdd(a.n_not_converged, bad);
+}
+
+// ---------------------------------------------------------------------------------------
+// Ideal-gas equation of state (A.2)-(A.3) PAPER.md:892-899:
+// Rm = sum_k Y_k R/W_k = R/W_mix per point, then rho = p/(Rm T) or p = rho Rm T.  One streaming
+// pass over Y, HBM-bound; planes prefetched into L2 like the temperature kernel.
+// ---------------------------------------------------------------------------------------
+template <int BD, int PPT>
+__global__ void __launch_bounds__(BD) eos_kernel(const EosArgs a) {
+    const int64_t base = (int64_t)blockIdx.x * (BD * PPT) + threadIdx.x;
+    int64_t pt[PPT];
+    double Rm[PPT];
+#pragma unroll
+    for (int i = 0; i < PPT; ++i) {
+        const int64_t p = base + (int64_t)i * BD;
+        pt[i] = p < a.n ? p : a.n - 1;
+        Rm[i] = 0.0;
+    }
+    constexpr int kAhead = 8;
+    for (int k = 0; k < a.n_species; ++k) {
+        if (k + kAhead < a.n_species && (threadIdx.x & 15) == 0) {
+#pragma unroll
+            for (int i = 0; i < PPT; ++i)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)(k + kAhead) * a.ld + pt[i]));
+        }
+        const double rw = __ldg(&a.energy[k].rw);
+#pragma unroll
+        for (int i = 0; i < PPT; ++i) Rm[i] = fma(a.Y[(int64_t)k * a.ld + pt[i]], rw, Rm[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < PPT; ++i) {
+        const int64_t p = base + (int64_t)i * BD;
+        if (p < a.n) {
+            const double rt = Rm[i] * a.T[p];
+            a.out[p] = a.to_density ? a.in[p] / rt : a.in[p] * rt;
+        }
+    }
 }
 
 // ---------------------------------------------------------------------------------------
@@ -310,6 +361,13 @@ cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream) {
 }
 
 const void *temperature_kernel_ptr() { return (const void *)temperature_kernel<kTempBD, kTempPPT>; }
+
+cudaError_t launch_eos(const EosArgs &a, cudaStream_t stream) {
+    const int64_t per_block = (int64_t)kTempBD * kTempPPT;
+    const int64_t blocks = (a.n + per_block - 1) / per_block;
+    eos_kernel<kTempBD, kTempPPT><<<dim3((unsigned)blocks), dim3(kTempBD), 0, stream>>>(a);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_dfma_probe(double *out, int iters, int blocks, cudaStream_t stream) {
     dfma_probe_kernel<<<blocks, 256, 0, stream>>>(out, iters, 1.0);

@@ -33,6 +33,15 @@ struct TempArgs {
     const EnergyRow *energy;     // device, [n_species]
     int32_t n_species, max_iter;
     double t_mid, tol;
+    int32_t enthalpy;            // 0: e given, Newton with c_v (A.27); 1: h given, Newton with c_p
+};
+
+struct EosArgs {                 // (A.2)-(A.3): out = in / (Rm T) (density from pressure) or in Rm T (pressure from density)
+    int64_t n, ld;
+    const double *in, *T, *Y;
+    double *out;
+    const EnergyRow *energy;
+    int32_t n_species, to_density;
 };
 
 const void *rates_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks);
@@ -40,6 +49,7 @@ const void *temperature_kernel_ptr();
 cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem,
                          bool two_blocks, size_t smem_bytes, cudaStream_t stream);
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream);
+cudaError_t launch_eos(const EosArgs &a, cudaStream_t stream);
 cudaError_t launch_dfma_probe(double *out, int iters, int blocks, cudaStream_t stream);
 
 }   // namespace pyro

@@ -433,6 +433,8 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         out.energy.assign(ns, EnergyRow{});
         for (int k = 0; k < ns; ++k) {
             const long double rw = kR / (long double)d->mol_weight[k];
+            out.energy[k].rw = (double)rw;
+            out.energy[k].pad = 0.0;
             for (int range = 0; range < 2; ++range) {
                 const double *a = (range ? d->nasa_hi : d->nasa_lo) + 7 * k;
                 double *c = range ? out.energy[k].hi : out.energy[k].lo;

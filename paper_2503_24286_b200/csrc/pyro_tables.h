@@ -121,8 +121,11 @@ struct GroupCounts {
 //   (a6, a1-1, a2/2, a3/3, a4/4, a5/5) * R/W_k
 // so that  e(T) = sum_k Y_k (c0 + c1 T + ... + c5 T^5)   (A.25)-(A.26) PAPER.md:1008-1012
 // and      c_v(T) = de/dT                                 (A.29)-(A.31) PAPER.md:1025-1034
-struct alignas(8) EnergyRow {
+// rw = R/W_k serves the enthalpy form (h_k = e_k + R T/W_k) and the equation of
+// state (A.2)-(A.3) PAPER.md:892-899: sum_k Y_k R/W_k = R / W_mix.
+struct alignas(16) EnergyRow {
     double lo[6], hi[6];
+    double rw, pad;
 };
 
 }   // namespace pyro

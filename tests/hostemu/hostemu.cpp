@@ -102,8 +102,32 @@ int emu_rates(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho,
     return PYRO_OK;
 }
 
+// enthalpy != 0: the enthalpy form, S1 += sum_k Y_k R/W_k as in the kernel
+int emu_temperature2(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *e, const double *Y,
+                     const double *Tg, double tol, int max_iter, double *T, int64_t *n_bad, int enthalpy);
+
 int emu_temperature(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *e, const double *Y,
                     const double *Tg, double tol, int max_iter, double *T, int64_t *n_bad) {
+    return emu_temperature2(d, n, ld, e, Y, Tg, tol, max_iter, T, n_bad, 0);
+}
+
+// the arithmetic of eos_kernel
+int emu_eos(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *in, const double *T, const double *Y,
+            double *out, int to_density) {
+    pyro::PackedMech pm;
+    int st = pyro::pack_mechanism(d, pm, g_err);
+    if (st != PYRO_OK) return st;
+    for (int64_t p = 0; p < n; ++p) {
+        double Rm = 0.0;
+        for (int k = 0; k < pm.n_species; ++k) Rm = std::fma(Y[k * ld + p], pm.energy[k].rw, Rm);
+        const double rt = Rm * T[p];
+        out[p] = to_density ? in[p] / rt : in[p] * rt;
+    }
+    return PYRO_OK;
+}
+
+int emu_temperature2(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *e, const double *Y,
+                     const double *Tg, double tol, int max_iter, double *T, int64_t *n_bad, int enthalpy) {
     pyro::PackedMech pm;
     int st = pyro::pack_mechanism(d, pm, g_err);
     if (st != PYRO_OK) return st;
@@ -111,12 +135,18 @@ int emu_temperature(const pyro_mech_desc *d, int64_t n, int64_t ld, const double
     const int ns = pm.n_species;
     int64_t bad = 0;
     for (int64_t p = 0; p < n; ++p) {
-        double Slo[6] = {0, 0, 0, 0, 0, 0}, Shi[6] = {0, 0, 0, 0, 0, 0};
-        for (int k = 0; k < ns; ++k)
+        double Slo[6] = {0, 0, 0, 0, 0, 0}, Shi[6] = {0, 0, 0, 0, 0, 0}, Rm = 0.0;
+        for (int k = 0; k < ns; ++k) {
             for (int m = 0; m < 6; ++m) {
                 Slo[m] = std::fma(Y[k * ld + p], pm.energy[k].lo[m], Slo[m]);
                 Shi[m] = std::fma(Y[k * ld + p], pm.energy[k].hi[m], Shi[m]);
             }
+            if (enthalpy) Rm = std::fma(Y[k * ld + p], pm.energy[k].rw, Rm);
+        }
+        if (enthalpy) {
+            Slo[1] += Rm;
+            Shi[1] += Rm;
+        }
         bool conv;
         pyro::newton_temperature(Slo, Shi, pm.lay.t_mid, e[p], Tg[p], tol, max_iter, &T[p], &conv);
         bad += conv ? 0 : 1;

@@ -7,6 +7,7 @@ import numpy as np
 
 OMEGA_TOL = 1e-11
 T_TOL = 1e-12
+EOS_TOL = 1e-13   # |d rho|/rho, |d p|/p: a sum of N_s positive terms in a different order
 
 
 def omega_residual(omega, omega_ref, bound):

@@ -307,3 +307,26 @@ def test_host_buffer_pipeline_matches_oracle(mechs, monkeypatch):
     om2 = np.empty((mech.n_species, n))
     gm.source_terms_host(st["rho"], st["e"], st["Y"], st["T_guess"], T2, om2)
     assert np.array_equal(T2, T.numpy()) and np.array_equal(om2, om.numpy())
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 5000), (2, 3001), (3, 700)])
+def test_enthalpy_inversion_and_equation_of_state(mechs, cfg, n):
+    """pyro_get_temperature_from_enthalpy, pyro_get_density, pyro_get_pressure."""
+    mech, gm, orc = mechs(cfg)
+    st = inputs.config_states(cfg, n=n)
+    Y = np.ascontiguousarray(st["Y"])
+    h = np.array([orc.mixture_h(float(st["T"][p]), Y[:, p]) for p in range(n)])
+    T_ref, _, conv = orc.get_temperature_from_enthalpy(h, Y, st["T_guess"])
+    bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T = gm.get_temperature_from_enthalpy(dev(h), dev(Y), dev(st["T_guess"]), n_not_converged=bad)
+    parity.assert_T_parity(T.cpu().numpy(), T_ref)
+    assert int(bad.item()) == 0 and conv.all()
+    # energy and enthalpy forms are different equations
+    T_e = gm.get_temperature(dev(h), dev(Y), dev(st["T_guess"])).cpu().numpy()
+    assert np.min(np.abs(T_e - T_ref) / T_ref) > 1e-3
+    p = inputs.P_ATM * np.linspace(0.1, 50.0, n)
+    rho = gm.get_density(dev(p), dev(st["T"]), dev(Y))
+    assert np.max(np.abs(rho.cpu().numpy() / orc.get_density(p, st["T"], Y) - 1)) <= parity.EOS_TOL
+    pp = gm.get_pressure(rho, dev(st["T"]), dev(Y), out=rho)          # in place
+    assert np.max(np.abs(pp.cpu().numpy() / p - 1)) <= 10 * parity.EOS_TOL
+    assert gm.get_density(dev(p[:0]), dev(st["T"][:0]), dev(Y[:, :0])).numel() == 0

@@ -69,6 +69,8 @@ def emu():
     L.emu_log2.argtypes = [C.c_double]
     L.emu_exp2_pair.argtypes = [C.c_double, vp, vp]
     L.emu_temperature.argtypes = [vp, i64, i64, vp, vp, vp, C.c_double, C.c_int, vp, vp]
+    L.emu_temperature2.argtypes = [vp, i64, i64, vp, vp, vp, C.c_double, C.c_int, vp, vp, C.c_int]
+    L.emu_eos.argtypes = [vp, i64, i64, vp, vp, vp, vp, C.c_int]
     return L
 
 
@@ -347,3 +349,30 @@ def test_emu_temperature_config_mechanisms(emu, cfg, n):
     T3, bad3 = emu_temperature(emu, mech, st["e"], st["Y"], st["T_guess"], max_iter=2)
     parity.assert_T_parity(T3, T_ref3)
     assert bad3 == int((conv3 == 0).sum())
+
+
+# ------------------------------------------------------------------ NEXT-1: enthalpy form, equation of state
+@pytest.mark.parametrize("cfg,n", [(0, 2048), (2, 512)])
+def test_emu_enthalpy_inversion_and_eos(emu, cfg, n):
+    mech = inputs.config_mechanism(cfg)
+    orc = oracle.Oracle(mech)
+    st = inputs.config_states(cfg, n=n)
+    desc, keep = binding.make_desc(mech)
+    Y = np.ascontiguousarray(st["Y"])
+    h = np.array([orc.mixture_h(float(st["T"][p]), Y[:, p]) for p in range(n)])
+    T_ref, _, conv = orc.get_temperature_from_enthalpy(h, Y, st["T_guess"])
+    T = np.empty(n)
+    bad = C.c_int64(0)
+    Tg = np.ascontiguousarray(st["T_guess"])
+    assert emu.emu_temperature2(C.byref(desc), n, n, h.ctypes.data, Y.ctypes.data, Tg.ctypes.data, 1e-6, 10,
+                                T.ctypes.data, C.byref(bad), 1) == 0
+    parity.assert_T_parity(T, T_ref)
+    assert bad.value == 0 and conv.all()
+    p = np.ascontiguousarray(inputs.P_ATM * np.linspace(0.1, 50.0, n))
+    Tt = np.ascontiguousarray(st["T"])
+    rho = np.empty(n)
+    assert emu.emu_eos(C.byref(desc), n, n, p.ctypes.data, Tt.ctypes.data, Y.ctypes.data, rho.ctypes.data, 1) == 0
+    assert np.max(np.abs(rho / orc.get_density(p, Tt, Y) - 1)) <= parity.EOS_TOL
+    pp = np.empty(n)
+    assert emu.emu_eos(C.byref(desc), n, n, rho.ctypes.data, Tt.ctypes.data, Y.ctypes.data, pp.ctypes.data, 0) == 0
+    assert np.max(np.abs(pp / orc.get_pressure(rho, Tt, Y) - 1)) <= parity.EOS_TOL
