@@ -289,8 +289,17 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     // device maximum so that a later, smaller mechanism cannot lower it under an earlier one
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
         return bail(ce, "cudaFuncSetAttribute(MaxDynamicSharedMemorySize)");
-    // all of the SM's L1/shared array as shared memory, so that several small blocks can be resident
-    if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
+    // Carve-out of the SM's L1/shared array: all of it as shared memory for the one-block shape; for the
+    // two-block shape of small mechanisms only what the two blocks need, the rest stays L1 for the
+    // spills of the 128-register build and for the global loads.
+    int carveout = cudaSharedmemCarveoutMaxShared;
+    if (m->two_blocks) {
+        const size_t need = 2 * (m->smem_bytes + static_smem + 1024) + 8192;
+        carveout = (int)((100 * need + prop.sharedMemPerMultiprocessor - 1) / prop.sharedMemPerMultiprocessor);
+        if (carveout > 100) carveout = 100;
+    }
+    if (const char *env = std::getenv("PYRO_CARVEOUT")) carveout = std::atoi(env);
+    if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, carveout)) != cudaSuccess)
         return bail(ce, "cudaFuncSetAttribute(PreferredSharedMemoryCarveout)");
     int nblk = 0;
     if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, threads, m->smem_bytes)) != cudaSuccess)
