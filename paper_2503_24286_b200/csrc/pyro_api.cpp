@@ -138,10 +138,12 @@ pyro::RatesArgs rates_args(const pyro_mech *m, int64_t n, int64_t ld, const doub
         a.groups.shape_g8[s] = l.shape_g8[s];
         a.groups.shape_g4[s] = l.shape_g4[s];
         a.groups.shape_g2[s] = l.shape_g2[s];
+        a.groups.shape_g1[s] = l.shape_g1[s];
     }
     for (int k = 0; k < 4; ++k) {
         a.groups.ext_g4[k] = l.ext_g4[k];
         a.groups.ext_g2[k] = l.ext_g2[k];
+        a.groups.ext_g1[k] = l.ext_g1[k];
     }
     return a;
 }
@@ -169,7 +171,7 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (!desc) return fail(PYRO_ERR_NULL, "desc is NULL");
     auto *m = new pyro_mech();
     std::string err;
-    int st = pyro::pack_mechanism(desc, m->packed, err);
+    int st = pyro::pack_mechanism(desc, m->packed, err, pyro::kLeftoverPad);
     if (st != PYRO_OK) {
         delete m;
         return fail(st, err);
@@ -324,6 +326,17 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         return fail(PYRO_ERR_TOO_LARGE, "the rates kernel does not fit one SM for this mechanism");
     }
     m->blocks_per_sm = nblk;
+    // The two-block kernel of small mechanisms contains the one-at-a-time loops: store the reactions
+    // that the lockstep grouping left alone as singles instead of coupling them with null records
+    // (the tables only shrink, so the shape chosen above stands).
+    if (m->two_blocks) {
+        pyro::PackedMech again;
+        if (pyro::pack_mechanism(desc, again, err, pyro::kLeftoverSingles) == PYRO_OK && again.lay.bytes <= lay.bytes) {
+            m->packed = again;
+            if ((ce = cudaMemcpy(m->d_blob, m->packed.blob.data(), m->packed.lay.bytes, cudaMemcpyHostToDevice)) != cudaSuccess)
+                return bail(ce, "cudaMemcpy(tables)");
+        }
+    }
     *out = m;
     return PYRO_OK;
 }

@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(kRatesMaxThreads, kMinBlocks) rates_kernel(con
             asm volatile("prefetch.global.L2 [%0];" ::"l"(a.T + pn));
             for (int k = 0; k < ns; ++k) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)k * a.ld + pn));
         }
-        accumulate_reactions(tab, a.groups, pt, ctot, mem);
+        accumulate_reactions<kMinBlocks == 2>(tab, a.groups, pt, ctot, mem);   // singles: small mechanisms only
         double *Wp = a.omega + p;
         int k = 0;
 #pragma unroll 1

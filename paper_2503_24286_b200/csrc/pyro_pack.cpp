@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <algorithm>
 #include <map>
@@ -54,7 +55,7 @@ uint32_t align16(uint32_t x) { return (x + 15u) & ~15u; }
 
 }   // namespace
 
-int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
+int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, int leftover) {
     try {
         PYRO_REQUIRE(d != nullptr, PYRO_ERR_NULL, "desc is NULL");
         const int ns = d->n_species, nr = d->n_reactions, ne = d->n_elements;
@@ -255,10 +256,19 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         // exponentials interleaved, their omega read-modify-writes batched), which needs the
         // scatter lists of a group to be mutually disjoint.  Greedy: every reaction joins the first
         // open group it is disjoint from; a full group (eight) is closed.  What is left open is cut
-        // into fours and couples; reactions left alone are re-coupled where possible and otherwise
-        // coupled with a null record (index -1).
+        // into fours and couples; reactions left alone are re-coupled where possible.  The rest is either
+        // coupled with a null record (index -1: every slot names the dummy species, so its rate is exactly
+        // zero and it rides along in the partner's lockstep for free -- measured faster for mechanisms of
+        // hundreds of reactions) or stored as singles that the kernels run one at a time (faster for small
+        // mechanisms, where null records would be a large share of the work: configs[1] 3.7 -> 2.6 ms).
+        bool pad_singles = leftover == kLeftoverPad;
+        if (leftover == kLeftoverAuto) {
+            pad_singles = nr >= 64;
+            if (const char *env = std::getenv("PYRO_PACK_SINGLES")) pad_singles = std::atoi(env) == 0;
+        }
         auto make_groups = [&](const std::vector<int> &members, const std::vector<std::vector<int>> &species,
-                               int largest, std::vector<int> &g8, std::vector<int> &g4, std::vector<int> &g2) {
+                               int largest, std::vector<int> &g8, std::vector<int> &g4, std::vector<int> &g2,
+                               std::vector<int> &g1) {
             auto disjoint = [&](int a, int b) {
                 for (int x : species[a])
                     for (int y : species[b])
@@ -311,9 +321,13 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
                     rest.push_back(i);
                 }
             }
-            for (int i : rest) {
-                g2.push_back(i);
-                g2.push_back(-1);
+            if (pad_singles) {
+                for (int i : rest) {
+                    g2.push_back(i);
+                    g2.push_back(-1);
+                }
+            } else {
+                g1 = rest;
             }
         };
         // plain class: by shape
@@ -321,16 +335,17 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         std::memset(&nullP, 0, sizeof nullP);
         for (int m = 0; m < 6; ++m) nullP.slot[m] = (uint32_t)ns;
         std::vector<RxnP> sortedP;
-        int shape_g8[9] = {0}, shape_g4[9] = {0}, shape_g2[9] = {0};
+        int shape_g8[9] = {0}, shape_g4[9] = {0}, shape_g2[9] = {0}, shape_g1[9] = {0};
         for (int shape = 0; shape < 9; ++shape) {
-            std::vector<int> members, g8, g4, g2;
+            std::vector<int> members, g8, g4, g2, g1;
             for (size_t i = 0; i < recP.size(); ++i)
                 if (shapeP[i] == shape) members.push_back((int)i);
-            make_groups(members, speciesP, 4, g8, g4, g2);   // (groups of eight: kept in the format, not formed yet)
+            make_groups(members, speciesP, 4, g8, g4, g2, g1);   // (groups of eight: kept in the format, not formed yet)
             shape_g8[shape] = (int)g8.size();
             shape_g4[shape] = (int)g4.size();
             shape_g2[shape] = (int)g2.size();
-            for (const std::vector<int> *g : {&g8, &g4, &g2})
+            shape_g1[shape] = (int)g1.size();
+            for (const std::vector<int> *g : {&g8, &g4, &g2, &g1})
                 for (int i : *g) {
                     sortedP.push_back(i < 0 ? nullP : recP[i]);
                     out.order.push_back(i < 0 ? -1 : orderP[i]);
@@ -345,14 +360,15 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
         nullX.eff_default = 1.0;
         std::vector<RxnX> sortedX;
         std::vector<EffEntry> effs;
-        int ext_g4[4] = {0, 0, 0, 0}, ext_g2[4] = {0, 0, 0, 0};
+        int ext_g4[4] = {0, 0, 0, 0}, ext_g2[4] = {0, 0, 0, 0}, ext_g1[4] = {0, 0, 0, 0};
         for (int kind = 0; kind < 4; ++kind) {
-            std::vector<int> members, g8, g4, g2;
+            std::vector<int> members, g8, g4, g2, g1;
             for (size_t i = 0; i < recX.size(); ++i)
                 if ((int)recX[i].type == kind) members.push_back((int)i);
-            make_groups(members, speciesX, 4, g8, g4, g2);
+            make_groups(members, speciesX, 4, g8, g4, g2, g1);
             ext_g4[kind] = (int)g4.size();
             ext_g2[kind] = (int)g2.size();
+            ext_g1[kind] = (int)g1.size();
             auto emit = [&](const std::vector<int> &g, size_t width) {
                 for (size_t at = 0; at < g.size(); at += width) {
                     size_t longest = 0;
@@ -378,6 +394,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
             };
             emit(g4, 4);
             emit(g2, 2);
+            emit(g1, 1);
         }
         recX.swap(sortedX);
 
@@ -405,10 +422,12 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err) {
             lay.shape_g8[s] = shape_g8[s];
             lay.shape_g4[s] = shape_g4[s];
             lay.shape_g2[s] = shape_g2[s];
+            lay.shape_g1[s] = shape_g1[s];
         }
         for (int k = 0; k < 4; ++k) {
             lay.ext_g4[k] = ext_g4[k];
             lay.ext_g2[k] = ext_g2[k];
+            lay.ext_g1[k] = ext_g1[k];
         }
         uint32_t off = 0;
         lay.off_spec = off;

@@ -22,6 +22,11 @@ struct PackedMech {
 };
 
 // Returns a pyro_status; on failure `err` says which entry was rejected.
-int pack_mechanism(const pyro_mech_desc *desc, PackedMech &out, std::string &err);
+// `leftover` says what happens to reactions that end up alone after the lockstep grouping:
+// kLeftoverPad couples each with a null record, kLeftoverSingles stores them as singles (the
+// kernel variant must then contain the one-at-a-time loops), kLeftoverAuto takes singles for
+// fewer than 64 reactions (environment PYRO_PACK_SINGLES=0/1 overrides; host tests).
+enum { kLeftoverAuto = -1, kLeftoverPad = 0, kLeftoverSingles = 1 };
+int pack_mechanism(const pyro_mech_desc *desc, PackedMech &out, std::string &err, int leftover = kLeftoverAuto);
 
 }   // namespace pyro

@@ -151,12 +151,15 @@ PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT &pt
 }
 
 // One shape of the plain class: its groups of eight and of four run four in lockstep, its
-// couples two in lockstep.
-template <int NR, int NP, class Tab, class Mem>
-PYRO_HD int plain_shape(const Tab &tab, int j, int g8, int g4, int g2, const PointT &pt, const Mem &mem) {
+// couples two in lockstep, the rest one at a time.
+// kSingles = false leaves the one-at-a-time loops out (the packer then stores no singles): for
+// large mechanisms their code alone costs 8 % (measured on configs[2]: instruction cache).
+template <int NR, int NP, bool kSingles, class Tab, class Mem>
+PYRO_HD int plain_shape(const Tab &tab, int j, int g8, int g4, int g2, int g1, const PointT &pt, const Mem &mem) {
     plain_reactions<NR, NP, 4>(tab, j, g8 + g4, pt, mem);
     plain_reactions<NR, NP, 2>(tab, j + g8 + g4, g2, pt, mem);
-    return j + g8 + g4 + g2;
+    if (kSingles) plain_reactions<NR, NP, 1>(tab, j + g8 + g4 + g2, g1, pt, mem);
+    return j + g8 + g4 + g2 + g1;
 }
 
 // Extended-class reactions of one kind, NB in lockstep: third body, falloff (Lindemann /
@@ -289,36 +292,37 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
     }
 }
 
-template <int KIND, class Tab, class Mem>
-PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, const PointT &pt, double ctot, const Mem &mem) {
+template <int KIND, bool kSingles, class Tab, class Mem>
+PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, int g1, const PointT &pt, double ctot, const Mem &mem) {
     // a group of four runs four in lockstep (Troe: two and two, its five exponentials per reaction
     // already fill the pipe), a couple two
     extended_reactions<KIND, KIND == kExtTroe ? 2 : 4>(tab, j, g4, pt, ctot, mem);
     extended_reactions<KIND, 2>(tab, j + g4, g2, pt, ctot, mem);
-    return j + g4 + g2;
+    if (kSingles) extended_reactions<KIND, 1>(tab, j + g4 + g2, g1, pt, ctot, mem);
+    return j + g4 + g2 + g1;
 }
 
 // Rows a5-a9 of SURVEY.md 8(a): rates of progress of every reaction and their stoichiometric
 // accumulation into plane W, (A.5)-(A.10) PAPER.md:908-934.  The planes hold n_species + 1
 // entries: the last one is the dummy species (A = B = 1, omega = sink) that pads the
-// extended records and the null records.
-template <class Tab, class Mem>
+// extended records and the efficiency lists.
+template <bool kSingles, class Tab, class Mem>
 PYRO_HD void accumulate_reactions(const Tab &tab, const GroupCounts &g, const PointT &pt, double ctot, const Mem &mem) {
     int j = 0;
-    j = plain_shape<1, 1>(tab, j, g.shape_g8[0], g.shape_g4[0], g.shape_g2[0], pt, mem);
-    j = plain_shape<1, 2>(tab, j, g.shape_g8[1], g.shape_g4[1], g.shape_g2[1], pt, mem);
-    j = plain_shape<1, 3>(tab, j, g.shape_g8[2], g.shape_g4[2], g.shape_g2[2], pt, mem);
-    j = plain_shape<2, 1>(tab, j, g.shape_g8[3], g.shape_g4[3], g.shape_g2[3], pt, mem);
-    j = plain_shape<2, 2>(tab, j, g.shape_g8[4], g.shape_g4[4], g.shape_g2[4], pt, mem);
-    j = plain_shape<2, 3>(tab, j, g.shape_g8[5], g.shape_g4[5], g.shape_g2[5], pt, mem);
-    j = plain_shape<3, 1>(tab, j, g.shape_g8[6], g.shape_g4[6], g.shape_g2[6], pt, mem);
-    j = plain_shape<3, 2>(tab, j, g.shape_g8[7], g.shape_g4[7], g.shape_g2[7], pt, mem);
-    j = plain_shape<3, 3>(tab, j, g.shape_g8[8], g.shape_g4[8], g.shape_g2[8], pt, mem);
+    j = plain_shape<1, 1, kSingles>(tab, j, g.shape_g8[0], g.shape_g4[0], g.shape_g2[0], g.shape_g1[0], pt, mem);
+    j = plain_shape<1, 2, kSingles>(tab, j, g.shape_g8[1], g.shape_g4[1], g.shape_g2[1], g.shape_g1[1], pt, mem);
+    j = plain_shape<1, 3, kSingles>(tab, j, g.shape_g8[2], g.shape_g4[2], g.shape_g2[2], g.shape_g1[2], pt, mem);
+    j = plain_shape<2, 1, kSingles>(tab, j, g.shape_g8[3], g.shape_g4[3], g.shape_g2[3], g.shape_g1[3], pt, mem);
+    j = plain_shape<2, 2, kSingles>(tab, j, g.shape_g8[4], g.shape_g4[4], g.shape_g2[4], g.shape_g1[4], pt, mem);
+    j = plain_shape<2, 3, kSingles>(tab, j, g.shape_g8[5], g.shape_g4[5], g.shape_g2[5], g.shape_g1[5], pt, mem);
+    j = plain_shape<3, 1, kSingles>(tab, j, g.shape_g8[6], g.shape_g4[6], g.shape_g2[6], g.shape_g1[6], pt, mem);
+    j = plain_shape<3, 2, kSingles>(tab, j, g.shape_g8[7], g.shape_g4[7], g.shape_g2[7], g.shape_g1[7], pt, mem);
+    j = plain_shape<3, 3, kSingles>(tab, j, g.shape_g8[8], g.shape_g4[8], g.shape_g2[8], g.shape_g1[8], pt, mem);
     int x = 0;
-    x = extended_kind<kExtGeneral>(tab, x, g.ext_g4[0], g.ext_g2[0], pt, ctot, mem);
-    x = extended_kind<kExtThreeBody>(tab, x, g.ext_g4[1], g.ext_g2[1], pt, ctot, mem);
-    x = extended_kind<kExtLindemann>(tab, x, g.ext_g4[2], g.ext_g2[2], pt, ctot, mem);
-    x = extended_kind<kExtTroe>(tab, x, g.ext_g4[3], g.ext_g2[3], pt, ctot, mem);
+    x = extended_kind<kExtGeneral, kSingles>(tab, x, g.ext_g4[0], g.ext_g2[0], g.ext_g1[0], pt, ctot, mem);
+    x = extended_kind<kExtThreeBody, kSingles>(tab, x, g.ext_g4[1], g.ext_g2[1], g.ext_g1[1], pt, ctot, mem);
+    x = extended_kind<kExtLindemann, kSingles>(tab, x, g.ext_g4[2], g.ext_g2[2], g.ext_g1[2], pt, ctot, mem);
+    x = extended_kind<kExtTroe, kSingles>(tab, x, g.ext_g4[3], g.ext_g2[3], g.ext_g1[3], pt, ctot, mem);
     mem.fence_st();
 }
 

@@ -42,8 +42,9 @@ struct alignas(16) SpecRow {
 // coefficients (so the scatter list is the slot list and the slots of one reaction never
 // collide).  Stored by shape (molecules per side), shape s = 3 (nreac-1) + (nprod-1); within a
 // shape first the groups of eight mutually species-disjoint reactions, then the groups of
-// four, then the couples (a reaction left alone is coupled with a null record: every slot
-// names the dummy species, so its rate is exactly zero).  48 bytes.
+// four, then the couples, then the reactions left alone.  Large mechanisms couple a reaction
+// left alone with a null record instead (every slot names the dummy species, so its rate is
+// exactly zero).  48 bytes.
 struct alignas(16) RxnP {
     double f[3];        // log2 k_f = f0 + f1 log2T + f2/T          (A.9) PAPER.md:925
     uint32_t slot[6];   // species: reactants 0..nreac-1, then products nreac..nreac+nprod-1
@@ -52,7 +53,7 @@ struct alignas(16) RxnP {
 // Extended class: three-body and falloff reactions, irreversible reactions, and reactions
 // with a repeated species (coefficient 2 or 3, or a species on both sides).  Stored by kind,
 // within a kind first the groups of four reactions with mutually disjoint scatter lists, then
-// the couples (null-padded like the plain class).  The six slots list every molecule (a
+// the couples, then the reactions left alone.  The six slots list every molecule (a
 // coefficient 2 repeats the species), reactants in 0..2 and products in 3..5; unused slots and
 // unused scatter entries name the dummy species n_species (A = B = 1, omega = sink), so that
 // the code is branch-free.  The scatter list holds each species once, with its net
@@ -97,12 +98,14 @@ struct TableLayout {
     uint32_t off_eff;        // EffEntry[n_eff]
     uint32_t bytes;
     int32_t n_species;
-    int32_t n_p, n_x, n_eff, n_fall;   // stored records (null padding included)
+    int32_t n_p, n_x, n_eff, n_fall;   // stored records (null records included)
     int32_t shape_g8[9];     // plain class, per shape: records stored as disjoint groups of eight
     int32_t shape_g4[9];     // ... of four
     int32_t shape_g2[9];     // ... as couples
+    int32_t shape_g1[9];     // ... alone
     int32_t ext_g4[4];       // extended class, per kind: records stored as disjoint groups of four
     int32_t ext_g2[4];       // ... as couples
+    int32_t ext_g1[4];       // ... alone
     int32_t needs_ctot;      // any extended reaction uses [M]
     int32_t single_t_mid;    // 1 if every species has the same T_mid (needed by the temperature solve)
     double t_mid;            // that T_mid
@@ -114,7 +117,7 @@ static_assert(sizeof(SpecRow) == 128 && sizeof(RxnP) == 48 && sizeof(RxnX) == 11
 
 // Loop counts of one mechanism, as the kernels take them (copied from TableLayout).
 struct GroupCounts {
-    int32_t shape_g8[9], shape_g4[9], shape_g2[9], ext_g4[4], ext_g2[4];
+    int32_t shape_g8[9], shape_g4[9], shape_g2[9], shape_g1[9], ext_g4[4], ext_g2[4], ext_g1[4];
 };
 
 // Energy table of the temperature solve: per species and NASA range the six coefficients

@@ -31,10 +31,12 @@ pyro::GroupCounts group_counts(const pyro::TableLayout &l) {
         g.shape_g8[s] = l.shape_g8[s];
         g.shape_g4[s] = l.shape_g4[s];
         g.shape_g2[s] = l.shape_g2[s];
+        g.shape_g1[s] = l.shape_g1[s];
     }
     for (int k = 0; k < 4; ++k) {
         g.ext_g4[k] = l.ext_g4[k];
         g.ext_g2[k] = l.ext_g2[k];
+        g.ext_g1[k] = l.ext_g1[k];
     }
     return g;
 }
@@ -48,6 +50,7 @@ const char *emu_last_error() { return g_err.c_str(); }
 //       [4] plain records stored in groups of eight [5] of four [6] single T_mid
 //       [7..15] per shape: records in eights, [16..24] in fours, [25..33] in couples
 //       [34..37] extended records per kind in fours, [38..41] in couples
+//       [42..50] plain records per shape alone, [51..54] extended records per kind alone
 int emu_pack_status(const pyro_mech_desc *d, int64_t *info) {
     pyro::PackedMech pm;
     int st = pyro::pack_mechanism(d, pm, g_err);
@@ -67,7 +70,9 @@ int emu_pack_status(const pyro_mech_desc *d, int64_t *info) {
         for (int k = 0; k < 4; ++k) {
             info[34 + k] = pm.lay.ext_g4[k];
             info[38 + k] = pm.lay.ext_g2[k];
+            info[51 + k] = pm.lay.ext_g1[k];
         }
+        for (int s = 0; s < 9; ++s) info[42 + s] = pm.lay.shape_g1[s];
         info[6] = pm.lay.single_t_mid;
     }
     return st;
@@ -96,7 +101,7 @@ int emu_rates(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho,
         const pyro::PointT pt = pyro::make_point(T[p]);
         const pyro::ArrayMem mem{A.data(), B.data(), W.data()};
         const double ctot = pyro::fill_planes(tab, ns, pt, rho[p], mem, [&](int k) { return Y[k * ld + p]; });
-        pyro::accumulate_reactions(tab, g, pt, ctot, mem);
+        pyro::accumulate_reactions<true>(tab, g, pt, ctot, mem);
         for (int k = 0; k < ns; ++k) omega[k * ld + p] = W[k];
     }
     return PYRO_OK;

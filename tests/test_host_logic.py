@@ -99,7 +99,7 @@ def pack_status(emu, mech, mutate=None):
     desc, keep = binding.make_desc(mech)
     if mutate:
         mutate(desc, keep)
-    info = (C.c_int64 * 42)()
+    info = (C.c_int64 * 55)()
     st = emu.emu_pack_status(C.byref(desc), info)
     return st, list(info), emu.emu_last_error().decode()
 
@@ -176,9 +176,9 @@ def test_packer_classes_and_table_size(emu):
         n_plain = _expected_plain(mech)
         order = pack_order(emu, mech, info[0] + info[1])
         assert st == 0
-        # records = reactions + null records that complete a couple
+        # records = reactions (+ null records that complete a couple, in mechanisms of 64 reactions or more)
         assert (order[:info[0]] >= 0).sum() == n_plain and (order[info[0]:] >= 0).sum() == mech.n_reactions - n_plain
-        assert info[0] % 2 == 0 and info[1] % 2 == 0
+        assert mech.n_reactions >= 64 or (order >= 0).all()
         assert info[3] >= len(mech.eff_species)      # efficiency lists padded to one length per lockstep group
     st, info, _ = pack_status(emu, inputs.config_mechanism(2))
     assert info[2] <= 40 * 1024          # configs[2] tables are staged in shared memory beside the planes
@@ -198,7 +198,8 @@ def pack_order(emu, mech, n_records):
 def test_packer_groups_are_species_disjoint_and_order_is_a_permutation(emu):
     """The lockstep groups batch their omega read-modify-writes: the members of a group must not
     share a species that they update.  `order` maps packed records back to the description
-    (-1 for the null records that complete a couple)."""
+    (-1 for the null records that complete a couple in large mechanisms; small ones store the
+    reactions left alone as singles)."""
     for mech in (inputs.config_mechanism(0), inputs.config_mechanism(2), inputs.config_mechanism(3),
                  hand_cases.all_paths_mechanism()):
         st, info, _ = pack_status(emu, mech)
@@ -227,11 +228,11 @@ def test_packer_groups_are_species_disjoint_and_order_is_a_permutation(emu):
             return pos + count
         pos = 0
         for sh in range(9):
-            for size, count in ((8, info[7 + sh]), (4, info[16 + sh]), (2, info[25 + sh])):
+            for size, count in ((8, info[7 + sh]), (4, info[16 + sh]), (2, info[25 + sh]), (1, info[42 + sh])):
                 pos = check(pos, size, count, lambda j: shape(j) == sh)
         assert pos == info[0]
         for k in range(4):
-            for size, count in ((4, info[34 + k]), (2, info[38 + k])):
+            for size, count in ((4, info[34 + k]), (2, info[38 + k]), (1, info[51 + k])):
                 pos = check(pos, size, count, lambda j: kind(j) == k)
         assert pos == info[0] + info[1]
 
@@ -316,6 +317,20 @@ def test_emu_rates_config_mechanisms(emu, cfg, n):
     om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
     r = parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"]), om_ref, bound)
     assert r < 1e-12   # typical residual is a few 1e-14; 1e-11 is the bar
+
+
+def test_emu_rates_both_packings_of_leftover_reactions(emu, monkeypatch):
+    """Reactions left alone after grouping: singles (small mechanisms) or null-padded couples (large)."""
+    for cfg, n in ((0, 1024), (2, 256)):
+        mech = inputs.config_mechanism(cfg)
+        st = inputs.config_states(cfg, n=n)
+        om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
+        for singles in ("0", "1"):
+            monkeypatch.setenv("PYRO_PACK_SINGLES", singles)
+            stt, info, _ = pack_status(emu, mech)
+            order = pack_order(emu, mech, info[0] + info[1])
+            assert (singles == "1") == bool((order >= 0).all()) or (order >= 0).all()
+            parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"]), om_ref, bound)
 
 
 def test_emu_rates_species_with_different_t_mid(emu):
