@@ -294,14 +294,9 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
 
 template <int KIND, bool kSingles, class Tab, class Mem>
 PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, int g1, const PointT &pt, double ctot, const Mem &mem) {
-    // a group of four runs four in lockstep, a couple two; Troe runs everything two by two (its five
-    // exponentials per reaction already fill the pipe) in ONE loop: code size matters
-    if (KIND == kExtTroe) {
-        extended_reactions<KIND, 2>(tab, j, g4 + g2, pt, ctot, mem);
-    } else {
-        extended_reactions<KIND, 4>(tab, j, g4, pt, ctot, mem);
-        extended_reactions<KIND, 2>(tab, j + g4, g2, pt, ctot, mem);
-    }
+    // groups of four and couples alike run two in lockstep, in ONE loop per kind: four in lockstep
+    // gains less than the second copy of the loop costs (instruction cache; measured on configs[2])
+    extended_reactions<KIND, 2>(tab, j, g4 + g2, pt, ctot, mem);
     if (kSingles) extended_reactions<KIND, 1>(tab, j + g4 + g2, g1, pt, ctot, mem);
     return j + g4 + g2 + g1;
 }
