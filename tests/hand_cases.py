@@ -63,3 +63,20 @@ def random_states(mech, n, seed=7):
     Y = rng.dirichlet(np.full(mech.n_species, 0.7), size=n).T.copy()
     rho = rng.uniform(0.05, 5.0, size=n)
     return rho, T, Y
+
+
+def degenerate_mechanisms():
+    """Degenerate cases the packer and the kernels must take: no reaction at all (omega = 0), a single
+    species, and a mechanism whose reactions are all in the extended class (nothing in the plain loops)."""
+    sp = species5()
+    none = simple_mechanism(sp, [])
+    one = simple_mechanism(sp[:1], [])
+    low = dict(A0=1e12, b0=-1.5, theta0=2000.0)
+    ext = simple_mechanism(sp, [
+        dict(reac={0: 2}, prod={1: 1, 2: 1}, A=3e9, b=0.5, theta=4000.0),                      # repeated species
+        dict(reac={1: 1, 3: 1}, prod={4: 1}, A=5e8, b=0.0, theta=1500.0, reversible=0),         # irreversible
+        dict(reac={2: 1, 3: 1}, prod={0: 1, 4: 1}, A=2e10, b=-0.3, theta=6000.0, type=1, eff={0: 2.5, 4: 0.4}),
+        dict(reac={0: 1, 1: 1}, prod={2: 1}, A=4e9, b=0.2, theta=900.0, type=3, troe=(0.6, 100.0, 1500.0, 5000.0),
+             eff={3: 6.0}, **low),
+    ])
+    return dict(none=none, one=one, ext=ext)

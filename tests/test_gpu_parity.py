@@ -330,3 +330,20 @@ def test_enthalpy_inversion_and_equation_of_state(mechs, cfg, n):
     pp = gm.get_pressure(rho, dev(st["T"]), dev(Y), out=rho)          # in place
     assert np.max(np.abs(pp.cpu().numpy() / p - 1)) <= 10 * parity.EOS_TOL
     assert gm.get_density(dev(p[:0]), dev(st["T"][:0]), dev(Y[:, :0])).numel() == 0
+
+
+def test_degenerate_mechanisms(mechs):
+    """No reaction at all, a single species, only extended-class reactions; T solve on each."""
+    for name, mech in hand_cases.degenerate_mechanisms().items():
+        gm = binding.Mechanism(mech)
+        orc = oracle.Oracle(mech)
+        rho, T, Y = hand_cases.random_states(mech, 777)
+        om_ref, bound = orc.get_net_production_rates(rho, T, Y)
+        om = gpu_rates(gm, rho, T, Y)
+        parity.assert_omega_parity(om, om_ref, bound)
+        if mech.n_reactions == 0:
+            assert not om.any()
+        e = np.array([orc.mixture_e(float(T[p]), Y[:, p]) for p in range(777)])
+        Tg = T * 1.07
+        T_ref, _, _ = orc.get_temperature(e, Y, Tg)
+        parity.assert_T_parity(gm.get_temperature(dev(e), dev(Y), dev(Tg)).cpu().numpy(), T_ref)

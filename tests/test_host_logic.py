@@ -391,3 +391,13 @@ def test_emu_enthalpy_inversion_and_eos(emu, cfg, n):
     pp = np.empty(n)
     assert emu.emu_eos(C.byref(desc), n, n, rho.ctypes.data, Tt.ctypes.data, Y.ctypes.data, pp.ctypes.data, 0) == 0
     assert np.max(np.abs(pp / orc.get_pressure(rho, Tt, Y) - 1)) <= parity.EOS_TOL
+
+
+def test_emu_rates_degenerate_mechanisms(emu):
+    for name, mech in hand_cases.degenerate_mechanisms().items():
+        rho, T, Y = hand_cases.random_states(mech, 200)
+        om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+        om = emu_rates(emu, mech, rho, T, Y)
+        parity.assert_omega_parity(om, om_ref, bound)
+        if mech.n_reactions == 0:
+            assert not om.any()
