@@ -164,6 +164,12 @@ double emu_exp2(double y) { return pyro::exp2_poly(y); }
 
 double emu_log2(double x) { return pyro::log2_pos(x); }
 
+double emu_exp2_rxn(double y) {
+    double v[1] = {y};
+    pyro::exp2_poly_n<1>(v);
+    return v[0];
+}
+
 void emu_exp2_pair(double y, double *e, double *b) {
     const double yy[1] = {y};
     double ee[1], bb[1];

@@ -65,6 +65,8 @@ def emu():
     L.emu_pack_status.argtypes = [vp, vp]
     L.emu_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp]
     L.emu_pack_order.argtypes = [vp, vp, C.c_int32]
+    L.emu_exp2_rxn.restype = C.c_double
+    L.emu_exp2_rxn.argtypes = [C.c_double]
     L.emu_log2.restype = C.c_double
     L.emu_log2.argtypes = [C.c_double]
     L.emu_exp2_pair.argtypes = [C.c_double, vp, vp]
@@ -121,6 +123,19 @@ def test_exp2_poly_accuracy_and_edges(emu):
     assert emu.emu_exp2(-1100.0) >= 0.0
     assert np.isnan(emu.emu_exp2(float("nan")))
     assert not np.isfinite(emu.emu_exp2(1100.0)) or emu.emu_exp2(1100.0) > 1e307
+
+
+def test_exp2_of_the_reaction_loops_degree_nine(emu):
+    """exp2_poly_n (rate coefficients, falloff): degree-9 polynomial, relative error below 5e-14."""
+    mp.mp.dps = 40
+    rng = np.random.default_rng(4)
+    ys = np.concatenate([rng.uniform(-1000, 1000, 3000), rng.uniform(-1, 1, 2000), np.arange(-20, 21) * 0.5])
+    worst = 0.0
+    for y in ys:
+        worst = max(worst, float(abs(mp.mpf(emu.emu_exp2_rxn(float(y))) / (mp.mpf(2) ** mp.mpf(float(y))) - 1)))
+    assert 1e-15 < worst < 5e-14, worst
+    assert emu.emu_exp2_rxn(0.0) == 1.0 and emu.emu_exp2_rxn(10.0) == 1024.0
+    assert 0.0 <= emu.emu_exp2_rxn(-1e9) < 1e-307 and np.isnan(emu.emu_exp2_rxn(float("nan")))
 
 
 def test_exp2_pair_is_exp2_and_its_reciprocal(emu):
