@@ -273,6 +273,86 @@ __global__ void __launch_bounds__(BD) temperature_kernel(const TempArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------
+// The same solve as a software-pipelined stream (used when the Y planes are 16-byte aligned):
+// thread t owns points 2t, 2t+1 of its block's 2 BD points and copies their 16 bytes of every
+// species plane into its own slot of a D-deep shared-memory ring with cp.async, D species ahead
+// of the arithmetic, so that the HBM latency is covered by D x 16 bytes in flight per thread
+// instead of by resident warps.  A thread only ever reads what it copied itself: no barrier
+// in the loop.  The energy table is staged in shared memory once per block.
+// ---------------------------------------------------------------------------------------
+template <int BD, int D>
+__global__ void __launch_bounds__(BD) temperature_stream_kernel(const TempArgs a) {
+    static_assert((D & (D - 1)) == 0, "ring depth must be a power of two");
+    extern __shared__ __align__(16) unsigned char tsm[];
+    EnergyRow *tab = reinterpret_cast<EnergyRow *>(tsm + (size_t)D * BD * 16);
+    const int tid = threadIdx.x, ns = a.n_species;
+    {
+        const double2 *src = reinterpret_cast<const double2 *>(a.energy);
+        double2 *dst = reinterpret_cast<double2 *>(tab);
+        for (int i = tid; i < ns * (int)(sizeof(EnergyRow) / 16); i += BD) dst[i] = __ldg(src + i);
+    }
+    const int64_t p0 = ((int64_t)blockIdx.x * BD + tid) * 2;   // the launcher passes whole blocks only
+    const double *Yp = a.Y + p0;
+    const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(tsm) + (uint32_t)tid * 16u;
+    auto issue = [&](int k) {
+        if (k < ns)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + (uint32_t)(k & (D - 1)) * (BD * 16u)),
+                         "l"(Yp + (int64_t)k * a.ld)
+                         : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");   // one group per species, empty past the end
+    };
+#pragma unroll
+    for (int s = 0; s < D; ++s) issue(s);
+    __syncthreads();   // the energy table is in place
+    double Slo[2][6], Shi[2][6], Rm[2] = {0.0, 0.0};
+#pragma unroll
+    for (int i = 0; i < 2; ++i)
+#pragma unroll
+        for (int m = 0; m < 6; ++m) Slo[i][m] = Shi[i][m] = 0.0;
+#pragma unroll 1
+    for (int k = 0; k < ns; ++k) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(D - 1) : "memory");
+        double y[2];
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(y[0]), "=d"(y[1]) : "r"(slot0 + (uint32_t)(k & (D - 1)) * (BD * 16u)));
+        issue(k + D);
+        const double2 *row = reinterpret_cast<const double2 *>(tab + k);
+        double c[12];
+#pragma unroll
+        for (int m = 0; m < 6; ++m) {
+            const double2 v = row[m];
+            c[2 * m] = v.x;
+            c[2 * m + 1] = v.y;
+        }
+#pragma unroll
+        for (int i = 0; i < 2; ++i)
+#pragma unroll
+            for (int m = 0; m < 6; ++m) {
+                Slo[i][m] = fma(y[i], c[m], Slo[i][m]);
+                Shi[i][m] = fma(y[i], c[6 + m], Shi[i][m]);
+            }
+        if (a.enthalpy) {   // h(T) = e(T) + T sum_k Y_k R/W_k
+            const double rw = tab[k].rw;
+#pragma unroll
+            for (int i = 0; i < 2; ++i) Rm[i] = fma(y[i], rw, Rm[i]);
+        }
+    }
+    int bad = 0;
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        if (a.enthalpy) {
+            Slo[i][1] += Rm[i];
+            Shi[i][1] += Rm[i];
+        }
+        double T;
+        bool conv;
+        newton_temperature(Slo[i], Shi[i], a.t_mid, a.e[p0 + i], a.T_guess[p0 + i], a.tol, a.max_iter, &T, &conv);
+        a.T[p0 + i] = T;
+        bad += conv ? 0 : 1;
+    }
+    if (a.n_not_converged != nullptr && bad) atomicAdd(a.n_not_converged, bad);
+}
+
+// ---------------------------------------------------------------------------------------
 // Ideal-gas equation of state (A.2)-(A.3) PAPER.md:892-899:
 // Rm = sum_k Y_k R/W_k = R/W_mix per point, then rho = p/(Rm T) or p = rho Rm T.  One streaming
 // pass over Y, HBM-bound; planes prefetched into L2 like the temperature kernel.
@@ -353,10 +433,26 @@ cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool table
 
 constexpr int kTempBD = 128, kTempPPT = 4;
 
+constexpr int kStreamBD = 128, kStreamDepth = 8;
+
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream) {
-    const int64_t per_block = (int64_t)kTempBD * kTempPPT;
-    const int64_t blocks = (a.n + per_block - 1) / per_block;
-    temperature_kernel<kTempBD, kTempPPT><<<dim3((unsigned)blocks), dim3(kTempBD), 0, stream>>>(a);
+    // whole blocks of 2 x kStreamBD points go through the cp.async stream when every species plane
+    // is 16-byte aligned; the rest (ragged tail, odd ld, unaligned Y) through the plain kernel
+    TempArgs rest = a;
+    const bool aligned = (a.ld % 2 == 0) && (reinterpret_cast<uintptr_t>(a.Y) % 16 == 0);
+    const size_t smem = (size_t)kStreamDepth * kStreamBD * 16 + (size_t)a.n_species * sizeof(EnergyRow);
+    const int64_t main_blocks = aligned && smem <= 48 * 1024 ? a.n / (2 * kStreamBD) : 0;
+    if (main_blocks > 0) {
+        temperature_stream_kernel<kStreamBD, kStreamDepth><<<dim3((unsigned)main_blocks), dim3(kStreamBD), smem, stream>>>(a);
+        const int64_t done = main_blocks * 2 * kStreamBD;
+        rest.n = a.n - done;
+        rest.e += done; rest.Y += done; rest.T_guess += done; rest.T += done;
+    }
+    if (rest.n > 0) {
+        const int64_t per_block = (int64_t)kTempBD * kTempPPT;
+        const int64_t blocks = (rest.n + per_block - 1) / per_block;
+        temperature_kernel<kTempBD, kTempPPT><<<dim3((unsigned)blocks), dim3(kTempBD), 0, stream>>>(rest);
+    }
     return cudaGetLastError();
 }
 

@@ -347,3 +347,34 @@ def test_degenerate_mechanisms(mechs):
         Tg = T * 1.07
         T_ref, _, _ = orc.get_temperature(e, Y, Tg)
         parity.assert_T_parity(gm.get_temperature(dev(e), dev(Y), dev(Tg)).cpu().numpy(), T_ref)
+
+
+def test_temperature_stream_and_plain_paths(mechs):
+    """pyro_get_temperature runs whole blocks of 256 points through the cp.async stream when the Y
+    planes are 16-byte aligned and the rest (ragged tail, odd leading dimension, unaligned Y) through
+    the plain kernel: same answers from every mix of the two."""
+    mech, gm, orc = mechs(2)
+    n = 256 * 5 + 77
+    st = inputs.config_states(2, n=n)
+    T_ref, _, _ = orc.get_temperature(st["e"], st["Y"], st["T_guess"])
+    ns = mech.n_species
+    for ld, shift in ((n + 1, 0), (n + 2, 0), (n + 2, 1), (n + 3, 1)):   # even / odd ld, aligned / unaligned base
+        buf = torch.zeros(ns * ld + 2, dtype=torch.float64, device="cuda")
+        Y = buf[shift:shift + ns * ld].view(ns, ld)[:, :n]
+        Y.copy_(dev(st["Y"]))
+        assert Y.stride(0) == ld and (Y.data_ptr() % 16 == 0) == (shift == 0)
+        bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+        T = gm.get_temperature(dev(st["e"]), Y, dev(st["T_guess"]), n_not_converged=bad)
+        parity.assert_T_parity(T.cpu().numpy(), T_ref)
+        assert int(bad.item()) == 0
+    # in place, stream path, with the iteration cap reported from both kernels
+    gm.set_newton(1e-300, 2)
+    try:
+        Tg = dev(st["T_guess"]).clone()
+        bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+        gm.get_temperature(dev(st["e"]), dev(st["Y"]), Tg, out=Tg, n_not_converged=bad)
+        T2_ref, _, conv2 = orc.get_temperature(st["e"], st["Y"], st["T_guess"], tol=1e-300, max_iter=2)
+        parity.assert_T_parity(Tg.cpu().numpy(), T2_ref)
+        assert int(bad.item()) == int((conv2 == 0).sum()) > n - 8
+    finally:
+        gm.set_newton(1e-6, 10)
