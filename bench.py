@@ -280,6 +280,30 @@ def main():
         # the host path and the device path compute the same thing
         assert torch.equal(om_h[:, :1024], omega[:, :1024].cpu()), "host pipeline and device path disagree"
 
+    # SURVEY.md 8(f) NEXT-1 helpers, outside the timed step: enthalpy form of the inversion and the
+    # equation of state (streaming kernels; algorithmic bytes 8(N_s + 3) per point each)
+    helpers = {}
+    if rank == 0:
+        p_in = torch.full((n,), 101325.0, dtype=torch.float64, device="cuda")
+        rho_out = torch.empty(n, dtype=torch.float64, device="cuda")
+        calls = {
+            "temperature_from_enthalpy": lambda: gm.get_temperature_from_enthalpy(d["e"], d["Y"], d["T_guess"], out=T,
+                                                                                  stream=stream),
+            "density": lambda: gm.get_density(p_in, T, d["Y"], out=rho_out, stream=stream),
+            "pressure": lambda: gm.get_pressure(rho_out, T, d["Y"], out=p_in, stream=stream),
+        }
+        for name, fn in calls.items():
+            fn()
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record(stream)
+            for _ in range(5):
+                fn()
+            t1.record(stream)
+            torch.cuda.synchronize()
+            helpers[name] = t0.elapsed_time(t1) / 5
+        gm.get_temperature(d["e"], d["Y"], d["T_guess"], rho=d["rho"], out=T, n_not_converged=bad, stream=stream)
+        torch.cuda.synchronize()
+
     if rank == 0:
         flops_pt = algorithmic_flops_per_point(mech)
         bytes_pt = algorithmic_bytes_per_point(ns)
@@ -325,6 +349,8 @@ def main():
                 "temperature_kernel_hbm": {"achieved_gbs": bytes_pt["temperature"] * n / (temp_ms * 1e-3) / 1e9,
                                            "frac": bytes_pt["temperature"] * n / (temp_ms * 1e-3) / 1e9 / hbm_peak},
             },
+            "next1_helpers_ms": {k: {"ms": v, "hbm_frac": 8.0 * (ns + 3) * n / (v * 1e-3) / 1e9 / hbm_peak}
+                                 for k, v in helpers.items()},
             "clocks": clocks.summary(),
             "gpu_launches": 2 * args.steps,
         }

@@ -389,6 +389,45 @@ __global__ void __launch_bounds__(BD) eos_kernel(const EosArgs a) {
     }
 }
 
+// The same as a cp.async stream (16-byte aligned planes), like temperature_stream_kernel.
+template <int BD, int D>
+__global__ void __launch_bounds__(BD) eos_stream_kernel(const EosArgs a) {
+    static_assert((D & (D - 1)) == 0, "ring depth must be a power of two");
+    extern __shared__ __align__(16) unsigned char tsm[];
+    double *rw = reinterpret_cast<double *>(tsm + (size_t)D * BD * 16);
+    const int tid = threadIdx.x, ns = a.n_species;
+    for (int k = tid; k < ns; k += BD) rw[k] = __ldg(&a.energy[k].rw);
+    const int64_t p0 = ((int64_t)blockIdx.x * BD + tid) * 2;
+    const double *Yp = a.Y + p0;
+    const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(tsm) + (uint32_t)tid * 16u;
+    auto issue = [&](int k) {
+        if (k < ns)
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + (uint32_t)(k & (D - 1)) * (BD * 16u)),
+                         "l"(Yp + (int64_t)k * a.ld)
+                         : "memory");
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+#pragma unroll
+    for (int s = 0; s < D; ++s) issue(s);
+    __syncthreads();
+    double Rm[2] = {0.0, 0.0};
+#pragma unroll 1
+    for (int k = 0; k < ns; ++k) {
+        asm volatile("cp.async.wait_group %0;" ::"n"(D - 1) : "memory");
+        double y[2];
+        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(y[0]), "=d"(y[1]) : "r"(slot0 + (uint32_t)(k & (D - 1)) * (BD * 16u)));
+        issue(k + D);
+        const double w = rw[k];
+        Rm[0] = fma(y[0], w, Rm[0]);
+        Rm[1] = fma(y[1], w, Rm[1]);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const double rt = Rm[i] * a.T[p0 + i];
+        a.out[p0 + i] = a.to_density ? a.in[p0 + i] / rt : a.in[p0 + i] * rt;
+    }
+}
+
 // ---------------------------------------------------------------------------------------
 // FP64 FMA peak probe: 8 independent DFMA chains per thread.
 // ---------------------------------------------------------------------------------------
@@ -459,9 +498,21 @@ cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream) {
 const void *temperature_kernel_ptr() { return (const void *)temperature_kernel<kTempBD, kTempPPT>; }
 
 cudaError_t launch_eos(const EosArgs &a, cudaStream_t stream) {
-    const int64_t per_block = (int64_t)kTempBD * kTempPPT;
-    const int64_t blocks = (a.n + per_block - 1) / per_block;
-    eos_kernel<kTempBD, kTempPPT><<<dim3((unsigned)blocks), dim3(kTempBD), 0, stream>>>(a);
+    EosArgs rest = a;
+    const bool aligned = (a.ld % 2 == 0) && (reinterpret_cast<uintptr_t>(a.Y) % 16 == 0);
+    const size_t smem = (size_t)kStreamDepth * kStreamBD * 16 + (size_t)a.n_species * sizeof(double);
+    const int64_t main_blocks = aligned ? a.n / (2 * kStreamBD) : 0;
+    if (main_blocks > 0) {
+        eos_stream_kernel<kStreamBD, kStreamDepth><<<dim3((unsigned)main_blocks), dim3(kStreamBD), smem, stream>>>(a);
+        const int64_t done = main_blocks * 2 * kStreamBD;
+        rest.n = a.n - done;
+        rest.in += done; rest.T += done; rest.Y += done; rest.out += done;
+    }
+    if (rest.n > 0) {
+        const int64_t per_block = (int64_t)kTempBD * kTempPPT;
+        const int64_t blocks = (rest.n + per_block - 1) / per_block;
+        eos_kernel<kTempBD, kTempPPT><<<dim3((unsigned)blocks), dim3(kTempBD), 0, stream>>>(rest);
+    }
     return cudaGetLastError();
 }
 

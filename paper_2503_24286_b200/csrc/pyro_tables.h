@@ -14,7 +14,8 @@
 //     (1, log2 T, 1/T, T, T^2, T^3, T^4).
 //
 // Every record is a multiple of 16 bytes and 16-byte aligned: the kernels read the tables
-// from shared memory with 128-bit loads at warp-uniform addresses (one wavefront each).
+// from shared memory with 128-bit loads at warp-uniform addresses (two wavefronts each, measured:
+// a uniform load moves 8 bytes per wavefront, so record size is shared-memory bandwidth).
 #pragma once
 #include <cstdint>
 
