@@ -36,9 +36,9 @@ METRIC = "source-term points/sec (FP64, 53 sp/325 rxn) and % of B200 FP64/HBM ro
 FLOPS_EXP, FLOPS_LOG, FLOPS_DIV = 30, 46, 15
 
 # DRAM traffic of the rates kernel measured once with `ncu --set full` (dram__bytes_read.sum +
-# dram__bytes_write.sum = 871.0 MB for 2^20 points of configs[2]; profiles/r01_v7_rates_kernel.md).
+# dram__bytes_write.sum = 866.3 MB for 2^20 points of configs[2]; profiles/r01_v8_kernels.md).
 # Reported as `traffic` for the configs[2]/[4] mechanism only, scaled to the points of one launch.
-NCU_RATES_DRAM_BYTES_PER_POINT_53SP = 871.0e6 / 1048576
+NCU_RATES_DRAM_BYTES_PER_POINT_53SP = 866.3e6 / 1048576
 
 # FP64 roof of one B200: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
