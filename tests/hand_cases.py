@@ -80,3 +80,12 @@ def degenerate_mechanisms():
              eff={3: 6.0}, **low),
     ])
     return dict(none=none, one=one, ext=ext)
+
+
+def fuzz_mechanisms():
+    """Seeded synthetic mechanisms of other shapes than the configs: reaction counts that leave ragged
+    lockstep groups, many / few special reactions, both sides of the 64-reaction packing switch."""
+    from paper_2503_24286_b200 import inputs
+    specs = [("h2", 13, 2, (1, 5), 2, 1, 11), ("h2", 40, 6, (2, 7), 3, 2, 12), ("gri", 63, 9, (4, 9), 5, 4, 13),
+             ("gri", 65, 0, (1, 1), 0, 0, 14), ("gri", 150, 40, (5, 12), 30, 10, 15), ("large", 90, 10, (6, 8), 7, 3, 16)]
+    return [inputs.make_mechanism(k, nr, ntb, ne, nt, nl, seed=sd, name=f"fuzz{sd}") for k, nr, ntb, ne, nt, nl, sd in specs]

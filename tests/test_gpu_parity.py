@@ -378,3 +378,17 @@ def test_temperature_stream_and_plain_paths(mechs):
         assert int(bad.item()) == int((conv2 == 0).sum()) > n - 8
     finally:
         gm.set_newton(1e-6, 10)
+
+
+def test_fuzz_mechanisms(mechs):
+    """Other shapes than the configs (ragged lockstep groups, both packings of leftover reactions,
+    120-species planes with few reactions): rates and temperature against the oracle."""
+    for mech in hand_cases.fuzz_mechanisms():
+        gm = binding.Mechanism(mech)
+        orc = oracle.Oracle(mech)
+        rho, T, Y = hand_cases.random_states(mech, 1500, seed=mech.n_reactions)
+        om_ref, bound = orc.get_net_production_rates(rho, T, Y)
+        parity.assert_omega_parity(gpu_rates(gm, rho, T, Y), om_ref, bound)
+        e = np.array([orc.mixture_e(float(T[p]), Y[:, p]) for p in range(1500)])
+        T_ref, _, _ = orc.get_temperature(e, Y, T * 0.93)
+        parity.assert_T_parity(gm.get_temperature(dev(e), dev(Y), dev(T * 0.93)).cpu().numpy(), T_ref)

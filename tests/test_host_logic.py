@@ -416,3 +416,10 @@ def test_emu_rates_degenerate_mechanisms(emu):
         parity.assert_omega_parity(om, om_ref, bound)
         if mech.n_reactions == 0:
             assert not om.any()
+
+
+def test_emu_rates_fuzz_mechanisms(emu):
+    for mech in hand_cases.fuzz_mechanisms():
+        rho, T, Y = hand_cases.random_states(mech, 96, seed=mech.n_reactions)
+        om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+        parity.assert_omega_parity(emu_rates(emu, mech, rho, T, Y), om_ref, bound)
