@@ -65,7 +65,8 @@ typedef struct {
     const uint8_t *type;         /* [n_reactions] PYRO_ELEMENTARY ... PYRO_FALLOFF_TROE            */
     const uint8_t *reversible;   /* [n_reactions] 1: reverse rate from K_c (A.10); 0: r_r = 0      */
     const double *eff_default;   /* [n_reactions] default third-body efficiency (usually 1)        */
-    const int32_t *eff_ptr, *eff_species; /* CSR of non-default efficiencies: ptr[n_reactions+1]   */
+    const int32_t *eff_ptr, *eff_species; /* CSR of non-default efficiencies: ptr[n_reactions+1];
+                                             within a reaction in any order, each species at most once */
     const double *eff_value;
     const double *A0, *b0, *theta0; /* [n_reactions] low-pressure limit, read when type >= 2       */
     const double *troe; /* [n_reactions][4] alpha, T***, T*, T** read when type == 3;

@@ -18,7 +18,8 @@
 //   get_temperature     P8 recovers generating T, W4 one-step convergence
 //   rate coefficient    W1 (the Arrhenius triple printed at PAPER.md:205-208)
 //   equilibrium const   W2 hand computation, P7 K_c(fwd) K_c(bwd) = 1, P6 detailed balance
-//   third body/falloff  W3 hand computation, P9 [M] = p/RT, P10 Lindemann limits, P11 Troe -> Lindemann
+//   third body/falloff  W3 hand computation, P9 [M] = p/RT, P10 Lindemann limits, P11 Troe -> Lindemann,
+//                       W5 where [M] multiplies: q_f, q_r, omega of a three-body and of falloff reactions (G8)
 //   production rates    P5 mass + element conservation, P12 scaling, P15 dense nu brute force, P16
 //   mixture_h / cp      N1 h - e = R T sum_k Y_k/W_k, N2 c_p = dh/dT, N3 c_p - c_v = R sum_k Y_k/W_k
 //   get_temperature_h   N4 recovers generating T, closed form for a constant-c_p species
@@ -190,18 +191,13 @@ ReactionDetail<Real> reaction_rate(const oracle_mech &m, int j, Real T, const Re
     Real kf = Real(m.A[j]) * std::pow(T, Real(m.b[j])) * std::exp(-Real(m.theta[j]) / T);
     d.k_inf = kf;
     // third-body concentration [M] = sum_k eff_jk C_k, eff = default unless listed (G6)
+    // (the listed efficiencies of a reaction may come in any order: plain search)
     Real M = 0;
-    {
-        int q = m.eff_ptr[j];
-        const int qend = m.eff_ptr[j + 1];
-        for (int k = 0; k < m.n_species; ++k) {
-            Real eff = Real(m.eff_default[j]);
-            if (q < qend && m.eff_species[q] == k) {
-                eff = Real(m.eff_value[q]);
-                ++q;
-            }
-            M += eff * C[k];
-        }
+    for (int k = 0; k < m.n_species; ++k) {
+        Real eff = Real(m.eff_default[j]);
+        for (int q = m.eff_ptr[j]; q < m.eff_ptr[j + 1]; ++q)
+            if (m.eff_species[q] == k) eff = Real(m.eff_value[q]);
+        M += eff * C[k];
     }
     d.M = M;
     d.F = 1;

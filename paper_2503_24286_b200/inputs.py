@@ -522,7 +522,8 @@ def simple_mechanism(species, reactions, elements=(), name="hand"):
                comp (optional element composition)}
     reactions: list of dicts {reac: {species: coeff}, prod: {species: coeff}, A, b, theta,
                type (default ELEMENTARY), reversible (default 1), eff_default (default 1),
-               eff: {species: value}, A0, b0, theta0, troe: (alpha, T3, T1, T2)}
+               eff: {species: value}, eff_order: [species...] (default ascending), A0, b0, theta0,
+               troe: (alpha, T3, T1, T2)}
     """
     ns = len(species)
     ne = len(elements)
@@ -556,7 +557,7 @@ def simple_mechanism(species, reactions, elements=(), name="hand"):
     troe[:, 0] = 1.0
     troe[:, 1:] = np.inf
     for j, r in enumerate(reactions):
-        for k in sorted(r.get("eff", {})):
+        for k in r.get("eff_order", sorted(r.get("eff", {}))):   # eff_order: list the efficiencies in that order
             esp.append(k)
             eval_.append(r["eff"][k])
         eptr.append(len(esp))

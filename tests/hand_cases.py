@@ -42,7 +42,8 @@ def all_paths_mechanism():
         dict(reac={3: 1}, prod={1: 2, 0: 1}, A=5e10, b=0.0, theta=15000.0),
         dict(reac={0: 3}, prod={2: 1, 4: 1}, A=2e9, b=-1.0, theta=500.0),
         dict(reac={2: 1, 1: 1}, prod={3: 1}, A=4e7, b=1.2, theta=-300.0, reversible=0),
-        dict(reac={0: 1, 1: 1}, prod={2: 1}, type=THREE_BODY, eff={0: 2.5, 2: 12.0}, A=1e10, b=-1.0, theta=0.0),
+        dict(reac={0: 1, 1: 1}, prod={2: 1}, type=THREE_BODY, eff={0: 2.5, 2: 12.0, 4: 0.3}, eff_order=[2, 4, 0],
+             A=1e10, b=-1.0, theta=0.0),   # efficiencies listed out of order
         dict(reac={1: 2}, prod={3: 1}, type=THREE_BODY, eff_default=0.5, eff={4: 1.5}, A=6e9, b=0.0, theta=100.0,
              reversible=0),
         dict(reac={2: 1}, prod={0: 1, 1: 1}, type=FALLOFF_LINDEMANN, eff={3: 6.0}, A=1e13, b=0.0, theta=20000.0,

@@ -155,6 +155,65 @@ def test_w4_newton_constant_cp_one_step(golden_dir):
         assert abs(T1[0] / 1234.5 - 1) < 1e-14
 
 
+def test_w5_three_body_factor_and_no_extra_factor_on_falloff(golden_dir):
+    """Reading G8: a three-body reaction has q_f = [M] k_f C_A C_B and q_r = [M] k_f/K_c C_AB; a falloff
+    reaction has [M] only inside P_r (q_f = k_eff C_A C_B, no extra factor) and its reverse rate uses the
+    same effective coefficient.  Closed-form values from the equations (make_w5.py), cross-checked here
+    against the W2 / W3 fixtures of SURVEY.md section 8(c)."""
+    g = {k: float(v) for k, v in read_golden(os.path.join(golden_dir, "w5_three_body_and_falloff_rates.txt")).items()}
+    g2 = {k: float(v) for k, v in read_golden(os.path.join(golden_dir, "w2_single_reaction.txt")).items()}
+    g3 = {k: float(v) for k, v in read_golden(os.path.join(golden_dir, "w3_falloff.txt")).items()}
+    # the fixture is consistent with the survey's hand computations
+    assert abs(g["tb_qf"] / (0.02 * g2["rf"]) - 1) < 1e-15 and abs(g["tb_qr"] / (0.02 * g2["rr"]) - 1) < 1e-15
+    assert abs(g["fo_qf_lindemann"] / (g3["k_lindemann"] * 0.004 * 0.005) - 1) < 1e-15
+    assert abs(g["fo_qf_troe"] / (g3["k_troe"] * 0.004 * 0.005) - 1) < 1e-15
+    assert abs(g["fo_qr_troe"] / (g3["k_troe"] / g["fo_Kc"] * 0.001) - 1) < 1e-15
+    # three-body
+    mech = _w2_mech(type=THREE_BODY, eff={0: 2.5, 2: 12.0})
+    for real, tol in (("f64", 2e-14), ("f80", 2e-15)):
+        o = oracle.Oracle(mech, real)
+        rho, Y = _state_from_C(mech, [2e-3, 3e-3, 1e-3])
+        d = o.reaction_detail(0, rho, 1500.0, Y)
+        assert abs(float(d["M"]) / g["tb_M"] - 1) < 1e-14
+        assert abs(float(d["kf"]) / g["tb_kf"] - 1) < 4e-15
+        assert abs(float(d["qf"]) / g["tb_qf"] - 1) < tol
+        assert abs(float(d["qr"]) / g["tb_qr"] - 1) < 50 * tol   # K_c carries exp(33): conditioning
+        om, bd = o.get_net_production_rates([rho], [1500.0], Y[:, None])
+        assert abs(float(om[2, 0]) / g["tb_omega_AB"] - 1) < tol
+        assert om[0, 0] == -om[2, 0] and om[1, 0] == -om[2, 0]
+        assert abs(float(bd[2, 0]) / (g["tb_qf"] + g["tb_qr"]) - 1) < tol
+    # falloff: no extra [M] on the rate of progress, reverse rate from the same effective coefficient
+    low = dict(A0=1e12, b0=-1.5, theta0=2000.0)
+    for rtype, troe, name in ((FALLOFF_LINDEMANN, None, "lindemann"), (FALLOFF_TROE, (0.6, 100.0, 1500.0, 5000.0), "troe")):
+        rx = dict(type=rtype, **low)
+        if troe:
+            rx["troe"] = troe
+        mech = _w2_mech(**rx)
+        o = oracle.Oracle(mech)
+        rho, Y = _state_from_C(mech, [0.004, 0.005, 0.001])
+        d = o.reaction_detail(0, rho, 1200.0, Y)
+        assert abs(d["M"] / g["fo_M"] - 1) < 1e-14
+        assert abs(d["Kc"] / g["fo_Kc"] - 1) < 1e-13
+        assert abs(d["qf"] / g["fo_qf_" + name] - 1) < 1e-13
+        assert abs(d["qr"] / g["fo_qr_" + name] - 1) < 2e-13
+        om, _ = o.get_net_production_rates([rho], [1200.0], Y[:, None])
+        assert abs(om[2, 0] / (g["fo_qf_" + name] - g["fo_qr_" + name]) - 1) < 1e-13
+
+
+def test_third_body_efficiency_lists_in_any_order():
+    """[M] = sum_k eff_k C_k (G6) does not depend on the order in which the non-default efficiencies are
+    listed (include/pyro.h: any order, each species at most once)."""
+    mech = _w2_mech(type=THREE_BODY, eff={0: 2.5, 2: 12.0})
+    rev = _w2_mech(type=THREE_BODY, eff={0: 2.5, 2: 12.0})
+    rev.eff_species = rev.eff_species[::-1].copy()
+    rev.eff_value = rev.eff_value[::-1].copy()
+    assert list(rev.eff_species) == [2, 0]
+    rho, Y = _state_from_C(mech, [2e-3, 3e-3, 1e-3])
+    a = oracle.Oracle(mech).reaction_detail(0, rho, 1500.0, Y)
+    b = oracle.Oracle(rev).reaction_detail(0, rho, 1500.0, Y)
+    assert a["M"] == b["M"] and abs(a["M"] / 0.02 - 1) < 1e-14 and a["qf"] == b["qf"]
+
+
 # ---------------------------------------------------------------- P1-P4 thermodynamics
 @pytest.fixture(scope="module")
 def cfg0():
