@@ -19,6 +19,11 @@
  *   stream) and return without synchronising; they allocate nothing and copy nothing.
  *   Concurrent calls on one handle from several host threads are allowed.
  *   There is no CPU fallback: without a CUDA device pyro_mech_create fails with PYRO_ERR_CUDA.
+ *   Environment variables read by pyro_mech_create are TEST HOOKS that force a launch shape the library would
+ *   not choose by itself (they exist so that the parity tests reach every kernel variant); they are not part of
+ *   the interface and change no result: PYRO_TABLES=shared|global, PYRO_RATES_BLOCK=<threads>,
+ *   PYRO_B_PLANE=shared, PYRO_CARVEOUT=<percent>, PYRO_RATES_TWO_BLOCKS=0|1, PYRO_PACK_SINGLES=0|1,
+ *   PYRO_HOST_SLAB=<points> (pyro_source_terms_host), PYRO_DEBUG=1 (prints the launch shape to stderr).
  */
 #ifndef PYRO_H
 #define PYRO_H
@@ -39,8 +44,14 @@ typedef enum {
     PYRO_ERR_TOO_LARGE = 4,   /* species / reactions beyond what the on-chip staging can hold (255 species) */
     PYRO_ERR_ALIGN = 5,       /* a field pointer is not 8-byte aligned                               */
     PYRO_ERR_CUDA = 6,        /* CUDA runtime error (text via pyro_last_error_string)                */
-    PYRO_ERR_UNSUPPORTED = 7  /* valid input that this build has no kernel for                      */
+    PYRO_ERR_UNSUPPORTED = 7  /* valid input that this build cannot evaluate (see PYRO_T_MIN / PYRO_T_MAX)  */
 } pyro_status;
+
+/* Supported temperature range of the rates (K).  pyro_mech_create examines the mechanism over this range
+ * and refuses (PYRO_ERR_UNSUPPORTED) one whose rates it could not evaluate in FP64 there -- see
+ * pyro_get_net_production_rates.  Outside the range nothing is checked. */
+#define PYRO_T_MIN 250.0
+#define PYRO_T_MAX 6000.0
 
 /* reaction types */
 enum { PYRO_ELEMENTARY = 0, PYRO_THREE_BODY = 1, PYRO_FALLOFF_LINDEMANN = 2, PYRO_FALLOFF_TROE = 3 };
@@ -83,7 +94,8 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out);
 int pyro_mech_destroy(pyro_mech *mech);
 
 /* Newton controls of pyro_get_temperature: stop when |dT| < abs_tol_K after the update,
- * at most max_iter iterations.  Defaults 1e-6 K and 10 (BASELINE.json configs[4]). */
+ * at most max_iter iterations.  Defaults 1e-6 K and 10 (BASELINE.json configs[4]).  May be called while other
+ * threads enqueue on the handle: a call enqueued concurrently uses either the old or the new pair member-wise. */
 int pyro_mech_set_newton(pyro_mech *mech, double abs_tol_K, int max_iter);
 
 /* Temperature from internal energy: solves  sum_k Y_k e_k(T) = e  per point by Newton's
@@ -93,7 +105,7 @@ int pyro_mech_set_newton(pyro_mech *mech, double abs_tol_K, int max_iter);
  *   Y        [n_species][ld] device, mass fractions (not clipped, not renormalised)
  *   T_guess  [n]            device, K, > 0
  *   T        [n]            device, out; may alias T_guess
- *   n_not_converged         device int32 or NULL: incremented once per point that hit max_iter
+ *   n_not_converged         device int32 (4-byte aligned) or NULL: incremented once per point that hit max_iter
  *                           (the last iterate is still written; this is not an error)
  * n == 0 returns PYRO_OK and launches nothing. */
 int pyro_get_temperature(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e,
@@ -117,7 +129,17 @@ int pyro_get_pressure(const pyro_mech *mech, int64_t n, int64_t ld, const double
 
 /* Net molar production rates omega[k*ld+p] = sum_j nu_kj R_j  (A.5)-(A.10) PAPER.md:908-934 from
  *   rho [n], T [n], Y [n_species][ld]   (device; T > 0, rho > 0, Y >= 0 are preconditions)
- *   omega [n_species][ld]               (device, out; must not alias Y) */
+ *   omega [n_species][ld]               (device, out; must not overlap Y)
+ * Range.  The kernel evaluates (A.7), (A.10) from one factor E_k = exp(g_k/RT - lambda_k(T)) RT/p0 per species
+ * and point, 1/K_c,j = prod_prod E_k / prod_reac E_k, where lambda_k(T) is the part of g_k/RT that every
+ * reversible reaction conserves (it cancels exactly in K_c; chosen at create time so that the E_k stay
+ * near 1).  Products of these factors must stay inside FP64 (2^+-1022) although K_c itself only holds their
+ * ratio.  pyro_mech_create therefore evaluates log2 E_k at 64 temperatures over [PYRO_T_MIN, PYRO_T_MAX]:
+ * a reaction whose per-side sums stay below 700 is evaluated side by side (fast path); any other reaction is
+ * evaluated in reactant/product pairs, whose partial products end at 1/K_c; and the call returns
+ * PYRO_ERR_UNSUPPORTED if even those partial sums exceed 900 (K_c within a factor 2^120 of the FP64 limits), or if
+ * log2 of a rate coefficient exceeds 2^30 in magnitude.  Inside the supported range the rates are thus finite
+ * wherever the definition's own K_c and rate coefficients are -- never a silent NaN. */
 int pyro_get_net_production_rates(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho,
                                   const double *T, const double *Y, double *omega, void *cuda_stream);
 

@@ -48,7 +48,7 @@ struct DeviceGuard {
 };
 
 constexpr int kMaxDevices = 64;
-constexpr uint32_t kWorkSlots = 4096;   // launches of one mechanism that may be in flight at once
+constexpr uint32_t kWorkSlots = 64;     // chunk counters of one mechanism: launches that run at the same time
 
 struct HostPipe {   // staging of pyro_source_terms_host
     static constexpr int kBuf = 3;
@@ -69,6 +69,8 @@ struct pyro_mech {
     pyro::EnergyRow *d_energy = nullptr;
     unsigned long long *d_work = nullptr;      // ring of chunk counters, one per launch in flight
     mutable std::atomic<uint32_t> next_work{0};
+    mutable std::vector<cudaEvent_t> work_done;   // recorded after the launch that used the slot
+    mutable std::mutex work_mu;
     bool tab_smem = false;     // tables staged in shared memory (else read from global memory)
     bool b_tmem = false;       // plane B in tensor memory beside omega (else in shared memory)
     bool two_blocks = false;   // the 128-register variant: two blocks resident per SM
@@ -78,8 +80,8 @@ struct pyro_mech {
     uint32_t tmem_cols = 32;
     int blocks_per_sm = 0;
     int sm_count = 0;
-    double newton_tol = 1e-6;
-    int newton_max_iter = 10;
+    std::atomic<double> newton_tol{1e-6};      // read by concurrent calls while pyro_mech_set_newton may write
+    std::atomic<int> newton_max_iter{10};
     std::mutex pipe_mu;
     HostPipe pipe;
 };
@@ -115,9 +117,15 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     int64_t blocks = (int64_t)m->sm_count * m->blocks_per_sm;
     if (blocks > (a.n_chunks + warps - 1) / warps) blocks = (a.n_chunks + warps - 1) / warps;
     pyro::RatesArgs args = a;
-    args.work = m->d_work + (m->next_work.fetch_add(1) % kWorkSlots);
+    // every launch in flight needs its own chunk counter: take the next slot of the ring and, before
+    // resetting it, make this stream wait for the launch that used the slot kWorkSlots launches ago
+    const uint32_t slot = m->next_work.fetch_add(1) % kWorkSlots;
+    args.work = m->d_work + slot;
+    std::lock_guard<std::mutex> lock(m->work_mu);
+    PYRO_CUDA(cudaStreamWaitEvent(stream, m->work_done[slot], 0));
     PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
     PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->smem_bytes, stream));
+    PYRO_CUDA(cudaEventRecord(m->work_done[slot], stream));
     return PYRO_OK;
 }
 
@@ -154,10 +162,11 @@ pyro::TempArgs temp_args(const pyro_mech *m, int64_t n, int64_t ld, const double
     a.n = n; a.ld = ld; a.e = e; a.Y = Y; a.T_guess = Tg; a.T = T; a.n_not_converged = bad;
     a.energy = m->d_energy;
     a.n_species = m->packed.n_species;
-    a.max_iter = m->newton_max_iter;
+    a.max_iter = m->newton_max_iter.load(std::memory_order_relaxed);
     a.t_mid = m->packed.lay.t_mid;
-    a.tol = m->newton_tol;
+    a.tol = m->newton_tol.load(std::memory_order_relaxed);
     a.enthalpy = 0;
+    a.single_t_mid = m->packed.lay.single_t_mid;
     return a;
 }
 
@@ -194,11 +203,16 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     }
     m->device = device;
     const pyro::TableLayout &lay = m->packed.lay;
-    auto bail = [&](cudaError_t e, const char *what) {
+    auto release = [&]() {
         cudaFree(m->d_blob);
         cudaFree(m->d_energy);
         cudaFree(m->d_work);
+        for (cudaEvent_t ev : m->work_done)
+            if (ev) cudaEventDestroy(ev);
         delete m;
+    };
+    auto bail = [&](cudaError_t e, const char *what) {
+        release();
         return cuda_fail(e, what);
     };
     if ((ce = cudaMalloc(&m->d_blob, lay.bytes > 0 ? lay.bytes : 8)) != cudaSuccess) return bail(ce, "cudaMalloc(tables)");
@@ -206,6 +220,10 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         return bail(ce, "cudaMemcpy(tables)");
     if ((ce = cudaMalloc(&m->d_work, kWorkSlots * sizeof(unsigned long long))) != cudaSuccess)
         return bail(ce, "cudaMalloc(work counters)");
+    m->work_done.assign(kWorkSlots, nullptr);
+    for (uint32_t i = 0; i < kWorkSlots; ++i)
+        if ((ce = cudaEventCreateWithFlags(&m->work_done[i], cudaEventDisableTiming)) != cudaSuccess)
+            return bail(ce, "cudaEventCreate(work counters)");
     const size_t ebytes = m->packed.energy.size() * sizeof(pyro::EnergyRow);
     if ((ce = cudaMalloc(&m->d_energy, ebytes)) != cudaSuccess) return bail(ce, "cudaMalloc(energy table)");
     if ((ce = cudaMemcpy(m->d_energy, m->packed.energy.data(), ebytes, cudaMemcpyHostToDevice)) != cudaSuccess)
@@ -256,10 +274,7 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         if (forced >= 32 && forced % 32 == 0 && forced <= threads) threads = forced;
     }
     if (threads < 32) {
-        cudaFree(m->d_blob);
-        cudaFree(m->d_energy);
-        cudaFree(m->d_work);
-        delete m;
+        release();
         return fail(PYRO_ERR_TOO_LARGE, "species arrays do not fit the on-chip memory of one block");
     }
     auto shape = [&](int t, size_t &smem, uint32_t &cols) {
@@ -319,10 +334,7 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (m->two_blocks && nblk < 2) nblk = 2;
     if (nblk > (int)(512 / m->tmem_cols)) nblk = (int)(512 / m->tmem_cols);   // resident blocks share 512 columns
     if (nblk < 1) {
-        cudaFree(m->d_blob);
-        cudaFree(m->d_energy);
-        cudaFree(m->d_work);
-        delete m;
+        release();
         return fail(PYRO_ERR_TOO_LARGE, "the rates kernel does not fit one SM for this mechanism");
     }
     m->blocks_per_sm = nblk;
@@ -346,11 +358,13 @@ int pyro_mech_destroy(pyro_mech *m) {
     DeviceGuard guard(m->device);
     {
         std::lock_guard<std::mutex> lock(m->pipe_mu);
-        if (m->pipe.ready) free_pipe(m->pipe);
+        free_pipe(m->pipe);
     }
     cudaFree(m->d_blob);
     cudaFree(m->d_energy);
     cudaFree(m->d_work);
+    for (cudaEvent_t ev : m->work_done)
+        if (ev) cudaEventDestroy(ev);
     delete m;
     return PYRO_OK;
 }
@@ -358,8 +372,8 @@ int pyro_mech_destroy(pyro_mech *m) {
 int pyro_mech_set_newton(pyro_mech *m, double abs_tol_K, int max_iter) {
     if (!m) return fail(PYRO_ERR_NULL, "mech is NULL");
     if (!(abs_tol_K >= 0) || max_iter < 1) return fail(PYRO_ERR_BAD_SIZE, "abs_tol_K must be >= 0 and max_iter >= 1");
-    m->newton_tol = abs_tol_K;
-    m->newton_max_iter = max_iter;
+    m->newton_tol.store(abs_tol_K, std::memory_order_relaxed);
+    m->newton_max_iter.store(max_iter, std::memory_order_relaxed);
     return PYRO_OK;
 }
 
@@ -373,10 +387,6 @@ int temperature_call(const pyro_mech *m, int64_t n, int64_t ld, const double *e,
     if (!aligned8(e) || !aligned8(Y) || !aligned8(T_guess) || !aligned8(T) ||
         (reinterpret_cast<uintptr_t>(n_not_converged) & 3u))
         return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
-    if (!m->packed.lay.single_t_mid)
-        return fail(PYRO_ERR_UNSUPPORTED,
-                    "species with different T_mid: the temperature solve of this build sums the energy "
-                    "polynomials per NASA range and needs one T_mid per mechanism");
     DeviceGuard guard(m->device);
     pyro::TempArgs a = temp_args(m, n, ld, e, Y, T_guess, T, n_not_converged);
     a.enthalpy = enthalpy ? 1 : 0;
@@ -434,7 +444,11 @@ int pyro_get_net_production_rates(const pyro_mech *m, int64_t n, int64_t ld, con
     if (!rho || !T || !Y || !omega) return fail(PYRO_ERR_NULL, "a field pointer is NULL");
     if (!aligned8(rho) || !aligned8(T) || !aligned8(Y) || !aligned8(omega))
         return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
-    if (omega == Y) return fail(PYRO_ERR_BAD_SIZE, "omega must not alias Y");
+    {   // omega is written while Y of other points is still being read: no overlap of the two fields at all
+        const uintptr_t span = (uintptr_t)(((int64_t)m->packed.n_species - 1) * ld + n) * sizeof(double);
+        const uintptr_t y0 = reinterpret_cast<uintptr_t>(Y), w0 = reinterpret_cast<uintptr_t>(omega);
+        if (y0 < w0 + span && w0 < y0 + span) return fail(PYRO_ERR_BAD_SIZE, "omega must not overlap Y");
+    }
     DeviceGuard guard(m->device);
     return enqueue_rates(m, rates_args(m, n, ld, rho, T, Y, omega), static_cast<cudaStream_t>(cuda_stream));
 }
@@ -451,6 +465,21 @@ int pyro_source_terms_host(pyro_mech *m, int64_t n, int64_t ld, const double *rh
     std::lock_guard<std::mutex> lock(m->pipe_mu);
     HostPipe &p = m->pipe;
     const int ns = m->packed.n_species;
+    // a failure leaves no half-built pipe behind and no copy in flight into the caller's buffers
+    auto drain = [&]() {
+        if (p.s_in) cudaStreamSynchronize(p.s_in);
+        if (p.s_run) cudaStreamSynchronize(p.s_run);
+        if (p.s_out) cudaStreamSynchronize(p.s_out);
+    };
+#define PYRO_PIPE(call)                                         \
+    do {                                                        \
+        cudaError_t e_ = (call);                                \
+        if (e_ != cudaSuccess) {                                \
+            drain();                                            \
+            if (!p.ready) free_pipe(p);                         \
+            return cuda_fail(e_, #call);                        \
+        }                                                       \
+    } while (0)
     if (!p.ready) {
         // slab of points: about 64 MB of mass fractions per buffer
         int64_t slab = (int64_t)(64.0 * 1024 * 1024 / (8.0 * ns));
@@ -459,50 +488,54 @@ int pyro_source_terms_host(pyro_mech *m, int64_t n, int64_t ld, const double *rh
         if (const char *env = std::getenv("PYRO_HOST_SLAB")) slab = std::atoll(env) > 0 ? std::atoll(env) : slab;
         p.slab = slab;
         for (int b = 0; b < HostPipe::kBuf; ++b) {
-            PYRO_CUDA(cudaMalloc(&p.rho[b], slab * 8));
-            PYRO_CUDA(cudaMalloc(&p.e[b], slab * 8));
-            PYRO_CUDA(cudaMalloc(&p.Tg[b], slab * 8));
-            PYRO_CUDA(cudaMalloc(&p.T[b], slab * 8));
-            PYRO_CUDA(cudaMalloc(&p.Y[b], slab * 8 * ns));
-            PYRO_CUDA(cudaMalloc(&p.omega[b], slab * 8 * ns));
-            PYRO_CUDA(cudaEventCreateWithFlags(&p.in_done[b], cudaEventDisableTiming));
-            PYRO_CUDA(cudaEventCreateWithFlags(&p.run_done[b], cudaEventDisableTiming));
-            PYRO_CUDA(cudaEventCreateWithFlags(&p.out_done[b], cudaEventDisableTiming));
+            PYRO_PIPE(cudaMalloc(&p.rho[b], slab * 8));
+            PYRO_PIPE(cudaMalloc(&p.e[b], slab * 8));
+            PYRO_PIPE(cudaMalloc(&p.Tg[b], slab * 8));
+            PYRO_PIPE(cudaMalloc(&p.T[b], slab * 8));
+            PYRO_PIPE(cudaMalloc(&p.Y[b], slab * 8 * ns));
+            PYRO_PIPE(cudaMalloc(&p.omega[b], slab * 8 * ns));
+            PYRO_PIPE(cudaEventCreateWithFlags(&p.in_done[b], cudaEventDisableTiming));
+            PYRO_PIPE(cudaEventCreateWithFlags(&p.run_done[b], cudaEventDisableTiming));
+            PYRO_PIPE(cudaEventCreateWithFlags(&p.out_done[b], cudaEventDisableTiming));
         }
-        PYRO_CUDA(cudaStreamCreateWithFlags(&p.s_in, cudaStreamNonBlocking));
-        PYRO_CUDA(cudaStreamCreateWithFlags(&p.s_run, cudaStreamNonBlocking));
-        PYRO_CUDA(cudaStreamCreateWithFlags(&p.s_out, cudaStreamNonBlocking));
-        PYRO_CUDA(cudaMalloc(&p.d_bad, sizeof(int32_t)));
+        PYRO_PIPE(cudaStreamCreateWithFlags(&p.s_in, cudaStreamNonBlocking));
+        PYRO_PIPE(cudaStreamCreateWithFlags(&p.s_run, cudaStreamNonBlocking));
+        PYRO_PIPE(cudaStreamCreateWithFlags(&p.s_out, cudaStreamNonBlocking));
+        PYRO_PIPE(cudaMalloc(&p.d_bad, sizeof(int32_t)));
         p.ready = true;
     }
-    PYRO_CUDA(cudaMemsetAsync(p.d_bad, 0, sizeof(int32_t), p.s_run));
+    PYRO_PIPE(cudaMemsetAsync(p.d_bad, 0, sizeof(int32_t), p.s_run));
     const int64_t slab = p.slab;
     int64_t i = 0;
     for (int64_t s0 = 0; s0 < n; s0 += slab, ++i) {
         const int b = (int)(i % HostPipe::kBuf);
         const int64_t cnt = (n - s0 < slab) ? (n - s0) : slab;
         // the buffer is free once the results of its previous slab have left
-        if (i >= HostPipe::kBuf) PYRO_CUDA(cudaStreamWaitEvent(p.s_in, p.out_done[b], 0));
-        PYRO_CUDA(cudaMemcpyAsync(p.rho[b], rho + s0, cnt * 8, cudaMemcpyHostToDevice, p.s_in));
-        PYRO_CUDA(cudaMemcpyAsync(p.e[b], e + s0, cnt * 8, cudaMemcpyHostToDevice, p.s_in));
-        PYRO_CUDA(cudaMemcpyAsync(p.Tg[b], T_guess + s0, cnt * 8, cudaMemcpyHostToDevice, p.s_in));
-        PYRO_CUDA(cudaMemcpy2DAsync(p.Y[b], slab * 8, Y + s0, ld * 8, cnt * 8, ns, cudaMemcpyHostToDevice, p.s_in));
-        PYRO_CUDA(cudaEventRecord(p.in_done[b], p.s_in));
-        PYRO_CUDA(cudaStreamWaitEvent(p.s_run, p.in_done[b], 0));
-        PYRO_CUDA(pyro::launch_temperature(temp_args(m, cnt, slab, p.e[b], p.Y[b], p.Tg[b], p.T[b], p.d_bad), p.s_run));
+        if (i >= HostPipe::kBuf) PYRO_PIPE(cudaStreamWaitEvent(p.s_in, p.out_done[b], 0));
+        PYRO_PIPE(cudaMemcpyAsync(p.rho[b], rho + s0, cnt * 8, cudaMemcpyHostToDevice, p.s_in));
+        PYRO_PIPE(cudaMemcpyAsync(p.e[b], e + s0, cnt * 8, cudaMemcpyHostToDevice, p.s_in));
+        PYRO_PIPE(cudaMemcpyAsync(p.Tg[b], T_guess + s0, cnt * 8, cudaMemcpyHostToDevice, p.s_in));
+        PYRO_PIPE(cudaMemcpy2DAsync(p.Y[b], slab * 8, Y + s0, ld * 8, cnt * 8, ns, cudaMemcpyHostToDevice, p.s_in));
+        PYRO_PIPE(cudaEventRecord(p.in_done[b], p.s_in));
+        PYRO_PIPE(cudaStreamWaitEvent(p.s_run, p.in_done[b], 0));
+        PYRO_PIPE(pyro::launch_temperature(temp_args(m, cnt, slab, p.e[b], p.Y[b], p.Tg[b], p.T[b], p.d_bad), p.s_run));
         st = enqueue_rates(m, rates_args(m, cnt, slab, p.rho[b], p.T[b], p.Y[b], p.omega[b]), p.s_run);
-        if (st != PYRO_OK) return st;
-        PYRO_CUDA(cudaEventRecord(p.run_done[b], p.s_run));
-        PYRO_CUDA(cudaStreamWaitEvent(p.s_out, p.run_done[b], 0));
-        PYRO_CUDA(cudaMemcpyAsync(T + s0, p.T[b], cnt * 8, cudaMemcpyDeviceToHost, p.s_out));
-        PYRO_CUDA(cudaMemcpy2DAsync(omega + s0, ld * 8, p.omega[b], slab * 8, cnt * 8, ns, cudaMemcpyDeviceToHost, p.s_out));
-        PYRO_CUDA(cudaEventRecord(p.out_done[b], p.s_out));
+        if (st != PYRO_OK) {
+            drain();
+            return st;
+        }
+        PYRO_PIPE(cudaEventRecord(p.run_done[b], p.s_run));
+        PYRO_PIPE(cudaStreamWaitEvent(p.s_out, p.run_done[b], 0));
+        PYRO_PIPE(cudaMemcpyAsync(T + s0, p.T[b], cnt * 8, cudaMemcpyDeviceToHost, p.s_out));
+        PYRO_PIPE(cudaMemcpy2DAsync(omega + s0, ld * 8, p.omega[b], slab * 8, cnt * 8, ns, cudaMemcpyDeviceToHost, p.s_out));
+        PYRO_PIPE(cudaEventRecord(p.out_done[b], p.s_out));
     }
     int32_t bad = 0;
-    PYRO_CUDA(cudaMemcpyAsync(&bad, p.d_bad, sizeof bad, cudaMemcpyDeviceToHost, p.s_run));
-    PYRO_CUDA(cudaStreamSynchronize(p.s_run));
-    PYRO_CUDA(cudaStreamSynchronize(p.s_out));
-    PYRO_CUDA(cudaStreamSynchronize(p.s_in));
+    PYRO_PIPE(cudaMemcpyAsync(&bad, p.d_bad, sizeof bad, cudaMemcpyDeviceToHost, p.s_run));
+    PYRO_PIPE(cudaStreamSynchronize(p.s_run));
+    PYRO_PIPE(cudaStreamSynchronize(p.s_out));
+    PYRO_PIPE(cudaStreamSynchronize(p.s_in));
+#undef PYRO_PIPE
     if (n_not_converged) *n_not_converged = bad;
     return PYRO_OK;
 }

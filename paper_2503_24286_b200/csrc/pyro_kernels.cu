@@ -273,6 +273,38 @@ __global__ void __launch_bounds__(BD) temperature_kernel(const TempArgs a) {
 }
 
 // ---------------------------------------------------------------------------------------
+// Row a4 for mechanisms whose species have different break temperatures (reading G10): one
+// thread per point, newton_temperature_general (pyro_point.cuh).  The first pass over Y streams from
+// HBM (planes prefetched into L2 ahead of the loads); a repeated pass -- an iterate crossed a break
+// temperature -- finds the point's column in L2.
+// ---------------------------------------------------------------------------------------
+template <int BD>
+__global__ void __launch_bounds__(BD) temperature_general_kernel(const TempArgs a) {
+    const int64_t p = (int64_t)blockIdx.x * BD + threadIdx.x;
+    const int64_t pc = p < a.n ? p : a.n - 1;
+    const int ns = a.n_species;
+    constexpr int kAhead = 8;
+    if ((threadIdx.x & 15) == 0)
+        for (int k = 0; k < ns && k < kAhead; ++k) asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)k * a.ld + pc));
+    const double *Yp = a.Y + pc;
+    double T;
+    bool conv;
+    newton_temperature_general(
+        ns,
+        [&](int k) {
+            if (k + kAhead < ns && (threadIdx.x & 15) == 0)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(Yp + (int64_t)(k + kAhead) * a.ld));
+            return Yp[(int64_t)k * a.ld];
+        },
+        [&](int k) -> const EnergyRow & { return a.energy[k]; }, a.enthalpy != 0, a.e[pc], a.T_guess[pc], a.tol, a.max_iter, &T,
+        &conv);
+    if (p < a.n) {
+        a.T[p] = T;
+        if (a.n_not_converged != nullptr && !conv) atomicAdd(a.n_not_converged, 1);
+    }
+}
+
+// ---------------------------------------------------------------------------------------
 // The same solve as a software-pipelined stream (used when the Y planes are 16-byte aligned):
 // thread t owns points 2t, 2t+1 of its block's 2 BD points and copies their 16 bytes of every
 // species plane into its own slot of a D-deep shared-memory ring with cp.async, D species ahead
@@ -475,6 +507,11 @@ constexpr int kTempBD = 128, kTempPPT = 4;
 constexpr int kStreamBD = 128, kStreamDepth = 8;
 
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream) {
+    if (!a.single_t_mid) {   // species with different break temperatures: the interval-wise solve
+        const int64_t blocks = (a.n + kTempBD - 1) / kTempBD;
+        temperature_general_kernel<kTempBD><<<dim3((unsigned)blocks), dim3(kTempBD), 0, stream>>>(a);
+        return cudaGetLastError();
+    }
     // whole blocks of 2 x kStreamBD points go through the cp.async stream when every species plane
     // is 16-byte aligned; the rest (ragged tail, odd ld, unaligned Y) through the plain kernel
     TempArgs rest = a;

@@ -34,6 +34,7 @@ struct TempArgs {
     int32_t n_species, max_iter;
     double t_mid, tol;
     int32_t enthalpy;            // 0: e given, Newton with c_v (A.27); 1: h given, Newton with c_p
+    int32_t single_t_mid;        // 1: every species switches NASA range at t_mid (streaming kernels); 0: general kernel
 };
 
 struct EosArgs {                 // (A.2)-(A.3): out = in / (Rm T) (density from pressure) or in Rm T (pressure from density)

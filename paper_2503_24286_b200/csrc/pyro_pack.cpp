@@ -7,11 +7,15 @@
 #include <cstdlib>
 #include <cstring>
 #include <algorithm>
+#include <array>
 #include <map>
 
 namespace pyro {
 namespace {
 
+constexpr long double kMaxSideLog2 = 700.0L;    // plain class: largest |sum over a reaction side of log2 E_k| (FP64 holds 2^+-1022)
+constexpr long double kMaxPairLog2 = 900.0L;    // extended class: largest |partial sum of product/reactant pair exponents|
+constexpr long double kMaxExp2Arg = 1073741824.0L;   // 2^30: exp2_poly reduces |y| < 2^31
 constexpr long double kR = 8314.46261815324L;   // J/(kmol K)
 constexpr long double kP0 = 101325.0L;          // Pa
 const long double kLog2e = 1.0L / std::log(2.0L);
@@ -40,22 +44,128 @@ template <class T> void put(std::vector<unsigned char> &blob, uint32_t off, cons
 //   g/RT = a1 (1 - ln T) - a2/2 T - a3/6 T^2 - a4/12 T^3 - a5/20 T^4 + a6/T - a7
 // which is h/RT - s/R of (A.12), (A.13) with the readings G2, G3.  The coefficient of log2 T
 // needs no log2e factor (a ln T = a log2 T / log2e).
-void species_row(const double *a, double dst[7]) {
+void species_row(const double *a, long double dst[7]) {
     const long double c0 = (long double)a[0] - (long double)a[6] + std::log(kR / kP0);
-    dst[0] = (double)(c0 * kLog2e);
-    dst[1] = (double)(1.0L - (long double)a[0]);
-    dst[2] = (double)((long double)a[5] * kLog2e);
-    dst[3] = (double)(-(long double)a[1] / 2 * kLog2e);
-    dst[4] = (double)(-(long double)a[2] / 6 * kLog2e);
-    dst[5] = (double)(-(long double)a[3] / 12 * kLog2e);
-    dst[6] = (double)(-(long double)a[4] / 20 * kLog2e);
+    dst[0] = c0 * kLog2e;
+    dst[1] = 1.0L - (long double)a[0];
+    dst[2] = (long double)a[5] * kLog2e;
+    dst[3] = -(long double)a[1] / 2 * kLog2e;
+    dst[4] = -(long double)a[2] / 6 * kLog2e;
+    dst[5] = -(long double)a[3] / 12 * kLog2e;
+    dst[6] = -(long double)a[4] / 20 * kLog2e;
+}
+
+// value of a row at T
+long double row_value(const long double c[7], long double T) {
+    const long double l2t = std::log2(T);
+    return c[0] + c[1] * l2t + c[2] / T + T * (c[3] + T * (c[4] + T * (c[5] + T * c[6])));
+}
+
+// Temperatures at which the packer examines a mechanism: kGuardPoints values spaced geometrically over
+// the supported range [PYRO_T_MIN, PYRO_T_MAX] of include/pyro.h.
+constexpr int kGuardPoints = 64;
+long double guard_temperature(int i) {
+    return (long double)PYRO_T_MIN * std::pow((long double)PYRO_T_MAX / (long double)PYRO_T_MIN, (long double)i / (kGuardPoints - 1));
+}
+
+// Conserved-quantity shift of the species rows (see pyro_tables.h "Range").  nu[j] lists the net
+// stoichiometric coefficients (species, coefficient) of the reversible reactions.  On return lam[k][f],
+// f = 0..2, is what is subtracted from the (1, log2 T, 1/T) coefficients of BOTH rows of species k.
+// Every lam[.][f] is orthogonal to every nu[j] (checked; all zeros are returned if the check fails), so
+// sum_k nu_kj log2 E_k -- the equilibrium constant -- is unchanged.
+void conserved_shift(int ns, const std::vector<std::vector<std::pair<int, int>>> &nu,
+                     const std::vector<std::array<long double, 7>> &lo, const std::vector<std::array<long double, 7>> &hi,
+                     const double *t_mid, std::vector<std::array<long double, 3>> &lam) {
+    lam.assign(ns, {0.0L, 0.0L, 0.0L});
+    // orthonormal basis Q of span{nu_j} by modified Gram-Schmidt (twice), in long double
+    std::vector<std::vector<long double>> Q;
+    std::vector<long double> v(ns);
+    for (const auto &col : nu) {
+        if ((int)Q.size() == ns) break;   // full rank: nothing is conserved, no shift possible
+        std::fill(v.begin(), v.end(), 0.0L);
+        long double n0 = 0;
+        for (auto &kc : col) v[kc.first] += kc.second;
+        for (int k = 0; k < ns; ++k) n0 += v[k] * v[k];
+        if (n0 == 0) continue;
+        for (int pass = 0; pass < 2; ++pass)
+            for (const auto &q : Q) {
+                long double d = 0;
+                for (int k = 0; k < ns; ++k) d += q[k] * v[k];
+                for (int k = 0; k < ns; ++k) v[k] -= d * q[k];
+            }
+        long double n1 = 0;
+        for (int k = 0; k < ns; ++k) n1 += v[k] * v[k];
+        if (n1 <= 1e-18L * n0) continue;   // dependent on the reactions seen so far
+        const long double inv = 1.0L / std::sqrt(n1);
+        for (int k = 0; k < ns; ++k) v[k] *= inv;
+        Q.push_back(v);
+    }
+    if ((int)Q.size() == ns) return;
+    auto project = [&](std::vector<long double> &x) {   // x <- (I - Q Q^T) x : the conserved part of x
+        for (int pass = 0; pass < 2; ++pass)
+            for (const auto &q : Q) {
+                long double d = 0;
+                for (int k = 0; k < ns; ++k) d += q[k] * x[k];
+                for (int k = 0; k < ns; ++k) x[k] -= d * q[k];
+            }
+    };
+    // least squares over the guard temperatures: lam_k(T) = lam[k][0] + lam[k][1] log2 T + lam[k][2]/T
+    // approximates the conserved part of log2 E(T) (each species on the NASA range it is in at T)
+    long double G[3][3] = {{0}}, phi[3];
+    std::vector<std::array<long double, 3>> rhs(ns, {0.0L, 0.0L, 0.0L});
+    std::vector<long double> L(ns);
+    for (int i = 0; i < kGuardPoints; ++i) {
+        const long double T = guard_temperature(i);
+        for (int k = 0; k < ns; ++k) L[k] = row_value(T < (long double)t_mid[k] ? lo[k].data() : hi[k].data(), T);
+        project(L);
+        phi[0] = 1.0L; phi[1] = std::log2(T); phi[2] = 1.0L / T;
+        for (int a = 0; a < 3; ++a) {
+            for (int b = 0; b < 3; ++b) G[a][b] += phi[a] * phi[b];
+            for (int k = 0; k < ns; ++k) rhs[k][a] += phi[a] * L[k];
+        }
+    }
+    // solve the 3x3 normal equations (Gauss-Jordan with pivoting), the same matrix for every species
+    long double inv[3][3] = {{1, 0, 0}, {0, 1, 0}, {0, 0, 1}};
+    for (int c = 0; c < 3; ++c) {
+        int piv = c;
+        for (int r = c + 1; r < 3; ++r)
+            if (std::fabs(G[r][c]) > std::fabs(G[piv][c])) piv = r;
+        if (G[piv][c] == 0) return;
+        for (int b = 0; b < 3; ++b) { std::swap(G[c][b], G[piv][b]); std::swap(inv[c][b], inv[piv][b]); }
+        const long double d = 1.0L / G[c][c];
+        for (int b = 0; b < 3; ++b) { G[c][b] *= d; inv[c][b] *= d; }
+        for (int r = 0; r < 3; ++r)
+            if (r != c) {
+                const long double m = G[r][c];
+                for (int b = 0; b < 3; ++b) { G[r][b] -= m * G[c][b]; inv[r][b] -= m * inv[c][b]; }
+            }
+    }
+    std::vector<long double> col(ns);
+    for (int f = 0; f < 3; ++f) {
+        for (int k = 0; k < ns; ++k) col[k] = inv[f][0] * rhs[k][0] + inv[f][1] * rhs[k][1] + inv[f][2] * rhs[k][2];
+        project(col);   // the solve amplifies rounding: put the coefficient vector back into the conserved space
+        for (int k = 0; k < ns; ++k) lam[k][f] = col[k];
+    }
+    // the shift must cancel in every reversible reaction: |nu_j . lam_f| at rounding level, else no shift
+    for (const auto &r : nu)
+        for (int f = 0; f < 3; ++f) {
+            long double dot = 0, mag = 0;
+            for (auto &kc : r) {
+                dot += kc.second * lam[kc.first][f];
+                mag += std::fabs(kc.second * lam[kc.first][f]);
+            }
+            if (std::fabs(dot) > 1e-16L * mag + 1e-300L) {
+                lam.assign(ns, {0.0L, 0.0L, 0.0L});
+                return;
+            }
+        }
 }
 
 uint32_t align16(uint32_t x) { return (x + 15u) & ~15u; }
 
 }   // namespace
 
-int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, int leftover) {
+int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, int leftover, int shift) {
     try {
         PYRO_REQUIRE(d != nullptr, PYRO_ERR_NULL, "desc is NULL");
         const int ns = d->n_species, nr = d->n_reactions, ne = d->n_elements;
@@ -159,6 +269,66 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
                 }
         }
 
+        // ---- species rows: log2 E_k folded in long double, shifted by the conserved part (pyro_tables.h
+        // "Range"), rounded once
+        std::vector<std::array<long double, 7>> rowLo(ns), rowHi(ns);
+        for (int k = 0; k < ns; ++k) {
+            species_row(d->nasa_lo + 7 * k, rowLo[k].data());
+            species_row(d->nasa_hi + 7 * k, rowHi[k].data());
+        }
+        std::vector<std::vector<std::pair<int, int>>> nuRev;   // net coefficients of the reversible reactions
+        for (int j = 0; j < nr; ++j) {
+            if (!d->reversible[j]) continue;
+            std::map<int, int> net;
+            for (int q = d->reac_ptr[j]; q < d->reac_ptr[j + 1]; ++q) net[d->reac_species[q]] -= d->reac_coeff[q];
+            for (int q = d->prod_ptr[j]; q < d->prod_ptr[j + 1]; ++q) net[d->prod_species[q]] += d->prod_coeff[q];
+            std::vector<std::pair<int, int>> col;
+            for (auto &kv : net)
+                if (kv.second != 0) col.push_back(kv);
+            if (!col.empty()) nuRev.push_back(col);
+        }
+        std::vector<std::array<long double, 3>> lam;
+        conserved_shift(ns, nuRev, rowLo, rowHi, d->t_mid, lam);
+        if (shift == kShiftOff) lam.assign(ns, {0.0L, 0.0L, 0.0L});
+        for (int k = 0; k < ns; ++k)
+            for (int f = 0; f < 3; ++f) {
+                rowLo[k][f] -= lam[k][f];
+                rowHi[k][f] -= lam[k][f];
+            }
+        // log2 E_k at the guard temperatures (row ns: the dummy species, E = 1); and the exponents of the rate
+        // coefficients, which exp2 must be able to reduce
+        std::vector<std::vector<long double>> Lg(kGuardPoints, std::vector<long double>(ns + 1, 0.0L));
+        for (int i = 0; i < kGuardPoints; ++i) {
+            const long double T = guard_temperature(i), l2t = std::log2(T);
+            for (int k = 0; k < ns; ++k) {
+                Lg[i][k] = row_value(T < (long double)d->t_mid[k] ? rowLo[k].data() : rowHi[k].data(), T);
+                PYRO_REQUIRE(std::fabs(Lg[i][k]) <= kMaxPairLog2, PYRO_ERR_UNSUPPORTED,
+                             "species %d: |log2 E| = %.0f at %.0f K is beyond what FP64 products of species factors can hold "
+                             "(limit %.0f; supported range %g-%g K)", k, (double)std::fabs(Lg[i][k]), (double)T,
+                             (double)kMaxPairLog2, (double)PYRO_T_MIN, (double)PYRO_T_MAX);
+            }
+            for (int j = 0; j < nr; ++j) {
+                const long double yk = std::log((long double)d->A[j]) * kLog2e + d->b[j] * l2t - (long double)d->theta[j] * kLog2e / T;
+                long double y0 = 0;
+                if (d->type[j] >= PYRO_FALLOFF_LINDEMANN)
+                    y0 = std::log((long double)d->A0[j]) * kLog2e + d->b0[j] * l2t - (long double)d->theta0[j] * kLog2e / T;
+                PYRO_REQUIRE(std::fabs(yk) < kMaxExp2Arg && std::fabs(y0) < kMaxExp2Arg, PYRO_ERR_UNSUPPORTED,
+                             "reaction %d: log2 of a rate coefficient reaches %.3g at %.0f K (exp2 reduces |y| < 2^30)", j,
+                             (double)std::max(std::fabs(yk), std::fabs(y0)), (double)T);
+            }
+        }
+        out.max_side_log2 = out.max_pair_log2 = 0.0;
+        out.n_wide = 0;
+        std::vector<SpecRow> spec(ns);
+        for (int k = 0; k < ns; ++k) {
+            spec[k].inv_w = (double)(1.0L / (long double)d->mol_weight[k]);
+            spec[k].t_mid = d->t_mid[k];
+            for (int f = 0; f < 7; ++f) {
+                spec[k].lo[f] = (double)rowLo[k][f];
+                spec[k].hi[f] = (double)rowHi[k][f];
+            }
+        }
+
         // ---- reactions: records
         std::vector<RxnP> recP;
         std::vector<RxnX> recX;
@@ -191,7 +361,23 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
             f[1] = d->b[j];
             f[2] = (double)(-(long double)d->theta[j] * kLog2e);
             const int type = d->type[j];
-            if (type == PYRO_ELEMENTARY && !repeated && reversible) {
+            // Range (pyro_tables.h): the plain class multiplies each side's species factors on their own, which
+            // is safe while |sum over a side of log2 E_k| <= kMaxSideLog2 over the supported temperatures; a
+            // reaction beyond that ("wide") goes to the extended class, whose products are formed in
+            // reactant/product pairs.
+            long double side = 0;
+            for (int i = 0; i < kGuardPoints; ++i) {
+                long double sr = 0, sp = 0;
+                for (int m = 0; m < 3; ++m) {
+                    sr += Lg[i][slot[m]];
+                    sp += Lg[i][slot[3 + m]];
+                }
+                side = std::max(side, std::max(std::fabs(sr), reversible ? std::fabs(sp) : 0.0L));
+            }
+            const bool wide = side > kMaxSideLog2;
+            if (wide && type == PYRO_ELEMENTARY && !repeated && reversible) ++out.n_wide;
+            if (!wide && (double)side > out.max_side_log2) out.max_side_log2 = (double)side;
+            if (type == PYRO_ELEMENTARY && !repeated && reversible && !wide) {
                 RxnP p;
                 std::memset(&p, 0, sizeof p);
                 for (int m = 0; m < 3; ++m) p.f[m] = f[m];
@@ -209,6 +395,43 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
             RxnX x;
             std::memset(&x, 0, sizeof x);
             for (int m = 0; m < 3; ++m) x.f[m] = f[m];
+            // The extended class forms the reverse product as prod_i (A_product,i B_reactant,i), i = 0..2 (padded
+            // with the dummy species), so only the partial sums of d_i = log2 E_product,i - log2 E_reactant,i
+            // must stay in range.  Order the slots so that the largest |d_i| and |partial sum| over the guard
+            // temperatures is smallest (36 orderings), and refuse the mechanism if even that is too large.
+            if (reversible) {
+                const int perms[6][3] = {{0, 1, 2}, {0, 2, 1}, {1, 0, 2}, {1, 2, 0}, {2, 0, 1}, {2, 1, 0}};
+                long double best = -1;
+                int bestR = 0, bestP = 0;
+                for (int pr = 0; pr < 6; ++pr)
+                    for (int pp = 0; pp < 6; ++pp) {
+                        long double cost = 0;
+                        for (int i = 0; i < kGuardPoints; ++i) {
+                            long double run = 0;
+                            for (int m = 0; m < 3; ++m) {
+                                const long double dm = Lg[i][slot[3 + perms[pp][m]]] - Lg[i][slot[perms[pr][m]]];
+                                run += dm;
+                                cost = std::max(cost, std::max(std::fabs(dm), std::fabs(run)));
+                            }
+                        }
+                        if (best < 0 || cost < best) {
+                            best = cost;
+                            bestR = pr;
+                            bestP = pp;
+                        }
+                    }
+                PYRO_REQUIRE(best <= kMaxPairLog2, PYRO_ERR_UNSUPPORTED,
+                             "reaction %d: products of its species factors reach 2^%.0f inside %g-%g K, beyond what FP64 "
+                             "holds (limit 2^%.0f); its equilibrium constant is out of range there", j, (double)best,
+                             (double)PYRO_T_MIN, (double)PYRO_T_MAX, (double)kMaxPairLog2);
+                if ((double)best > out.max_pair_log2) out.max_pair_log2 = (double)best;
+                uint32_t ordered[6];
+                for (int m = 0; m < 3; ++m) {
+                    ordered[m] = slot[perms[bestR][m]];
+                    ordered[3 + m] = slot[3 + perms[bestP][m]];
+                }
+                for (int m = 0; m < 6; ++m) slot[m] = ordered[m];
+            }
             for (int m = 0; m < 6; ++m) x.slot[m] = slot[m];
             x.rev = reversible ? 1 : 0;
             x.type = (int16_t)type;
@@ -239,10 +462,16 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
                 if (type == PYRO_FALLOFF_TROE) {
                     const double *t = d->troe + 4 * j;
                     fl.troe_alpha = t[0];
-                    fl.troe_t3 = (double)(-kLog2e / (long double)t[1]);
-                    fl.troe_t1 = std::isinf(t[2]) ? 0.0 : (double)(-kLog2e / (long double)t[2]);
+                    // Sentinel temperatures of real mechanisms (T*** = 1e-30, T** = 1e30 ...) make the exponent
+                    // exceed what exp2 reduces (|y| < 2^31).  Clamp the coefficients where the term is exactly
+                    // zero in FP64 anyway: exp(-T/T***) with T*** < 1.4e-4 K is 0 for every T >= 1 K, and
+                    // exp(-T**/T) with T** > 7.4e8 K is 0 for every T <= 1e5 K; the clamped exponents stay
+                    // below 2^31 for 1 K <= T <= 1e5 K and still underflow to zero there.
+                    const long double kMaxSlope = 1.0e4L, kMaxT2 = 1073741824.0L;
+                    fl.troe_t3 = (double)std::max(-kLog2e / (long double)t[1], -kMaxSlope);
+                    fl.troe_t1 = std::isinf(t[2]) ? 0.0 : (double)std::max(-kLog2e / (long double)t[2], -kMaxSlope);
                     fl.troe_has_t2 = std::isinf(t[3]) ? 0.0 : 1.0;
-                    fl.troe_t2 = std::isinf(t[3]) ? 0.0 : (double)(-kLog2e * (long double)t[3]);
+                    fl.troe_t2 = std::isinf(t[3]) ? 0.0 : (double)std::max(-kLog2e * (long double)t[3], -kMaxT2);
                 }
                 x.fall_index = (uint32_t)recFall.size();
                 recFall.push_back(fl);
@@ -398,15 +627,6 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
         }
         recX.swap(sortedX);
 
-        // ---- species rows
-        std::vector<SpecRow> spec(ns);
-        for (int k = 0; k < ns; ++k) {
-            spec[k].inv_w = (double)(1.0L / (long double)d->mol_weight[k]);
-            spec[k].t_mid = d->t_mid[k];
-            species_row(d->nasa_lo + 7 * k, spec[k].lo);
-            species_row(d->nasa_hi + 7 * k, spec[k].hi);
-        }
-
         // ---- blob
         TableLayout &lay = out.lay;
         std::memset(&lay, 0, sizeof lay);
@@ -453,7 +673,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
         for (int k = 0; k < ns; ++k) {
             const long double rw = kR / (long double)d->mol_weight[k];
             out.energy[k].rw = (double)rw;
-            out.energy[k].pad = 0.0;
+            out.energy[k].t_mid = d->t_mid[k];
             for (int range = 0; range < 2; ++range) {
                 const double *a = (range ? d->nasa_hi : d->nasa_lo) + 7 * k;
                 double *c = range ? out.energy[k].hi : out.energy[k].lo;

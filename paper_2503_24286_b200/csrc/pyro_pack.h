@@ -19,6 +19,9 @@ struct PackedMech {
     std::vector<EnergyRow> energy;     // temperature-solve table [n_species]
     std::vector<int> order;            // packed record -> reaction index of the description (-1: null record)
     int n_species = 0, n_reactions = 0;
+    double max_side_log2 = 0.0;        // plain class: largest |sum over a reaction side of log2 E_k| over the guard temperatures
+    double max_pair_log2 = 0.0;        // extended class: largest |partial sum of pair exponents| (pyro_tables.h "Range")
+    int n_wide = 0;                    // reactions that are in the extended class only because a side sum exceeds the plain limit
 };
 
 // Returns a pyro_status; on failure `err` says which entry was rejected.
@@ -27,6 +30,10 @@ struct PackedMech {
 // kernel variant must then contain the one-at-a-time loops), kLeftoverAuto takes singles for
 // fewer than 64 reactions (environment PYRO_PACK_SINGLES=0/1 overrides; host tests).
 enum { kLeftoverAuto = -1, kLeftoverPad = 0, kLeftoverSingles = 1 };
-int pack_mechanism(const pyro_mech_desc *desc, PackedMech &out, std::string &err, int leftover = kLeftoverAuto);
+// `shift`: kShiftOn subtracts the conserved part of log2 E_k from the species rows (pyro_tables.h "Range");
+// kShiftOff leaves the rows as folded (host tests: the two must give the same rates).
+enum { kShiftOn = 1, kShiftOff = 0 };
+int pack_mechanism(const pyro_mech_desc *desc, PackedMech &out, std::string &err, int leftover = kLeftoverAuto,
+                   int shift = kShiftOn);
 
 }   // namespace pyro

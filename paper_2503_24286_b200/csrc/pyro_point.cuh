@@ -281,10 +281,13 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
         mem.fence_ld();
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            const double pf = a[b][0] * a[b][1] * a[b][2];
-            const double pr = rev[b] != 0.0 ? a[b][3] * a[b][4] * a[b][5] : 0.0;   // irreversible: r_r = 0 (G19)
-            const double pb = mem.value(br[b][0]) * mem.value(br[b][1]) * mem.value(br[b][2]);
-            double R = (y[b * NE] * pb) * (pf - pr) * fall[b];
+            // Pair form (pyro_tables.h "Range"): prod_reac C_k = prod_i (A_ri B_ri) and
+            // prod_prod C_k / K_c = prod_i (A_pi B_ri), multiplied left to right in the slot order the packer
+            // chose, so that no partial product leaves the FP64 range while the rate itself is in it.
+            const double b0 = mem.value(br[b][0]), b1 = mem.value(br[b][1]), b2 = mem.value(br[b][2]);
+            const double pf = (a[b][0] * b0) * (a[b][1] * b1) * (a[b][2] * b2);
+            const double pr = rev[b] != 0.0 ? (a[b][3] * b0) * (a[b][4] * b1) * (a[b][5] * b2) : 0.0;   // irreversible: r_r = 0 (G19)
+            double R = y[b * NE] * (pf - pr) * fall[b];
             if (KIND == kExtThreeBody) R *= M[b];   // R = [M](q_f - q_r), reading G8
 #pragma unroll
             for (int m = 0; m < 6; ++m) mem.stW(hW[b][m], fma(nu[b][m], R, mem.value(wr[b][m])));
@@ -403,6 +406,55 @@ PYRO_HD int newton_temperature(const double *Slo, const double *Shi, double t_mi
             conv = true;
             break;
         }
+    }
+    *T_out = T;
+    *converged = conv;
+    return it;
+}
+
+// The same solve for mechanisms whose species switch NASA range at different temperatures (G10: the
+// range is chosen per species at every iterate).  The mixture polynomial S = sum_k Y_k c_k(range of k at T) is
+// valid on the whole interval [t_below, t_above) between the two break temperatures that enclose T, so it
+// is summed once (one pass over the species: `load_y(k)` and the energy row of k) and the Newton
+// iteration continues on it at O(1) per step until an iterate leaves the interval; then the pass is
+// repeated for the interval the iterate fell into.  Iterates, stop rule and count are those of
+// newton_temperature.  `enthalpy`: S[1] += sum_k Y_k R/W_k (h = e + T R/W_mix).
+template <class LoadY, class Row>
+PYRO_HD int newton_temperature_general(int ns, const LoadY &load_y, const Row &row_of, bool enthalpy, double e, double T,
+                                       double tol, int max_iter, double *T_out, bool *converged) {
+    int it = 0;
+    bool conv = false;
+    while (it < max_iter && !conv) {
+        double S[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, Rm = 0.0;
+        double t_below = -1.0, t_above = 1.7976931348623157e308;
+#pragma unroll 1
+        for (int k = 0; k < ns; ++k) {
+            const EnergyRow &r = row_of(k);
+            const double y = load_y(k), tm = r.t_mid;
+            const bool low = T < tm;
+            const double *c = low ? r.lo : r.hi;
+#pragma unroll
+            for (int m = 0; m < 6; ++m) S[m] = fma(y, c[m], S[m]);
+            Rm = fma(y, r.rw, Rm);
+            t_above = low && tm < t_above ? tm : t_above;
+            t_below = !low && tm > t_below ? tm : t_below;
+        }
+        if (enthalpy) S[1] += Rm;
+        do {
+            double eT = fma(S[5], T, S[4]);
+            eT = fma(eT, T, S[3]);
+            eT = fma(eT, T, S[2]);
+            eT = fma(eT, T, S[1]);
+            eT = fma(eT, T, S[0]);
+            double cv = fma(5.0 * S[5], T, 4.0 * S[4]);
+            cv = fma(cv, T, 3.0 * S[3]);
+            cv = fma(cv, T, 2.0 * S[2]);
+            cv = fma(cv, T, S[1]);
+            const double dT = -(eT - e) / cv;
+            T += dT;
+            ++it;
+            conv = fabs(dT) < tol;
+        } while (!conv && it < max_iter && T >= t_below && T < t_above);   // NaN leaves the loop and the pass repeats until the cap
     }
     *T_out = T;
     *converged = conv;

@@ -13,6 +13,24 @@
 // All exponents are stored in log2 units on the per-point features
 //     (1, log2 T, 1/T, T, T^2, T^3, T^4).
 //
+// Range.  Taken literally the E_k are huge or tiny (|log2 E_k| ~ 1.44 |a6|/T: hundreds at 300 K) and a
+// reaction side multiplies up to three of them, which overflows FP64 long before K_c -- which only holds
+// the DIFFERENCE sum_k nu_kj log2 E_k -- does.  The identity above holds unchanged for
+//     E'_k = E_k 2^(-lambda_k(T))   whenever   sum_k nu_kj lambda_k(T) = 0 for every reversible reaction j,
+// i.e. for any lambda(T) in the left null space of the stoichiometric matrix (the conserved quantities:
+// element counts, inert species, ...); C_k = A_k B_k is unchanged too.  The packer takes
+//     lambda_k(T) = l_k0 + l_k1 log2 T + l_k2 / T
+// as the least-squares fit, over the supported temperature range, of the projection of log2 E(T) onto that
+// null space (pyro_pack.cpp: conserved_shift), and stores log2 E'_k: the same seven features, the first
+// three coefficients shifted, both NASA ranges of a species by the same amount.  What is left in log2 E'_k
+// is the part of the Gibbs energies that the reactions can actually see.  The packer then evaluates
+// |sum over a side of log2 E'_k| of every reaction over the supported range: up to 700 the reaction may
+// be in the plain class (sides multiplied on their own); beyond, it goes to the extended class, which
+// multiplies in reactant/product pairs, so that only partial sums of log2 E'_p - log2 E'_r occur -- they
+// end at -log2 K_c (up to the p0/RT factor), which is finite wherever the definition's own K_c is.  The
+// packer orders the pairs for the smallest partial sums and refuses (PYRO_ERR_UNSUPPORTED) a mechanism whose
+// partial sums exceed 900 inside [PYRO_T_MIN, PYRO_T_MAX] (include/pyro.h).
+//
 // Every record is a multiple of 16 bytes and 16-byte aligned: the kernels read the tables
 // from shared memory with 128-bit loads at warp-uniform addresses (two wavefronts each, measured:
 // a uniform load moves 8 bytes per wavefront, so record size is shared-memory bandwidth).
@@ -51,8 +69,11 @@ struct alignas(16) RxnP {
     uint32_t slot[6];   // species: reactants 0..nreac-1, then products nreac..nreac+nprod-1
 };
 
-// Extended class: three-body and falloff reactions, irreversible reactions, and reactions
-// with a repeated species (coefficient 2 or 3, or a species on both sides).  Stored by kind,
+// Extended class: three-body and falloff reactions, irreversible reactions, reactions
+// with a repeated species (coefficient 2 or 3, or a species on both sides), and "wide" reactions
+// (a side's sum of log2 E_k exceeds 700 somewhere in the supported temperature range).  The rate is
+// formed in reactant/product pairs, R = k [prod_i (A_ri B_ri) - prod_i (A_pi B_ri)], i = 0..2 left to
+// right, with the slots ordered by the packer so that the partial products stay in range.  Stored by kind,
 // within a kind first the groups of four reactions with mutually disjoint scatter lists, then
 // the couples, then the reactions left alone.  The six slots list every molecule (a
 // coefficient 2 repeats the species), reactants in 0..2 and products in 3..5; unused slots and
@@ -127,9 +148,10 @@ struct GroupCounts {
 // and      c_v(T) = de/dT                                 (A.29)-(A.31) PAPER.md:1025-1034
 // rw = R/W_k serves the enthalpy form (h_k = e_k + R T/W_k) and the equation of
 // state (A.2)-(A.3) PAPER.md:892-899: sum_k Y_k R/W_k = R / W_mix.
+// t_mid: the species' own break temperature (the general solve for mechanisms with several of them).
 struct alignas(16) EnergyRow {
     double lo[6], hi[6];
-    double rw, pad;
+    double rw, t_mid;
 };
 
 }   // namespace pyro

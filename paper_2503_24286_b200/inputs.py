@@ -394,27 +394,48 @@ def mixture_energy(mech, T, Y, dtype=np.longdouble):
     numpy.longdouble (the default for small n) "Newton recovers T" tests the solve and
     not this generator; at bench sizes float64 is used because e is then just an input."""
     ld = dtype
-    n = T.shape[0]
-    e = np.empty(n, dtype=np.float64)
-    low = T < T_MID
-    for mask, coef in ((low, mech.nasa_lo), (~low, mech.nasa_hi)):
-        idx = np.nonzero(mask)[0]
-        if idx.size == 0:
-            continue
-        Ts = T[idx].astype(ld)
-        acc = np.zeros(idx.size, dtype=ld)
-        for k in range(mech.n_species):
-            a = coef[k].astype(ld)
-            # (h/(R T) - 1) T = (a1-1) T + a2/2 T^2 + ... + a5/5 T^5 + a6
-            poly = a[4] / 5
-            poly = poly * Ts + a[3] / 4
-            poly = poly * Ts + a[2] / 3
-            poly = poly * Ts + a[1] / 2
-            poly = poly * Ts + (a[0] - 1)
-            poly = poly * Ts + a[5]
-            acc += Y[k, idx].astype(ld) * poly / ld(mech.mol_weight[k])
-        e[idx] = (acc * ld(R_UNIVERSAL)).astype(np.float64)
-    return e
+    Ts = T.astype(ld)
+    acc = np.zeros(T.shape[0], dtype=ld)
+    for tm in np.unique(mech.t_mid):   # each species on its own range (reading G10); one mask per break temperature
+        low = T < tm
+        for mask, coef in ((low, mech.nasa_lo), (~low, mech.nasa_hi)):
+            idx = np.nonzero(mask)[0]
+            if idx.size == 0:
+                continue
+            Tk = Ts[idx]
+            part = np.zeros(idx.size, dtype=ld)
+            for k in np.nonzero(mech.t_mid == tm)[0]:
+                a = coef[k].astype(ld)
+                # (h/(R T) - 1) T = (a1-1) T + a2/2 T^2 + ... + a5/5 T^5 + a6
+                poly = a[4] / 5
+                poly = poly * Tk + a[3] / 4
+                poly = poly * Tk + a[2] / 3
+                poly = poly * Tk + a[1] / 2
+                poly = poly * Tk + (a[0] - 1)
+                poly = poly * Tk + a[5]
+                part += Y[k, idx].astype(ld) * poly / ld(mech.mol_weight[k])
+            acc[idx] += part
+    return (acc * ld(R_UNIVERSAL)).astype(np.float64)
+
+
+def with_species_break_temperatures(mech, t_mids):
+    """A copy of `mech` whose species k switches NASA range at t_mids[k % len(t_mids)] instead of T_MID.  The
+    high range keeps its a3..a5; a1, a2, a6, a7 are solved again so that c_p, dc_p/dT, h and s are continuous
+    at the species' own break temperature (rule H1 at another T_mid).  Real NASA-7 files carry one break
+    temperature per species; the configs use 1000 K throughout."""
+    import copy
+    out = copy.deepcopy(mech)
+    out.t_mid = np.array([t_mids[k % len(t_mids)] for k in range(mech.n_species)], dtype=np.float64)
+    out.nasa_hi = mech.nasa_hi.copy()
+    for k in range(mech.n_species):
+        lo, hi, Tm = mech.nasa_lo[k], out.nasa_hi[k], out.t_mid[k]
+        dlo = lo[1] + 2 * lo[2] * Tm + 3 * lo[3] * Tm**2 + 4 * lo[4] * Tm**3
+        hi[1] = dlo - (2 * hi[2] * Tm + 3 * hi[3] * Tm**2 + 4 * hi[4] * Tm**3)
+        hi[0] = _cp_R(lo, Tm) - (hi[1] * Tm + hi[2] * Tm**2 + hi[3] * Tm**3 + hi[4] * Tm**4)
+        hi[5] = lo[5] + sum((lo[m] - hi[m]) * Tm ** (m + 1) / (m + 1) for m in range(5))
+        hi[6] = lo[6] + (lo[0] - hi[0]) * np.log(Tm) + sum((lo[m] - hi[m]) * Tm**m / m for m in range(1, 5))
+    out.name = mech.name + "_tmids"
+    return out
 
 
 def _dirichlet(rng, alpha, ns, n):

@@ -90,3 +90,43 @@ def fuzz_mechanisms():
     specs = [("h2", 13, 2, (1, 5), 2, 1, 11), ("h2", 40, 6, (2, 7), 3, 2, 12), ("gri", 63, 9, (4, 9), 5, 4, 13),
              ("gri", 65, 0, (1, 1), 0, 0, 14), ("gri", 150, 40, (5, 12), 30, 10, 15), ("large", 90, 10, (6, 8), 7, 3, 16)]
     return [inputs.make_mechanism(k, nr, ntb, ne, nt, nl, seed=sd, name=f"fuzz{sd}") for k, nr, ntb, ne, nt, nl, sd in specs]
+
+
+def extreme_thermo_mechanisms(a6):
+    """Species whose a6 (formation enthalpy / R) is `a6` for every species: |g/RT| ~ |a6|/T is far beyond what a
+    product of per-species factors exp(g/RT) can hold in FP64, while the Gibbs-energy DIFFERENCES that the
+    equilibrium constants see are small or moderate.
+      "balanced":  A + B <=> C + D in all four reaction types (sum nu = 0: the common a6 cancels in K_c)
+      "assoc":     A + B <=> AB, A + AB <=> B + A2-like ... (sum nu != 0: K_c keeps one a6/T)"""
+    def sp(W, a1, a7, dh=0.0):
+        lo = [a1, 4.0e-4, -5.0e-8, 0.0, 0.0, a6 + dh, a7]
+        return dict(W=W, lo=lo)   # one range
+    low = dict(A0=1e12, b0=-1.5, theta0=2000.0)
+    four = [sp(10.0, 3.5, 2.0), sp(12.0, 3.0, 4.0, 800.0), sp(9.0, 3.2, 3.0, -600.0), sp(13.0, 3.3, 2.5, 300.0)]
+    balanced = simple_mechanism(four, [
+        dict(reac={0: 1, 1: 1}, prod={2: 1, 3: 1}, A=3e9, b=0.3, theta=2500.0),
+        dict(reac={0: 1, 1: 1}, prod={2: 1, 3: 1}, type=THREE_BODY, eff={0: 2.0, 3: 5.0}, A=1e10, b=-0.5, theta=500.0),
+        dict(reac={2: 1, 3: 1}, prod={0: 1, 1: 1}, type=FALLOFF_TROE, troe=(0.6, 100.0, 1500.0, 5000.0), eff={1: 3.0},
+             A=2e10, b=0.0, theta=1500.0, **low),
+        dict(reac={0: 1, 1: 1}, prod={2: 1, 3: 1}, A=4e8, b=0.0, theta=1000.0, reversible=0),
+    ], name=f"balanced{a6:g}")
+    three = [sp(10.0, 3.5, 2.0), sp(12.0, 3.0, 4.0, 800.0), sp(22.0, 4.2, 5.0, -900.0)]
+    assoc = simple_mechanism(three, [
+        dict(reac={0: 1, 1: 1}, prod={2: 1}, A=3e9, b=0.3, theta=2500.0),
+        dict(reac={2: 1}, prod={0: 1, 1: 1}, type=FALLOFF_LINDEMANN, eff={0: 2.0}, A=1e13, b=0.0, theta=20000.0,
+             A0=1e14, b0=-0.5, theta0=18000.0),
+    ], name=f"assoc{a6:g}")
+    return dict(balanced=balanced, assoc=assoc)
+
+
+def troe_sentinel_mechanism():
+    """Troe parameter sets with the sentinel temperatures real mechanism files carry (T*** = 1e-30, T* = 1e30,
+    T** = 1e30): the exponents -T/T***, -T**/T are astronomically large, the terms themselves exactly 0 or 1."""
+    low = dict(A0=1e12, b0=-1.5, theta0=2000.0)
+    return simple_mechanism(species5(), [
+        dict(reac={0: 1, 1: 1}, prod={2: 1}, type=FALLOFF_TROE, troe=(0.7, 1e-30, 1e30, np.inf), **W1, **low),
+        dict(reac={4: 1, 0: 1}, prod={3: 1}, type=FALLOFF_TROE, troe=(0.5, 120.0, 1800.0, 1e30), A=2e10, b=0.3, theta=900.0, **low),
+        dict(reac={1: 2}, prod={3: 1}, type=FALLOFF_TROE, troe=(0.4, 1e-8, 900.0, 1e30), A=6e9, b=0.0, theta=100.0, **low),
+        dict(reac={2: 1}, prod={0: 1, 1: 1}, type=FALLOFF_TROE, troe=(0.62, 1e-30, 1e30, 4000.0), A=1e13, b=0.0,
+             theta=20000.0, A0=1e14, b0=-0.5, theta0=18000.0),
+    ], name="troe_sentinels")

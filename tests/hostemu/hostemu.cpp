@@ -87,11 +87,28 @@ int emu_pack_order(const pyro_mech_desc *d, int32_t *order, int32_t cap) {
     return st;
 }
 
+// largest |sum over a reaction side of log2 E_k| over the guard temperatures, with (shift = 1) and without
+// (shift = 0) the conserved-quantity shift of the species rows; the range guard is what may reject
+int emu_pack_side_log2(const pyro_mech_desc *d, int shift, double *out) {
+    pyro::PackedMech pm;
+    int st = pyro::pack_mechanism(d, pm, g_err, pyro::kLeftoverAuto, shift ? pyro::kShiftOn : pyro::kShiftOff);
+    out[0] = pm.max_side_log2; out[1] = pm.max_pair_log2; out[2] = pm.n_wide;
+    return st;
+}
+
+int emu_rates2(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
+               double *omega, int shift);
+
 // the per-point functions of the rates kernel, one point after the other
 int emu_rates(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
               double *omega) {
+    return emu_rates2(d, n, ld, rho, T, Y, omega, 1);
+}
+
+int emu_rates2(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
+               double *omega, int shift) {
     pyro::PackedMech pm;
-    int st = pyro::pack_mechanism(d, pm, g_err);
+    int st = pyro::pack_mechanism(d, pm, g_err, pyro::kLeftoverAuto, shift ? pyro::kShiftOn : pyro::kShiftOff);
     if (st != PYRO_OK) return st;
     HostTab tab{pm.blob.data(), pm.lay};
     const pyro::GroupCounts g = group_counts(pm.lay);
@@ -136,9 +153,19 @@ int emu_temperature2(const pyro_mech_desc *d, int64_t n, int64_t ld, const doubl
     pyro::PackedMech pm;
     int st = pyro::pack_mechanism(d, pm, g_err);
     if (st != PYRO_OK) return st;
-    if (!pm.lay.single_t_mid) return PYRO_ERR_UNSUPPORTED;
     const int ns = pm.n_species;
     int64_t bad = 0;
+    if (!pm.lay.single_t_mid) {   // the arithmetic of temperature_general_kernel
+        for (int64_t p = 0; p < n; ++p) {
+            bool conv;
+            pyro::newton_temperature_general(
+                ns, [&](int k) { return Y[k * ld + p]; }, [&](int k) -> const pyro::EnergyRow & { return pm.energy[k]; },
+                enthalpy != 0, e[p], Tg[p], tol, max_iter, &T[p], &conv);
+            bad += conv ? 0 : 1;
+        }
+        if (n_bad) *n_bad = bad;
+        return PYRO_OK;
+    }
     for (int64_t p = 0; p < n; ++p) {
         double Slo[6] = {0, 0, 0, 0, 0, 0}, Shi[6] = {0, 0, 0, 0, 0, 0}, Rm = 0.0;
         for (int k = 0; k < ns; ++k) {

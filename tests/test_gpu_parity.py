@@ -194,6 +194,26 @@ def test_abi_error_codes_on_device(mechs):
     g = lib.pyro_get_temperature
     assert g(h, 64, 64, None, None, Y.data_ptr(), T.data_ptr(), T.data_ptr(), None, None) == 1
     assert g(h, 64, 10, None, rho.data_ptr(), Y.data_ptr(), T.data_ptr(), T.data_ptr(), None, None) == 2
+    # partial overlap of omega with Y (not only pointer equality): the second plane of Y, and a range that ends inside Y
+    assert f(h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), Y.data_ptr() + 8 * 64, None) == 2
+    assert f(h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr() + 8 * 64 * (mech.n_species - 1), Y.data_ptr(), None) == 2
+    # ld < n and alignment on every entry point, including the NEXT-1 helpers
+    bad32 = torch.zeros(4, dtype=torch.int32, device="cuda")
+    assert g(h, 64, 64, None, rho.data_ptr(), Y.data_ptr(), T.data_ptr(), T.data_ptr(), bad32.data_ptr() + 2, None) == 5
+    assert g(h, 64, 64, None, rho.data_ptr() + 4, Y.data_ptr(), T.data_ptr(), T.data_ptr(), None, None) == 5
+    ge = lib.pyro_get_temperature_from_enthalpy
+    assert ge(h, 64, 63, rho.data_ptr(), Y.data_ptr(), T.data_ptr(), T.data_ptr(), None, None) == 2
+    assert ge(h, 64, 64, rho.data_ptr(), Y.data_ptr(), T.data_ptr(), T.data_ptr(), bad32.data_ptr() + 1, None) == 5
+    assert ge(h, 64, 64, None, Y.data_ptr(), T.data_ptr(), T.data_ptr(), None, None) == 1
+    for eos in (lib.pyro_get_density, lib.pyro_get_pressure):
+        assert eos(h, 64, 63, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), om.data_ptr(), None) == 2
+        assert eos(h, -5, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), om.data_ptr(), None) == 2
+        assert eos(h, 64, 64, rho.data_ptr(), T.data_ptr() + 4, Y.data_ptr(), om.data_ptr(), None) == 5
+        assert eos(h, 64, 64, rho.data_ptr(), None, Y.data_ptr(), om.data_ptr(), None) == 1
+        assert eos(h, 0, 0, None, None, None, None, None) == 0   # n == 0 launches nothing
+    hs = lib.pyro_source_terms_host
+    assert hs(h, 64, 63, None, None, None, None, None, None, None) == 2
+    assert hs(h, 64, 64, None, None, None, None, None, None, None) == 1
     assert lib.pyro_mech_set_newton(h, -1.0, 10) == 2 and lib.pyro_mech_set_newton(h, 1e-6, 0) == 2
     assert lib.pyro_last_error_string()
     out = C.c_void_p()
@@ -271,19 +291,69 @@ def test_plane_b_in_shared_memory_path(mechs, monkeypatch):
 
 
 def test_species_with_different_t_mid(mechs):
-    """The rates path switches NASA range per species; the temperature solve of this build refuses."""
-    import copy
-    mech = copy.deepcopy(inputs.config_mechanism(0))
-    mech.t_mid = mech.t_mid.copy()
-    mech.t_mid[::2] = 1400.0
-    mech.t_mid[1::3] = 800.0
+    """Per-species break temperatures (G10): the rates path switches range per species and point, and the
+    temperature solve (energy and enthalpy form) re-sums the mixture polynomial whenever an iterate crosses a
+    break temperature -- both against the oracle, which chooses the range per species at every iterate."""
+    from test_host_logic import _mixed_tmid_case
+    for cfg, n in ((0, 5000), (2, 1111)):
+        mech, T, Y, e, h, Tg = _mixed_tmid_case(cfg, n)
+        gm = binding.Mechanism(mech)
+        orc = oracle.Oracle(mech)
+        rho = np.full(n, 0.7)
+        om_ref, bound = orc.get_net_production_rates(rho, T, Y)
+        parity.assert_omega_parity(gpu_rates(gm, rho, T, Y), om_ref, bound)
+        T_ref, _, conv = orc.get_temperature(e, Y, Tg)
+        assert conv.all()
+        bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+        T_gpu = gm.get_temperature(dev(e), dev(Y), dev(Tg), n_not_converged=bad).cpu().numpy()
+        parity.assert_T_parity(T_gpu, T_ref)
+        assert int(bad.item()) == 0
+        Th_ref, _, _ = orc.get_temperature_from_enthalpy(h, Y, Tg)
+        parity.assert_T_parity(gm.get_temperature_from_enthalpy(dev(h), dev(Y), dev(Tg)).cpu().numpy(), Th_ref)
+        # padded leading dimension and an iteration cap of 2: last iterates and the count as the oracle's
+        ld = n + 37
+        Yp = torch.full((mech.n_species, ld), float("nan"), dtype=torch.float64, device="cuda")
+        Yp[:, :n] = dev(Y)
+        gm.set_newton(1e-6, 2)
+        T2_ref, _, conv2 = orc.get_temperature(e, Y, Tg, max_iter=2)
+        bad.zero_()
+        T2 = gm.get_temperature(dev(e), Yp[:, :n], dev(Tg), n_not_converged=bad).cpu().numpy()
+        parity.assert_T_parity(T2, T2_ref)
+        assert int(bad.item()) == int((conv2 == 0).sum())
+        gm.set_newton(1e-6, 10)
+        gm.close()
+
+
+@pytest.mark.parametrize("a6", [1.2e5, -1.2e5, 2.5e5, -2.5e5])
+def test_rates_finite_wherever_the_oracle_is_extreme_formation_enthalpies(a6):
+    """|g_k/RT| up to 1000 per species at 250 K (SURVEY.md section 7 hard part 4; (A.10) PAPER.md:932): the shifted
+    species factors and the pair form of wide reactions keep the kernel finite and within tolerance wherever
+    the oracle is; a mechanism whose K_c itself leaves FP64 inside the supported range is refused at create."""
+    from test_host_logic import _cold_to_hot_states
+    for name, mech in hand_cases.extreme_thermo_mechanisms(a6).items():
+        rho, T, Y = _cold_to_hot_states(mech, 1500)
+        om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+        if name == "assoc" and abs(a6) > 2e5:
+            with pytest.raises(binding.PyroError) as ei:
+                binding.Mechanism(mech)
+            assert ei.value.status == 7 and "250" in str(ei.value)
+            continue
+        assert np.isfinite(om_ref).all() and np.isfinite(bound).all()
+        gm = binding.Mechanism(mech)
+        parity.assert_omega_parity(gpu_rates(gm, rho, T, Y), om_ref, bound)
+        gm.close()
+
+
+def test_troe_sentinel_temperatures():
+    """T*** = 1e-30, T* = 1e30, T** = 1e30 as real mechanism files carry them."""
+    mech = hand_cases.troe_sentinel_mechanism()
+    rho, T, Y = hand_cases.random_states(mech, 2000)
+    T[:4] = [250.0, 1234.5, 3000.0, 6000.0]
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+    assert np.isfinite(om_ref).all()
     gm = binding.Mechanism(mech)
-    st = inputs.config_states(0, n=3000)
-    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
-    parity.assert_omega_parity(gpu_rates(gm, st["rho"], st["T"], st["Y"]), om_ref, bound)
-    with pytest.raises(binding.PyroError) as ei:
-        gm.get_temperature(dev(st["e"]), dev(st["Y"]), dev(st["T_guess"]))
-    assert ei.value.status == 7
+    parity.assert_omega_parity(gpu_rates(gm, rho, T, Y), om_ref, bound)
+    gm.close()
 
 
 def test_host_buffer_pipeline_matches_oracle(mechs, monkeypatch):

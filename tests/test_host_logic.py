@@ -73,6 +73,8 @@ def emu():
     L.emu_temperature.argtypes = [vp, i64, i64, vp, vp, vp, C.c_double, C.c_int, vp, vp]
     L.emu_temperature2.argtypes = [vp, i64, i64, vp, vp, vp, C.c_double, C.c_int, vp, vp, C.c_int]
     L.emu_eos.argtypes = [vp, i64, i64, vp, vp, vp, vp, C.c_int]
+    L.emu_rates2.argtypes = [vp, i64, i64, vp, vp, vp, vp, C.c_int]
+    L.emu_pack_side_log2.argtypes = [vp, C.c_int, vp]
     return L
 
 
@@ -84,6 +86,24 @@ def emu_rates(emu, mech, rho, T, Y):
                        Y.ctypes.data, om.ctypes.data)
     assert st == 0, emu.emu_last_error()
     return om
+
+
+def emu_rates_status(emu, mech, rho, T, Y, shift=1):
+    """(status, omega, message) of the host build of the rates path; shift = 0 packs without the conserved shift."""
+    desc, keep = binding.make_desc(mech)
+    rho, T, Y = (np.ascontiguousarray(x, dtype=np.float64) for x in (rho, T, Y))
+    om = np.empty_like(Y)
+    st = emu.emu_rates2(C.byref(desc), rho.shape[0], rho.shape[0], rho.ctypes.data, T.ctypes.data,
+                        Y.ctypes.data, om.ctypes.data, shift)
+    return st, om, emu.emu_last_error().decode()
+
+
+def pack_range(emu, mech, shift=1):
+    """(status, largest side sum of the plain class, largest pair partial sum, wide reactions)."""
+    desc, keep = binding.make_desc(mech)
+    out = (C.c_double * 3)()
+    st = emu.emu_pack_side_log2(C.byref(desc), shift, out)
+    return st, out[0], out[1], int(out[2])
 
 
 def emu_temperature(emu, mech, e, Y, Tg, tol=1e-6, max_iter=10):
@@ -188,7 +208,8 @@ def _expected_plain(mech):
 def test_packer_classes_and_table_size(emu):
     for mech in (inputs.config_mechanism(0), inputs.config_mechanism(2), hand_cases.all_paths_mechanism()):
         st, info, _ = pack_status(emu, mech)
-        n_plain = _expected_plain(mech)
+        # wide reactions (a side's species factors beyond 2^700 at the cold end) leave the plain class
+        n_plain = _expected_plain(mech) - pack_range(emu, mech)[3]
         order = pack_order(emu, mech, info[0] + info[1])
         assert st == 0
         # records = reactions (+ null records that complete a couple, in mechanisms of 64 reactions or more)
@@ -325,6 +346,90 @@ def _reaction_dict(mech, j):
     return d
 
 
+def _cold_to_hot_states(mech, n, seed=3):
+    rng = np.random.default_rng(seed)
+    T = np.concatenate([[250.0, 251.0, 300.0, 6000.0], rng.uniform(250.0, 3500.0, size=n - 4)])
+    Y = rng.dirichlet(np.full(mech.n_species, 0.8), size=n).T.copy()
+    rho = rng.uniform(0.05, 5.0, size=n)
+    return rho, T, Y
+
+
+@pytest.mark.parametrize("a6", [1.2e5, -1.2e5, 2.5e5, -2.5e5])
+def test_emu_rates_finite_wherever_the_oracle_is_extreme_formation_enthalpies(emu, a6):
+    """SURVEY.md section 7 hard part 4 / (A.10) PAPER.md:932: |g_k/RT| ~ |a6|/T up to 1000 per species at 250 K.
+    The per-species factors are shifted by what the reactions conserve and wide reactions are multiplied in
+    pairs, so the rates are finite and within tolerance wherever the oracle's are; a mechanism whose K_c
+    itself leaves the FP64 range inside the supported temperatures is refused with a message, never NaN."""
+    for name, mech in hand_cases.extreme_thermo_mechanisms(a6).items():
+        rho, T, Y = _cold_to_hot_states(mech, 400)
+        om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+        st, om, msg = emu_rates_status(emu, mech, rho, T, Y)
+        if name == "assoc" and abs(a6) > 2e5:
+            # K_c ~ exp(+-a6/T) = 2^+-1440 at 250 K: out of range for the definition itself
+            assert not np.isfinite(om_ref[:, T < 300]).all()
+            assert st == 7 and "K" in msg and "250" in msg
+            continue
+        assert st == 0, msg
+        ok = np.isfinite(om_ref).all(axis=0) & np.isfinite(bound).all(axis=0)
+        assert ok.all(), "the oracle is finite on the whole supported range for the accepted mechanisms"
+        assert np.isfinite(om).all()
+        parity.assert_omega_parity(om, om_ref, bound)
+
+
+def test_conserved_shift_changes_nothing_but_the_range(emu):
+    """Packing with and without the shift of the species rows gives the same rates (it cancels exactly in K_c
+    and in C_k = A_k B_k); without it the extreme mechanism is out of range and is refused."""
+    for cfg, n in ((0, 512), (2, 128)):
+        mech = inputs.config_mechanism(cfg)
+        st = inputs.config_states(cfg, n=n)
+        om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
+        for shift in (0, 1):
+            s, om, msg = emu_rates_status(emu, mech, st["rho"], st["T"], st["Y"], shift)
+            assert s == 0, msg
+            assert parity.assert_omega_parity(om, om_ref, bound) < 1e-12
+        s1, side1, pair1, wide1 = pack_range(emu, mech, 1)
+        assert s1 == 0 and side1 <= 700.0 and pair1 <= 900.0
+    mech = hand_cases.extreme_thermo_mechanisms(-2.5e5)["balanced"]
+    s0, *_ = pack_range(emu, mech, 0)
+    s1, side1, pair1, wide1 = pack_range(emu, mech, 1)
+    assert s0 == 7 and s1 == 0 and side1 < 50.0 and wide1 == 0   # the common a6/T is gone entirely
+
+
+def test_wide_reactions_take_the_pair_form(emu):
+    """A reaction whose side sums exceed 2^700 at the cold end goes to the extended class, which multiplies in
+    reactant/product pairs.  Packed without the shift, A + B <=> AB with |log2 E_k| = 692 each at 250 K is
+    such a reaction; the rates still match the oracle from 250 K up."""
+    mech = hand_cases.extreme_thermo_mechanisms(-1.2e5)["assoc"]
+    s, side, pair, wide = pack_range(emu, mech, 0)
+    assert s == 0 and wide == 1 and 600.0 < pair <= 900.0   # (the Lindemann reaction is in the extended class anyway)
+    assert pack_range(emu, mech, 1)[3] == 0   # with the shift the sides stay below 2^700
+    rho, T, Y = _cold_to_hot_states(mech, 300)
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+    for shift in (0, 1):
+        st, om, msg = emu_rates_status(emu, mech, rho, T, Y, shift)
+        assert st == 0, msg
+        parity.assert_omega_parity(om, om_ref, bound)
+
+
+def test_troe_sentinel_temperatures(emu):
+    """T*** = 1e-30, T* = 1e30, T** = 1e30 as real mechanism files carry them: the exponents are
+    clamped at pack time where the term is exactly 0 (or 1) in FP64, so exp2's reduction never sees |y| >= 2^31."""
+    mech = hand_cases.troe_sentinel_mechanism()
+    rho, T, Y = hand_cases.random_states(mech, 600)
+    T[:4] = [250.0, 1234.5, 3000.0, 6000.0]
+    om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
+    assert np.isfinite(om_ref).all()
+    st, om, msg = emu_rates_status(emu, mech, rho, T, Y)
+    assert st == 0, msg
+    parity.assert_omega_parity(om, om_ref, bound)
+
+
+def test_rate_coefficient_exponent_out_of_exp2_range_is_refused(emu):
+    mech = hand_cases.simple_mechanism(hand_cases.species5(), [dict(reac={0: 1, 1: 1}, prod={2: 1}, A=1e10, b=0.0, theta=1e12)])
+    st, _, msg = pack_status(emu, mech)
+    assert st == 7 and "rate coefficient" in msg
+
+
 @pytest.mark.parametrize("cfg,n", [(0, 4096), (1, 2048), (2, 1024), (3, 256)])
 def test_emu_rates_config_mechanisms(emu, cfg, n):
     mech = inputs.config_mechanism(cfg)
@@ -358,12 +463,45 @@ def test_emu_rates_species_with_different_t_mid(emu):
     st = inputs.config_states(0, n=2048)
     om_ref, bound = oracle.Oracle(mech).get_net_production_rates(st["rho"], st["T"], st["Y"])
     parity.assert_omega_parity(emu_rates(emu, mech, st["rho"], st["T"], st["Y"]), om_ref, bound)
-    # the temperature solve of this build needs one T_mid
-    desc, keep = binding.make_desc(mech)
-    e = np.ascontiguousarray(st["e"], dtype=np.float64)
-    T = np.empty_like(e)
-    assert emu.emu_temperature(C.byref(desc), e.shape[0], e.shape[0], e.ctypes.data, st["Y"].ctypes.data,
-                               st["T_guess"].ctypes.data, 1e-6, 10, T.ctypes.data, None) == 7
+
+
+def _mixed_tmid_case(cfg, n, seed=11):
+    """A config mechanism with four different break temperatures (ranges re-matched at each), states from
+    250 K to 3200 K, guesses within 10 % -- so that some land on the other side of a break temperature and
+    some iterates cross one -- plus guesses placed exactly on and one ulp around the break temperatures."""
+    mech = inputs.with_species_break_temperatures(inputs.config_mechanism(cfg), [800.0, 1000.0, 1400.0, 1250.0])
+    rng = np.random.default_rng(seed)
+    T = rng.uniform(250.0, 3200.0, size=n)
+    T[: n // 4] = rng.choice([800.0, 1000.0, 1250.0, 1400.0], size=n // 4) * (1.0 + rng.uniform(-0.04, 0.04, size=n // 4))
+    Y = rng.dirichlet(np.full(mech.n_species, 0.5), size=n).T.copy()
+    e = inputs.mixture_energy(mech, T, Y)
+    h = e + inputs.R_UNIVERSAL * T * (Y / mech.mol_weight[:, None]).sum(axis=0)
+    Tg = T * (1.0 + rng.uniform(-0.1, 0.1, size=n))
+    Tg[:8] = [800.0, np.nextafter(800.0, 0), np.nextafter(800.0, 1e4), 1250.0, 1400.0, np.nextafter(1400.0, 0), 1000.0, 999.0]
+    return mech, T, Y, e, h, Tg
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 3000), (2, 600)])
+def test_emu_temperature_species_with_different_t_mid(emu, cfg, n):
+    """Row a4 with per-species break temperatures (G10; (A.12)-(A.13) PAPER.md:941-945, listing 22 :672-695): the
+    interval-wise solve agrees with the oracle's per-species, per-iterate range choice to 1e-12, in both the
+    energy and the enthalpy form, and recovers the generating temperature."""
+    mech, T, Y, e, h, Tg = _mixed_tmid_case(cfg, n)
+    orc = oracle.Oracle(mech)
+    for enthalpy, rhs in ((0, e), (1, h)):
+        T_ref, it, conv = (orc.get_temperature_from_enthalpy if enthalpy else orc.get_temperature)(rhs, Y, Tg)
+        assert conv.all()
+        desc, keep = binding.make_desc(mech)
+        rhs_c, Y_c, Tg_c = (np.ascontiguousarray(x, dtype=np.float64) for x in (rhs, Y, Tg))
+        out = np.empty_like(rhs_c)
+        bad = C.c_int64(-1)
+        st = emu.emu_temperature2(C.byref(desc), n, n, rhs_c.ctypes.data, Y_c.ctypes.data, Tg_c.ctypes.data, 1e-6, 10,
+                                  out.ctypes.data, C.byref(bad), enthalpy)
+        assert st == 0 and bad.value == 0
+        parity.assert_T_parity(out, T_ref)
+        assert np.max(np.abs(out - T) / T) < 1e-11   # the generating temperature (e was formed in long double)
+        crossed = ((Tg[:, None] < mech.t_mid[None, :]) != (T[:, None] < mech.t_mid[None, :])).any(axis=1)
+        assert crossed.sum() > n // 10   # the case does exercise the re-summation
 
 
 @pytest.mark.parametrize("cfg,n", [(0, 4096), (2, 1024), (3, 256), (4, 512)])
