@@ -72,6 +72,8 @@ def _load():
                 C.c_void_p, C.c_void_p, C.c_void_p]
             getattr(_lib, f"oracle_get_net_production_rates_{sfx}").argtypes = [
                 C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 7
+            getattr(_lib, f"oracle_get_jacobian_{sfx}").argtypes = [
+                C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
     return _lib
 
 
@@ -219,3 +221,22 @@ class Oracle:
         if want_rates:
             return omega, bound, rf, rr
         return omega, bound
+
+    def get_jacobian(self, rho, T, Y, mode=0):
+        """Chemical Jacobian J[i, k, p] = dS_i/dY_k (S_i = W_i omega_i, eq. (6), (A.36)) and
+        dSdT[i, p] = dS_i/dT at fixed (rho, Y).  mode 0: Y-derivatives at fixed (rho, T); mode 1: at fixed
+        (rho, e), i.e. through the temperature inversion as the paper's listing 23 (reading G26).
+        Returns J, dSdT and the sums of absolute terms boundJ, bounddSdT that scale the parity tolerance."""
+        rho = self._vec(rho)
+        T = self._vec(T)
+        Y = self._vec(Y)
+        n = rho.shape[0]
+        ns = self.n_species
+        assert Y.shape == (ns, n)
+        J = np.empty((ns, ns, n), dtype=self.dtype)
+        bJ = np.empty((ns, ns, n), dtype=self.dtype)
+        dSdT = np.empty((ns, n), dtype=self.dtype)
+        bT = np.empty((ns, n), dtype=self.dtype)
+        self._fn("get_jacobian")(C.byref(self._m), n, n, rho.ctypes.data, T.ctypes.data, Y.ctypes.data, int(mode),
+                                 J.ctypes.data, dSdT.ctypes.data, bJ.ctypes.data, bT.ctypes.data)
+        return J, dSdT, bJ, bT

@@ -24,6 +24,8 @@
 //   mixture_h / cp      N1 h - e = R T sum_k Y_k/W_k, N2 c_p = dh/dT, N3 c_p - c_v = R sum_k Y_k/W_k
 //   get_temperature_h   N4 recovers generating T, closed form for a constant-c_p species
 //   density / pressure  N5 single species rho = p W/(R T), N6 p(rho(p)) = p, N7 sum_k C_k = p/(R T)
+//   jacobian            J1 differences of the oracle's omega (long double), J2 closed forms (W6), J3 conservation
+//                       per column, J4 the (rho, e) form through the Newton solve, J5 dS/dT by central differences
 //   No function is "parity unpinned".
 //
 // Readings of garbled / silent passages are
@@ -313,6 +315,204 @@ void get_temperature(const oracle_mech &m, int64_t n, int64_t ld, const Real *e,
     }
 }
 
+// ---------------------------------------------------------------------------------------------------
+// the chemical Jacobian, analytic.  PAPER.md:697-714 eq. (6) J = dS/dY with
+// S_i = W_i omega_i (A.1) PAPER.md:888; (A.36) PAPER.md:1057.  Written out from (A.5)-(A.13) by the chain and
+// product rules, reaction by reaction, dense in the species index (slow and plain on purpose).
+//   C_k = rho Y_k / W_k (A.8): at fixed rho,  d/dY_k = (rho/W_k) d/dC_k ; the Y_k are independent variables
+//   (no sum-to-one constraint is applied, as automatic differentiation of (A.5) would not apply one).
+// Readings: G26 what is held fixed -- mode 0: (rho, T); mode 1: (rho, e), the paper's J: listing 23
+// differentiates through the temperature inversion, i.e.  dT/dY_k|_e = -e_k(T)/c_v  from (A.25): 0 = e_k dY_k + c_v dT.
+// Pins (tests/test_oracle_pins.py): J1 finite differences of this oracle's own omega in long double, error linear in
+// delta for one-sided differences as in eq. (7) / fig. 8 and quadratic for central ones; J2 closed forms of the
+// single reaction W2/W6 (dR/dC_A = k C_B); J3 mass and element conservation per column; J4 the
+// (rho, e) form against differences through the oracle's own Newton solve; J5 dS/dT by central differences for
+// every reaction type.
+// Every derivative comes with the sum of the absolute values of the terms it is made of ("a..." twins); the
+// harness scales the parity tolerance of the CUDA path with them, exactly as bound_i does for omega.
+template <class Real> struct ReactionDerivative {
+    std::vector<Real> dqf_dC, dqr_dC, aqf_dC, aqr_dC;   // [n_species]
+    Real dqf_dT = 0, dqr_dT = 0, aqf_dT = 0, aqr_dT = 0;
+};
+
+template <class Real>
+ReactionDerivative<Real> reaction_derivative(const oracle_mech &m, int j, Real T, const Real *C, const Real *g,
+                                             const Real *h_RT) {
+    const int ns = m.n_species;
+    ReactionDerivative<Real> d;
+    d.dqf_dC.assign(ns, Real(0)); d.dqr_dC.assign(ns, Real(0)); d.aqf_dC.assign(ns, Real(0)); d.aqr_dC.assign(ns, Real(0));
+    const Real ln10 = std::log(Real(10));
+    // (A.9): k = A T^b exp(-theta/T);  d ln k / dT = (b + theta/T)/T
+    const Real kinf = Real(m.A[j]) * std::pow(T, Real(m.b[j])) * std::exp(-Real(m.theta[j]) / T);
+    const Real dlnkinf_dT = (Real(m.b[j]) + Real(m.theta[j]) / T) / T;
+    const Real a_dlnkinf_dT = (std::fabs(Real(m.b[j])) + std::fabs(Real(m.theta[j])) / T) / T;
+    // [M] = sum_k eff_k C_k  (G6):  d[M]/dC_k = eff_k
+    std::vector<Real> eff(ns);
+    Real M = 0;
+    for (int k = 0; k < ns; ++k) {
+        eff[k] = Real(m.eff_default[j]);
+        for (int q = m.eff_ptr[j]; q < m.eff_ptr[j + 1]; ++q)
+            if (m.eff_species[q] == k) eff[k] = Real(m.eff_value[q]);
+        M += eff[k] * C[k];
+    }
+    const int type = m.type[j];
+    Real k = kinf, dlnk_dT = dlnkinf_dT, a_dlnk_dT = a_dlnkinf_dT, dlnk_dM = 0, a_dlnk_dM = 0;
+    if (type >= 2) {   // falloff (G6-G8): k = k_inf L(Pr) F(T, Pr), L = Pr/(1+Pr), Pr = k0 [M]/k_inf
+        const Real k0 = Real(m.A0[j]) * std::pow(T, Real(m.b0[j])) * std::exp(-Real(m.theta0[j]) / T);
+        const Real dlnk0_dT = (Real(m.b0[j]) + Real(m.theta0[j]) / T) / T;
+        const Real a_dlnk0_dT = (std::fabs(Real(m.b0[j])) + std::fabs(Real(m.theta0[j])) / T) / T;
+        const Real Pr = k0 * M / kinf;
+        const Real dlnPr_dT = dlnk0_dT - dlnkinf_dT;          // at fixed concentrations
+        const Real a_dlnPr_dT = a_dlnk0_dT + a_dlnkinf_dT;
+        const Real dlnL_dlnPr = Real(1) / (Real(1) + Pr);     // d ln[Pr/(1+Pr)] / d ln Pr
+        Real F = 1, dlnF_dlnPr = 0, dlnF_dT = 0, a_dlnF_dT = 0;   // dlnF_dT: at fixed Pr
+        if (type == 3) {
+            const Real alpha = m.troe[4 * j + 0], T3 = m.troe[4 * j + 1], T1 = m.troe[4 * j + 2], T2 = m.troe[4 * j + 3];
+            const Real e3 = std::exp(-T / T3), e1 = std::exp(-T / T1);
+            const bool has2 = std::isfinite(m.troe[4 * j + 3]);
+            const Real e2 = has2 ? std::exp(-T2 / T) : Real(0);
+            const Real Fc = (Real(1) - alpha) * e3 + alpha * e1 + e2;
+            const Real t3 = -(Real(1) - alpha) / T3 * e3, t1 = -alpha / T1 * e1, t2 = has2 ? T2 / (T * T) * e2 : Real(0);
+            const Real dlFc_dT = (t3 + t1 + t2) / (Fc * ln10);             // lFc = log10 Fc
+            const Real a_dlFc_dT = (std::fabs(t3) + std::fabs(t1) + std::fabs(t2)) / (std::fabs(Fc) * ln10);
+            const Real lFc = std::log10(Fc);
+            const Real c = Real(-0.4L) - Real(0.67L) * lFc;
+            const Real n = Real(0.75L) - Real(1.27L) * lFc;
+            const Real x = std::log10(Pr) + c;
+            const Real den = n - Real(0.14L) * x;
+            const Real f1 = x / den;
+            const Real gg = Real(1) / (Real(1) + f1 * f1);                 // log10 F = lFc gg
+            F = std::pow(Real(10), lFc * gg);
+            const Real df1_dx = n / (den * den), df1_dn = -x / (den * den);
+            const Real dgg_df1 = -Real(2) * f1 * gg * gg;
+            // vary Pr at fixed T: dx/d ln Pr = 1/ln 10, so d ln F/d ln Pr = ln10 lFc dgg/df1 df1/dx / ln10
+            dlnF_dlnPr = lFc * dgg_df1 * df1_dx;
+            // vary T at fixed Pr: c and n move with lFc
+            const Real dx_dT = -Real(0.67L) * dlFc_dT, dn_dT = -Real(1.27L) * dlFc_dT;
+            dlnF_dT = ln10 * (dlFc_dT * gg + lFc * dgg_df1 * (df1_dx * dx_dT + df1_dn * dn_dT));
+            a_dlnF_dT = ln10 * a_dlFc_dT *
+                        (gg + std::fabs(lFc * dgg_df1) * (std::fabs(df1_dx) * Real(0.67L) + std::fabs(df1_dn) * Real(1.27L)));
+        }
+        k = kinf * (Pr / (Real(1) + Pr)) * F;
+        dlnk_dT = dlnkinf_dT + (dlnL_dlnPr + dlnF_dlnPr) * dlnPr_dT + dlnF_dT;
+        a_dlnk_dT = a_dlnkinf_dT + (std::fabs(dlnL_dlnPr) + std::fabs(dlnF_dlnPr)) * a_dlnPr_dT + a_dlnF_dT;
+        dlnk_dM = (dlnL_dlnPr + dlnF_dlnPr) / M;              // d ln Pr / d[M] = 1/[M]
+        a_dlnk_dM = (std::fabs(dlnL_dlnPr) + std::fabs(dlnF_dlnPr)) / std::fabs(M);
+    }
+    // dense nu', nu'' of this reaction
+    std::vector<int> nup(ns, 0), nupp(ns, 0);
+    for (int q = m.reac_ptr[j]; q < m.reac_ptr[j + 1]; ++q) nup[m.reac_species[q]] += m.reac_coeff[q];
+    for (int q = m.prod_ptr[j]; q < m.prod_ptr[j + 1]; ++q) nupp[m.prod_species[q]] += m.prod_coeff[q];
+    // P = prod_l C_l^nu_l  and  dP/dC_k = nu_k C_k^(nu_k - 1) prod_{l != k} C_l^nu_l   (no division: C_k may be 0)
+    auto power_product = [&](const std::vector<int> &nu, int skip_one_of) {
+        Real P = 1;
+        for (int l = 0; l < ns; ++l)
+            for (int r = 0; r < nu[l] - (l == skip_one_of ? 1 : 0); ++r) P *= C[l];
+        return P;
+    };
+    const Real Pf = power_product(nup, -1);
+    Real kr = 0, Pr_ = 0, dlnKc_dT = 0, a_dlnKc_dT = 0;
+    if (m.reversible[j]) {
+        int dnu = 0;
+        Real dg = 0, dh = 0, adh = 0;
+        for (int l = 0; l < ns; ++l) {
+            const int nu = nupp[l] - nup[l];
+            if (nu == 0) continue;
+            dnu += nu;
+            dg += Real(nu) * g[l];
+            dh += Real(nu) * h_RT[l];
+            adh += std::fabs(Real(nu) * h_RT[l]);
+        }
+        const Real Kc = std::pow(Const<Real>::p0 / (Const<Real>::R * T), Real(dnu)) * std::exp(-dg);   // (A.10; G1)
+        kr = k / Kc;
+        Pr_ = power_product(nupp, -1);
+        // ln Kc = dnu ln(p0/RT) - sum nu g/RT, d(g/RT)/dT = -(h/RT)/T  (from (A.11)-(A.13)):
+        dlnKc_dT = (-Real(dnu) + dh) / T;
+        a_dlnKc_dT = (std::fabs(Real(dnu)) + adh) / T;
+    }
+    const Real qf0 = k * Pf, qr0 = kr * Pr_;
+    const Real Mfac = (type == 1) ? M : Real(1);   // three-body: R = [M](qf0 - qr0)  (G8)
+    for (int l = 0; l < ns; ++l) {
+        const Real direct_f = nup[l] > 0 ? k * Real(nup[l]) * power_product(nup, l) : Real(0);
+        const Real direct_r = (m.reversible[j] && nupp[l] > 0) ? kr * Real(nupp[l]) * power_product(nupp, l) : Real(0);
+        const Real viaM_f = qf0 * dlnk_dM * eff[l], viaM_r = qr0 * dlnk_dM * eff[l];
+        d.dqf_dC[l] = Mfac * (direct_f + viaM_f);
+        d.dqr_dC[l] = Mfac * (direct_r + viaM_r);
+        d.aqf_dC[l] = std::fabs(Mfac) * (std::fabs(direct_f) + std::fabs(qf0 * a_dlnk_dM * eff[l]));
+        d.aqr_dC[l] = std::fabs(Mfac) * (std::fabs(direct_r) + std::fabs(qr0 * a_dlnk_dM * eff[l]));
+        if (type == 1) {
+            d.dqf_dC[l] += eff[l] * qf0;
+            d.dqr_dC[l] += eff[l] * qr0;
+            d.aqf_dC[l] += std::fabs(eff[l] * qf0);
+            d.aqr_dC[l] += std::fabs(eff[l] * qr0);
+        }
+    }
+    d.dqf_dT = Mfac * qf0 * dlnk_dT;
+    d.dqr_dT = Mfac * qr0 * (dlnk_dT - dlnKc_dT);
+    d.aqf_dT = std::fabs(Mfac * qf0) * a_dlnk_dT;
+    d.aqr_dT = std::fabs(Mfac * qr0) * (a_dlnk_dT + a_dlnKc_dT);
+    return d;
+}
+
+// One point.  J[(i n_s + k) ldj] = dS_i/dY_k, dSdT[i ldj] = dS_i/dT at fixed (rho, Y); the same shapes for the
+// bounds.  mode 0: Y-derivatives at fixed (rho, T); mode 1: at fixed (rho, e)  (reading G26).
+template <class Real>
+void jacobian_point(const oracle_mech &m, Real rho, Real T, const Real *Y, int64_t ld, int mode, Real *J, Real *dSdT,
+                    Real *boundJ, Real *bounddSdT, int64_t ldj) {
+    const int ns = m.n_species, nr = m.n_reactions;
+    std::vector<Real> C(ns), g(ns), h_RT(ns), cp_R(ns), Yv(ns);
+    for (int k = 0; k < ns; ++k) {
+        Yv[k] = Y[k * ld];
+        C[k] = rho * Yv[k] / Real(m.mol_weight[k]);
+        Real s_R;
+        species_thermo<Real>(m, k, T, cp_R[k], h_RT[k], s_R, g[k]);
+    }
+    std::vector<Real> dwdC((size_t)ns * ns, Real(0)), adwdC((size_t)ns * ns, Real(0)), dwdT(ns, Real(0)), adwdT(ns, Real(0));
+    for (int j = 0; j < nr; ++j) {
+        const ReactionDerivative<Real> d = reaction_derivative<Real>(m, j, T, C.data(), g.data(), h_RT.data());
+        std::vector<int> nu(ns, 0);
+        for (int q = m.reac_ptr[j]; q < m.reac_ptr[j + 1]; ++q) nu[m.reac_species[q]] -= m.reac_coeff[q];
+        for (int q = m.prod_ptr[j]; q < m.prod_ptr[j + 1]; ++q) nu[m.prod_species[q]] += m.prod_coeff[q];
+        for (int i = 0; i < ns; ++i) {
+            if (nu[i] == 0) continue;
+            for (int k = 0; k < ns; ++k) {   // (A.5): d omega_i/dC_k = sum_j nu_ij (dqf_j/dC_k - dqr_j/dC_k)
+                dwdC[(size_t)i * ns + k] += Real(nu[i]) * (d.dqf_dC[k] - d.dqr_dC[k]);
+                adwdC[(size_t)i * ns + k] += std::fabs(Real(nu[i])) * (d.aqf_dC[k] + d.aqr_dC[k]);
+            }
+            dwdT[i] += Real(nu[i]) * (d.dqf_dT - d.dqr_dT);
+            adwdT[i] += std::fabs(Real(nu[i])) * (d.aqf_dT + d.aqr_dT);
+        }
+    }
+    Real cv = 0;
+    if (mode == 1) cv = mixture_cv<Real>(m, T, Yv.data(), 1);
+    for (int i = 0; i < ns; ++i) {
+        const Real Wi = Real(m.mol_weight[i]);
+        const Real sT = Wi * dwdT[i], asT = Wi * adwdT[i];
+        if (dSdT) dSdT[i * ldj] = sT;
+        if (bounddSdT) bounddSdT[i * ldj] = asT;
+        for (int k = 0; k < ns; ++k) {
+            const Real scale = Wi * rho / Real(m.mol_weight[k]);
+            Real v = scale * dwdC[(size_t)i * ns + k], a = scale * adwdC[(size_t)i * ns + k];
+            if (mode == 1) {   // + dS_i/dT dT/dY_k|_e,  dT/dY_k|_e = -e_k/c_v,  e_k = (h_RT_k - 1) R T / W_k  (A.26)
+                const Real ek = (h_RT[k] - Real(1)) * Const<Real>::R * T / Real(m.mol_weight[k]);
+                v -= sT * ek / cv;
+                a += std::fabs(asT * ek / cv);
+            }
+            J[((size_t)i * ns + k) * ldj] = v;
+            if (boundJ) boundJ[((size_t)i * ns + k) * ldj] = a;
+        }
+    }
+}
+
+template <class Real>
+void get_jacobian(const oracle_mech &m, int64_t n, int64_t ld, const Real *rho, const Real *T, const Real *Y, int mode,
+                  Real *J, Real *dSdT, Real *boundJ, Real *bounddSdT) {
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < n; ++p)
+        jacobian_point<Real>(m, rho[p], T[p], Y + p, ld, mode, J + p, dSdT ? dSdT + p : nullptr,
+                             boundJ ? boundJ + p : nullptr, bounddSdT ? bounddSdT + p : nullptr, ld);
+}
+
 template <class Real>
 void reaction_detail(const oracle_mech &m, int j, Real rho, Real T, const Real *Y, Real *out9) {
     const int ns = m.n_species;
@@ -384,6 +584,11 @@ int oracle_sizeof_real80() { return (int)sizeof(long double); }
     void oracle_get_pressure_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *rho,           \
                                       const Real *T, const Real *Y, Real *p) {                                \
         for (int64_t i = 0; i < n; ++i) p[i] = pressure_point<Real>(*m, rho[i], T[i], Y + i, ld);             \
+    }                                                                                                         \
+    void oracle_get_jacobian_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *rho, const Real *T, \
+                                      const Real *Y, int mode, Real *J, Real *dSdT, Real *boundJ,              \
+                                      Real *bounddSdT) {                                                       \
+        get_jacobian<Real>(*m, n, ld, rho, T, Y, mode, J, dSdT, boundJ, bounddSdT);                            \
     }                                                                                                         \
     void oracle_get_net_production_rates_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld,                \
                                                   const Real *rho, const Real *T, const Real *Y, Real *omega, \
