@@ -165,6 +165,31 @@ uint32_t align16(uint32_t x) { return (x + 15u) & ~15u; }
 
 }   // namespace
 
+// Falloff row of reaction j (type >= PYRO_FALLOFF_LINDEMANN): low-pressure Arrhenius coefficients in log2 form and
+// the Troe parameters as slopes of base-2 exponents.
+RxnFall fall_row(const pyro_mech_desc *d, int j) {
+    RxnFall fl;
+    std::memset(&fl, 0, sizeof fl);
+    fl.l[0] = (double)(std::log((long double)d->A0[j]) * kLog2e);
+    fl.l[1] = d->b0[j];
+    fl.l[2] = (double)(-(long double)d->theta0[j] * kLog2e);
+    if (d->type[j] == PYRO_FALLOFF_TROE) {
+        const double *t = d->troe + 4 * j;
+        fl.troe_alpha = t[0];
+        // Sentinel temperatures of real mechanisms (T*** = 1e-30, T** = 1e30 ...) make the exponent
+        // exceed what exp2 reduces (|y| < 2^31).  Clamp the coefficients where the term is exactly
+        // zero in FP64 anyway: exp(-T/T***) with T*** < 1.4e-4 K is 0 for every T >= 1 K, and
+        // exp(-T**/T) with T** > 7.4e8 K is 0 for every T <= 1e5 K; the clamped exponents stay
+        // below 2^31 for 1 K <= T <= 1e5 K and still underflow to zero there.
+        const long double kMaxSlope = 1.0e4L, kMaxT2 = 1073741824.0L;
+        fl.troe_t3 = (double)std::max(-kLog2e / (long double)t[1], -kMaxSlope);
+        fl.troe_t1 = std::isinf(t[2]) ? 0.0 : (double)std::max(-kLog2e / (long double)t[2], -kMaxSlope);
+        fl.troe_has_t2 = std::isinf(t[3]) ? 0.0 : 1.0;
+        fl.troe_t2 = std::isinf(t[3]) ? 0.0 : (double)std::max(-kLog2e * (long double)t[3], -kMaxT2);
+    }
+    return fl;
+}
+
 int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, int leftover, int shift) {
     try {
         PYRO_REQUIRE(d != nullptr, PYRO_ERR_NULL, "desc is NULL");
@@ -454,25 +479,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
                     effs.push_back(EffEntry{d->eff_value[q] - d->eff_default[j], (uint32_t)d->eff_species[q], 0u});
             }
             if (type >= PYRO_FALLOFF_LINDEMANN) {
-                RxnFall fl;
-                std::memset(&fl, 0, sizeof fl);
-                fl.l[0] = (double)(std::log((long double)d->A0[j]) * kLog2e);
-                fl.l[1] = d->b0[j];
-                fl.l[2] = (double)(-(long double)d->theta0[j] * kLog2e);
-                if (type == PYRO_FALLOFF_TROE) {
-                    const double *t = d->troe + 4 * j;
-                    fl.troe_alpha = t[0];
-                    // Sentinel temperatures of real mechanisms (T*** = 1e-30, T** = 1e30 ...) make the exponent
-                    // exceed what exp2 reduces (|y| < 2^31).  Clamp the coefficients where the term is exactly
-                    // zero in FP64 anyway: exp(-T/T***) with T*** < 1.4e-4 K is 0 for every T >= 1 K, and
-                    // exp(-T**/T) with T** > 7.4e8 K is 0 for every T <= 1e5 K; the clamped exponents stay
-                    // below 2^31 for 1 K <= T <= 1e5 K and still underflow to zero there.
-                    const long double kMaxSlope = 1.0e4L, kMaxT2 = 1073741824.0L;
-                    fl.troe_t3 = (double)std::max(-kLog2e / (long double)t[1], -kMaxSlope);
-                    fl.troe_t1 = std::isinf(t[2]) ? 0.0 : (double)std::max(-kLog2e / (long double)t[2], -kMaxSlope);
-                    fl.troe_has_t2 = std::isinf(t[3]) ? 0.0 : 1.0;
-                    fl.troe_t2 = std::isinf(t[3]) ? 0.0 : (double)std::max(-kLog2e * (long double)t[3], -kMaxT2);
-                }
+                const RxnFall fl = fall_row(d, j);
                 x.fall_index = (uint32_t)recFall.size();
                 recFall.push_back(fl);
             }

@@ -4,6 +4,7 @@
 #include <vector>
 
 #include "../../include/pyro.h"
+#include "pyro_jac_tables.h"
 #include "pyro_tables.h"
 
 namespace pyro {
@@ -35,5 +36,17 @@ enum { kLeftoverAuto = -1, kLeftoverPad = 0, kLeftoverSingles = 1 };
 enum { kShiftOn = 1, kShiftOff = 0 };
 int pack_mechanism(const pyro_mech_desc *desc, PackedMech &out, std::string &err, int leftover = kLeftoverAuto,
                    int shift = kShiftOn);
+
+// Tables of the chemical-Jacobian kernel (pyro_jac_tables.h) of a description that pack_mechanism accepted.
+// The kernel keeps two accumulators per species in tensor memory: at most kJacMaxSpecies species.
+constexpr int kJacMaxSpecies = 127;
+struct JacPacked {
+    JacLayout lay;
+    std::vector<unsigned char> blob;
+};
+int pack_jacobian(const pyro_mech_desc *desc, JacPacked &out, std::string &err);
+
+// Falloff row of reaction j of a validated description (shared by the rates and the Jacobian tables).
+RxnFall fall_row(const pyro_mech_desc *desc, int j);
 
 }   // namespace pyro

@@ -12,6 +12,7 @@
 
 #include "../../paper_2503_24286_b200/csrc/pyro_pack.h"
 #include "../../paper_2503_24286_b200/csrc/pyro_point.cuh"
+#include "../../paper_2503_24286_b200/csrc/pyro_jac.cuh"
 
 namespace {
 struct HostTab {
@@ -22,6 +23,21 @@ struct HostTab {
     const pyro::RxnX &rxn_x(int j) const { return reinterpret_cast<const pyro::RxnX *>(base + lay.off_rxn_x)[j]; }
     const pyro::RxnFall &rxn_fall(int j) const { return reinterpret_cast<const pyro::RxnFall *>(base + lay.off_fall)[j]; }
     const pyro::EffEntry &eff(int q) const { return reinterpret_cast<const pyro::EffEntry *>(base + lay.off_eff)[q]; }
+};
+struct HostJacTab {
+    const unsigned char *base;       // rates blob (species rows)
+    pyro::TableLayout lay;
+    const pyro::EnergyRow *en;
+    const unsigned char *jbase;      // Jacobian blob
+    pyro::JacLayout jl;
+    const pyro::SpecRow &spec(int k) const { return reinterpret_cast<const pyro::SpecRow *>(base + lay.off_spec)[k]; }
+    const pyro::EnergyRow &energy(int k) const { return en[k]; }
+    const pyro::JacRxn &rxn(int j) const { return reinterpret_cast<const pyro::JacRxn *>(jbase + jl.off_rxn)[j]; }
+    const pyro::JacInc &inc(int q) const { return reinterpret_cast<const pyro::JacInc *>(jbase + jl.off_inc)[q]; }
+    const pyro::JacEffInc &effinc(int q) const { return reinterpret_cast<const pyro::JacEffInc *>(jbase + jl.off_effinc)[q]; }
+    const pyro::EffEntry &eff(int q) const { return reinterpret_cast<const pyro::EffEntry *>(jbase + jl.off_eff)[q]; }
+    const pyro::RxnFall &rxn_fall(int j) const { return reinterpret_cast<const pyro::RxnFall *>(jbase + jl.off_fall)[j]; }
+    const pyro::JacCol &col(int k) const { return reinterpret_cast<const pyro::JacCol *>(jbase + jl.off_col)[k]; }
 };
 thread_local std::string g_err;
 
@@ -184,6 +200,28 @@ int emu_temperature2(const pyro_mech_desc *d, int64_t n, int64_t ld, const doubl
         bad += conv ? 0 : 1;
     }
     if (n_bad) *n_bad = bad;
+    return PYRO_OK;
+}
+
+// the per-point functions of the Jacobian kernel, one point after the other; J[(i ns + k) ld + p], dSdT[i ld + p]
+int emu_jacobian(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
+                 int mode, double *J, double *dSdT) {
+    pyro::PackedMech pm;
+    int st = pyro::pack_mechanism(d, pm, g_err);
+    if (st != PYRO_OK) return st;
+    pyro::JacPacked jp;
+    st = pyro::pack_jacobian(d, jp, g_err);
+    if (st != PYRO_OK) return st;
+    const HostJacTab tab{pm.blob.data(), pm.lay, pm.energy.data(), jp.blob.data(), jp.lay};
+    const int ns = pm.n_species;
+    std::vector<double> C(ns + 1), G(ns + 1), DG(ns + 1), a0(ns + 1), a1(ns + 1), a2(ns + 1), ext(1 + 2 * jp.lay.n_ext);
+    for (int64_t p = 0; p < n; ++p) {
+        const pyro::JacArrayMem mem{C.data(), G.data(), DG.data(), {a0.data(), a1.data(), a2.data()}, ext.data()};
+        pyro::jacobian_point(
+            tab, jp.lay, T[p], rho[p], mode, dSdT != nullptr, mem, [&](int k) { return Y[k * ld + p]; },
+            [&](int i, int k, double v) { J[((int64_t)i * ns + k) * ld + p] = v; },
+            [&](int i, double v) { dSdT[i * ld + p] = v; });
+    }
     return PYRO_OK;
 }
 

@@ -37,3 +37,15 @@ def assert_T_parity(T, T_ref):
     r = float(np.max(np.abs(T - T_ref) / np.abs(T_ref))) if T.size else 0.0
     assert r <= T_TOL, f"max |dT|/T = {r:.3e} > {T_TOL}"
     return r
+
+
+JAC_TOL = 1e-11   # chemical Jacobian and dS/dT: relative to the sum of the absolute terms of the entry
+
+
+def assert_jacobian_parity(J, J_ref, bound):
+    """|J_ik - J_ik^oracle| <= JAC_TOL * (sum of the absolute values of the entry's terms, as the oracle returns it);
+    entries with no term at all must be exactly zero."""
+    assert np.isfinite(J).all()
+    r = omega_residual(J, J_ref, bound)
+    assert r <= JAC_TOL, f"max |dJ|/bound = {r:.3e} > {JAC_TOL}"
+    return r
