@@ -23,7 +23,8 @@
  *   not choose by itself (they exist so that the parity tests reach every kernel variant); they are not part of
  *   the interface and change no result: PYRO_TABLES=shared|global, PYRO_RATES_BLOCK=<threads>,
  *   PYRO_B_PLANE=shared, PYRO_CARVEOUT=<percent>, PYRO_RATES_TWO_BLOCKS=0|1, PYRO_PACK_SINGLES=0|1,
- *   PYRO_HOST_SLAB=<points> (pyro_source_terms_host), PYRO_DEBUG=1 (prints the launch shape to stderr).
+ *   PYRO_HOST_SLAB=<points> (pyro_source_terms_host), PYRO_JAC_V_PLANE=shared, PYRO_JAC_BLOCK=<threads>
+ *   (pyro_get_jacobian), PYRO_DEBUG=1 (prints the launch shape to stderr).
  */
 #ifndef PYRO_H
 #define PYRO_H
@@ -142,6 +143,23 @@ int pyro_get_pressure(const pyro_mech *mech, int64_t n, int64_t ld, const double
  * wherever the definition's own K_c and rate coefficients are -- never a silent NaN. */
 int pyro_get_net_production_rates(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho,
                                   const double *T, const double *Y, double *omega, void *cuda_stream);
+
+/* Chemical Jacobian (eq. (6); (A.36) PAPER.md:1057) of the source terms S_i = W_i omega_i
+ * ((A.1) PAPER.md:888), analytic:
+ *   J[(i*n_species + k)*ld + p] = dS_i/dY_k     [n_species*n_species][ld], device, out; must not overlap Y
+ *   dSdT[i*ld + p]              = dS_i/dT at fixed (rho, Y)   [n_species][ld], device, out, or NULL
+ * from rho [n], T [n], Y [n_species][ld] as in pyro_get_net_production_rates.  The mass fractions are independent
+ * variables (no sum-to-one constraint is applied), C_k = rho Y_k / W_k (A.8).  `mode` says what is held fixed
+ * while Y_k varies:
+ *   PYRO_JAC_FIXED_T   rho and T:  J_ik = W_i (rho/W_k) sum_j nu_ij dR_j/dC_k
+ *   PYRO_JAC_FIXED_E   rho and the internal energy e (an adiabatic isochoric reactor (A.1); what the paper's listing 23
+ *                      differentiates, through the temperature inversion):  J_ik - dS_i/dT e_k(T)/c_v(T,Y)
+ * The derivatives of the third-body and Lindemann / Troe forms are included (through [M] and through T).
+ * Mechanisms of more than 127 species: PYRO_ERR_UNSUPPORTED.  Launches on one handle share a scratch buffer and are
+ * ordered after one another (also across streams). */
+enum { PYRO_JAC_FIXED_T = 0, PYRO_JAC_FIXED_E = 1 };
+int pyro_get_jacobian(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *T,
+                      const double *Y, int mode, double *J, double *dSdT, void *cuda_stream);
 
 /* The whole source-term step from HOST buffers: (rho, e, Y, T_guess) -> (T, omega).  Copies the
  * inputs to the device in slabs of points, runs the temperature solve and the rates kernel on

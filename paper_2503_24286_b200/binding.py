@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libpyro.so")
 EXPORTS = (
     "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
     "pyro_get_temperature_from_enthalpy", "pyro_get_density", "pyro_get_pressure",
-    "pyro_get_net_production_rates", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
+    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
     "pyro_status_string", "pyro_last_error_string",
 )
 
@@ -69,6 +69,7 @@ def load_library():
     lib.pyro_get_density.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_get_pressure.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_get_net_production_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
+    lib.pyro_get_jacobian.argtypes = [vp, i64, i64, vp, vp, vp, C.c_int, vp, vp, vp]
     lib.pyro_source_terms_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]
     lib.pyro_mech_info.argtypes = [vp, C.POINTER(i64), C.c_int]
     lib.pyro_probe_fp64_peak.argtypes = [C.c_int, dbl, C.POINTER(dbl)]
@@ -214,6 +215,22 @@ class Mechanism:
         _check(self._lib.pyro_get_net_production_rates(self._h, n, ld, _ptr(rho), _ptr(T), _ptr(Y), _ptr(out),
                                                        _stream(stream)))
         return out
+
+    def get_jacobian(self, rho, T, Y, mode=0, out=None, dSdT=None, want_dSdT=True, stream=None):
+        """pyro_get_jacobian: J[i, k, p] = dS_i/dY_k (mode 0: fixed (rho, T); mode 1: fixed (rho, e)) and
+        dSdT[i, p]; returns (J, dSdT).  J has shape [n_species, n_species, ld]."""
+        import torch
+        n = rho.shape[0]
+        ns = Y.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        if out is None:
+            out = torch.empty((ns, ns, ld), dtype=torch.float64, device=Y.device)
+        assert out.is_contiguous() and out.shape[2] == ld
+        if dSdT is None and want_dSdT:
+            dSdT = torch.empty((ns, ld), dtype=torch.float64, device=Y.device)
+        _check(self._lib.pyro_get_jacobian(self._h, n, ld, _ptr(rho), _ptr(T), _ptr(Y), int(mode), _ptr(out),
+                                           _ptr(dSdT), _stream(stream)))
+        return out[:, :, :n], (None if dSdT is None else dSdT[:, :n])
 
     def source_terms_host(self, rho, e, Y, T_guess, T_out, omega_out):
         """pyro_source_terms_host on HOST buffers (numpy arrays or CPU torch tensors, float64,

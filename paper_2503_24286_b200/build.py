@@ -11,8 +11,9 @@ import sys
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libpyro.so")
-SOURCES = ["pyro_kernels.cu", "pyro_api.cpp", "pyro_pack.cpp"]
-HEADERS = ["pyro_kernels.h", "pyro_pack.h", "pyro_tables.h", "pyro_math.cuh", "pyro_point.cuh",
+SOURCES = ["pyro_kernels.cu", "pyro_jac_kernels.cu", "pyro_api.cpp", "pyro_pack.cpp", "pyro_jac_pack.cpp"]
+HEADERS = ["pyro_kernels.h", "pyro_pack.h", "pyro_tables.h", "pyro_math.cuh", "pyro_point.cuh", "pyro_jac.cuh",
+           "pyro_jac_tables.h",
            os.path.join("..", "..", "include", "pyro.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "--shared", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

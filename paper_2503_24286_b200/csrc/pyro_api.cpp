@@ -84,6 +84,17 @@ struct pyro_mech {
     std::atomic<int> newton_max_iter{10};
     std::mutex pipe_mu;
     HostPipe pipe;
+    // chemical Jacobian (pyro_get_jacobian)
+    bool jac_ok = false;       // false: more species than the kernel holds (pyro_get_jacobian returns PYRO_ERR_UNSUPPORTED)
+    bool jac_small = true;     // plane V in tensor memory (else in shared memory)
+    pyro::JacPacked jac;
+    unsigned char *d_jblob = nullptr;
+    double *d_jext = nullptr;  // per-thread scratch of the [M] reactions, [1 + 2 n_ext][jac_grid_threads]
+    int jac_threads = 0, jac_blocks_per_sm = 0;
+    size_t jac_smem = 0;
+    uint32_t jac_tmem_cols = 32;
+    mutable std::mutex jac_mu;
+    cudaEvent_t jac_done = nullptr;   // launches on one handle share the scratch: each waits for the one before
 };
 
 namespace {
@@ -207,6 +218,9 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         cudaFree(m->d_blob);
         cudaFree(m->d_energy);
         cudaFree(m->d_work);
+        cudaFree(m->d_jblob);
+        cudaFree(m->d_jext);
+        if (m->jac_done) cudaEventDestroy(m->jac_done);
         for (cudaEvent_t ev : m->work_done)
             if (ev) cudaEventDestroy(ev);
         delete m;
@@ -349,6 +363,59 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
                 return bail(ce, "cudaMemcpy(tables)");
         }
     }
+    // ---- chemical Jacobian: tables, launch shape, scratch (mechanisms beyond its species limit keep everything else)
+    if (lay.n_species <= pyro::kJacMaxSpecies) {
+        st = pyro::pack_jacobian(desc, m->jac, err);
+        if (st != PYRO_OK) {
+            release();
+            return fail(st, err);
+        }
+        const pyro::JacLayout &jl = m->jac.lay;
+        if ((ce = cudaMalloc(&m->d_jblob, jl.bytes > 0 ? jl.bytes : 16)) != cudaSuccess) return bail(ce, "cudaMalloc(Jacobian tables)");
+        if ((ce = cudaMemcpy(m->d_jblob, m->jac.blob.data(), jl.bytes, cudaMemcpyHostToDevice)) != cudaSuccess)
+            return bail(ce, "cudaMemcpy(Jacobian tables)");
+        // Per point: planes C, G, dG/dT in shared memory; accumulators W, V, dS/dT in tensor memory, 6 columns per
+        // species row (one warp per lane quarter: at most 128 threads per block) if they fit 512 columns, else V
+        // moves to a fourth shared-memory plane (4 columns per row).
+        m->jac_small = 6 * rows + 2 <= 512;
+        if (const char *env = std::getenv("PYRO_JAC_V_PLANE")) {
+            if (!std::strcmp(env, "shared")) m->jac_small = false;
+        }
+        const size_t planes = m->jac_small ? 3 : 4;
+        cudaFuncAttributes fa{};
+        const void *jfn = pyro::jacobian_kernel_ptr(m->jac_small);
+        if ((ce = cudaFuncGetAttributes(&fa, jfn)) != cudaSuccess) return bail(ce, "cudaFuncGetAttributes(jacobian)");
+        const size_t jsmem_max = (size_t)prop.sharedMemPerBlockOptin - fa.sharedSizeBytes;
+        size_t jt = jsmem_max / (planes * 8 * rows);
+        jt = (jt / 32) * 32;
+        if (jt > (size_t)pyro::kJacMaxThreads) jt = pyro::kJacMaxThreads;
+        if (const char *env = std::getenv("PYRO_JAC_BLOCK")) {
+            const size_t forced = (size_t)std::atoi(env);
+            if (forced >= 32 && forced % 32 == 0 && forced <= jt) jt = forced;
+        }
+        if (jt >= 32) {
+            m->jac_threads = (int)jt;
+            m->jac_smem = planes * 8 * rows * jt;
+            const uint32_t need = (uint32_t)((m->jac_small ? 6 : 4) * rows + (m->jac_small ? 2 : 0));
+            m->jac_tmem_cols = 32;
+            while (m->jac_tmem_cols < need) m->jac_tmem_cols *= 2;
+            if ((ce = cudaFuncSetAttribute(jfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jsmem_max)) != cudaSuccess)
+                return bail(ce, "cudaFuncSetAttribute(jacobian)");
+            int jblk = 0;
+            if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&jblk, jfn, m->jac_threads, m->jac_smem)) != cudaSuccess)
+                return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor(jacobian)");
+            if (jblk > (int)(512 / m->jac_tmem_cols)) jblk = (int)(512 / m->jac_tmem_cols);
+            if (jblk >= 1) {
+                m->jac_blocks_per_sm = jblk;
+                const size_t grid_threads = (size_t)m->sm_count * jblk * jt;
+                if ((ce = cudaMalloc(&m->d_jext, (size_t)(1 + 2 * jl.n_ext) * grid_threads * sizeof(double))) != cudaSuccess)
+                    return bail(ce, "cudaMalloc(Jacobian scratch)");
+                if ((ce = cudaEventCreateWithFlags(&m->jac_done, cudaEventDisableTiming)) != cudaSuccess)
+                    return bail(ce, "cudaEventCreate(jacobian)");
+                m->jac_ok = true;
+            }
+        }
+    }
     *out = m;
     return PYRO_OK;
 }
@@ -363,6 +430,9 @@ int pyro_mech_destroy(pyro_mech *m) {
     cudaFree(m->d_blob);
     cudaFree(m->d_energy);
     cudaFree(m->d_work);
+    cudaFree(m->d_jblob);
+    cudaFree(m->d_jext);
+    if (m->jac_done) cudaEventDestroy(m->jac_done);
     for (cudaEvent_t ev : m->work_done)
         if (ev) cudaEventDestroy(ev);
     delete m;
@@ -451,6 +521,59 @@ int pyro_get_net_production_rates(const pyro_mech *m, int64_t n, int64_t ld, con
     }
     DeviceGuard guard(m->device);
     return enqueue_rates(m, rates_args(m, n, ld, rho, T, Y, omega), static_cast<cudaStream_t>(cuda_stream));
+}
+
+int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
+                      int mode, double *J, double *dSdT, void *cuda_stream) {
+    int st = check_fields(m, n, ld);
+    if (st != PYRO_OK) return st;
+    if (mode != PYRO_JAC_FIXED_T && mode != PYRO_JAC_FIXED_E) return fail(PYRO_ERR_BAD_SIZE, "mode must be PYRO_JAC_FIXED_T or PYRO_JAC_FIXED_E");
+    if (n == 0) return PYRO_OK;
+    if (!rho || !T || !Y || !J) return fail(PYRO_ERR_NULL, "a field pointer is NULL");
+    if (!aligned8(rho) || !aligned8(T) || !aligned8(Y) || !aligned8(J) || !aligned8(dSdT))
+        return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
+    if (!m->jac_ok) return fail(PYRO_ERR_UNSUPPORTED, "the Jacobian kernel holds at most 127 species");
+    const int64_t ns = m->packed.n_species;
+    {   // J (and dSdT) are written while Y of other points is still being read
+        const uintptr_t y0 = reinterpret_cast<uintptr_t>(Y), ys = (uintptr_t)((ns - 1) * ld + n) * sizeof(double);
+        const uintptr_t j0 = reinterpret_cast<uintptr_t>(J), js = (uintptr_t)((ns * ns - 1) * ld + n) * sizeof(double);
+        if (y0 < j0 + js && j0 < y0 + ys) return fail(PYRO_ERR_BAD_SIZE, "J must not overlap Y");
+        const uintptr_t t0 = reinterpret_cast<uintptr_t>(dSdT);
+        if (dSdT && ((y0 < t0 + ys && t0 < y0 + ys) || (j0 < t0 + ys && t0 < j0 + js)))
+            return fail(PYRO_ERR_BAD_SIZE, "dSdT must not overlap Y or J");
+    }
+    DeviceGuard guard(m->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    pyro::JacArgs a{};
+    a.n = n; a.ld = ld; a.n_chunks = (n + 31) / 32;
+    a.rho = rho; a.T = T; a.Y = Y; a.J = J; a.dSdT = dSdT;
+    a.gtab = m->d_blob;
+    a.off_spec = m->packed.lay.off_spec;
+    a.energy = m->d_energy;
+    a.jtab = m->d_jblob;
+    a.ext = m->d_jext;
+    a.tmem_cols = m->jac_tmem_cols;
+    a.mode = mode;
+    a.lay = m->jac.lay;
+    const int warps = m->jac_threads / 32;
+    int64_t blocks = (int64_t)m->sm_count * m->jac_blocks_per_sm;
+    if (blocks > (a.n_chunks + warps - 1) / warps) blocks = (a.n_chunks + warps - 1) / warps;
+    const uint32_t slot = m->next_work.fetch_add(1) % kWorkSlots;
+    a.work = m->d_work + slot;
+    std::lock_guard<std::mutex> lock(m->jac_mu);
+    {
+        std::lock_guard<std::mutex> wl(m->work_mu);
+        PYRO_CUDA(cudaStreamWaitEvent(stream, m->work_done[slot], 0));
+    }
+    PYRO_CUDA(cudaStreamWaitEvent(stream, m->jac_done, 0));   // the scratch is shared by the launches of one handle
+    PYRO_CUDA(cudaMemsetAsync(a.work, 0, sizeof(unsigned long long), stream));
+    PYRO_CUDA(pyro::launch_jacobian(a, m->jac_small, m->jac_threads, (int)blocks, m->jac_smem, stream));
+    PYRO_CUDA(cudaEventRecord(m->jac_done, stream));
+    {
+        std::lock_guard<std::mutex> wl(m->work_mu);
+        PYRO_CUDA(cudaEventRecord(m->work_done[slot], stream));
+    }
+    return PYRO_OK;
 }
 
 int pyro_source_terms_host(pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e,

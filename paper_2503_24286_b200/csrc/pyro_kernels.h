@@ -5,6 +5,7 @@
 #include <cstddef>
 #include <cstdint>
 
+#include "pyro_jac_tables.h"
 #include "pyro_tables.h"
 
 namespace pyro {
@@ -44,6 +45,25 @@ struct EosArgs {                 // (A.2)-(A.3): out = in / (Rm T) (density from
     const EnergyRow *energy;
     int32_t n_species, to_density;
 };
+
+constexpr int kJacMaxThreads = 128;     // threads (= points) per block of the Jacobian kernel: one warp per tensor-memory lane quarter
+
+struct JacArgs {                 // chemical Jacobian (pyro_jac_tables.h)
+    int64_t n, ld, n_chunks;
+    unsigned long long *work;    // chunk counter, zero at launch
+    const double *rho, *T, *Y;
+    double *J, *dSdT;            // J[(i n_s + k) ld + p]; dSdT[i ld + p] or NULL
+    const unsigned char *gtab;   // rates blob (species rows at off_spec)
+    const EnergyRow *energy;
+    const unsigned char *jtab;   // Jacobian blob
+    double *ext;                 // scratch of the [M] reactions: [1 + 2 n_ext][threads of the grid]
+    uint32_t off_spec, tmem_cols;
+    int32_t mode;                // 0: fixed (rho, T); 1: fixed (rho, e)
+    JacLayout lay;
+};
+
+const void *jacobian_kernel_ptr(bool small);
+cudaError_t launch_jacobian(const JacArgs &a, bool small, int threads, int blocks, size_t smem_bytes, cudaStream_t stream);
 
 const void *rates_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks);
 const void *temperature_kernel_ptr();

@@ -462,3 +462,94 @@ def test_fuzz_mechanisms(mechs):
         e = np.array([orc.mixture_e(float(T[p]), Y[:, p]) for p in range(1500)])
         T_ref, _, _ = orc.get_temperature(e, Y, T * 0.93)
         parity.assert_T_parity(gm.get_temperature(dev(e), dev(Y), dev(T * 0.93)).cpu().numpy(), T_ref)
+
+
+# ------------------------------------------------------------------ chemical Jacobian
+def gpu_jacobian(gm, rho, T, Y, mode, **kw):
+    J, sT = gm.get_jacobian(dev(rho), dev(T), dev(Y), mode=mode, **kw)
+    torch.cuda.synchronize()
+    return J.cpu().numpy(), (None if sT is None else sT.cpu().numpy())
+
+
+@pytest.mark.parametrize("mode", [0, 1])
+@pytest.mark.parametrize("cfg,n", [(0, 1500), (2, 333), (3, 70)])
+def test_jacobian_every_entry(mechs, cfg, n, mode):
+    """pyro_get_jacobian against the oracle's analytic Jacobian: every entry J[i, k, p] and dS/dT, several
+    blocks and a ragged tail; both readings of what is held fixed (G26)."""
+    mech, gm, orc = mechs(cfg)
+    st = inputs.config_states(cfg, n=n)
+    Y = st["Y"].copy()
+    Y[:, :3] = 0.0           # exact zeros in the composition: no division by a concentration
+    Y[mech.n_species - 1, :3] = 1.0
+    Jr, sTr, bJ, bT = orc.get_jacobian(st["rho"], st["T"], Y, mode=mode)
+    J, sT = gpu_jacobian(gm, st["rho"], st["T"], Y, mode)
+    r1 = parity.assert_jacobian_parity(J, Jr, bJ)
+    r2 = parity.assert_jacobian_parity(sT, sTr, bT)
+    print(f"cfg {cfg} mode {mode}: max |dJ|/bound = {r1:.2e}, max |d dSdT|/bound = {r2:.2e}")
+
+
+def test_jacobian_hand_mechanism_padded_ld_and_no_dSdT():
+    """Every reaction class; leading dimension larger than n with NaN padding left untouched; dSdT = NULL."""
+    mech = hand_cases.all_paths_mechanism()
+    gm = binding.Mechanism(mech)
+    n, ld, ns = 77, 96, mech.n_species
+    rho, T, Y = hand_cases.random_states(mech, n)
+    Yp = np.full((ns, ld), np.nan)
+    Yp[:, :n] = Y
+    Jr, sTr, bJ, bT = oracle.Oracle(mech).get_jacobian(rho, T, Y, mode=1)
+    out = torch.full((ns, ns, ld), float("nan"), dtype=torch.float64, device="cuda")
+    Yd, rd, Td = dev(Yp), dev(rho), dev(T)
+    binding._check(gm._lib.pyro_get_jacobian(gm._h, n, ld, rd.data_ptr(), Td.data_ptr(), Yd.data_ptr(), 1,
+                                             out.data_ptr(), None, None))
+    torch.cuda.synchronize()
+    o = out.cpu().numpy()
+    parity.assert_jacobian_parity(o[:, :, :n], Jr, bJ)
+    assert np.isnan(o[:, :, n:]).all()
+
+
+def test_jacobian_v_plane_in_shared_memory_and_small_blocks(mechs, monkeypatch):
+    """The large-mechanism layout (V in shared memory, 4 tensor-memory columns per species) forced on configs[0],
+    and 32-thread blocks."""
+    mech, _, orc = mechs(0)
+    st = inputs.config_states(0, n=700)
+    Jr, sTr, bJ, bT = orc.get_jacobian(st["rho"], st["T"], st["Y"], mode=0)
+    for env in ({"PYRO_JAC_V_PLANE": "shared"}, {"PYRO_JAC_BLOCK": "32"}):
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        gm = binding.Mechanism(mech)
+        J, sT = gpu_jacobian(gm, st["rho"], st["T"], st["Y"], 0)
+        parity.assert_jacobian_parity(J, Jr, bJ)
+        parity.assert_jacobian_parity(sT, sTr, bT)
+        for k in env:
+            monkeypatch.delenv(k)
+
+
+def test_jacobian_full_size_sampled_columns(mechs):
+    """configs[2] at the size bench.py times the Jacobian on (2^18 points): sampled points against the oracle."""
+    mech, gm, orc = mechs(2)
+    n = 1 << 18
+    st = inputs.config_states(2, n=n)
+    J, sT = gm.get_jacobian(dev(st["rho"]), dev(st["T"]), dev(st["Y"]), mode=1)
+    torch.cuda.synchronize()
+    idx = _sample(n, 96)
+    Jr, sTr, bJ, bT = orc.get_jacobian(st["rho"][idx], st["T"][idx], st["Y"][:, idx], mode=1)
+    parity.assert_jacobian_parity(J[:, :, idx].cpu().numpy(), Jr, bJ)
+    parity.assert_jacobian_parity(sT[:, idx].cpu().numpy(), sTr, bT)
+    # conservation of mass per column holds at any size: sum_i J_ik = 0 relative to the column's terms
+    s = J.sum(dim=0).abs().max().item()
+    assert s <= 1e-9 * J.abs().sum(dim=0).max().item()
+
+
+def test_jacobian_error_codes(mechs):
+    mech, gm, _ = mechs(0)
+    ns = mech.n_species
+    st = inputs.config_states(0, n=64)
+    rho, T, Y = dev(st["rho"]), dev(st["T"]), dev(st["Y"])
+    J = torch.empty((ns, ns, 64), dtype=torch.float64, device="cuda")
+    f = gm._lib.pyro_get_jacobian
+    assert f(gm._h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), 2, J.data_ptr(), None, None) == 2   # mode
+    assert f(gm._h, 64, 32, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), 0, J.data_ptr(), None, None) == 2   # ld < n
+    assert f(gm._h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), 0, None, None, None) == 1           # NULL
+    assert f(gm._h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), 0, J.data_ptr() + 4, None, None) == 5   # alignment
+    assert f(gm._h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), 0, Y.data_ptr(), None, None) == 2   # J overlaps Y
+    assert f(gm._h, 0, 0, None, None, None, 0, None, None, None) == 0                                       # n = 0
