@@ -144,6 +144,16 @@ int pyro_get_pressure(const pyro_mech *mech, int64_t n, int64_t ld, const double
 int pyro_get_net_production_rates(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho,
                                   const double *T, const double *Y, double *omega, void *cuda_stream);
 
+/* The whole source-term step in ONE launch (the source terms "for a given
+ * density, mass fractions, and internal energy"): per point the Newton solve of pyro_get_temperature from
+ * (e, Y, T_guess), then the production rates at that temperature.  All pointers device:
+ *   rho, e, T_guess [n], Y [n_species][ld]  in;   T [n] (may alias T_guess), omega [n_species][ld] (must not overlap Y)  out;
+ *   n_not_converged as in pyro_get_temperature.
+ * Results are those of pyro_get_temperature followed by pyro_get_net_production_rates (same iterates, same rates). */
+int pyro_source_terms(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e,
+                      const double *Y, const double *T_guess, double *T, double *omega, int32_t *n_not_converged,
+                      void *cuda_stream);
+
 /* Chemical Jacobian (eq. (6); (A.36) PAPER.md:1057) of the source terms S_i = W_i omega_i
  * ((A.1) PAPER.md:888), analytic:
  *   J[(i*n_species + k)*ld + p] = dS_i/dY_k     [n_species*n_species][ld], device, out; must not overlap Y

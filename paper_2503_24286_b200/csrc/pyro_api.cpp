@@ -123,7 +123,7 @@ int check_fields(const pyro_mech *m, int64_t n, int64_t ld) {
 bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7u) == 0; }
 
 // Enqueue the rates kernel of `m` on `stream`: persistent blocks, blocks_per_sm per SM at most.
-int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t stream) {
+int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t stream, bool fused = false) {
     const int warps = m->block_threads / 32;
     int64_t blocks = (int64_t)m->sm_count * m->blocks_per_sm;
     if (blocks > (a.n_chunks + warps - 1) / warps) blocks = (a.n_chunks + warps - 1) / warps;
@@ -135,7 +135,8 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     std::lock_guard<std::mutex> lock(m->work_mu);
     PYRO_CUDA(cudaStreamWaitEvent(stream, m->work_done[slot], 0));
     PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
-    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->smem_bytes, stream));
+    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->smem_bytes, stream,
+                                 fused));
     PYRO_CUDA(cudaEventRecord(m->work_done[slot], stream));
     return PYRO_OK;
 }
@@ -332,6 +333,13 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (const char *env = std::getenv("PYRO_CARVEOUT")) carveout = std::atoi(env);
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, carveout)) != cudaSuccess)
         return bail(ce, "cudaFuncSetAttribute(PreferredSharedMemoryCarveout)");
+    {   // the fused temperature + rates kernel of the same shape (pyro_source_terms)
+        const void *ffn = pyro::fused_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks);
+        if ((ce = cudaFuncSetAttribute(ffn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
+            return bail(ce, "cudaFuncSetAttribute(fused, MaxDynamicSharedMemorySize)");
+        if ((ce = cudaFuncSetAttribute(ffn, cudaFuncAttributePreferredSharedMemoryCarveout, carveout)) != cudaSuccess)
+            return bail(ce, "cudaFuncSetAttribute(fused, PreferredSharedMemoryCarveout)");
+    }
     int nblk = 0;
     if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nblk, fn, threads, m->smem_bytes)) != cudaSuccess)
         return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor");
@@ -521,6 +529,31 @@ int pyro_get_net_production_rates(const pyro_mech *m, int64_t n, int64_t ld, con
     }
     DeviceGuard guard(m->device);
     return enqueue_rates(m, rates_args(m, n, ld, rho, T, Y, omega), static_cast<cudaStream_t>(cuda_stream));
+}
+
+int pyro_source_terms(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e, const double *Y,
+                      const double *T_guess, double *T, double *omega, int32_t *n_not_converged, void *cuda_stream) {
+    int st = check_fields(m, n, ld);
+    if (st != PYRO_OK) return st;
+    if (n == 0) return PYRO_OK;
+    if (!rho || !e || !Y || !T_guess || !T || !omega) return fail(PYRO_ERR_NULL, "a field pointer is NULL");
+    if (!aligned8(rho) || !aligned8(e) || !aligned8(Y) || !aligned8(T_guess) || !aligned8(T) || !aligned8(omega) ||
+        (reinterpret_cast<uintptr_t>(n_not_converged) & 3u))
+        return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
+    {
+        const uintptr_t span = (uintptr_t)(((int64_t)m->packed.n_species - 1) * ld + n) * sizeof(double);
+        const uintptr_t y0 = reinterpret_cast<uintptr_t>(Y), w0 = reinterpret_cast<uintptr_t>(omega);
+        if (y0 < w0 + span && w0 < y0 + span) return fail(PYRO_ERR_BAD_SIZE, "omega must not overlap Y");
+    }
+    DeviceGuard guard(m->device);
+    pyro::RatesArgs a = rates_args(m, n, ld, rho, nullptr, Y, omega);
+    a.e = e; a.T_guess = T_guess; a.T_out = T; a.n_not_converged = n_not_converged;
+    a.energy = m->d_energy;
+    a.tol = m->newton_tol.load(std::memory_order_relaxed);
+    a.max_iter = m->newton_max_iter.load(std::memory_order_relaxed);
+    a.t_mid = m->packed.lay.t_mid;
+    a.single_t_mid = m->packed.lay.single_t_mid;
+    return enqueue_rates(m, a, static_cast<cudaStream_t>(cuda_stream), true);
 }
 
 int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,

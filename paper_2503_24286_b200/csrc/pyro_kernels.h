@@ -24,6 +24,13 @@ struct RatesArgs {
     uint32_t off_spec, off_rxn_p, off_rxn_x, off_fall, off_eff;
     int32_t n_species;
     GroupCounts groups;
+    // fused temperature + rates kernel only (pyro_source_terms): T is solved from (e, Y, T_guess) and written to T_out
+    const double *e, *T_guess;
+    double *T_out;
+    int32_t *n_not_converged;
+    const EnergyRow *energy;
+    double tol, t_mid;
+    int32_t max_iter, single_t_mid;
 };
 
 struct TempArgs {
@@ -66,9 +73,10 @@ const void *jacobian_kernel_ptr(bool small);
 cudaError_t launch_jacobian(const JacArgs &a, bool small, int threads, int blocks, size_t smem_bytes, cudaStream_t stream);
 
 const void *rates_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks);
+const void *fused_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks);
 const void *temperature_kernel_ptr();
 cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem,
-                         bool two_blocks, size_t smem_bytes, cudaStream_t stream);
+                         bool two_blocks, size_t smem_bytes, cudaStream_t stream, bool fused = false);
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream);
 cudaError_t launch_eos(const EosArgs &a, cudaStream_t stream);
 cudaError_t launch_dfma_probe(double *out, int iters, int blocks, cudaStream_t stream);

@@ -427,10 +427,9 @@ PYRO_HD int newton_temperature_general(int ns, const LoadY &load_y, const Row &r
     while (it < max_iter && !conv) {
         double S[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, Rm = 0.0;
         double t_below = -1.0, t_above = 1.7976931348623157e308;
-#pragma unroll 1
-        for (int k = 0; k < ns; ++k) {
+        auto add_species = [&](int k, double y) {
             const EnergyRow &r = row_of(k);
-            const double y = load_y(k), tm = r.t_mid;
+            const double tm = r.t_mid;
             const bool low = T < tm;
             const double *c = low ? r.lo : r.hi;
 #pragma unroll
@@ -438,7 +437,18 @@ PYRO_HD int newton_temperature_general(int ns, const LoadY &load_y, const Row &r
             Rm = fma(y, r.rw, Rm);
             t_above = low && tm < t_above ? tm : t_above;
             t_below = !low && tm > t_below ? tm : t_below;
+        };
+        int k = 0;
+#pragma unroll 1
+        for (; k + 4 <= ns; k += 4) {   // four mass fractions in flight: the pass is bound by the latency of these loads
+            const double y0 = load_y(k), y1 = load_y(k + 1), y2 = load_y(k + 2), y3 = load_y(k + 3);
+            add_species(k, y0);
+            add_species(k + 1, y1);
+            add_species(k + 2, y2);
+            add_species(k + 3, y3);
         }
+#pragma unroll 1
+        for (; k < ns; ++k) add_species(k, load_y(k));
         if (enthalpy) S[1] += Rm;
         do {
             double eT = fma(S[5], T, S[4]);

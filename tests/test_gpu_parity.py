@@ -553,3 +553,49 @@ def test_jacobian_error_codes(mechs):
     assert f(gm._h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), 0, J.data_ptr() + 4, None, None) == 5   # alignment
     assert f(gm._h, 64, 64, rho.data_ptr(), T.data_ptr(), Y.data_ptr(), 0, Y.data_ptr(), None, None) == 2   # J overlaps Y
     assert f(gm._h, 0, 0, None, None, None, 0, None, None, None) == 0                                       # n = 0
+
+
+# ------------------------------------------------------------------ fused temperature + rates
+@pytest.mark.parametrize("cfg,n", [(0, 4096), (2, 2500), (3, 700), (4, 13**3)])
+def test_fused_source_terms_every_point(mechs, cfg, n):
+    """pyro_source_terms: T against the oracle's Newton solve, omega against the oracle's rates at the GPU's T
+    (the same split of the comparison as the two-launch step of configs[4])."""
+    mech, gm, orc = mechs(cfg)
+    st = inputs.config_states(cfg, n=n)
+    T_ref, it, conv = orc.get_temperature(st["e"], st["Y"], st["T_guess"])
+    bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T, om = gm.source_terms(dev(st["rho"]), dev(st["e"]), dev(st["Y"]), dev(st["T_guess"]), n_not_converged=bad)
+    torch.cuda.synchronize()
+    T = T.cpu().numpy()
+    parity.assert_T_parity(T, T_ref)
+    assert int(bad.item()) == 0
+    om_ref, bound = orc.get_net_production_rates(st["rho"], T, st["Y"])
+    parity.assert_omega_parity(om.cpu().numpy(), om_ref, bound)
+    # and it is the two-launch step: same temperatures bit for bit, hence same rates
+    T2 = gm.get_temperature(dev(st["e"]), dev(st["Y"]), dev(st["T_guess"]))
+    om2 = gm.get_net_production_rates(dev(st["rho"]), T2, dev(st["Y"]))
+    torch.cuda.synchronize()
+    assert np.max(np.abs(T2.cpu().numpy() - T) / T) <= 1e-14
+    parity.assert_omega_parity(om.cpu().numpy(), om2.cpu().numpy(), bound)
+
+
+def test_fused_source_terms_mixed_t_mid_cap_and_in_place(mechs):
+    """Species with different break temperatures; T in place of T_guess; iteration cap reported."""
+    mech0, _, _ = mechs(0)
+    mech = inputs.with_species_break_temperatures(mech0, np.linspace(700.0, 1500.0, mech0.n_species))
+    gm, orc = binding.Mechanism(mech), oracle.Oracle(mech)
+    st = inputs.config_states(0, n=3000)
+    e = np.array([orc.mixture_e(st["T"][p], st["Y"][:, p]) for p in range(3000)])
+    T_ref, _, _ = orc.get_temperature(e, st["Y"], st["T_guess"])
+    Tg = dev(st["T_guess"])
+    T, om = gm.source_terms(dev(st["rho"]), dev(e), dev(st["Y"]), Tg, T_out=Tg)
+    torch.cuda.synchronize()
+    parity.assert_T_parity(Tg.cpu().numpy(), T_ref)
+    om_ref, bound = orc.get_net_production_rates(st["rho"], Tg.cpu().numpy(), st["Y"])
+    parity.assert_omega_parity(om.cpu().numpy(), om_ref, bound)
+    gm.set_newton(1e-6, 1)
+    bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+    gm.source_terms(dev(st["rho"]), dev(e), dev(st["Y"]), dev(st["T_guess"]), n_not_converged=bad)
+    torch.cuda.synchronize()
+    _, _, conv1 = orc.get_temperature(e, st["Y"], st["T_guess"], max_iter=1)
+    assert int(bad.item()) == int((conv1 == 0).sum()) > 0
