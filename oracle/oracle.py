@@ -72,6 +72,9 @@ def _load():
                 C.c_void_p, C.c_void_p, C.c_void_p]
             getattr(_lib, f"oracle_get_net_production_rates_{sfx}").argtypes = [
                 C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 7
+            getattr(_lib, f"oracle_reactor_rk4_{sfx}").argtypes = [
+                C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, real, C.c_int, real,
+                C.c_int, C.c_void_p, C.c_void_p]
             getattr(_lib, f"oracle_get_jacobian_{sfx}").argtypes = [
                 C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int] + [C.c_void_p] * 4
     return _lib
@@ -240,3 +243,20 @@ class Oracle:
         self._fn("get_jacobian")(C.byref(self._m), n, n, rho.ctypes.data, T.ctypes.data, Y.ctypes.data, int(mode),
                                  J.ctypes.data, dSdT.ctypes.data, bJ.ctypes.data, bT.ctypes.data)
         return J, dSdT, bJ, bT
+
+    def reactor_rk4(self, rho, e, Y, T_guess, dt, n_steps, tol=1e-6, max_iter=10):
+        """n_steps classical Runge-Kutta steps of size dt of the adiabatic isochoric reactors (A.1) PAPER.md:886-888
+        (PAPER.md:616), one reactor per point.  Returns (Y, T, Ybound, n_not_converged): final mass fractions,
+        temperature of the final state, the accumulated size of the terms added into each Y_k."""
+        rho = self._vec(rho)
+        e = self._vec(e)
+        Y = self._vec(Y).copy()
+        T = self._vec(T_guess).copy()
+        n = rho.shape[0]
+        assert Y.shape == (self.n_species, n)
+        Yb = np.empty_like(Y)
+        bad = C.c_int64(0)
+        self._fn("reactor_rk4")(C.byref(self._m), n, n, rho.ctypes.data, e.ctypes.data, Y.ctypes.data, T.ctypes.data,
+                                self._creal(dt), int(n_steps), self._creal(tol), int(max_iter), Yb.ctypes.data,
+                                C.byref(bad))
+        return Y, T, Yb, int(bad.value)

@@ -26,6 +26,8 @@
 //   density / pressure  N5 single species rho = p W/(R T), N6 p(rho(p)) = p, N7 sum_k C_k = p/(R T)
 //   jacobian            J1 differences of the oracle's omega (long double), J2 closed forms (W6), J3 conservation
 //                       per column, J4 the (rho, e) form through the Newton solve, J5 dS/dT by central differences
+//   reactor_rk4         R1 a step = degree-4 Taylor polynomial for a linear decay, R2 fourth order in dt, R3 mass and
+//                       element conservation, R4 energy, R5 equilibrium is a fixed point
 //   No function is "parity unpinned".
 //
 // Readings of garbled / silent passages are
@@ -513,6 +515,80 @@ void get_jacobian(const oracle_mech &m, int64_t n, int64_t ld, const Real *rho, 
                              boundJ ? boundJ + p : nullptr, bounddSdT ? bounddSdT + p : nullptr, ld);
 }
 
+// ---------------------------------------------------------------------------------------------------
+// homogeneous adiabatic isochoric reactors (A.1) PAPER.md:886-888,
+//     rho dY_k/dt = W_k omega_k(rho, T, Y),   rho and e constant,   T from (e, Y) by the Newton inversion (A.25)-(A.28),
+// marched with the classical fourth-order Runge-Kutta scheme at a fixed step ("standard fourth-order
+// accurate explicit Runge-Kutta ... a time step of 10 ns").  Written out stage by stage:
+//     k1 = f(Y0), k2 = f(Y0 + dt/2 k1), k3 = f(Y0 + dt/2 k2), k4 = f(Y0 + dt k3),  Y1 = Y0 + dt/6 (k1 + 2 k2 + 2 k3 + k4),
+//     f_k(Y) = W_k omega_k(rho, T(e, Y), Y) / rho.
+// Readings (G27): every stage inverts the temperature from the stage's mass fractions, starting the Newton
+// iteration from the temperature of the stage before (stop rule G11); mass fractions are neither clipped nor
+// renormalised (G17); the temperature returned is that of the final state.
+// Ybound_k accumulates the sizes of the terms that were added into Y_k (dt/6 (B1 + 2 B2 + 2 B3 + B4) W_k/rho with B the
+// bound_i of (A.5)): the scale of the parity tolerance.
+// Pins (tests/test_oracle_reactor_pins.py): R1 one irreversible reaction with constant rate coefficient: a step is
+// the degree-4 Taylor polynomial of exp(-k dt) exactly; R2 fourth-order convergence in dt; R3 mass and element
+// conservation; R4 energy: e(T_final, Y_final) = e; R5 a steady state (equilibrium composition) stays put.
+template <class Real>
+void reactor_rk4_point(const oracle_mech &m, Real rho, Real e, Real *Y, int64_t ld, Real &T, Real dt, int n_steps, Real tol,
+                       int max_iter, Real *Ybound, int64_t ldb, int &not_converged) {
+    const int ns = m.n_species;
+    std::vector<Real> Y0(ns), Ys(ns), om(ns), bd(ns), k1(ns), k2(ns), k3(ns), k4(ns), B(ns);
+    not_converged = 0;
+    auto f = [&](const std::vector<Real> &y, std::vector<Real> &k, Real weight) {
+        int it, cv;
+        Real Tn;
+        get_temperature_point<Real>(m, e, y.data(), 1, T, tol, max_iter, Tn, it, cv);
+        if (!cv) ++not_converged;
+        T = Tn;
+        production_rates_point<Real>(m, rho, T, y.data(), 1, om.data(), bd.data(), 1, nullptr, nullptr, 1);
+        for (int i = 0; i < ns; ++i) {
+            k[i] = Real(m.mol_weight[i]) * om[i] / rho;
+            B[i] += weight * Real(m.mol_weight[i]) * bd[i] / rho;
+        }
+    };
+    for (int i = 0; i < ns; ++i) {
+        Y0[i] = Y[i * ld];
+        if (Ybound) Ybound[i * ldb] = 0;
+    }
+    for (int step = 0; step < n_steps; ++step) {
+        for (int i = 0; i < ns; ++i) B[i] = 0;
+        f(Y0, k1, Real(1));
+        for (int i = 0; i < ns; ++i) Ys[i] = Y0[i] + dt / Real(2) * k1[i];
+        f(Ys, k2, Real(2));
+        for (int i = 0; i < ns; ++i) Ys[i] = Y0[i] + dt / Real(2) * k2[i];
+        f(Ys, k3, Real(2));
+        for (int i = 0; i < ns; ++i) Ys[i] = Y0[i] + dt * k3[i];
+        f(Ys, k4, Real(1));
+        for (int i = 0; i < ns; ++i) {
+            Y0[i] = Y0[i] + dt / Real(6) * (k1[i] + Real(2) * k2[i] + Real(2) * k3[i] + k4[i]);
+            if (Ybound) Ybound[i * ldb] += dt / Real(6) * B[i];
+        }
+    }
+    {   // temperature of the final state
+        int it, cv;
+        Real Tn;
+        get_temperature_point<Real>(m, e, Y0.data(), 1, T, tol, max_iter, Tn, it, cv);
+        if (!cv) ++not_converged;
+        T = Tn;
+    }
+    for (int i = 0; i < ns; ++i) Y[i * ld] = Y0[i];
+}
+
+template <class Real>
+void reactor_rk4(const oracle_mech &m, int64_t n, int64_t ld, const Real *rho, const Real *e, Real *Y, Real *T, Real dt,
+                 int n_steps, Real tol, int max_iter, Real *Ybound, int64_t *n_not_converged) {
+    int64_t bad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : bad)
+    for (int64_t p = 0; p < n; ++p) {
+        int nc;
+        reactor_rk4_point<Real>(m, rho[p], e[p], Y + p, ld, T[p], dt, n_steps, tol, max_iter, Ybound ? Ybound + p : nullptr, ld, nc);
+        bad += nc;
+    }
+    if (n_not_converged) *n_not_converged = bad;
+}
+
 template <class Real>
 void reaction_detail(const oracle_mech &m, int j, Real rho, Real T, const Real *Y, Real *out9) {
     const int ns = m.n_species;
@@ -589,6 +665,11 @@ int oracle_sizeof_real80() { return (int)sizeof(long double); }
                                       const Real *Y, int mode, Real *J, Real *dSdT, Real *boundJ,              \
                                       Real *bounddSdT) {                                                       \
         get_jacobian<Real>(*m, n, ld, rho, T, Y, mode, J, dSdT, boundJ, bounddSdT);                            \
+    }                                                                                                         \
+    void oracle_reactor_rk4_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *rho, const Real *e,    \
+                                     Real *Y, Real *T, Real dt, int n_steps, Real tol, int max_iter, Real *Ybound, \
+                                     int64_t *n_not_converged) {                                              \
+        reactor_rk4<Real>(*m, n, ld, rho, e, Y, T, dt, n_steps, tol, max_iter, Ybound, n_not_converged);      \
     }                                                                                                         \
     void oracle_get_net_production_rates_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld,                \
                                                   const Real *rho, const Real *T, const Real *Y, Real *omega, \
