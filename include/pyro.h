@@ -154,6 +154,21 @@ int pyro_source_terms(const pyro_mech *mech, int64_t n, int64_t ld, const double
                       const double *Y, const double *T_guess, double *T, double *omega, int32_t *n_not_converged,
                       void *cuda_stream);
 
+/* Batched reactor march: one adiabatic isochoric reactor (A.1) PAPER.md:886-888 per point,
+ *     rho dY_k/dt = W_k omega_k(rho, T, Y),   rho and e constant,   T from (e, Y) by the Newton solve of pyro_get_temperature,
+ * advanced by n_steps classical fourth-order Runge-Kutta steps of size dt (s) in ONE launch, the state
+ * staying on chip across the stages.  All pointers device:
+ *   rho, e [n]            in
+ *   Y [n_species][ld]     in: initial mass fractions; out: mass fractions after n_steps steps (not clipped, not renormalised)
+ *   T [n]                 in: Newton starting guess; out: temperature of the final state
+ *   work [n_species][ld]  scratch (contents undefined afterwards); must not overlap Y
+ *   n_not_converged       as in pyro_get_temperature: incremented once per Newton solve (4 per step + 1) that hit the cap
+ * Every stage starts its Newton iteration from the temperature of the stage before.  The step is the caller's: the
+ * scheme is explicit and unstable beyond the chemical time scale (the paper's H2 case needs 10 ns). n_steps = 0 only
+ * inverts the temperature. */
+int pyro_reactor_rk4(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e, double *Y,
+                     double *T, double dt, int32_t n_steps, double *work, int32_t *n_not_converged, void *cuda_stream);
+
 /* Chemical Jacobian (eq. (6); (A.36) PAPER.md:1057) of the source terms S_i = W_i omega_i
  * ((A.1) PAPER.md:888), analytic:
  *   J[(i*n_species + k)*ld + p] = dS_i/dY_k     [n_species*n_species][ld], device, out; must not overlap Y

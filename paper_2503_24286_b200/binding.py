@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libpyro.so")
 EXPORTS = (
     "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
     "pyro_get_temperature_from_enthalpy", "pyro_get_density", "pyro_get_pressure",
-    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
+    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
     "pyro_status_string", "pyro_last_error_string",
 )
 
@@ -70,6 +70,7 @@ def load_library():
     lib.pyro_get_pressure.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_get_net_production_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_get_jacobian.argtypes = [vp, i64, i64, vp, vp, vp, C.c_int, vp, vp, vp]
+    lib.pyro_reactor_rk4.argtypes = [vp, i64, i64, vp, vp, vp, vp, dbl, C.c_int32, vp, vp, vp]
     lib.pyro_source_terms.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.pyro_source_terms_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]
     lib.pyro_mech_info.argtypes = [vp, C.POINTER(i64), C.c_int]
@@ -230,6 +231,18 @@ class Mechanism:
         _check(self._lib.pyro_source_terms(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T_guess), _ptr(T_out),
                                            _ptr(omega_out), _ptr(n_not_converged), _stream(stream)))
         return T_out, omega_out
+
+    def reactor_rk4(self, rho, e, Y, T, dt, n_steps, work=None, n_not_converged=None, stream=None):
+        """pyro_reactor_rk4: marches Y (in place) by n_steps RK4 steps of size dt; T: guess in, final temperature out."""
+        import torch
+        n = rho.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        if work is None:
+            work = torch.empty_like(Y)
+        assert work.stride(0) == ld or n == 0
+        _check(self._lib.pyro_reactor_rk4(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T), float(dt), int(n_steps),
+                                          _ptr(work), _ptr(n_not_converged), _stream(stream)))
+        return Y, T
 
     def get_jacobian(self, rho, T, Y, mode=0, out=None, dSdT=None, want_dSdT=True, stream=None):
         """pyro_get_jacobian: J[i, k, p] = dS_i/dY_k (mode 0: fixed (rho, T); mode 1: fixed (rho, e)) and

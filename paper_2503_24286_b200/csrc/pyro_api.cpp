@@ -79,6 +79,9 @@ struct pyro_mech {
     uint32_t planes_off = 0;
     uint32_t tmem_cols = 32;
     int blocks_per_sm = 0;
+    size_t reactor_smem = 0;         // its dynamic shared memory: that of the rates kernel + the staged energy table
+    uint32_t reactor_energy_off = 0;
+    int reactor_blocks_per_sm = 1;   // resident blocks of the reactor kernel (same block shape as the rates kernel)
     int sm_count = 0;
     std::atomic<double> newton_tol{1e-6};      // read by concurrent calls while pyro_mech_set_newton may write
     std::atomic<int> newton_max_iter{10};
@@ -333,6 +336,27 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (const char *env = std::getenv("PYRO_CARVEOUT")) carveout = std::atoi(env);
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, carveout)) != cudaSuccess)
         return bail(ce, "cudaFuncSetAttribute(PreferredSharedMemoryCarveout)");
+    {   // the reactor kernel of the same shape (pyro_reactor_rk4)
+        const void *rfn = pyro::reactor_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks);
+        if ((ce = cudaFuncSetAttribute(rfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
+            return bail(ce, "cudaFuncSetAttribute(reactor, MaxDynamicSharedMemorySize)");
+        if ((ce = cudaFuncSetAttribute(rfn, cudaFuncAttributePreferredSharedMemoryCarveout, carveout)) != cudaSuccess)
+            return bail(ce, "cudaFuncSetAttribute(reactor, PreferredSharedMemoryCarveout)");
+        m->reactor_smem = m->smem_bytes;
+        m->reactor_energy_off = 0;
+        const size_t etab = (size_t)lay.n_species * sizeof(pyro::EnergyRow);
+        const size_t eoff = (m->smem_bytes + 15) & ~(size_t)15;
+        // (two-block shape of small mechanisms: the table is a few KB, inside the slack of the carve-out above)
+        if (eoff + etab <= smem_max && (!m->two_blocks || etab <= 4096)) {
+            m->reactor_energy_off = (uint32_t)eoff;
+            m->reactor_smem = eoff + etab;
+        }
+        int rblk = 0;
+        if ((ce = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&rblk, rfn, threads, m->reactor_smem)) != cudaSuccess)
+            return bail(ce, "cudaOccupancyMaxActiveBlocksPerMultiprocessor(reactor)");
+        if (rblk > (int)(512 / m->tmem_cols)) rblk = (int)(512 / m->tmem_cols);
+        m->reactor_blocks_per_sm = rblk < 1 ? 1 : rblk;
+    }
     {   // the fused temperature + rates kernel of the same shape (pyro_source_terms)
         const void *ffn = pyro::fused_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks);
         if ((ce = cudaFuncSetAttribute(ffn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)
@@ -554,6 +578,47 @@ int pyro_source_terms(const pyro_mech *m, int64_t n, int64_t ld, const double *r
     a.t_mid = m->packed.lay.t_mid;
     a.single_t_mid = m->packed.lay.single_t_mid;
     return enqueue_rates(m, a, static_cast<cudaStream_t>(cuda_stream), true);
+}
+
+int pyro_reactor_rk4(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e, double *Y, double *T,
+                     double dt, int32_t n_steps, double *work, int32_t *n_not_converged, void *cuda_stream) {
+    int st = check_fields(m, n, ld);
+    if (st != PYRO_OK) return st;
+    if (n_steps < 0 || !(dt == dt)) return fail(PYRO_ERR_BAD_SIZE, "n_steps must be >= 0 and dt a number");
+    if (n == 0) return PYRO_OK;
+    if (!rho || !e || !Y || !T || !work) return fail(PYRO_ERR_NULL, "a field pointer is NULL");
+    if (!aligned8(rho) || !aligned8(e) || !aligned8(Y) || !aligned8(T) || !aligned8(work) ||
+        (reinterpret_cast<uintptr_t>(n_not_converged) & 3u))
+        return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
+    {
+        const uintptr_t span = (uintptr_t)(((int64_t)m->packed.n_species - 1) * ld + n) * sizeof(double);
+        const uintptr_t y0 = reinterpret_cast<uintptr_t>(Y), w0 = reinterpret_cast<uintptr_t>(work);
+        if (y0 < w0 + span && w0 < y0 + span) return fail(PYRO_ERR_BAD_SIZE, "work must not overlap Y");
+    }
+    DeviceGuard guard(m->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    pyro::ReactorArgs a{};
+    a.rates = rates_args(m, n, ld, rho, nullptr, nullptr, nullptr);
+    a.rates.e = e;
+    a.rates.n_not_converged = n_not_converged;
+    a.rates.energy = m->d_energy;
+    a.rates.tol = m->newton_tol.load(std::memory_order_relaxed);
+    a.rates.max_iter = m->newton_max_iter.load(std::memory_order_relaxed);
+    a.rates.t_mid = m->packed.lay.t_mid;
+    a.rates.single_t_mid = m->packed.lay.single_t_mid;
+    a.Y = Y; a.T = T; a.acc = work; a.dt = dt; a.n_steps = n_steps;
+    a.energy_smem_off = m->reactor_energy_off;
+    const int warps = m->block_threads / 32;
+    int64_t blocks = (int64_t)m->sm_count * m->reactor_blocks_per_sm;
+    if (blocks > (a.rates.n_chunks + warps - 1) / warps) blocks = (a.rates.n_chunks + warps - 1) / warps;
+    const uint32_t slot = m->next_work.fetch_add(1) % kWorkSlots;
+    a.rates.work = m->d_work + slot;
+    std::lock_guard<std::mutex> lock(m->work_mu);
+    PYRO_CUDA(cudaStreamWaitEvent(stream, m->work_done[slot], 0));
+    PYRO_CUDA(cudaMemsetAsync(a.rates.work, 0, sizeof(unsigned long long), stream));
+    PYRO_CUDA(pyro::launch_reactor(a, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->reactor_smem, stream));
+    PYRO_CUDA(cudaEventRecord(m->work_done[slot], stream));
+    return PYRO_OK;
 }
 
 int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,

@@ -53,6 +53,20 @@ struct EosArgs {                 // (A.2)-(A.3): out = in / (Rm T) (density from
     int32_t n_species, to_density;
 };
 
+struct ReactorArgs {             // batched RK4 reactor march (pyro_reactor_rk4)
+    RatesArgs rates;             // tables, launch shape, rho, e, Newton controls, energy table, n_not_converged (Y, T, omega unused)
+    double *Y;                   // [n_species][ld] state, in/out
+    double *T;                   // [n] guess in, temperature of the final state out
+    double *acc;                 // [n_species][ld] scratch: running sum of the weighted stage slopes
+    double dt;
+    int32_t n_steps;
+    uint32_t energy_smem_off;    // byte offset of the staged energy table in dynamic shared memory (0: read it from global memory)
+};
+
+const void *reactor_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool singles);
+cudaError_t launch_reactor(const ReactorArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem, bool singles,
+                           size_t smem_bytes, cudaStream_t stream);
+
 constexpr int kJacMaxThreads = 128;     // threads (= points) per block of the Jacobian kernel: one warp per tensor-memory lane quarter
 
 struct JacArgs {                 // chemical Jacobian (pyro_jac_tables.h)

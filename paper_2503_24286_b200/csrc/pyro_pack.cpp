@@ -681,6 +681,7 @@ int pack_mechanism(const pyro_mech_desc *d, PackedMech &out, std::string &err, i
             const long double rw = kR / (long double)d->mol_weight[k];
             out.energy[k].rw = (double)rw;
             out.energy[k].t_mid = d->t_mid[k];
+            out.energy[k].w = d->mol_weight[k];
             for (int range = 0; range < 2; ++range) {
                 const double *a = (range ? d->nasa_hi : d->nasa_lo) + 7 * k;
                 double *c = range ? out.energy[k].hi : out.energy[k].lo;

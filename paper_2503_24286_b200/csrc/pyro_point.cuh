@@ -359,6 +359,7 @@ struct ArrayMem {
     PYRO_HD uint32_t atB(uint32_t k) const { return k; }
     PYRO_HD uint32_t atW(uint32_t k) const { return k; }
     PYRO_HD double ldA(uint32_t h) const { return A[h]; }
+    PYRO_HD void stA(uint32_t h, double v) const { A[h] = v; }
     PYRO_HD WRaw ldW(uint32_t h) const { return W[h]; }
     PYRO_HD WRaw ldB(uint32_t, uint32_t hB) const { return B[hB]; }
     PYRO_HD WBRaw ldWB(uint32_t hW, uint32_t hB) const { return WBRaw{W[hW], B[hB]}; }
@@ -469,6 +470,100 @@ PYRO_HD int newton_temperature_general(int ns, const LoadY &load_y, const Row &r
     *T_out = T;
     *converged = conv;
     return it;
+}
+
+// n_steps classical Runge-Kutta steps of one adiabatic isochoric reactor (A.1) PAPER.md:886-888,
+//     rho dY_k/dt = W_k omega_k(rho, T(e, Y), Y),     rho, e constant      (RK4 at a fixed step).
+// The state stays where the rates path keeps it: a stage's mass fractions are written into plane A, the Newton solve
+// of row a4 runs on them, fill_planes turns plane A into A_k = C_k E_k in place, accumulate_reactions leaves the
+// stage's omega in plane W, and the next stage's first sweep reads it from there.  Only Y0 (the caller's Y, updated in
+// place once per step) and the running sum of the weighted stage slopes (`acc`, a caller-provided scratch field)
+// live in global memory, one coalesced access per species and stage.
+//   y0_ld(k), y0_st(k, v)    mass fraction of species k at the start of the step (caller's Y)
+//   acc_ld(k), acc_st(k, v)  dt/6 k1 + dt/3 k2 + dt/3 k3 so far
+//   row_of(k)                energy row of species k (c_v polynomial, W_k, T_mid)
+// Returns the number of Newton solves that hit the iteration cap; *T is the guess on entry and the temperature of
+// the final state on return.
+template <bool kSingles, class Tab, class Mem, class Y0Ld, class Y0St, class AccLd, class AccSt, class Row>
+PYRO_HD int reactor_rk4_point(const Tab &tab, const GroupCounts &g, int ns, bool single_t_mid, double t_mid, double rho,
+                              double e, double *T, double dt, int n_steps, double tol, int max_iter, const Mem &mem,
+                              const Y0Ld &y0_ld, const Y0St &y0_st, const AccLd &acc_ld, const AccSt &acc_st, const Row &row_of) {
+    const double inv_rho = 1.0 / rho;
+    const double dt6 = dt / 6.0, dt3 = dt / 3.0, dth = dt / 2.0;
+    double Tc = *T;
+    int bad = 0;
+    for (int step = 0; step <= n_steps; ++step) {
+        const int n_stage = step < n_steps ? 4 : 1;   // after the last step: the final update and its temperature
+#pragma unroll 1
+        for (int s = 0; s < n_stage; ++s) {
+            double Slo[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0}, Shi[6] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+            const bool have_slope = step > 0 || s > 0;   // plane W holds the omega of the stage before
+            if (have_slope) mem.fence_st();
+            // eight species at a time: their omega (tensor memory) and their two global values are requested
+            // together, so the L2 latency of the state is paid once per batch
+            constexpr int NB = 8;
+            const bool need_acc = s != 1 && have_slope;
+#pragma unroll 1
+            for (int k = 0; k < ns; k += NB) {
+                typename Mem::WRaw wr[NB];
+                double y0v[NB], accv[NB];
+                if (have_slope) {
+#pragma unroll
+                    for (int i = 0; i < NB; ++i) wr[i] = mem.ldW(mem.atW((uint32_t)(k + i < ns ? k + i : ns)));
+                }
+#pragma unroll
+                for (int i = 0; i < NB; ++i) {
+                    const int ki = k + i < ns ? k + i : ns - 1;
+                    y0v[i] = y0_ld(ki);
+                    accv[i] = need_acc ? acc_ld(ki) : 0.0;
+                }
+                if (have_slope) mem.fence_ld();
+#pragma unroll
+                for (int i = 0; i < NB; ++i) {
+                    const int ki = k + i;
+                    if (ki < ns) {
+                        const EnergyRow &er = row_of(ki);
+                        const double slope = have_slope ? mem.value(wr[i]) * (er.w * inv_rho) : 0.0;   // W_k omega_k / rho
+                        double y0 = y0v[i], ys;
+                        if (s == 0) {
+                            if (have_slope) {   // Y1 = Y0 + dt/6 (k1 + 2 k2 + 2 k3 + k4)
+                                y0 = y0 + fma(dt6, slope, accv[i]);
+                                y0_st(ki, y0);
+                            }
+                            ys = y0;
+                        } else if (s == 1) {
+                            acc_st(ki, dt6 * slope);
+                            ys = fma(dth, slope, y0);
+                        } else {
+                            acc_st(ki, fma(dt3, slope, accv[i]));
+                            ys = fma(s == 2 ? dth : dt, slope, y0);
+                        }
+                        mem.stA(mem.atA((uint32_t)ki), ys);
+                        if (single_t_mid) {
+#pragma unroll
+                            for (int m = 0; m < 6; ++m) {
+                                Slo[m] = fma(ys, er.lo[m], Slo[m]);
+                                Shi[m] = fma(ys, er.hi[m], Shi[m]);
+                            }
+                        }
+                    }
+                }
+            }
+            bool conv;
+            if (single_t_mid)
+                newton_temperature(Slo, Shi, t_mid, e, Tc, tol, max_iter, &Tc, &conv);
+            else
+                newton_temperature_general(
+                    ns, [&](int q) { return mem.ldA(mem.atA((uint32_t)q)); }, row_of, false, e, Tc, tol, max_iter, &Tc, &conv);
+            bad += conv ? 0 : 1;
+            if (step == n_steps) break;
+            const PointT pt = make_point(Tc);
+            const double ctot = fill_planes(tab, ns, pt, rho, mem, [&](int q) { return mem.ldA(mem.atA((uint32_t)q)); });
+            accumulate_reactions<kSingles>(tab, g, pt, ctot, mem);
+        }
+    }
+    *T = Tc;
+    return bad;
 }
 
 }   // namespace pyro

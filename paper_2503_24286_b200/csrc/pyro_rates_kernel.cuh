@@ -46,6 +46,7 @@ template <bool kBTmem> struct DevMem {
     }
     __device__ __forceinline__ void sts(uint32_t h, double v) const { asm volatile("st.shared.f64 [%0], %1;" ::"r"(h), "d"(v)); }
     __device__ __forceinline__ double ldA(uint32_t h) const { return lds(h); }
+    __device__ __forceinline__ void stA(uint32_t h, double v) const { sts(h, v); }
     __device__ __forceinline__ WRaw ldtm2(uint32_t t) const {
         WRaw r;
         asm volatile("tcgen05.ld.sync.aligned.32x32b.x2.b32 {%0, %1}, [%2];" : "=r"(r.lo), "=r"(r.hi) : "r"(t));

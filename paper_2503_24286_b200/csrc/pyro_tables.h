@@ -149,9 +149,11 @@ struct GroupCounts {
 // rw = R/W_k serves the enthalpy form (h_k = e_k + R T/W_k) and the equation of
 // state (A.2)-(A.3) PAPER.md:892-899: sum_k Y_k R/W_k = R / W_mix.
 // t_mid: the species' own break temperature (the general solve for mechanisms with several of them).
+// w = W_k serves the reactor march (A.1): dY_k/dt = W_k omega_k / rho.  128 bytes.
 struct alignas(16) EnergyRow {
     double lo[6], hi[6];
     double rw, t_mid;
+    double w, pad;
 };
 
 }   // namespace pyro

@@ -225,6 +225,29 @@ int emu_jacobian(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *r
     return PYRO_OK;
 }
 
+// the per-point reactor march of reactor_kernel, one point after the other; Y in/out, T in (guess) / out, work scratch
+int emu_reactor(const pyro_mech_desc *d, int64_t n, int64_t ld, const double *rho, const double *e, double *Y, double *T,
+                double dt, int n_steps, double tol, int max_iter, double *work, int64_t *n_bad) {
+    pyro::PackedMech pm;
+    int st = pyro::pack_mechanism(d, pm, g_err);
+    if (st != PYRO_OK) return st;
+    HostTab tab{pm.blob.data(), pm.lay};
+    const pyro::GroupCounts g = group_counts(pm.lay);
+    const int ns = pm.n_species;
+    std::vector<double> A(ns + 1), B(ns + 1), W(ns + 1);
+    int64_t bad = 0;
+    for (int64_t p = 0; p < n; ++p) {
+        const pyro::ArrayMem mem{A.data(), B.data(), W.data()};
+        bad += pyro::reactor_rk4_point<true>(
+            tab, g, ns, pm.lay.single_t_mid != 0, pm.lay.t_mid, rho[p], e[p], &T[p], dt, n_steps, tol, max_iter, mem,
+            [&](int k) { return Y[k * ld + p]; }, [&](int k, double v) { Y[k * ld + p] = v; },
+            [&](int k) { return work[k * ld + p]; }, [&](int k, double v) { work[k * ld + p] = v; },
+            [&](int k) -> const pyro::EnergyRow & { return pm.energy[k]; });
+    }
+    if (n_bad) *n_bad = bad;
+    return PYRO_OK;
+}
+
 double emu_exp2(double y) { return pyro::exp2_poly(y); }
 
 double emu_log2(double x) { return pyro::log2_pos(x); }

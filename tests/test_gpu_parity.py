@@ -599,3 +599,82 @@ def test_fused_source_terms_mixed_t_mid_cap_and_in_place(mechs):
     torch.cuda.synchronize()
     _, _, conv1 = orc.get_temperature(e, st["Y"], st["T_guess"], max_iter=1)
     assert int(bad.item()) == int((conv1 == 0).sum()) > 0
+
+
+# ------------------------------------------------------------------ batched reactor march
+REACTOR_TOL = 1e-10   # |dY_k| <= REACTOR_TOL * (sum of the sizes of the terms added into Y_k + |Y_k|)
+
+
+def stable_dt(orc, rho, T, Y, safety=0.05):
+    """A step that resolves the fastest chemical time scale of the batch (largest Jacobian row sum of dY/dt = S/rho)."""
+    J, _, _, _ = orc.get_jacobian(rho, T, Y, mode=1)
+    return safety / float(np.max(np.abs(J).sum(axis=1) / np.asarray(rho)[None, :]))
+
+
+def assert_reactor_parity(Y, T, Y_ref, T_ref, Yb):
+    assert np.isfinite(Y).all() and np.isfinite(T).all()
+    rY = float(np.max(np.abs(Y - Y_ref) / (Yb + np.abs(Y_ref) + 1e-300)))
+    rT = float(np.max(np.abs(T - T_ref) / T_ref))
+    assert rY <= REACTOR_TOL, f"max |dY|/(Ybound + |Y|) = {rY:.3e}"
+    assert rT <= 1e-9, f"max |dT|/T = {rT:.3e}"
+    return rY, rT
+
+
+@pytest.mark.parametrize("case,n", [("all_paths", 333), ("cfg0", 3001), ("cfg2", 700), ("cfg3", 150), ("mixed_t_mid", 1000)])
+def test_reactor_rk4_every_point(mechs, case, n):
+    """pyro_reactor_rk4 against the oracle's RK4 march: final mass fractions and temperature of every reactor,
+    0, 1 and 7 steps, ragged tails, every reaction class, per-species break temperatures."""
+    if case == "all_paths":
+        mech = hand_cases.all_paths_mechanism()
+        rho, T, Y = hand_cases.random_states(mech, n)
+    else:
+        cfg = {"cfg0": 0, "cfg2": 2, "cfg3": 3, "mixed_t_mid": 0}[case]
+        mech = inputs.config_mechanism(cfg)
+        if case == "mixed_t_mid":
+            mech = inputs.with_species_break_temperatures(mech, np.linspace(800.0, 1400.0, mech.n_species))
+        st = inputs.config_states(cfg, n=n)
+        rho, T, Y = st["rho"], st["T"], st["Y"]
+    orc = oracle.Oracle(mech)
+    gm = binding.Mechanism(mech)
+    e = np.array([orc.mixture_e(T[p], Y[:, p]) for p in range(n)])
+    Tg = T * 1.03
+    ns_dt = min(n, 64)
+    dt = stable_dt(orc, rho[:ns_dt], T[:ns_dt], Y[:, :ns_dt], safety=0.02)
+    for n_steps in (0, 1, 7):
+        Yr, Tr, Yb, bad_r = orc.reactor_rk4(rho, e, Y, Tg, dt, n_steps)
+        ok = np.isfinite(Yr).all(axis=0) & np.isfinite(Tr) & (np.abs(Yr).max(axis=0) < 10.0)   # reactors the step is stable for
+        assert ok.sum() >= 0.5 * n
+        Yd, Td = dev(Y), dev(Tg)
+        bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+        gm.reactor_rk4(dev(rho), dev(e), Yd, Td, dt, n_steps, n_not_converged=bad)
+        torch.cuda.synchronize()
+        rY, rT = assert_reactor_parity(Yd.cpu().numpy()[:, ok], Td.cpu().numpy()[ok], Yr[:, ok], Tr[ok], Yb[:, ok])
+        if ok.all():
+            assert int(bad.item()) == bad_r
+        print(f"{case} steps {n_steps}: max |dY|/scale = {rY:.2e}, max |dT|/T = {rT:.2e}, stable reactors {int(ok.sum())}/{n}")
+
+
+def test_reactor_rk4_padded_ld_and_error_codes(mechs):
+    mech, gm, orc = mechs(0)
+    n, ld, ns = 100, 128, mech.n_species
+    st = inputs.config_states(0, n=n)
+    dt = stable_dt(orc, st["rho"][:32], st["T"][:32], st["Y"][:, :32], safety=0.02)
+    Yr, Tr, Yb, _ = orc.reactor_rk4(st["rho"], st["e"], st["Y"], st["T_guess"], dt, 3)
+    Yp = np.full((ns, ld), np.nan)
+    Yp[:, :n] = st["Y"]
+    Yd, Td = dev(Yp), dev(st["T_guess"])
+    work = torch.full((ns, ld), float("nan"), dtype=torch.float64, device="cuda")
+    rd, ed = dev(st["rho"]), dev(st["e"])
+    f = gm._lib.pyro_reactor_rk4
+    assert f(gm._h, n, ld, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr(), Td.data_ptr(), dt, 3, work.data_ptr(), None, None) == 0
+    torch.cuda.synchronize()
+    Yh = Yd.cpu().numpy()
+    ok = np.isfinite(Yr).all(axis=0) & (np.abs(Yr).max(axis=0) < 10.0)
+    assert_reactor_parity(Yh[:, :n][:, ok], Td.cpu().numpy()[ok], Yr[:, ok], Tr[ok], Yb[:, ok])
+    assert np.isnan(Yh[:, n:]).all() and torch.isnan(work[:, n:]).all()
+    assert f(gm._h, n, ld, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr(), Td.data_ptr(), dt, -1, work.data_ptr(), None, None) == 2
+    assert f(gm._h, n, 50, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr(), Td.data_ptr(), dt, 1, work.data_ptr(), None, None) == 2
+    assert f(gm._h, n, ld, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr(), Td.data_ptr(), dt, 1, None, None, None) == 1
+    assert f(gm._h, n, ld, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr(), Td.data_ptr(), dt, 1, Yd.data_ptr(), None, None) == 2
+    assert f(gm._h, n, ld, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr() + 4, Td.data_ptr(), dt, 1, work.data_ptr(), None, None) == 5
+    assert f(gm._h, 0, 0, None, None, None, None, dt, 1, None, None, None) == 0

@@ -78,6 +78,7 @@ def emu():
     L.emu_rates2.argtypes = [vp, i64, i64, vp, vp, vp, vp, C.c_int]
     L.emu_pack_side_log2.argtypes = [vp, C.c_int, vp]
     L.emu_jacobian.argtypes = [vp, i64, i64, vp, vp, vp, C.c_int, vp, vp]
+    L.emu_reactor.argtypes = [vp, i64, i64, vp, vp, vp, vp, C.c_double, C.c_int, C.c_double, C.c_int, vp, vp]
     return L
 
 
@@ -602,3 +603,59 @@ def test_jacobian_point_code_matches_oracle(emu, case, mode):
     assert np.all(np.isfinite(J)) and np.all(np.isfinite(sT))
     parity.assert_jacobian_parity(J, Jr, bJ)
     parity.assert_jacobian_parity(sT, sTr, bT)
+
+
+# ------------------------------------------------------------------ reactor march
+def stable_dt(orc, rho, T, Y, safety=0.05):
+    """A step that resolves the fastest chemical time scale of the batch (largest Jacobian row sum of dY/dt = S/rho)."""
+    J, _, _, _ = orc.get_jacobian(rho, T, Y, mode=1)
+    return safety / float(np.max(np.abs(J).sum(axis=1) / np.asarray(rho)[None, :]))
+
+
+def emu_reactor(emu, mech, rho, e, Y, Tg, dt, n_steps, tol=1e-6, max_iter=10):
+    desc, keep = binding.make_desc(mech)
+    rho, e = (np.ascontiguousarray(x, dtype=np.float64) for x in (rho, e))
+    Y = np.array(Y, dtype=np.float64, order="C")
+    T = np.array(Tg, dtype=np.float64)
+    work = np.full_like(Y, np.nan)
+    bad = C.c_int64(0)
+    st = emu.emu_reactor(C.byref(desc), rho.shape[0], rho.shape[0], rho.ctypes.data, e.ctypes.data, Y.ctypes.data,
+                         T.ctypes.data, dt, n_steps, tol, max_iter, work.ctypes.data, C.byref(bad))
+    assert st == 0, emu.emu_last_error()
+    return Y, T, int(bad.value)
+
+
+REACTOR_TOL = 1e-10   # |dY_k| <= REACTOR_TOL * (sum of the sizes of the terms added into Y_k + |Y_k|) (DESIGN.md section 5)
+
+
+def assert_reactor_parity(Y, T, Y_ref, T_ref, Yb):
+    assert np.isfinite(Y).all() and np.isfinite(T).all()
+    rY = float(np.max(np.abs(Y - Y_ref) / (Yb + np.abs(Y_ref) + 1e-300)))
+    rT = float(np.max(np.abs(T - T_ref) / T_ref))
+    assert rY <= REACTOR_TOL, f"max |dY|/(Ybound + |Y|) = {rY:.3e}"
+    assert rT <= 1e-9, f"max |dT|/T = {rT:.3e}"
+    return rY, rT
+
+
+@pytest.mark.parametrize("case", ["all_paths", "cfg0", "cfg2", "mixed_t_mid"])
+def test_reactor_point_code_matches_oracle(emu, case):
+    if case == "all_paths":
+        mech = hand_cases.all_paths_mechanism()
+        rho, T, Y = hand_cases.random_states(mech, 48)
+    else:
+        cfg = 2 if case == "cfg2" else 0
+        mech = inputs.config_mechanism(cfg)
+        if case == "mixed_t_mid":
+            mech = inputs.with_species_break_temperatures(mech, np.linspace(800.0, 1400.0, mech.n_species))
+        st = inputs.config_states(cfg, n=24 if cfg == 2 else 128)
+        rho, T, Y = st["rho"], st["T"], st["Y"]
+    orc = oracle.Oracle(mech)
+    e = np.array([orc.mixture_e(T[p], Y[:, p]) for p in range(len(T))])
+    Tg = T * 1.03
+    dt = stable_dt(orc, rho, T, Y)
+    for n_steps in (0, 1, 6):
+        Yr, Tr, Yb, bad_r = orc.reactor_rk4(rho, e, Y, Tg, dt, n_steps)
+        Ye, Te, bad_e = emu_reactor(emu, mech, rho, e, Y, Tg, dt, n_steps)
+        assert bad_r == bad_e == 0
+        rY, rT = assert_reactor_parity(Ye, Te, Yr, Tr, Yb)
+    assert np.any(np.abs(Yr - Y) > 1e-6 * np.abs(Y))
