@@ -72,6 +72,7 @@ def _load():
                 C.c_void_p, C.c_void_p, C.c_void_p]
             getattr(_lib, f"oracle_get_net_production_rates_{sfx}").argtypes = [
                 C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 7
+            getattr(_lib, f"oracle_get_transport_{sfx}").argtypes = [C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 5
             getattr(_lib, f"oracle_reactor_rk4_{sfx}").argtypes = [
                 C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, real, C.c_int, real,
                 C.c_int, C.c_void_p, C.c_void_p]
@@ -260,3 +261,37 @@ class Oracle:
                                 self._creal(dt), int(n_steps), self._creal(tol), int(max_iter), Yb.ctypes.data,
                                 C.byref(bad))
         return Y, T, Yb, int(bad.value)
+
+
+class _Transport(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("mol_weight", C.c_void_p), ("visc", C.c_void_p), ("cond", C.c_void_p),
+                ("diff", C.c_void_p)]
+
+
+class TransportOracle:
+    """Mixture-averaged transport properties (A.18)-(A.24) PAPER.md:968-996 for a table of polynomial fits
+    (`paper_2503_24286_b200.inputs.Transport` or any object with mol_weight [ns], visc [ns,5], cond [ns,5],
+    diff [ns,ns,5])."""
+
+    def __init__(self, tr, real="f64"):
+        self._lib = _load()
+        self.real = real
+        self.dtype = np.float64 if real == "f64" else np.longdouble
+        self.n_species = int(np.asarray(tr.mol_weight).shape[0])
+        self._keep = [np.ascontiguousarray(np.asarray(getattr(tr, k)), dtype=np.float64)
+                      for k in ("mol_weight", "visc", "cond", "diff")]
+        assert self._keep[1].shape == (self.n_species, 5) and self._keep[3].shape == (self.n_species, self.n_species, 5)
+        self._t = _Transport(self.n_species, *[a.ctypes.data for a in self._keep])
+
+    def get_transport(self, T, Y):
+        """Returns (mu [n], kappa [n], D_km [n_species, n])."""
+        T = np.ascontiguousarray(np.asarray(T), dtype=self.dtype)
+        Y = np.ascontiguousarray(np.asarray(Y), dtype=self.dtype)
+        n = T.shape[0]
+        assert Y.shape == (self.n_species, n)
+        mu = np.empty(n, dtype=self.dtype)
+        ka = np.empty(n, dtype=self.dtype)
+        D = np.empty((self.n_species, n), dtype=self.dtype)
+        getattr(self._lib, f"oracle_get_transport_{self.real}")(C.byref(self._t), n, n, T.ctypes.data, Y.ctypes.data,
+                                                                mu.ctypes.data, ka.ctypes.data, D.ctypes.data)
+        return mu, ka, D

@@ -26,6 +26,8 @@
 //   density / pressure  N5 single species rho = p W/(R T), N6 p(rho(p)) = p, N7 sum_k C_k = p/(R T)
 //   jacobian            J1 differences of the oracle's omega (long double), J2 closed forms (W6), J3 conservation
 //                       per column, J4 the (rho, e) form through the Newton solve, J5 dS/dT by central differences
+//   transport           X1 single species, X2 identical species, X3 the W7 fixture (50-digit evaluation), X4 binary
+//                       D_1,m = W_2 D_12/W, X5 permutation of the species, X6 Wilke limits
 //   reactor_rk4         R1 a step = degree-4 Taylor polynomial for a linear decay, R2 fourth order in dt, R3 mass and
 //                       element conservation, R4 energy, R5 equilibrium is a fixed point
 //   No function is "parity unpinned".
@@ -589,6 +591,88 @@ void reactor_rk4(const oracle_mech &m, int64_t n, int64_t ld, const Real *rho, c
     if (n_not_converged) *n_not_converged = bad;
 }
 
+// ---------------------------------------------------------------------------------------------------
+// mixture-averaged transport properties, Appendix A.2, as printed:
+//   X_k = W Y_k / W_k,  W = (sum_i Y_i/W_i)^-1                                              (A.3)
+//   mu_k    = sqrt(T) [sum_{m=0..4} b_km (ln T)^m]^2                                         (A.22)
+//   Phi_kj  = [1 + sqrt((mu_k/mu_j) sqrt(W_j/W_k))]^2 / sqrt(8 (1 + W_k/W_j))                (A.21)
+//   mu      = sum_k X_k mu_k / sum_j Phi_kj X_j                                              (A.20)
+//   kappa_k = sqrt(T) sum_m c_km (ln T)^m                                                    (A.24)
+//   kappa   = 1/2 [sum_k X_k kappa_k + (sum_k X_k/kappa_k)^-1]                               (A.23)
+//   D_kj    = sqrt(T) sum_m a_kjm (ln T)^m                                                   (A.19)
+//   D_k,m   = (W - X_k W_k)/W (sum_{j != k} X_j/D_kj)^-1                                     (A.18)
+// Readings: G28 the binary diffusivities are taken exactly as (A.19) prints them (sqrt(T) times the
+// polynomial, no pressure factor: the fits are the caller's, at the caller's pressure); G29 (A.18) is singular for a
+// pure species (0/0): left as printed, a mixture of at least two species is a documented precondition; G30 the
+// polynomial is evaluated by Horner's rule in ln T.
+// Pins (tests/test_oracle_transport_pins.py): X1 a single species returns its own mu_k, kappa_k; X2 identical species
+// mix to the species value at any composition; X3 the W7 fixture (50-digit mpmath evaluation of a three-species
+// mixture); X4 binary mixture D_1,m = W_2 D_12 / W; X5 permuting the species permutes the result; X6 Wilke's
+// identity Phi_jk = (mu_j/mu_k)(W_k/W_j) Phi_kj through the mixture formula (equal-mass, equal-viscosity limits).
+extern "C" {
+struct oracle_transport {
+    int32_t n_species;
+    const double *mol_weight;   // [n_species]
+    const double *visc;         // [n_species][5]  b_km
+    const double *cond;         // [n_species][5]  c_km
+    const double *diff;         // [n_species][n_species][5]  a_kjm
+};
+}
+
+template <class Real> Real poly4(const double *c, Real x) {   // sum_{m=0..4} c_m x^m, Horner (G30)
+    Real p = Real(c[4]);
+    for (int m = 3; m >= 0; --m) p = p * x + Real(c[m]);
+    return p;
+}
+
+template <class Real>
+void transport_point(const oracle_transport &t, Real T, const Real *Y, int64_t ld, Real &mu, Real &kappa, Real *Dkm,
+                     int64_t ldd) {
+    const int ns = t.n_species;
+    const Real lnT = std::log(T), sqT = std::sqrt(T);
+    std::vector<Real> X(ns), muk(ns), kak(ns);
+    Real s = 0;
+    for (int k = 0; k < ns; ++k) s += Y[k * ld] / Real(t.mol_weight[k]);
+    const Real W = Real(1) / s;                                                   // (A.3)
+    for (int k = 0; k < ns; ++k) {
+        X[k] = W * Y[k * ld] / Real(t.mol_weight[k]);
+        const Real pb = poly4<Real>(t.visc + 5 * k, lnT);
+        muk[k] = sqT * pb * pb;                                                   // (A.22)
+        kak[k] = sqT * poly4<Real>(t.cond + 5 * k, lnT);                          // (A.24)
+    }
+    mu = 0;
+    for (int k = 0; k < ns; ++k) {
+        Real den = 0;
+        for (int j = 0; j < ns; ++j) {
+            const Real Wk = t.mol_weight[k], Wj = t.mol_weight[j];
+            const Real a = Real(1) + std::sqrt(muk[k] / muk[j] * std::sqrt(Wj / Wk));
+            den += a * a / std::sqrt(Real(8) * (Real(1) + Wk / Wj)) * X[j];       // (A.21)
+        }
+        mu += X[k] * muk[k] / den;                                                // (A.20)
+    }
+    Real s1 = 0, s2 = 0;
+    for (int k = 0; k < ns; ++k) {
+        s1 += X[k] * kak[k];
+        s2 += X[k] / kak[k];
+    }
+    kappa = (s1 + Real(1) / s2) / Real(2);                                        // (A.23)
+    for (int k = 0; k < ns; ++k) {
+        Real sum = 0;
+        for (int j = 0; j < ns; ++j) {
+            if (j == k) continue;
+            sum += X[j] / (sqT * poly4<Real>(t.diff + 5 * ((size_t)k * ns + j), lnT));   // (A.19)
+        }
+        Dkm[k * ldd] = (W - X[k] * Real(t.mol_weight[k])) / W / sum;              // (A.18)
+    }
+}
+
+template <class Real>
+void get_transport(const oracle_transport &t, int64_t n, int64_t ld, const Real *T, const Real *Y, Real *mu, Real *kappa,
+                   Real *Dkm) {
+#pragma omp parallel for schedule(static)
+    for (int64_t p = 0; p < n; ++p) transport_point<Real>(t, T[p], Y + p, ld, mu[p], kappa[p], Dkm + p, ld);
+}
+
 template <class Real>
 void reaction_detail(const oracle_mech &m, int j, Real rho, Real T, const Real *Y, Real *out9) {
     const int ns = m.n_species;
@@ -670,6 +754,10 @@ int oracle_sizeof_real80() { return (int)sizeof(long double); }
                                      Real *Y, Real *T, Real dt, int n_steps, Real tol, int max_iter, Real *Ybound, \
                                      int64_t *n_not_converged) {                                              \
         reactor_rk4<Real>(*m, n, ld, rho, e, Y, T, dt, n_steps, tol, max_iter, Ybound, n_not_converged);      \
+    }                                                                                                         \
+    void oracle_get_transport_##SUFFIX(const oracle_transport *t, int64_t n, int64_t ld, const Real *T, const Real *Y, \
+                                       Real *mu, Real *kappa, Real *Dkm) {                                   \
+        get_transport<Real>(*t, n, ld, T, Y, mu, kappa, Dkm);                                                 \
     }                                                                                                         \
     void oracle_get_net_production_rates_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld,                \
                                                   const Real *rho, const Real *T, const Real *Y, Real *omega, \

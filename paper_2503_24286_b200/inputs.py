@@ -597,3 +597,64 @@ def simple_mechanism(species, reactions, elements=(), name="hand"):
         A0=f("A0", 1.0), b0=f("b0", 0.0), theta0=f("theta0", 0.0), troe=troe, name=name,
         meta={"kind": "hand"},
     )
+
+
+# --------------------------------------------------------------------------
+# transport fits: inputs of the mixture-averaged transport path (A.18)-(A.24)
+# --------------------------------------------------------------------------
+@dataclass
+class Transport:
+    """Polynomial fits in ln T of the species transport properties, in the forms the paper prints:
+    mu_k = sqrt(T) (sum_m visc[k,m] (ln T)^m)^2 (A.22), kappa_k = sqrt(T) sum_m cond[k,m] (ln T)^m (A.24),
+    D_kj = sqrt(T) sum_m diff[k,j,m] (ln T)^m (A.19).  SI units (Pa s, W/(m K), m^2/s)."""
+
+    mol_weight: np.ndarray  # [n_species]
+    visc: np.ndarray        # [n_species][5]
+    cond: np.ndarray        # [n_species][5]
+    diff: np.ndarray        # [n_species][n_species][5], symmetric in the species pair
+    name: str = ""
+
+    @property
+    def n_species(self) -> int:
+        return int(self.mol_weight.shape[0])
+
+
+def make_transport(mol_weight, seed, name="transport"):
+    """Synthetic fits shaped like those a kinetic-theory code produces (the paper takes them from Cantera,
+    which is not available here): per species a Lennard-Jones diameter sigma ~ U(2.5, 5.5) Angstrom and well depth
+    eps/k ~ U(30, 600) K; Chapman-Enskog viscosity, an Eucken-like conductivity and binary diffusivities at 1 atm from
+    the textbook collision-integral fits (Neufeld), sampled at 32 temperatures over 250-3500 K and least-squares
+    fitted in ln T in the printed forms.  These are input DATA: neither the oracle nor the CUDA path uses this code."""
+    rng = np.random.default_rng(seed)
+    W = np.asarray(mol_weight, dtype=np.float64)
+    ns = W.shape[0]
+    sigma = rng.uniform(2.5, 5.5, size=ns)
+    eps = rng.uniform(30.0, 600.0, size=ns)
+    eucken = rng.uniform(1.0, 2.0, size=ns)
+    T = np.geomspace(250.0, 3500.0, 32)
+    lnT = np.log(T)
+    V = np.vander(lnT, 5, increasing=True)
+    om22 = lambda ts: 1.16145 * ts ** -0.14874 + 0.52487 * np.exp(-0.7732 * ts) + 2.16178 * np.exp(-2.43787 * ts)
+    om11 = lambda ts: 1.06036 * ts ** -0.1561 + 0.193 * np.exp(-0.47635 * ts) + 1.03587 * np.exp(-1.52996 * ts) \
+        + 1.76474 * np.exp(-3.89411 * ts)
+    visc = np.zeros((ns, 5))
+    cond = np.zeros((ns, 5))
+    diff = np.zeros((ns, ns, 5))
+    for k in range(ns):
+        mu = 2.6693e-6 * np.sqrt(W[k] * T) / (sigma[k] ** 2 * om22(T / eps[k]))           # Pa s
+        visc[k] = np.linalg.lstsq(V, np.sqrt(mu / np.sqrt(T)), rcond=None)[0]
+        ka = mu * 3.75 * R_UNIVERSAL / W[k] * eucken[k]                                     # W/(m K)
+        cond[k] = np.linalg.lstsq(V, ka / np.sqrt(T), rcond=None)[0]
+    for k in range(ns):
+        for j in range(k, ns):
+            s_kj = 0.5 * (sigma[k] + sigma[j])
+            e_kj = np.sqrt(eps[k] * eps[j])
+            d = 2.6628e-7 * np.sqrt(T ** 3 * (W[k] + W[j]) / (2.0 * W[k] * W[j])) / (s_kj ** 2 * om11(T / e_kj))   # m^2/s at 1 atm
+            diff[k, j] = diff[j, k] = np.linalg.lstsq(V, d / np.sqrt(T), rcond=None)[0]
+    return Transport(mol_weight=W.copy(), visc=visc, cond=cond, diff=diff, name=name)
+
+
+def config_transport(cfg):
+    """Transport fits for the species of configs[cfg] (seed 3000 + cfg; cfg 4 shares cfg 2's)."""
+    c = 2 if cfg == 4 else cfg
+    return make_transport(config_mechanism(cfg).mol_weight, 3000 + c, name=f"cfg{c}")
