@@ -186,6 +186,31 @@ enum { PYRO_JAC_FIXED_T = 0, PYRO_JAC_FIXED_E = 1 };
 int pyro_get_jacobian(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *T,
                       const double *Y, int mode, double *J, double *dSdT, void *cuda_stream);
 
+/* Mixture-averaged transport properties, Appendix A.2 as printed, from
+ * polynomial fits in ln T that the caller supplies (the paper takes them from Cantera):
+ *   mu_k = sqrt(T) (sum_m visc[k][m] (ln T)^m)^2 (A.22)      kappa_k = sqrt(T) sum_m cond[k][m] (ln T)^m (A.24)
+ *   D_kj = sqrt(T) sum_m diff[k][j][m] (ln T)^m (A.19), m = 0..4; no pressure factor is applied (the fits are at the
+ *   caller's pressure); the diagonal diff[k][k] is never read.
+ * pyro_get_transport evaluates, per point, the Wilke mixture viscosity (A.20)-(A.21), the mixture conductivity
+ * (A.23) and the mixture-averaged diffusivities (A.18) with mole fractions X_k = W Y_k/W_k (A.3):
+ *   T [n], Y [n_species][ld]                         device, in
+ *   mu [n] (Pa s), kappa [n] (W/(m K)), D [n_species][ld] (m^2/s)    device, out; D must not overlap Y
+ * (A.18) is singular for a pure species (0/0): at least two species present is a precondition; T > 0.
+ * The description is HOST memory, borrowed during pyro_transport_create only.  Same status codes and error text
+ * (pyro_last_error_string) as the rest of the library; no CPU fallback. */
+typedef struct pyro_transport pyro_transport;
+typedef struct {
+    int32_t n_species;
+    const double *mol_weight; /* [n_species] kg/kmol                     */
+    const double *visc;       /* [n_species][5]                          */
+    const double *cond;       /* [n_species][5]                          */
+    const double *diff;       /* [n_species][n_species][5]               */
+} pyro_transport_desc;
+int pyro_transport_create(const pyro_transport_desc *desc, int device, pyro_transport **out);
+int pyro_transport_destroy(pyro_transport *tr);
+int pyro_get_transport(const pyro_transport *tr, int64_t n, int64_t ld, const double *T, const double *Y, double *mu,
+                       double *kappa, double *D, void *cuda_stream);
+
 /* The whole source-term step from HOST buffers: (rho, e, Y, T_guess) -> (T, omega).  Copies the
  * inputs to the device in slabs of points, runs the temperature solve and the rates kernel on
  * each slab and copies T and omega back, the three stages overlapped on separate streams.

@@ -18,7 +18,8 @@ EXPORTS = (
     "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
     "pyro_get_temperature_from_enthalpy", "pyro_get_density", "pyro_get_pressure",
     "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
-    "pyro_status_string", "pyro_last_error_string",
+    "pyro_status_string", "pyro_last_error_string", "pyro_transport_create", "pyro_transport_destroy",
+    "pyro_get_transport",
 )
 
 PYRO_OK = 0
@@ -51,6 +52,11 @@ class MechDesc(C.Structure):
 _lib = None
 
 
+class TransportDesc(C.Structure):
+    _fields_ = [("n_species", C.c_int32), ("mol_weight", C.c_void_p), ("visc", C.c_void_p), ("cond", C.c_void_p),
+                ("diff", C.c_void_p)]
+
+
 def load_library():
     """Loads libpyro.so (building it with nvcc first if the sources are newer)."""
     global _lib
@@ -73,6 +79,9 @@ def load_library():
     lib.pyro_reactor_rk4.argtypes = [vp, i64, i64, vp, vp, vp, vp, dbl, C.c_int32, vp, vp, vp]
     lib.pyro_source_terms.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.pyro_source_terms_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]
+    lib.pyro_transport_create.argtypes = [C.POINTER(TransportDesc), C.c_int, C.POINTER(vp)]
+    lib.pyro_transport_destroy.argtypes = [vp]
+    lib.pyro_get_transport.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
     lib.pyro_mech_info.argtypes = [vp, C.POINTER(i64), C.c_int]
     lib.pyro_probe_fp64_peak.argtypes = [C.c_int, dbl, C.POINTER(dbl)]
     lib.pyro_status_string.argtypes = [C.c_int]
@@ -284,3 +293,40 @@ def probe_fp64_peak(device=0, millis=200.0):
     out = C.c_double(0.0)
     _check(load_library().pyro_probe_fp64_peak(int(device), float(millis), C.byref(out)))
     return float(out.value)
+
+
+class Transport:
+    """Owns a pyro_transport handle (mixture-averaged transport fits of one species set)."""
+
+    def __init__(self, tr, device=0):
+        self._lib = load_library()
+        keep = [np.ascontiguousarray(np.asarray(getattr(tr, k)), dtype=np.float64)
+                for k in ("mol_weight", "visc", "cond", "diff")]
+        self.n_species = int(keep[0].shape[0])
+        desc = TransportDesc(self.n_species, *[a.ctypes.data for a in keep])
+        h = C.c_void_p()
+        _check(self._lib.pyro_transport_create(C.byref(desc), int(device), C.byref(h)))
+        self._h = h
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.pyro_transport_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def get_transport(self, T, Y, mu=None, kappa=None, D=None, stream=None):
+        """pyro_get_transport: (mu [n], kappa [n], D_km [n_species, ld]) from (T, Y)."""
+        import torch
+        n = T.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        mu = torch.empty_like(T) if mu is None else mu
+        kappa = torch.empty_like(T) if kappa is None else kappa
+        D = torch.empty_like(Y) if D is None else D
+        assert D.stride(0) == ld or n == 0
+        _check(self._lib.pyro_get_transport(self._h, n, ld, _ptr(T), _ptr(Y), _ptr(mu), _ptr(kappa), _ptr(D), _stream(stream)))
+        return mu, kappa, D

@@ -62,6 +62,10 @@ struct HostPipe {   // staging of pyro_source_terms_host
 
 }   // namespace
 
+namespace pyro {
+int set_last_error(int status, const std::string &msg) { return fail(status, msg); }
+}   // namespace pyro
+
 struct pyro_mech {
     int device = 0;
     pyro::PackedMech packed;

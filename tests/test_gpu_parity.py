@@ -678,3 +678,68 @@ def test_reactor_rk4_padded_ld_and_error_codes(mechs):
     assert f(gm._h, n, ld, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr(), Td.data_ptr(), dt, 1, Yd.data_ptr(), None, None) == 2
     assert f(gm._h, n, ld, rd.data_ptr(), ed.data_ptr(), Yd.data_ptr() + 4, Td.data_ptr(), dt, 1, work.data_ptr(), None, None) == 5
     assert f(gm._h, 0, 0, None, None, None, None, dt, 1, None, None, None) == 0
+
+
+# ------------------------------------------------------------------ mixture-averaged transport
+TRANSPORT_TOL = 1e-11   # relative, on mu, kappa and every D_k,m
+
+
+def assert_transport_parity(got, ref):
+    worst = 0.0
+    for g, r in zip(got, ref):
+        g = g.cpu().numpy() if hasattr(g, "cpu") else np.asarray(g)
+        assert np.isfinite(g).all()
+        worst = max(worst, float(np.max(np.abs(g - r) / np.abs(r))))
+    assert worst <= TRANSPORT_TOL, f"max relative difference {worst:.3e}"
+    return worst
+
+
+@pytest.mark.parametrize("cfg,n", [(0, 3001), (2, 1500), (3, 333)])
+def test_transport_every_point(cfg, n):
+    """pyro_get_transport against the oracle's (A.18)-(A.24): mu, kappa and every D_k,m of every point; several
+    blocks and a ragged tail; a composition with exact zeros."""
+    tr = inputs.config_transport(cfg)
+    st = inputs.config_states(cfg, n=n)
+    Y = st["Y"].copy()
+    Y[:, 0] = 0.0
+    Y[:2, 0] = 0.5            # only two species present
+    ref = oracle.TransportOracle(tr).get_transport(st["T"], Y)
+    gt = binding.Transport(tr)
+    got = gt.get_transport(dev(st["T"]), dev(Y))
+    torch.cuda.synchronize()
+    w = assert_transport_parity(got, ref)
+    print(f"transport cfg {cfg}: max relative difference {w:.2e}")
+
+
+def test_transport_w7_padded_ld_and_error_codes(golden_dir):
+    """The hand-written W7 mixture through the C ABI; leading dimension > n with NaN padding untouched; error codes."""
+    from test_oracle_transport_pins import _w7
+    from conftest import read_golden
+    mk, tr = _w7(golden_dir)
+    g = {k: float(v) for k, v in read_golden(os.path.join(golden_dir, "w7_transport.txt")).items()}
+    gt = binding.Transport(tr)
+    n, ld = 5, 8
+    Yp = np.full((3, ld), np.nan)
+    Yp[:, :n] = np.array([[float(y)] for y in mk.Y])
+    Td = dev(np.full(n, float(mk.T)))
+    Yd = dev(Yp)
+    mu = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
+    ka = torch.full((n,), float("nan"), dtype=torch.float64, device="cuda")
+    D = torch.full((3, ld), float("nan"), dtype=torch.float64, device="cuda")
+    f = gt._lib.pyro_get_transport
+    assert f(gt._h, n, ld, Td.data_ptr(), Yd.data_ptr(), mu.data_ptr(), ka.data_ptr(), D.data_ptr(), None) == 0
+    torch.cuda.synchronize()
+    assert abs(mu[0].item() / g["mu_mix"] - 1) < 1e-13 and abs(ka[4].item() / g["kappa_mix"] - 1) < 1e-13
+    for k in range(3):
+        assert abs(D[k, 2].item() / g[f"D_{k}m"] - 1) < 1e-13
+    assert torch.isnan(D[:, n:]).all()
+    assert f(gt._h, n, 3, Td.data_ptr(), Yd.data_ptr(), mu.data_ptr(), ka.data_ptr(), D.data_ptr(), None) == 2
+    assert f(gt._h, n, ld, Td.data_ptr(), Yd.data_ptr(), None, ka.data_ptr(), D.data_ptr(), None) == 1
+    assert f(gt._h, n, ld, Td.data_ptr(), Yd.data_ptr(), mu.data_ptr() + 4, ka.data_ptr(), D.data_ptr(), None) == 5
+    assert f(gt._h, n, ld, Td.data_ptr(), Yd.data_ptr(), mu.data_ptr(), ka.data_ptr(), Yd.data_ptr(), None) == 2
+    assert f(gt._h, 0, 0, None, None, None, None, None, None) == 0
+    assert f(None, n, ld, Td.data_ptr(), Yd.data_ptr(), mu.data_ptr(), ka.data_ptr(), D.data_ptr(), None) == 1
+    bad = binding.TransportDesc(0, None, None, None, None)
+    h = C.c_void_p()
+    assert gt._lib.pyro_transport_create(C.byref(bad), 0, C.byref(h)) == 2 and not h.value
+    assert gt._lib.pyro_transport_destroy(None) == 0
