@@ -147,6 +147,98 @@ def time_oracle(cfg, target_seconds, with_temperature=True):
                                               f"{dt:.1f} s", "n": n, "seconds": dt}
 
 
+def _event_times(fn, stream, reps, warm=2):
+    import torch
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    ts = []
+    for _ in range(reps):
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        fn()
+        b.record(stream)
+        torch.cuda.synchronize()
+        ts.append(a.elapsed_time(b))
+    return float(np.median(ts)), float(min(ts))
+
+
+def time_widened_rows(gm, mech, cfg, d, T, stream, device):
+    """SURVEY.md 8(f) rows beyond the step, each timed on its own (CUDA events, median of 5 after 2 warm-ups) on a
+    bounded slice of the same states: NEXT-2 chemical Jacobian, NEXT-3 mixture-averaged transport, NEXT-4 batched
+    RK4 reactors.  Rooflines: DESIGN.md section 7."""
+    import torch
+    from paper_2503_24286_b200 import binding
+    ns = mech.n_species
+    n = d["rho"].shape[0]
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = float(peaks.get("hbm_gbs", 6650.0))
+    out = {}
+    # ---- NEXT-2: J = dS/dY at fixed (rho, e) and dS/dT; output 8 ns^2 bytes per point dominates the traffic
+    nj = int(min(n, max(4096, (6 << 30) // (8 * ns * ns))))
+    nj = 1 << (nj.bit_length() - 1)
+    sl = lambda x: x[..., :nj].contiguous()
+    rho_j, T_j, Y_j = sl(d["rho"]), sl(T), sl(d["Y"])
+    J = torch.empty((ns, ns, nj), dtype=torch.float64, device="cuda")
+    sT = torch.empty((ns, nj), dtype=torch.float64, device="cuda")
+    try:
+        ms, mn = _event_times(lambda: gm.get_jacobian(rho_j, T_j, Y_j, mode=1, out=J, dSdT=sT, stream=stream), stream, 5)
+        byt = 8.0 * (ns * ns + 3 * ns + 2) * nj
+        out["next2_jacobian"] = {
+            "points": nj, "ms": ms, "ms_min": mn, "points_per_s": nj / (ms * 1e-3), "mode": "fixed (rho, e)",
+            "roofline": {"bound": "hbm", "achieved": byt / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                         "frac": byt / (ms * 1e-3) / 1e9 / hbm_peak, "bytes_per_point": 8.0 * (ns * ns + 3 * ns + 2)}}
+        # a stable explicit step for the reactors: the largest row sum of |J|/rho over the slice bounds the stiffness
+        rate = float((J.abs().sum(dim=1) / rho_j[None, :]).max().item())
+    except binding.PyroError as ex:
+        out["next2_jacobian"] = {"unavailable": str(ex)}
+        rate = None
+    del J, sT
+    # ---- NEXT-3: mixture-averaged transport, O(ns^2) FP64 per point
+    tr = inputs.config_transport(cfg)
+    gt = binding.Transport(tr, device=device)
+    nt = int(min(n, 1 << 20))
+    T_t, Y_t = T[:nt].contiguous(), d["Y"][:, :nt].contiguous()
+    mu, ka, D = torch.empty_like(T_t), torch.empty_like(T_t), torch.empty_like(Y_t)
+    ms, mn = _event_times(lambda: gt.get_transport(T_t, Y_t, mu, ka, D, stream=stream), stream, 5)
+    # per ordered pair: Phi 7 flops, Horner 8, reciprocal counted as a division, accumulate 2; per species 2 Horner + 3 divisions
+    fl = ns * ns * (7 + 8 + FLOPS_DIV + 2) + ns * (16 + 3 * FLOPS_DIV + 12) + FLOPS_LOG + 2 * FLOPS_DIV
+    out["next3_transport"] = {
+        "points": nt, "ms": ms, "ms_min": mn, "points_per_s": nt / (ms * 1e-3),
+        "roofline": {"bound": "alu", "achieved": fl * nt / (ms * 1e-3) / 1e12, "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s",
+                     "frac": fl * nt / (ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS, "flops_per_point": float(fl)}}
+    gt.close()
+    # ---- NEXT-4: RK4 reactors, 4 stages (Newton solve + rates) per step
+    if rate:
+        nr = int(min(n, 1 << 20))
+        steps = 4
+        dt = 1e-3 / rate
+        rho_r, e_r = d["rho"][:nr].contiguous(), d["e"][:nr].contiguous()
+        work = torch.empty((ns, nr), dtype=torch.float64, device="cuda")
+        Y_r, T_r = d["Y"][:, :nr].clone(), d["T_guess"][:nr].clone()
+
+        def march():
+            Y_r.copy_(d["Y"][:, :nr])
+            T_r.copy_(d["T_guess"][:nr])
+            gm.reactor_rk4(rho_r, e_r, Y_r, T_r, dt, steps, work=work, stream=stream)
+        copy_ms, _ = _event_times(lambda: (Y_r.copy_(d["Y"][:, :nr]), T_r.copy_(d["T_guess"][:nr])), stream, 5)
+        ms, mn = _event_times(march, stream, 5)
+        ms, mn = ms - copy_ms, mn - copy_ms
+        fl = 4 * algorithmic_flops_per_point(mech) + 4 * (25 * ns + FLOPS_DIV + 4) * 4
+        out["next4_reactor_rk4"] = {
+            "reactors": nr, "steps": steps, "dt": dt, "ms": ms, "ms_min": mn,
+            "reactor_steps_per_s": nr * steps / (ms * 1e-3), "ns_per_reactor_stage": ms * 1e6 / nr / steps / 4,
+            "finite_fraction": float(torch.isfinite(Y_r).all(dim=0).float().mean().item()),
+            "roofline": {"bound": "alu", "achieved": fl * nr * steps / (ms * 1e-3) / 1e12, "peak": FP64_PEAK_TFLOPS,
+                         "unit": "TFLOP/s", "frac": fl * nr * steps / (ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS,
+                         "flops_per_reactor_step": float(fl)}}
+    return out
+
+
 def reference_arm(args, rank):
     """--impl reference: the oracle timed on the host cores (this tier's reference arm)."""
     if rank != 0:
@@ -185,6 +277,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-widened", action="store_true", help="skip the SURVEY 8(f) rows (Jacobian, transport, reactors)")
     ap.add_argument("--points", type=int, default=0, help="override the number of points (profiling runs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -252,8 +345,10 @@ def main():
         t_end.record(stream)
         barrier()
     total_ms = t_begin.elapsed_time(t_end)
-    temp_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in ev]))
-    rates_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in ev]))
+    temp_all = [e[0].elapsed_time(e[1]) for e in ev]
+    rates_all = [e[1].elapsed_time(e[2]) for e in ev]
+    temp_ms = float(np.median(temp_all))      # per-launch CUDA-event times: median (and min) over the timed steps
+    rates_ms = float(np.median(rates_all))
     total_ms = sharding.max_over_ranks(total_ms, device="cuda")
     ms_per_step = total_ms / args.steps
     value = sharding.job_throughput(n, world, ms_per_step)
@@ -304,6 +399,10 @@ def main():
         gm.get_temperature(d["e"], d["Y"], d["T_guess"], rho=d["rho"], out=T, n_not_converged=bad, stream=stream)
         torch.cuda.synchronize()
 
+    widened = {}
+    if rank == 0 and not args.no_widened:
+        widened = time_widened_rows(gm, mech, cfg, d, T, stream, local_rank)
+
     if rank == 0:
         flops_pt = algorithmic_flops_per_point(mech)
         bytes_pt = algorithmic_bytes_per_point(ns)
@@ -333,7 +432,8 @@ def main():
                 "registers": info["registers"], "spill_bytes": info["local_bytes"],
                 "newton_not_converged": not_converged,
             },
-            "kernels_ms": {"temperature": temp_ms, "rates": rates_ms},
+            "kernels_ms": {"temperature": temp_ms, "rates": rates_ms, "temperature_min": float(min(temp_all)),
+                           "rates_min": float(min(rates_all)), "statistic": "median and min of the per-launch event times"},
             "roofline": {
                 "bound": "alu", "kernel": "rates_kernel", "achieved": achieved_tflops, "peak": FP64_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved_tflops / FP64_PEAK_TFLOPS,
@@ -354,6 +454,7 @@ def main():
             "clocks": clocks.summary(),
             "gpu_launches": 2 * args.steps,
         }
+        line.update(widened)
         if e2e:
             line["e2e"] = e2e
         if not args.no_cpu_baseline and world == 1:
