@@ -99,6 +99,7 @@ struct pyro_mech {
     double *d_jext = nullptr;  // per-thread scratch of the [M] reactions, [1 + 2 n_ext][jac_grid_threads]
     int jac_threads = 0, jac_blocks_per_sm = 0;
     size_t jac_smem = 0;
+    uint32_t jac_planes_bytes = 0;
     uint32_t jac_tmem_cols = 32;
     mutable std::mutex jac_mu;
     cudaEvent_t jac_done = nullptr;   // launches on one handle share the scratch: each waits for the one before
@@ -422,7 +423,7 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         const void *jfn = pyro::jacobian_kernel_ptr(m->jac_small);
         if ((ce = cudaFuncGetAttributes(&fa, jfn)) != cudaSuccess) return bail(ce, "cudaFuncGetAttributes(jacobian)");
         const size_t jsmem_max = (size_t)prop.sharedMemPerBlockOptin - fa.sharedSizeBytes;
-        size_t jt = jsmem_max / (planes * 8 * rows);
+        size_t jt = jsmem_max / (planes * 8 * rows + pyro::kJacRingBytes / 32);   // + the warp's share of its record ring
         jt = (jt / 32) * 32;
         if (jt > (size_t)pyro::kJacMaxThreads) jt = pyro::kJacMaxThreads;
         if (const char *env = std::getenv("PYRO_JAC_BLOCK")) {
@@ -431,7 +432,8 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         }
         if (jt >= 32) {
             m->jac_threads = (int)jt;
-            m->jac_smem = planes * 8 * rows * jt;
+            m->jac_planes_bytes = (uint32_t)(planes * 8 * rows * jt);
+            m->jac_smem = m->jac_planes_bytes + (jt / 32) * pyro::kJacRingBytes;
             const uint32_t need = (uint32_t)((m->jac_small ? 6 : 4) * rows + (m->jac_small ? 2 : 0));
             m->jac_tmem_cols = 32;
             while (m->jac_tmem_cols < need) m->jac_tmem_cols *= 2;
@@ -655,6 +657,7 @@ int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *r
     a.jtab = m->d_jblob;
     a.ext = m->d_jext;
     a.tmem_cols = m->jac_tmem_cols;
+    a.planes_bytes = m->jac_planes_bytes;
     a.mode = mode;
     a.lay = m->jac.lay;
     const int warps = m->jac_threads / 32;

@@ -107,6 +107,7 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
     mem.fill((uint32_t)ns, 1.0, 0.0, 0.0);
     mem.st_ext(0u, 1.0);
     // ---- phase 1: third-body and falloff reactions (readings G6-G8), once per point
+    tab.begin_rxn(lay.n_plain, lay.n_ext);   // the records of a phase are read front to back (kernel: streamed through shared memory)
 #pragma unroll 1
     for (int x = 0; x < lay.n_ext; ++x) {
         const JacRxn &r = tab.rxn(lay.n_plain + x);
@@ -163,6 +164,7 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
         jac_scatter<PV>(mem, r.sc_species, r.sc_w, g * r.eff_default);
     }
     // ---- phase 2: temperature derivative of the other reactions
+    tab.begin_rxn(0, lay.n_plain);
 #pragma unroll 1
     for (int j = 0; j < lay.n_plain; ++j) {
         const JacRxn &r = tab.rxn(j);
@@ -180,6 +182,7 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
     }
     // ---- phase 3: the columns
     const double rcv = mode == 1 ? 1.0 / cv : 0.0;
+    tab.begin_inc();
 #pragma unroll 1
     for (int k = 0; k < ns; ++k) {
         const JacCol &col = tab.col(k);
@@ -193,11 +196,6 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
             const double m = e.coef * mem.ld_ext(e.mul);
             exp2_poly_n<1>(y);
             jac_scatter<PW>(mem, e.sc_species, e.sc_w, (m * y[0]) * others);
-        }
-#pragma unroll 1
-        for (uint32_t q = col.eff_begin; q < col.eff_end; ++q) {
-            const JacEffInc &e = tab.effinc((int)q);
-            jac_scatter<PW>(mem, e.sc_species, e.sc_w, e.delta * mem.ld_ext(e.g));
         }
         mem.fence_st();
         // J_ik = (column_i + V_i) rho/W_k - dS_i/dT e_k/c_v ; the column accumulator is cleared for the next one
@@ -214,11 +212,17 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
             ekcv = ek * rcv;
         }
 #pragma unroll 1
-        for (int i = 0; i < ns; ++i) {
-            const typename Mem::Out o = mem.ld_out((uint32_t)i);
+        for (int i = 0; i < ns; i += 4) {   // four rows in flight per tensor-memory round trip
+            typename Mem::Out o[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u) o[u] = mem.ld_out((uint32_t)(i + u < ns ? i + u : ns));
             mem.fence_ld();
-            store_J(i, k, fma(mem.out_w(o) + mem.out_v(o), scale, -(mem.out_dt(o) * ekcv)));
-            mem.template st_acc<PW>((uint32_t)i, 0.0);
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+                if (i + u < ns) {
+                    store_J(i + u, k, fma(mem.out_w(o[u]) + mem.out_v(o[u]), scale, -(mem.out_dt(o[u]) * ekcv)));
+                    mem.template st_acc<PW>((uint32_t)(i + u), 0.0);
+                }
         }
     }
 }

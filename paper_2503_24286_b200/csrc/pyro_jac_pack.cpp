@@ -23,7 +23,7 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
     std::vector<EffEntry> effs;
     std::vector<RxnFall> falls;
     std::vector<std::vector<JacInc>> inc(ns);
-    std::vector<std::vector<JacEffInc>> effinc(ns);
+    std::vector<std::vector<JacInc>> effinc(ns);   // incidences through a listed third-body efficiency
     for (int j = 0; j < nr; ++j) {
         JacRxn r;
         std::memset(&r, 0, sizeof r);
@@ -63,14 +63,18 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
             for (int q = d->eff_ptr[j]; q < d->eff_ptr[j + 1]; ++q) {
                 const double delta = d->eff_value[q] - d->eff_default[j];
                 effs.push_back(EffEntry{delta, (uint32_t)d->eff_species[q], 0u});
-                JacEffInc e;
+                // species eff_species[q] enters R through [M]: d = delta * g_x, written as an incidence whose
+                // exponent is 0 (2^0 = 1 exactly) and whose other molecules are the dummy species (C = 1)
+                JacInc e;
                 std::memset(&e, 0, sizeof e);
-                e.delta = delta;
+                e.coef = delta;
                 for (int m = 0; m < 6; ++m) {
                     e.sc_w[m] = r.sc_w[m];
                     e.sc_species[m] = r.sc_species[m];
+                    e.gslot[m] = dummy;
                 }
-                e.g = (uint16_t)(2u + 2u * r.ext);
+                e.other[0] = e.other[1] = dummy;
+                e.mul = (uint16_t)(2u + 2u * r.ext);
                 effinc[d->eff_species[q]].push_back(e);
             }
             r.eff_count = (uint32_t)effs.size() - r.eff_begin;
@@ -124,17 +128,13 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
     lay.n_fall = (int)falls.size();
     std::vector<JacCol> cols(ns);
     std::vector<JacInc> inc_all;
-    std::vector<JacEffInc> effinc_all;
     for (int k = 0; k < ns; ++k) {
         cols[k].inc_begin = (uint32_t)inc_all.size();
         inc_all.insert(inc_all.end(), inc[k].begin(), inc[k].end());
+        inc_all.insert(inc_all.end(), effinc[k].begin(), effinc[k].end());
         cols[k].inc_end = (uint32_t)inc_all.size();
-        cols[k].eff_begin = (uint32_t)effinc_all.size();
-        effinc_all.insert(effinc_all.end(), effinc[k].begin(), effinc[k].end());
-        cols[k].eff_end = (uint32_t)effinc_all.size();
     }
     lay.n_inc = (int)inc_all.size();
-    lay.n_effinc = (int)effinc_all.size();
     std::vector<JacRxn> rxn(rxn_plain);
     rxn.insert(rxn.end(), rxn_ext.begin(), rxn_ext.end());
     uint32_t off = 0;
@@ -142,8 +142,6 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
     off = align16j(off + (uint32_t)(rxn.size() * sizeof(JacRxn)));
     lay.off_inc = off;
     off = align16j(off + (uint32_t)(inc_all.size() * sizeof(JacInc)));
-    lay.off_effinc = off;
-    off = align16j(off + (uint32_t)(effinc_all.size() * sizeof(JacEffInc)));
     lay.off_eff = off;
     off = align16j(off + (uint32_t)(effs.size() * sizeof(EffEntry)));
     lay.off_fall = off;
@@ -157,7 +155,6 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
     };
     put(lay.off_rxn, rxn.data(), rxn.size() * sizeof(JacRxn));
     put(lay.off_inc, inc_all.data(), inc_all.size() * sizeof(JacInc));
-    put(lay.off_effinc, effinc_all.data(), effinc_all.size() * sizeof(JacEffInc));
     put(lay.off_eff, effs.data(), effs.size() * sizeof(EffEntry));
     put(lay.off_fall, falls.data(), falls.size() * sizeof(RxnFall));
     put(lay.off_col, cols.data(), cols.size() * sizeof(JacCol));

@@ -55,26 +55,20 @@ struct alignas(16) JacInc {
     uint16_t pad;
 };
 
-// Species k is listed in the efficiency list of [M]-reaction x:  d = delta * scratch[g].  80 bytes.
-struct alignas(16) JacEffInc {
-    double delta;
-    double sc_w[6];
-    uint16_t sc_species[6];
-    uint16_t g;
-    uint16_t pad;
-};
-
-// Ranges of the two incidence lists of one species.  16 bytes.
+// The incidence list of one species: records [inc_begin, inc_end) of the JacInc table, in the order the kernel walks
+// them (the whole table is read front to back once per point).  A species that is listed in the efficiency list of
+// an [M]-reaction x has one more incidence for it: d = delta * scratch[g_x], stored as a JacInc whose exponent is 0
+// (2^0 = 1 exactly), whose other molecules are the dummy species and whose multiplier slot is g_x.  16 bytes.
 struct alignas(16) JacCol {
-    uint32_t inc_begin, inc_end, eff_begin, eff_end;
+    uint32_t inc_begin, inc_end, pad0, pad1;
 };
 
 struct JacLayout {
-    uint32_t off_rxn, off_inc, off_effinc, off_eff, off_fall, off_col, bytes;
-    int32_t n_species, n_plain, n_ext, n_inc, n_effinc, n_eff, n_fall;
+    uint32_t off_rxn, off_inc, off_eff, off_fall, off_col, bytes;
+    int32_t n_species, n_plain, n_ext, n_inc, n_eff, n_fall;
 };
 
-static_assert(sizeof(JacRxn) == 128 && sizeof(JacInc) == 112 && sizeof(JacEffInc) == 80 && sizeof(JacCol) == 16,
+static_assert(sizeof(JacRxn) == 128 && sizeof(JacInc) == 112 && sizeof(JacCol) == 16,
               "Jacobian table records are multiples of 16 bytes");
 
 }   // namespace pyro

@@ -67,7 +67,8 @@ const void *reactor_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool singl
 cudaError_t launch_reactor(const ReactorArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem, bool singles,
                            size_t smem_bytes, cudaStream_t stream);
 
-constexpr int kJacMaxThreads = 128;     // threads (= points) per block of the Jacobian kernel: one warp per tensor-memory lane quarter
+constexpr int kJacMaxThreads = 128;
+constexpr size_t kJacRingBytes = 8192;  // per warp: two segments of 32 records of up to 128 bytes (RecordRing)     // threads (= points) per block of the Jacobian kernel: one warp per tensor-memory lane quarter
 
 struct JacArgs {                 // chemical Jacobian (pyro_jac_tables.h)
     int64_t n, ld, n_chunks;
@@ -79,6 +80,7 @@ struct JacArgs {                 // chemical Jacobian (pyro_jac_tables.h)
     const unsigned char *jtab;   // Jacobian blob
     double *ext;                 // scratch of the [M] reactions: [1 + 2 n_ext][threads of the grid]
     uint32_t off_spec, tmem_cols;
+    uint32_t planes_bytes;       // dynamic shared memory taken by the planes; the per-warp record rings (8 KB each) follow
     int32_t mode;                // 0: fixed (rho, T); 1: fixed (rho, e)
     JacLayout lay;
 };
