@@ -132,47 +132,60 @@ __global__ void __launch_bounds__(BD) temperature_general_kernel(const TempArgs 
 
 // ---------------------------------------------------------------------------------------
 // The same solve as a software-pipelined stream (used when the Y planes are 16-byte aligned):
-// thread t owns points 2t, 2t+1 of its block's 2 BD points and copies their 16 bytes of every
-// species plane into its own slot of a D-deep shared-memory ring with cp.async, D species ahead
-// of the arithmetic, so that the HBM latency is covered by D x 16 bytes in flight per thread
-// instead of by resident warps.  A thread only ever reads what it copied itself: no barrier
+// thread t owns NV pairs of points (2t, 2t+1, then 2 BD further on, ...) of its block's 2 NV BD points and copies
+// their 16 bytes of every species plane into its own slots of a D-deep shared-memory ring with cp.async, D
+// species ahead of the arithmetic, so that the HBM latency is covered by D x NV x 16 bytes in flight per thread
+// instead of by resident warps.  NV = 2: the twelve coefficients of a species serve four points per thread, which
+// halves the warp-uniform table reads that bound the NV = 1 version (ncu: 14 of 18 shared-memory wavefronts per
+// species and warp).  A thread only ever reads what it copied itself: no barrier
 // in the loop.  The energy table is staged in shared memory once per block.
 // ---------------------------------------------------------------------------------------
-template <int BD, int D>
+template <int BD, int D, int NV>
 __global__ void __launch_bounds__(BD) temperature_stream_kernel(const TempArgs a) {
     static_assert((D & (D - 1)) == 0, "ring depth must be a power of two");
+    constexpr int NP = 2 * NV;   // points per thread: NV 16-byte vectors, 2 BD points apart (every copy of a warp is 512 contiguous bytes)
     extern __shared__ __align__(16) unsigned char tsm[];
-    EnergyRow *tab = reinterpret_cast<EnergyRow *>(tsm + (size_t)D * BD * 16);
+    EnergyRow *tab = reinterpret_cast<EnergyRow *>(tsm + (size_t)D * NV * BD * 16);
     const int tid = threadIdx.x, ns = a.n_species;
     {
         const double2 *src = reinterpret_cast<const double2 *>(a.energy);
         double2 *dst = reinterpret_cast<double2 *>(tab);
         for (int i = tid; i < ns * (int)(sizeof(EnergyRow) / 16); i += BD) dst[i] = __ldg(src + i);
     }
-    const int64_t p0 = ((int64_t)blockIdx.x * BD + tid) * 2;   // the launcher passes whole blocks only
+    const int64_t p0 = (int64_t)blockIdx.x * (BD * NP) + tid * 2;   // the launcher passes whole blocks only
     const double *Yp = a.Y + p0;
     const uint32_t slot0 = (uint32_t)__cvta_generic_to_shared(tsm) + (uint32_t)tid * 16u;
     auto issue = [&](int k) {
-        if (k < ns)
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + (uint32_t)(k & (D - 1)) * (BD * 16u)),
-                         "l"(Yp + (int64_t)k * a.ld)
-                         : "memory");
+        if (k < ns) {
+#pragma unroll
+            for (int v = 0; v < NV; ++v)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(slot0 + (uint32_t)((k & (D - 1)) * NV + v) * (BD * 16u)),
+                             "l"(Yp + (int64_t)k * a.ld + v * (2 * BD))
+                             : "memory");
+        }
         asm volatile("cp.async.commit_group;" ::: "memory");   // one group per species, empty past the end
     };
 #pragma unroll
     for (int s = 0; s < D; ++s) issue(s);
     __syncthreads();   // the energy table is in place
-    double Slo[2][6], Shi[2][6], Rm[2] = {0.0, 0.0};
+    double Slo[NP][6], Shi[NP][6], Rm[NP];
 #pragma unroll
-    for (int i = 0; i < 2; ++i)
+    for (int i = 0; i < NP; ++i) {
+        Rm[i] = 0.0;
 #pragma unroll
         for (int m = 0; m < 6; ++m) Slo[i][m] = Shi[i][m] = 0.0;
+    }
 #pragma unroll 1
     for (int k = 0; k < ns; ++k) {
         asm volatile("cp.async.wait_group %0;" ::"n"(D - 1) : "memory");
-        double y[2];
-        asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(y[0]), "=d"(y[1]) : "r"(slot0 + (uint32_t)(k & (D - 1)) * (BD * 16u)));
+        double y[NP];
+#pragma unroll
+        for (int v = 0; v < NV; ++v)
+            asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];"
+                         : "=d"(y[2 * v]), "=d"(y[2 * v + 1])
+                         : "r"(slot0 + (uint32_t)((k & (D - 1)) * NV + v) * (BD * 16u)));
         issue(k + D);
+        // the twelve coefficients of the species are read once (six warp-uniform 128-bit loads) for the thread's NP points
         const double2 *row = reinterpret_cast<const double2 *>(tab + k);
         double c[12];
 #pragma unroll
@@ -182,7 +195,7 @@ __global__ void __launch_bounds__(BD) temperature_stream_kernel(const TempArgs a
             c[2 * m + 1] = v.y;
         }
 #pragma unroll
-        for (int i = 0; i < 2; ++i)
+        for (int i = 0; i < NP; ++i)
 #pragma unroll
             for (int m = 0; m < 6; ++m) {
                 Slo[i][m] = fma(y[i], c[m], Slo[i][m]);
@@ -191,20 +204,21 @@ __global__ void __launch_bounds__(BD) temperature_stream_kernel(const TempArgs a
         if (a.enthalpy) {   // h(T) = e(T) + T sum_k Y_k R/W_k
             const double rw = tab[k].rw;
 #pragma unroll
-            for (int i = 0; i < 2; ++i) Rm[i] = fma(y[i], rw, Rm[i]);
+            for (int i = 0; i < NP; ++i) Rm[i] = fma(y[i], rw, Rm[i]);
         }
     }
     int bad = 0;
 #pragma unroll
-    for (int i = 0; i < 2; ++i) {
+    for (int i = 0; i < NP; ++i) {
         if (a.enthalpy) {
             Slo[i][1] += Rm[i];
             Shi[i][1] += Rm[i];
         }
+        const int64_t p = p0 + (i >> 1) * (2 * BD) + (i & 1);
         double T;
         bool conv;
-        newton_temperature(Slo[i], Shi[i], a.t_mid, a.e[p0 + i], a.T_guess[p0 + i], a.tol, a.max_iter, &T, &conv);
-        a.T[p0 + i] = T;
+        newton_temperature(Slo[i], Shi[i], a.t_mid, a.e[p], a.T_guess[p], a.tol, a.max_iter, &T, &conv);
+        a.T[p] = T;
         bad += conv ? 0 : 1;
     }
     if (a.n_not_converged != nullptr && bad) atomicAdd(a.n_not_converged, bad);
@@ -332,6 +346,7 @@ cudaError_t launch_rates(const RatesArgs &a, int threads, int blocks, bool table
 constexpr int kTempBD = 128, kTempPPT = 4;
 
 constexpr int kStreamBD = 128, kStreamDepth = 8;
+constexpr int kStreamNV = 2;   // 16-byte vectors (pairs of points) per thread of the temperature stream
 
 cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream) {
     if (!a.single_t_mid) {   // species with different break temperatures: the interval-wise solve
@@ -343,11 +358,17 @@ cudaError_t launch_temperature(const TempArgs &a, cudaStream_t stream) {
     // is 16-byte aligned; the rest (ragged tail, odd ld, unaligned Y) through the plain kernel
     TempArgs rest = a;
     const bool aligned = (a.ld % 2 == 0) && (reinterpret_cast<uintptr_t>(a.Y) % 16 == 0);
-    const size_t smem = (size_t)kStreamDepth * kStreamBD * 16 + (size_t)a.n_species * sizeof(EnergyRow);
-    const int64_t main_blocks = aligned && smem <= 48 * 1024 ? a.n / (2 * kStreamBD) : 0;
+    // four points per thread pay off when the pass over the species dominates (measured: configs[2] 0.364 -> 0.349 ms);
+    // for a handful of species the four Newton solves per thread do (configs[1] 0.53 -> 0.62 ms): two points there
+    const int nv = a.n_species >= 24 ? kStreamNV : 1;
+    const size_t smem = (size_t)kStreamDepth * nv * kStreamBD * 16 + (size_t)a.n_species * sizeof(EnergyRow);
+    const int64_t main_blocks = aligned && smem <= 48 * 1024 ? a.n / (2 * nv * kStreamBD) : 0;
     if (main_blocks > 0) {
-        temperature_stream_kernel<kStreamBD, kStreamDepth><<<dim3((unsigned)main_blocks), dim3(kStreamBD), smem, stream>>>(a);
-        const int64_t done = main_blocks * 2 * kStreamBD;
+        if (nv == kStreamNV)
+            temperature_stream_kernel<kStreamBD, kStreamDepth, kStreamNV><<<dim3((unsigned)main_blocks), dim3(kStreamBD), smem, stream>>>(a);
+        else
+            temperature_stream_kernel<kStreamBD, kStreamDepth, 1><<<dim3((unsigned)main_blocks), dim3(kStreamBD), smem, stream>>>(a);
+        const int64_t done = main_blocks * 2 * nv * kStreamBD;
         rest.n = a.n - done;
         rest.e += done; rest.Y += done; rest.T_guess += done; rest.T += done;
     }
