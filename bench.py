@@ -38,7 +38,11 @@ FLOPS_EXP, FLOPS_LOG, FLOPS_DIV = 30, 46, 15
 # DRAM traffic of the rates kernel measured once with `ncu --set full` (dram__bytes_read.sum +
 # dram__bytes_write.sum = 866.3 MB for 2^20 points of configs[2]; profiles/r01_v8_kernels.md).
 # Reported as `traffic` for the configs[2]/[4] mechanism only, scaled to the points of one launch.
-NCU_RATES_DRAM_BYTES_PER_POINT_53SP = 866.3e6 / 1048576
+NCU_RATES_DRAM_BYTES_PER_POINT_53SP = 864.1e6 / 1048576
+# Executed FP64 work of the rates kernel from the same ncu capture (profiles/r02_kernels.md): DADD + DMUL + 2 DFMA
+# thread instructions per point, and the busy share of the FP64 pipe.  configs[2]/[4] mechanism only.
+NCU_RATES_EXECUTED_FLOPS_PER_POINT_53SP = 24.2e3
+NCU_RATES_FP64_PIPE_PCT_53SP = 45.0
 
 # FP64 roof of one B200: 148 SMs x 64 FP64 FMA lanes x 2 flop x 1.965 GHz.
 FP64_PEAK_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
@@ -278,6 +282,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-widened", action="store_true", help="skip the SURVEY 8(f) rows (Jacobian, transport, reactors)")
+    ap.add_argument("--probes", action="store_true", help="print the design probes (DMMA peak, indexed RMW) and exit")
     ap.add_argument("--points", type=int, default=0, help="override the number of points (profiling runs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -300,6 +305,17 @@ def main():
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    if args.probes:
+        if rank == 0:
+            out = {"fp64_dfma_tflops": binding.probe_fp64_peak(local_rank, 200.0),
+                   "fp64_dmma_m8n8k4_tflops": binding.probe_dmma_peak(local_rank, 200.0),
+                   "indexed_rmw_cycles_per_iteration": {
+                       f"{w}_warps": {name: binding.probe_indexed_rmw(local_rank, w, mode)
+                                      for mode, name in ((0, "shared_rmw"), (1, "tensor_rmw"), (2, "tensor_loads"))}
+                       for w in (1, 4, 8)}}
+            print(json.dumps(out), flush=True)
+        return
 
     cfg = args.config
     mech = inputs.config_mechanism(cfg)
@@ -441,6 +457,12 @@ def main():
                 "traffic_note": "bytes per launch, ncu dram read + write of one profiled launch scaled by points; "
                                 "algorithmic bytes per launch = %.4g" % (bytes_pt["rates"] * n),
                 "flops_per_point": flops_pt,
+                "frac_is": "algorithmic flops (SURVEY 8(d): two libm exponentials per reversible reaction) / time / peak",
+                "executed_frac": (NCU_RATES_EXECUTED_FLOPS_PER_POINT_53SP * n / (rates_ms * 1e-3) / 1e12 / FP64_PEAK_TFLOPS
+                                  if ns == 53 else None),
+                "fp64_pipe_pct": NCU_RATES_FP64_PIPE_PCT_53SP if ns == 53 else None,
+                "executed_note": "executed flops per point and FP64-pipe busy share from the committed ncu capture "
+                                 "(profiles/r02_kernels.md), scaled by this run's time",
                 "peak_source": "148 SMs x 64 FP64 FMA lanes x 2 x 1.965 GHz (DESIGN.md); measured DFMA probe alongside",
                 "measured_dfma_tflops": measured_peak,
                 "hbm": {"achieved_gbs": bytes_pt["rates"] * n / (rates_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
@@ -449,7 +471,9 @@ def main():
                 "temperature_kernel_hbm": {"achieved_gbs": bytes_pt["temperature"] * n / (temp_ms * 1e-3) / 1e9,
                                            "frac": bytes_pt["temperature"] * n / (temp_ms * 1e-3) / 1e9 / hbm_peak},
             },
-            "next1_helpers_ms": {k: {"ms": v, "hbm_frac": 8.0 * (ns + 3) * n / (v * 1e-3) / 1e9 / hbm_peak}
+            "next1_helpers_ms": {k: {"ms": v, "hbm_frac": min(1.0, 8.0 * (ns + 3) * n / (v * 1e-3) / 1e9 / hbm_peak),
+                                     "gbs": 8.0 * (ns + 3) * n / (v * 1e-3) / 1e9,
+                                     "note": "peak = measured COPY bandwidth; a read-only stream can exceed it: fraction capped at 1"}
                                  for k, v in helpers.items()},
             "clocks": clocks.summary(),
             "gpu_launches": 2 * args.steps,

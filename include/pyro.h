@@ -237,6 +237,16 @@ int pyro_mech_info(const pyro_mech *mech, int64_t *out, int cap);
  * `millis` ms; *tflops = 2 * FMAs / time.  Used as the roofline denominator cross-check. */
 int pyro_probe_fp64_peak(int device, double millis, double *tflops);
 
+/* Probes behind two design decisions (`python bench.py --probes` prints them):
+ * pyro_probe_dmma_peak: sustained rate of the FP64 tensor-core instruction mma.sync.m8n8k4.f64 (8 independent
+ *   accumulators per warp, every SM) for about `millis` ms; *tflops = 2 flops per multiply-add.
+ * pyro_probe_indexed_rmw: one block of `warps_per_sm` warps (1..8) per SM; every thread performs, per iteration, sixteen
+ *   independent read-modify-writes of a double at pseudo-random warp-uniform slots out of 64, in shared memory
+ *   (mode 0), in tensor memory with tcgen05.ld / wait / add / tcgen05.st / wait (mode 1), or only the tensor-memory
+ *   loads (mode 2); *cycles_per_iteration = SM clock cycles per iteration of block 0. */
+int pyro_probe_dmma_peak(int device, double millis, double *tflops);
+int pyro_probe_indexed_rmw(int device, int warps_per_sm, int mode, double *cycles_per_iteration);
+
 const char *pyro_status_string(int status); /* static text for a pyro_status                       */
 const char *pyro_last_error_string(void);   /* detail of the last error on this thread (may be "") */
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libpyro.so")
 EXPORTS = (
     "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
     "pyro_get_temperature_from_enthalpy", "pyro_get_density", "pyro_get_pressure",
-    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak",
+    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak", "pyro_probe_dmma_peak", "pyro_probe_indexed_rmw",
     "pyro_status_string", "pyro_last_error_string", "pyro_transport_create", "pyro_transport_destroy",
     "pyro_get_transport",
 )
@@ -52,6 +52,21 @@ class MechDesc(C.Structure):
 _lib = None
 
 
+def probe_dmma_peak(device=0, millis=200.0):
+    """Measured mma.sync.m8n8k4.f64 peak of the device in TFLOP/s."""
+    out = C.c_double(0.0)
+    _check(load_library().pyro_probe_dmma_peak(int(device), float(millis), C.byref(out)))
+    return float(out.value)
+
+
+def probe_indexed_rmw(device=0, warps_per_sm=8, mode=1):
+    """SM cycles per iteration of sixteen indexed read-modify-writes per thread (mode 0 shared memory, 1 tensor memory,
+    2 tensor-memory loads only)."""
+    out = C.c_double(0.0)
+    _check(load_library().pyro_probe_indexed_rmw(int(device), int(warps_per_sm), int(mode), C.byref(out)))
+    return float(out.value)
+
+
 class TransportDesc(C.Structure):
     _fields_ = [("n_species", C.c_int32), ("mol_weight", C.c_void_p), ("visc", C.c_void_p), ("cond", C.c_void_p),
                 ("diff", C.c_void_p)]
@@ -84,6 +99,8 @@ def load_library():
     lib.pyro_get_transport.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp]
     lib.pyro_mech_info.argtypes = [vp, C.POINTER(i64), C.c_int]
     lib.pyro_probe_fp64_peak.argtypes = [C.c_int, dbl, C.POINTER(dbl)]
+    lib.pyro_probe_dmma_peak.argtypes = [C.c_int, dbl, C.POINTER(dbl)]
+    lib.pyro_probe_indexed_rmw.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(dbl)]
     lib.pyro_status_string.argtypes = [C.c_int]
     lib.pyro_status_string.restype = C.c_char_p
     lib.pyro_last_error_string.restype = C.c_char_p
