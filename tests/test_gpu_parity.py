@@ -743,3 +743,38 @@ def test_transport_w7_padded_ld_and_error_codes(golden_dir):
     h = C.c_void_p()
     assert gt._lib.pyro_transport_create(C.byref(bad), 0, C.byref(h)) == 2 and not h.value
     assert gt._lib.pyro_transport_destroy(None) == 0
+
+
+# ------------------------------------------------------------------ ABI: size and alignment checks of every field entry point
+def test_abi_ld_and_alignment_on_every_entry_point(mechs):
+    """ld < n is PYRO_ERR_BAD_SIZE and a misaligned pointer PYRO_ERR_ALIGN on every device entry point, including the
+    widened ones; n_not_converged must be 4-byte aligned."""
+    mech, gm, _ = mechs(0)
+    ns, n = mech.n_species, 64
+    st = inputs.config_states(0, n=n)
+    rho, e, Y, Tg, T = (dev(st[k]) for k in ("rho", "e", "Y", "T_guess", "T"))
+    out1 = torch.empty(n, dtype=torch.float64, device="cuda")
+    outY = torch.empty((ns, n), dtype=torch.float64, device="cuda")
+    J = torch.empty((ns, ns, n), dtype=torch.float64, device="cuda")
+    bad = torch.zeros(2, dtype=torch.int32, device="cuda")
+    L, h = gm._lib, gm._h
+    p = lambda t: t.data_ptr()
+    calls = {
+        "temperature": lambda ld, o=0: L.pyro_get_temperature(h, n, ld, p(rho), p(e), p(Y), p(Tg), p(out1) + o, None, None),
+        "temperature_h": lambda ld, o=0: L.pyro_get_temperature_from_enthalpy(h, n, ld, p(e), p(Y), p(Tg), p(out1) + o, None, None),
+        "density": lambda ld, o=0: L.pyro_get_density(h, n, ld, p(rho), p(T), p(Y), p(out1) + o, None),
+        "pressure": lambda ld, o=0: L.pyro_get_pressure(h, n, ld, p(rho), p(T), p(Y), p(out1) + o, None),
+        "rates": lambda ld, o=0: L.pyro_get_net_production_rates(h, n, ld, p(rho), p(T), p(Y), p(outY) + o, None),
+        "source_terms": lambda ld, o=0: L.pyro_source_terms(h, n, ld, p(rho), p(e), p(Y), p(Tg), p(out1) + o, p(outY), None, None),
+        "jacobian": lambda ld, o=0: L.pyro_get_jacobian(h, n, ld, p(rho), p(T), p(Y), 0, p(J) + o, None, None),
+        "reactor": lambda ld, o=0: L.pyro_reactor_rk4(h, n, ld, p(rho), p(e), p(Y), p(out1) + o, 1e-300, 0, p(outY), None, None),
+    }
+    for name, f in calls.items():
+        assert f(n - 1) == 2, name          # ld < n
+        assert f(n, 4) == 5, name           # 4-byte offset: not 8-byte aligned
+    # n_not_converged: device int32, 4-byte aligned
+    assert L.pyro_get_temperature(h, n, n, p(rho), p(e), p(Y), p(Tg), p(out1), p(bad) + 2, None) == 5
+    assert L.pyro_get_temperature(h, n, n, p(rho), p(e), p(Y), p(Tg), p(out1), p(bad) + 4, None) == 0
+    assert L.pyro_source_terms(h, n, n, p(rho), p(e), p(Y), p(Tg), p(out1), p(outY), p(bad) + 1, None) == 5
+    assert L.pyro_reactor_rk4(h, n, n, p(rho), p(e), p(Y), p(out1), 1e-300, 0, p(outY), p(bad) + 2, None) == 5
+    torch.cuda.synchronize()
