@@ -83,6 +83,11 @@ struct pyro_mech {
     uint32_t planes_off = 0;
     uint32_t tmem_cols = 32;
     int blocks_per_sm = 0;
+    // two-points-per-thread rates kernel (pyro_rates2_kernels.cu), used by pyro_get_net_production_rates when it fits
+    bool two_points = false;
+    bool tab_smem2 = false;
+    size_t smem2 = 0;
+    uint32_t planes_off2 = 0, tmem_cols2 = 32;
     size_t reactor_smem = 0;         // its dynamic shared memory: that of the rates kernel + the staged energy table
     uint32_t reactor_energy_off = 0;
     int reactor_blocks_per_sm = 1;   // resident blocks of the reactor kernel (same block shape as the rates kernel)
@@ -136,6 +141,15 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     int64_t blocks = (int64_t)m->sm_count * m->blocks_per_sm;
     if (blocks > (a.n_chunks + warps - 1) / warps) blocks = (a.n_chunks + warps - 1) / warps;
     pyro::RatesArgs args = a;
+    const bool two = m->two_points && !fused;
+    if (two) {   // 64-point chunks, one warp per lane quarter
+        args.n_chunks = (a.n + 63) / 64;
+        args.planes_off = m->planes_off2;
+        args.tmem_cols = m->tmem_cols2;
+        blocks = (int64_t)m->sm_count;
+        const int64_t need = (args.n_chunks + pyro::kRates2Threads / 32 - 1) / (pyro::kRates2Threads / 32);
+        if (blocks > need) blocks = need;
+    }
     // every launch in flight needs its own chunk counter: take the next slot of the ring and, before
     // resetting it, make this stream wait for the launch that used the slot kWorkSlots launches ago
     const uint32_t slot = m->next_work.fetch_add(1) % kWorkSlots;
@@ -143,8 +157,11 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     std::lock_guard<std::mutex> lock(m->work_mu);
     PYRO_CUDA(cudaStreamWaitEvent(stream, m->work_done[slot], 0));
     PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
-    PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->smem_bytes, stream,
-                                 fused));
+    if (two)
+        PYRO_CUDA(pyro::launch_rates2(args, pyro::kRates2Threads, (int)blocks, m->tab_smem2, m->smem2, stream));
+    else
+        PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->smem_bytes, stream,
+                                     fused));
     PYRO_CUDA(cudaEventRecord(m->work_done[slot], stream));
     return PYRO_OK;
 }
@@ -341,6 +358,42 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     if (const char *env = std::getenv("PYRO_CARVEOUT")) carveout = std::atoi(env);
     if ((ce = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, carveout)) != cudaSuccess)
         return bail(ce, "cudaFuncSetAttribute(PreferredSharedMemoryCarveout)");
+    // Two points per thread (pyro_rates2_kernels.cu): 128 threads hold the same 256 points; needs eight tensor-memory
+    // columns per species row and the A plane of both points (16 bytes per row and thread) in shared memory.  Used for
+    // mechanisms that run the one-block shape (not the two-block shape of small mechanisms).
+    if (!m->two_blocks && 8 * rows <= 512) {
+        const size_t planes2 = 16 * rows * (size_t)pyro::kRates2Threads;
+        const void *fn2s = pyro::rates2_kernel_ptr(true), *fn2g = pyro::rates2_kernel_ptr(false);
+        cudaFuncAttributes fa2{};
+        if ((ce = cudaFuncGetAttributes(&fa2, fn2s)) != cudaSuccess) return bail(ce, "cudaFuncGetAttributes(rates2)");
+        const size_t smem_max2 = (size_t)prop.sharedMemPerBlockOptin - fa2.sharedSizeBytes;
+        bool ok = false;
+        if (tab_room + planes2 <= smem_max2 && m->tab_smem) {
+            m->tab_smem2 = true;
+            m->planes_off2 = (uint32_t)tab_room;
+            m->smem2 = tab_room + planes2;
+            ok = true;
+        } else if (planes2 <= smem_max2) {
+            m->tab_smem2 = false;
+            m->planes_off2 = 0;
+            m->smem2 = planes2;
+            ok = true;
+        }
+        if (ok) {
+            m->tmem_cols2 = 32;
+            while (m->tmem_cols2 < 8 * rows) m->tmem_cols2 *= 2;
+            for (const void *f2 : {fn2s, fn2g}) {
+                if ((ce = cudaFuncSetAttribute(f2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max2)) != cudaSuccess)
+                    return bail(ce, "cudaFuncSetAttribute(rates2, MaxDynamicSharedMemorySize)");
+                if ((ce = cudaFuncSetAttribute(f2, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
+                    return bail(ce, "cudaFuncSetAttribute(rates2, carveout)");
+            }
+            // Measured slower than the one-point kernel (configs[2]: 7.58 against 7.09 ms -- 27 % fewer instructions, but
+            // one warp per scheduler issues on 45 % of the cycles against 66 % for two; profiles/r02_dead_ends.md):
+            // available to tests and measurements through PYRO_RATES_POINTS=2, not chosen by the library.
+            if (const char *env = std::getenv("PYRO_RATES_POINTS")) m->two_points = std::atoi(env) == 2;
+        }
+    }
     {   // the reactor kernel of the same shape (pyro_reactor_rk4)
         const void *rfn = pyro::reactor_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks);
         if ((ce = cudaFuncSetAttribute(rfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max)) != cudaSuccess)

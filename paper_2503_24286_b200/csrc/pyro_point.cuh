@@ -21,10 +21,11 @@ namespace pyro {
 
 constexpr double kLog10of2 = 0.30102999566398119521;   // log10(2)
 
-// Per-thread temperature features of its point.
-struct PointT {
-    double T, invT, L2T;
+// Per-thread temperature features of its point (V = double) or of its two points (V = D2, pyro_math.cuh).
+template <class V> struct PointTV {
+    V T, invT, L2T;
 };
+typedef PointTV<double> PointT;
 
 PYRO_HD PointT make_point(double T) {
     PointT pt;
@@ -33,9 +34,16 @@ PYRO_HD PointT make_point(double T) {
     pt.L2T = log2(T);
     return pt;
 }
+PYRO_HD PointTV<D2> make_point(D2 T) {
+    PointTV<D2> pt;
+    pt.T = T;
+    pt.invT = D2{1.0 / T.x, 1.0 / T.y};
+    pt.L2T = D2{log2(T.x), log2(T.y)};
+    return pt;
+}
 
 // log2 k = c0 + c1 log2T + c2/T                               (A.9) PAPER.md:925
-PYRO_HD double arrhenius_log2(double c0, double c1, double c2, double L2T, double invT) {
+template <class V> PYRO_HD V arrhenius_log2(double c0, double c1, double c2, V L2T, V invT) {
     return fma(c1, L2T, fma(c2, invT, c0));
 }
 
@@ -48,23 +56,28 @@ PYRO_HD double species_log2E(const double *c, double T, double L2T, double invT)
     y = fma(c[1], L2T, y);
     return fma(c[2], invT, y);
 }
+// the same with the NASA range chosen per point (T < T_mid,k: low; G10) by fetching only that coefficient set
+PYRO_HD double species_log2E_row(const SpecRow &row, const PointT &pt) {
+    return species_log2E(pt.T < row.t_mid ? row.lo : row.hi, pt.T, pt.L2T, pt.invT);
+}
+PYRO_HD D2 species_log2E_row(const SpecRow &row, const PointTV<D2> &pt) {
+    return D2{species_log2E(pt.T.x < row.t_mid ? row.lo : row.hi, pt.T.x, pt.L2T.x, pt.invT.x),
+              species_log2E(pt.T.y < row.t_mid ? row.lo : row.hi, pt.T.y, pt.L2T.y, pt.invT.y)};
+}
 
 // Rows a2, a3 of SURVEY.md 8(a) for NK species in lockstep: C_k = rho Y_k / W_k (A.8)
-// PAPER.md:921, the NASA range chosen per point (T < T_mid,k: low; G10) by fetching only that
-// coefficient set, E_k and 1/E_k by one paired exponential.  Writes A_k = C_k E_k, B_k = 1/E_k,
-// omega_k = 0 and adds C_k to ctot.
-template <int NK, class Tab, class Mem>
-PYRO_HD void species_planes(const Tab &tab, int k0, const PointT &pt, double rho, const double (&Y)[NK], double &ctot,
-                            const Mem &mem) {
-    double y[NK], e[NK], b[NK], C[NK];
+// PAPER.md:921, the NASA range chosen per point, E_k and 1/E_k by one paired exponential.  Writes A_k = C_k E_k,
+// B_k = 1/E_k, omega_k = 0 and adds C_k to ctot.
+template <int NK, class Tab, class Mem, class PT, class V>
+PYRO_HD void species_planes(const Tab &tab, int k0, const PT &pt, V rho, const V (&Y)[NK], V &ctot, const Mem &mem) {
+    V y[NK], e[NK], b[NK], C[NK];
 #pragma unroll
     for (int i = 0; i < NK; ++i) {
         const SpecRow &row = tab.spec(k0 + i);
-        const double *c = pt.T < row.t_mid ? row.lo : row.hi;
-        y[i] = species_log2E(c, pt.T, pt.L2T, pt.invT);
+        y[i] = species_log2E_row(row, pt);
         C[i] = rho * Y[i] * row.inv_w;
     }
-    exp2_pair_n<NK>(y, e, b);
+    exp2_pair_nv<NK>(y, e, b);
 #pragma unroll
     for (int i = 0; i < NK; ++i) {
         ctot += C[i];
@@ -88,14 +101,15 @@ template <int N> PYRO_HD void load_slots(const uint32_t (&src)[6], uint32_t (&ds
 //   omega -= R on reactants, += R on products                (A.5)
 // Branch-free.  The NB exponentials run as interleaved Horner chains; all species touched in
 // one iteration are distinct, so the omega read-modify-writes are one batch of loads, the
-// adds, one batch of stores.
-template <int NR, int NP, int NB, class Tab, class Mem>
-PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT &pt, const Mem &mem) {
+// adds, one batch of stores.  V = typename Mem::V: one point per thread or two.
+template <int NR, int NP, int NB, class Tab, class Mem, class PT>
+PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PT &pt, const Mem &mem) {
+    typedef typename Mem::V V;
     constexpr int NS = NR + NP;
 #pragma unroll 1
     for (int j = j0; j < j0 + count; j += NB) {
         uint32_t hA[NB][NS], hB[NB][NR], hW[NB][NS];
-        double y[NB];
+        V y[NB];
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
             const RxnP &r = tab.rxn_p(j + b);
@@ -119,16 +133,16 @@ PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT &pt
 #pragma unroll
             for (int m = 0; m < NP; ++m) wr[b][m] = mem.ldW(hW[b][NR + m]);
         }
-        double a[NB][NS];
+        V a[NB][NS];
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
             for (int m = 0; m < NS; ++m) a[b][m] = mem.ldA(hA[b][m]);
-        exp2_poly_n<NB>(y);
-        double pd[NB];   // k_f (prod_reac A - prod_prod A)
+        exp2_poly_nv<NB>(y);
+        V pd[NB];   // k_f (prod_reac A - prod_prod A)
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            double pf = a[b][0], pr = a[b][NR];
+            V pf = a[b][0], pr = a[b][NR];
 #pragma unroll
             for (int m = 1; m < NR; ++m) pf *= a[b][m];
 #pragma unroll
@@ -138,10 +152,10 @@ PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT &pt
         mem.fence_ld();
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
-            double pb = mem.value_b(wbr[b][0]);
+            V pb = mem.value_b(wbr[b][0]);
 #pragma unroll
             for (int m = 1; m < NR; ++m) pb *= mem.value_b(wbr[b][m]);
-            const double R = pb * pd[b];
+            const V R = pb * pd[b];
 #pragma unroll
             for (int m = 0; m < NR; ++m) mem.stW(hW[b][m], mem.value_w(wbr[b][m]) - R);
 #pragma unroll
@@ -154,8 +168,8 @@ PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PointT &pt
 // couples two in lockstep, the rest one at a time.
 // kSingles = false leaves the one-at-a-time loops out (the packer then stores no singles): for
 // large mechanisms their code alone costs 8 % (measured on configs[2]: instruction cache).
-template <int NR, int NP, bool kSingles, class Tab, class Mem>
-PYRO_HD int plain_shape(const Tab &tab, int j, int g8, int g4, int g2, int g1, const PointT &pt, const Mem &mem) {
+template <int NR, int NP, bool kSingles, class Tab, class Mem, class PT>
+PYRO_HD int plain_shape(const Tab &tab, int j, int g8, int g4, int g2, int g1, const PT &pt, const Mem &mem) {
     plain_reactions<NR, NP, 4>(tab, j, g8 + g4, pt, mem);
     plain_reactions<NR, NP, 2>(tab, j + g8 + g4, g2, pt, mem);
     if (kSingles) plain_reactions<NR, NP, 1>(tab, j + g8 + g4 + g2, g1, pt, mem);
@@ -168,14 +182,15 @@ PYRO_HD int plain_shape(const Tab &tab, int j, int g8, int g4, int g2, int g1, c
 // dummy species and the efficiency lists of a group have one length, so there are no
 // data-dependent branches; logarithms and divisions are the branch-free log2_pos and
 // rcp_newton of pyro_math.cuh.
-template <int KIND, int NB, class Tab, class Mem>
-PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT &pt, double ctot, const Mem &mem) {
+template <int KIND, int NB, class Tab, class Mem, class PT, class V>
+PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PT &pt, V ctot, const Mem &mem) {
     constexpr int NE = KIND == kExtTroe ? 5 : (KIND == kExtLindemann ? 2 : 1);   // exponentials per reaction
 #pragma unroll 1
     for (int j = j0; j < j0 + count; j += NB) {
         uint32_t hA[NB][6], hB[NB][3], hWs[NB][3], hW[NB][6];   // hWs: tensor-memory handle of a reactant slot (its B)
-        double nu[NB][6], rev[NB], M[NB], alpha[NB], has_t2[NB];
-        double y[NB * NE];
+        double nu[NB][6], rev[NB], alpha[NB], has_t2[NB];
+        V M[NB];
+        V y[NB * NE];
         uint32_t q0[NB], nq = 0;
 #pragma unroll
         for (int b = 0; b < NB; ++b) {
@@ -219,7 +234,7 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
                 wr[b][m] = mem.ldW(hW[b][m]);
                 if (m < 3) br[b][m] = mem.ldB(hWs[b][m], hB[b][m]);
             }
-        double a[NB][6];
+        V a[NB][6];
 #pragma unroll
         for (int b = 0; b < NB; ++b)
 #pragma unroll
@@ -230,7 +245,8 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
 #pragma unroll 1
             for (uint32_t q = 0; q < nq; q += 4) {
                 typename Mem::WRaw cb[NB * 4];
-                double dl[NB * 4], ca[NB * 4];
+                double dl[NB * 4];
+                V ca[NB * 4];
 #pragma unroll
                 for (int b = 0; b < NB; ++b)
 #pragma unroll
@@ -247,33 +263,33 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
                     for (int u = 0; u < 4; ++u) M[b] = fma(dl[b * 4 + u], ca[b * 4 + u] * mem.value(cb[b * 4 + u]), M[b]);
             }
         }
-        exp2_poly_n<NB * NE>(y);
-        double fall[NB];
+        exp2_poly_nv<NB * NE>(y);
+        V fall[NB];
 #pragma unroll
-        for (int b = 0; b < NB; ++b) fall[b] = 1.0;
+        for (int b = 0; b < NB; ++b) fall[b] = splat<V>(1.0);
         if (KIND >= kExtLindemann) {
-            double Pr[NB];
+            V Pr[NB];
 #pragma unroll
             for (int b = 0; b < NB; ++b) {
                 Pr[b] = y[b * NE + 1] * M[b];                    // Pr = k0 [M] / k_inf
                 fall[b] = Pr[b] * rcp_newton(1.0 + Pr[b]);       // k = k_inf Pr/(1+Pr) F
             }
             if (KIND == kExtTroe) {
-                double z[NB];
+                V z[NB];
 #pragma unroll
                 for (int b = 0; b < NB; ++b) {
-                    const double Fc = fma(1.0 - alpha[b], y[b * NE + 2], fma(alpha[b], y[b * NE + 3], has_t2[b] * y[b * NE + 4]));
-                    const double l2Fc = log2_pos(Fc);
-                    const double lFc = l2Fc * kLog10of2;
-                    const double cc = -0.4 - 0.67 * lFc;
-                    const double n = 0.75 - 1.27 * lFc;
-                    const double lPr = log2_pos(Pr[b]) * kLog10of2 + cc;
+                    const V Fc = fma(1.0 - alpha[b], y[b * NE + 2], fma(alpha[b], y[b * NE + 3], has_t2[b] * y[b * NE + 4]));
+                    const V l2Fc = log2_pos(Fc);
+                    const V lFc = l2Fc * kLog10of2;
+                    const V cc = -0.4 - 0.67 * lFc;
+                    const V n = 0.75 - 1.27 * lFc;
+                    const V lPr = log2_pos(Pr[b]) * kLog10of2 + cc;
                     // F = Fcent^(1/(1+f1^2)), f1 = lPr/d, d = n - 0.14 lPr:  1/(1+f1^2) = d^2/(d^2 + lPr^2)
-                    const double d = n - 0.14 * lPr;
-                    const double d2 = d * d;
+                    const V d = n - 0.14 * lPr;
+                    const V d2 = d * d;
                     z[b] = l2Fc * (d2 * rcp_newton(fma(lPr, lPr, d2)));
                 }
-                exp2_poly_n<NB>(z);
+                exp2_poly_nv<NB>(z);
 #pragma unroll
                 for (int b = 0; b < NB; ++b) fall[b] *= z[b];
             }
@@ -284,10 +300,10 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
             // Pair form (pyro_tables.h "Range"): prod_reac C_k = prod_i (A_ri B_ri) and
             // prod_prod C_k / K_c = prod_i (A_pi B_ri), multiplied left to right in the slot order the packer
             // chose, so that no partial product leaves the FP64 range while the rate itself is in it.
-            const double b0 = mem.value(br[b][0]), b1 = mem.value(br[b][1]), b2 = mem.value(br[b][2]);
-            const double pf = (a[b][0] * b0) * (a[b][1] * b1) * (a[b][2] * b2);
-            const double pr = rev[b] != 0.0 ? (a[b][3] * b0) * (a[b][4] * b1) * (a[b][5] * b2) : 0.0;   // irreversible: r_r = 0 (G19)
-            double R = y[b * NE] * (pf - pr) * fall[b];
+            const V b0 = mem.value(br[b][0]), b1 = mem.value(br[b][1]), b2 = mem.value(br[b][2]);
+            const V pf = (a[b][0] * b0) * (a[b][1] * b1) * (a[b][2] * b2);
+            const V pr = rev[b] != 0.0 ? (a[b][3] * b0) * (a[b][4] * b1) * (a[b][5] * b2) : splat<V>(0.0);   // irreversible: r_r = 0 (G19)
+            V R = y[b * NE] * (pf - pr) * fall[b];
             if (KIND == kExtThreeBody) R *= M[b];   // R = [M](q_f - q_r), reading G8
 #pragma unroll
             for (int m = 0; m < 6; ++m) mem.stW(hW[b][m], fma(nu[b][m], R, mem.value(wr[b][m])));
@@ -295,8 +311,8 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PointT 
     }
 }
 
-template <int KIND, bool kSingles, class Tab, class Mem>
-PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, int g1, const PointT &pt, double ctot, const Mem &mem) {
+template <int KIND, bool kSingles, class Tab, class Mem, class PT, class V>
+PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, int g1, const PT &pt, V ctot, const Mem &mem) {
     // groups of four and couples alike run two in lockstep, in ONE loop per kind: four in lockstep
     // gains less than the second copy of the loop costs (instruction cache; measured on configs[2])
     extended_reactions<KIND, 2>(tab, j, g4 + g2, pt, ctot, mem);
@@ -308,8 +324,8 @@ PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, int g1, const P
 // accumulation into plane W, (A.5)-(A.10) PAPER.md:908-934.  The planes hold n_species + 1
 // entries: the last one is the dummy species (A = B = 1, omega = sink) that pads the
 // extended records and the efficiency lists.
-template <bool kSingles, class Tab, class Mem>
-PYRO_HD void accumulate_reactions(const Tab &tab, const GroupCounts &g, const PointT &pt, double ctot, const Mem &mem) {
+template <bool kSingles, class Tab, class Mem, class PT, class V>
+PYRO_HD void accumulate_reactions(const Tab &tab, const GroupCounts &g, const PT &pt, V ctot, const Mem &mem) {
     int j = 0;
     j = plain_shape<1, 1, kSingles>(tab, j, g.shape_g8[0], g.shape_g4[0], g.shape_g2[0], g.shape_g1[0], pt, mem);
     j = plain_shape<1, 2, kSingles>(tab, j, g.shape_g8[1], g.shape_g4[1], g.shape_g2[1], g.shape_g1[1], pt, mem);
@@ -329,27 +345,28 @@ PYRO_HD void accumulate_reactions(const Tab &tab, const GroupCounts &g, const Po
 }
 
 // Rows a2, a3 for every species, then the dummy species (A = B = 1, omega = sink): fills the
-// three planes.  `load_y(k)` fetches the thread's mass fraction of species k.  Returns C_tot.
-template <class Tab, class Mem, class LoadY>
-PYRO_HD double fill_planes(const Tab &tab, int ns, const PointT &pt, double rho, const Mem &mem, const LoadY &load_y) {
-    double ctot = 0.0;
+// three planes.  `load_y(k)` fetches the thread's mass fraction(s) of species k.  Returns C_tot.
+template <class Tab, class Mem, class PT, class V, class LoadY>
+PYRO_HD V fill_planes(const Tab &tab, int ns, const PT &pt, V rho, const Mem &mem, const LoadY &load_y) {
+    V ctot = splat<V>(0.0);
     int k = 0;
 #pragma unroll 1
     for (; k + 4 <= ns; k += 4) {
-        const double y[4] = {load_y(k), load_y(k + 1), load_y(k + 2), load_y(k + 3)};
+        const V y[4] = {load_y(k), load_y(k + 1), load_y(k + 2), load_y(k + 3)};
         species_planes<4>(tab, k, pt, rho, y, ctot, mem);
     }
 #pragma unroll 1
     for (; k < ns; ++k) {
-        const double y[1] = {load_y(k)};
+        const V y[1] = {load_y(k)};
         species_planes<1>(tab, k, pt, rho, y, ctot, mem);
     }
-    mem.st_species((uint32_t)ns, 1.0, 1.0);
+    mem.st_species((uint32_t)ns, splat<V>(1.0), splat<V>(1.0));
     return ctot;
 }
 
 // Plain arrays of n_species + 1 entries per plane (host build, tests).
 struct ArrayMem {
+    typedef double V;
     typedef double WRaw;
     struct WBRaw {
         double w, b;

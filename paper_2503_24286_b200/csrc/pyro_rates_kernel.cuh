@@ -28,6 +28,7 @@ struct DevTab {
 //   shared-memory plane and omega alone in tensor memory (columns tw + 2k).
 // All accesses are volatile asm, so they keep their program order.
 template <bool kBTmem> struct DevMem {
+    typedef double V;
     struct WRaw {
         uint32_t lo, hi;
     };
