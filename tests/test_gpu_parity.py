@@ -784,10 +784,10 @@ def test_two_points_per_thread_rates_kernel(mechs, monkeypatch):
     """The two-points-per-thread variant of the rates kernel (PYRO_RATES_POINTS=2; measured slower, kept as a
     variant): every entry against the oracle, ragged tail of a 64-point chunk, hand mechanism with every class."""
     monkeypatch.setenv("PYRO_RATES_POINTS", "2")
-    for mech, (rho, T, Y) in ((inputs.config_mechanism(2), None), (hand_cases.all_paths_mechanism(), hand_cases.random_states(hand_cases.all_paths_mechanism(), 333))):
-        if rho is None:
-            st = inputs.config_states(2, n=2500 + 33)
-            rho, T, Y = st["rho"], st["T"], st["Y"]
+    st = inputs.config_states(2, n=2500 + 33)
+    hand = hand_cases.all_paths_mechanism()
+    cases = [(inputs.config_mechanism(2), (st["rho"], st["T"], st["Y"])), (hand, hand_cases.random_states(hand, 333))]
+    for mech, (rho, T, Y) in cases:
         gm = binding.Mechanism(mech)
         om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
         parity.assert_omega_parity(gpu_rates(gm, rho, T, Y), om_ref, bound)
