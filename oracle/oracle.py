@@ -73,6 +73,9 @@ def _load():
             getattr(_lib, f"oracle_get_net_production_rates_{sfx}").argtypes = [
                 C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 7
             getattr(_lib, f"oracle_get_transport_{sfx}").argtypes = [C.c_void_p, C.c_int64, C.c_int64] + [C.c_void_p] * 5
+            getattr(_lib, f"oracle_reactor_cn_{sfx}").argtypes = [
+                C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, real, C.c_int, C.c_int,
+                real, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p]
             getattr(_lib, f"oracle_reactor_rk4_{sfx}").argtypes = [
                 C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, real, C.c_int, real,
                 C.c_int, C.c_void_p, C.c_void_p]
@@ -261,6 +264,23 @@ class Oracle:
                                 self._creal(dt), int(n_steps), self._creal(tol), int(max_iter), Yb.ctypes.data,
                                 C.byref(bad))
         return Y, T, Yb, int(bad.value)
+
+    def reactor_cn(self, rho, e, Y, T_guess, dt, n_steps, newton_iters=4, tol=1e-6, max_iter=10):
+        """n_steps Crank-Nicolson steps (A.32)-(A.36) PAPER.md:1043-1062 of the reactors, `newton_iters` Newton
+        iterations each.  Returns (Y, T, Ybound, last_update, n_not_converged)."""
+        rho = self._vec(rho)
+        e = self._vec(e)
+        Y = self._vec(Y).copy()
+        T = self._vec(T_guess).copy()
+        n = rho.shape[0]
+        assert Y.shape == (self.n_species, n)
+        Yb = np.empty_like(Y)
+        lu = np.empty(n, dtype=self.dtype)
+        bad = C.c_int64(0)
+        self._fn("reactor_cn")(C.byref(self._m), n, n, rho.ctypes.data, e.ctypes.data, Y.ctypes.data, T.ctypes.data,
+                               self._creal(dt), int(n_steps), int(newton_iters), self._creal(tol), int(max_iter),
+                               Yb.ctypes.data, lu.ctypes.data, C.byref(bad))
+        return Y, T, Yb, lu, int(bad.value)
 
 
 class _Transport(C.Structure):

@@ -30,6 +30,8 @@
 //                       D_1,m = W_2 D_12/W, X5 permutation of the species, X6 Wilke limits
 //   reactor_rk4         R1 a step = degree-4 Taylor polynomial for a linear decay, R2 fourth order in dt, R3 mass and
 //                       element conservation, R4 energy, R5 equilibrium is a fixed point
+//   reactor_cn          C1 a step of a linear decay = y (1 - z/2)/(1 + z/2), C2 second order in dt, C3 conservation,
+//                       C4 bounded where RK4 diverges
 //   No function is "parity unpinned".
 //
 // Readings of garbled / silent passages are
@@ -673,6 +675,103 @@ void get_transport(const oracle_transport &t, int64_t n, int64_t ld, const Real 
     for (int64_t p = 0; p < n; ++p) transport_point<Real>(t, T[p], Y + p, ld, mu[p], kappa[p], Dkm + p, ld);
 }
 
+// Implicit march of the same reactors with the Crank-Nicolson scheme of Appendix A.3.2:
+//     F_k = Y_k^{m+1} - Y_k^m - dt/2 (s_k^{m+1} + s_k^m) = 0,   s_k = W_k omega_k / rho  (the right-hand side of (A.1)),   (A.32)
+// solved per step by Newton iterations (A.33)-(A.35) started from Y^m:
+//     (delta_jk - dt/2 ds_j/dY_k) dY_k = -F_j,    Y <- Y + dY,
+// with the chemical Jacobian (A.36) at fixed (rho, e) (reading G26: ds_j/dY_k = J_jk / rho of jacobian_point, mode 1).
+// Readings (G31): a fixed number of Newton iterations per step (data-independent control flow, as the paper's
+// JAX version needs); the temperature is re-inverted from (e, Y) before every evaluation of omega
+// and J, starting from the last temperature; the linear system is solved by Gaussian elimination with partial
+// pivoting; the size of the last Newton update max_k |dY_k| is returned per point.
+// Pins (tests/test_oracle_reactor_pins.py): C1 linear decay: a step is y (1 - z/2)/(1 + z/2) exactly, after one Newton
+// iteration; C2 second-order convergence in dt; C3 mass and element conservation; C4 bounded at dt where RK4 diverges.
+template <class Real>
+void solve_dense(int n, std::vector<Real> &A, std::vector<Real> &b) {   // A x = b, partial pivoting; x returned in b
+    for (int c = 0; c < n; ++c) {
+        int piv = c;
+        for (int r = c + 1; r < n; ++r)
+            if (std::fabs(A[(size_t)r * n + c]) > std::fabs(A[(size_t)piv * n + c])) piv = r;
+        if (piv != c) {
+            for (int j = 0; j < n; ++j) std::swap(A[(size_t)c * n + j], A[(size_t)piv * n + j]);
+            std::swap(b[c], b[piv]);
+        }
+        for (int r = c + 1; r < n; ++r) {
+            const Real f = A[(size_t)r * n + c] / A[(size_t)c * n + c];
+            for (int j = c; j < n; ++j) A[(size_t)r * n + j] -= f * A[(size_t)c * n + j];
+            b[r] -= f * b[c];
+        }
+    }
+    for (int r = n - 1; r >= 0; --r) {
+        Real s = b[r];
+        for (int j = r + 1; j < n; ++j) s -= A[(size_t)r * n + j] * b[j];
+        b[r] = s / A[(size_t)r * n + r];
+    }
+}
+
+template <class Real>
+void reactor_cn_point(const oracle_mech &m, Real rho, Real e, Real *Y, int64_t ld, Real &T, Real dt, int n_steps,
+                      int newton_iters, Real tol, int max_iter, Real *Ybound, int64_t ldb, Real &last_update, int &not_converged) {
+    const int ns = m.n_species;
+    std::vector<Real> Ym(ns), Yn(ns), sm(ns), om(ns), bd(ns), bdm(ns), J((size_t)ns * ns), A((size_t)ns * ns), F(ns);
+    not_converged = 0;
+    last_update = 0;
+    auto rates = [&](const std::vector<Real> &y, std::vector<Real> &w, std::vector<Real> &b) {
+        int it, cv;
+        Real Tn;
+        get_temperature_point<Real>(m, e, y.data(), 1, T, tol, max_iter, Tn, it, cv);
+        if (!cv) ++not_converged;
+        T = Tn;
+        production_rates_point<Real>(m, rho, T, y.data(), 1, w.data(), b.data(), 1, nullptr, nullptr, 1);
+    };
+    for (int i = 0; i < ns; ++i) {
+        Yn[i] = Y[i * ld];
+        if (Ybound) Ybound[i * ldb] = 0;
+    }
+    rates(Yn, om, bd);
+    for (int step = 0; step < n_steps; ++step) {
+        for (int i = 0; i < ns; ++i) {
+            Ym[i] = Yn[i];
+            sm[i] = Real(m.mol_weight[i]) * om[i] / rho;
+            bdm[i] = bd[i];
+        }
+        for (int it = 0; it < newton_iters; ++it) {
+            jacobian_point<Real>(m, rho, T, Yn.data(), 1, 1, J.data(), nullptr, nullptr, nullptr, 1);
+            for (int i = 0; i < ns; ++i) {
+                F[i] = -(Yn[i] - Ym[i] - dt / Real(2) * (Real(m.mol_weight[i]) * om[i] / rho + sm[i]));      // (A.32)
+                for (int k = 0; k < ns; ++k)
+                    A[(size_t)i * ns + k] = (i == k ? Real(1) : Real(0)) - dt / Real(2) * J[(size_t)i * ns + k] / rho;   // (A.35)
+            }
+            solve_dense<Real>(ns, A, F);                                                                      // (A.34)
+            last_update = 0;
+            for (int i = 0; i < ns; ++i) {
+                Yn[i] += F[i];                                                                                 // (A.33)
+                last_update = std::fmax(last_update, std::fabs(F[i]));
+            }
+            rates(Yn, om, bd);
+        }
+        if (Ybound)
+            for (int i = 0; i < ns; ++i) Ybound[i * ldb] += dt / Real(2) * Real(m.mol_weight[i]) * (bd[i] + bdm[i]) / rho;
+    }
+    for (int i = 0; i < ns; ++i) Y[i * ld] = Yn[i];
+}
+
+template <class Real>
+void reactor_cn(const oracle_mech &m, int64_t n, int64_t ld, const Real *rho, const Real *e, Real *Y, Real *T, Real dt,
+                int n_steps, int newton_iters, Real tol, int max_iter, Real *Ybound, Real *last_update, int64_t *n_not_converged) {
+    int64_t bad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : bad)
+    for (int64_t p = 0; p < n; ++p) {
+        int nc;
+        Real lu;
+        reactor_cn_point<Real>(m, rho[p], e[p], Y + p, ld, T[p], dt, n_steps, newton_iters, tol, max_iter,
+                               Ybound ? Ybound + p : nullptr, ld, lu, nc);
+        if (last_update) last_update[p] = lu;
+        bad += nc;
+    }
+    if (n_not_converged) *n_not_converged = bad;
+}
+
 template <class Real>
 void reaction_detail(const oracle_mech &m, int j, Real rho, Real T, const Real *Y, Real *out9) {
     const int ns = m.n_species;
@@ -758,6 +857,12 @@ int oracle_sizeof_real80() { return (int)sizeof(long double); }
     void oracle_get_transport_##SUFFIX(const oracle_transport *t, int64_t n, int64_t ld, const Real *T, const Real *Y, \
                                        Real *mu, Real *kappa, Real *Dkm) {                                   \
         get_transport<Real>(*t, n, ld, T, Y, mu, kappa, Dkm);                                                 \
+    }                                                                                                         \
+    void oracle_reactor_cn_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld, const Real *rho, const Real *e,     \
+                                    Real *Y, Real *T, Real dt, int n_steps, int newton_iters, Real tol,           \
+                                    int max_iter, Real *Ybound, Real *last_update, int64_t *n_not_converged) {     \
+        reactor_cn<Real>(*m, n, ld, rho, e, Y, T, dt, n_steps, newton_iters, tol, max_iter, Ybound, last_update,  \
+                         n_not_converged);                                                                    \
     }                                                                                                         \
     void oracle_get_net_production_rates_##SUFFIX(const oracle_mech *m, int64_t n, int64_t ld,                \
                                                   const Real *rho, const Real *T, const Real *Y, Real *omega, \

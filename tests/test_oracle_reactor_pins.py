@@ -137,3 +137,67 @@ def test_double_reactor_agrees_with_long_double():
     b = o8.reactor_rk4(rho, e, Y, T, dt, 10)
     assert np.isfinite(a[0]).all() and a[3] == 0
     assert np.all(np.abs(a[0] - b[0].astype(np.float64)) <= 1e-12 * (a[2] + np.abs(a[0])))
+
+
+# ---------------------------------------------------------------- Crank-Nicolson march (A.32)-(A.36) PAPER.md:1043-1062
+def _decay_mech(k):
+    z4 = [0.0] * 4
+    sp = [dict(W=20.0, lo=[3.5, *z4, -1000.0, 2.0]), dict(W=20.0, lo=[3.0, *z4, -3000.0, 3.0])]
+    return simple_mechanism(sp, [dict(reac={0: 1}, prod={1: 1}, A=k, b=0.0, theta=0.0, reversible=0)])
+
+
+def test_c1_linear_decay_step_and_c4_stability_where_rk4_diverges():
+    """dY_A/dt = -k Y_A: one Crank-Nicolson step is y (1 - z/2)/(1 + z/2), z = k dt, reached by ONE Newton iteration
+    (the problem is linear and the Jacobian exact).  At z = 20 RK4 grows by |P(z)| = 5e3 per step, CN stays bounded
+    (the implicit scheme allows larger steps)."""
+    k = 2.5e5
+    mech = _decay_mech(k)
+    for real, tol in (("f64", 1e-14), ("f80", 1e-17)):
+        o = oracle.Oracle(mech, real)
+        Y0 = np.array([[0.7], [0.3]])
+        T0, rho = 1100.0, 0.4
+        e = o.mixture_e(T0, Y0[:, 0])
+        for dt, steps, iters in ((1e-6, 1, 1), (2e-6, 7, 1), (4e-7, 40, 3), (8e-5, 5, 2)):
+            z = LD(k) * LD(dt)
+            g = (1 - z / 2) / (1 + z / 2)
+            Y, T, Yb, lu, bad = o.reactor_cn([rho], [e], Y0, [T0], dt, steps, newton_iters=iters)
+            yA = LD(Y0[0, 0]) * g ** steps
+            assert bad == 0
+            assert abs(LD(Y[0, 0]) - yA) <= tol * steps * 4 and abs(LD(Y[1, 0]) - (LD(Y0[1, 0]) + LD(Y0[0, 0]) - yA)) <= tol * steps * 4
+            if iters > 1:
+                assert float(lu[0]) <= 1e-15          # the second Newton update of a linear problem is rounding
+            assert abs(float(o.mixture_e(T[0], Y[:, 0])) / float(e) - 1) < 1e-12
+    # z = 20: RK4 diverges, CN does not
+    o = oracle.Oracle(mech)
+    Yr, _, _, _ = o.reactor_rk4([rho], [e], Y0, [T0], 8e-5, 5)
+    Yc, _, _, _, _ = o.reactor_cn([rho], [e], Y0, [T0], 8e-5, 5, newton_iters=1)
+    assert abs(Yr[0, 0]) > 1e10 and abs(Yc[0, 0]) <= 0.7
+
+
+def test_c2_second_order_convergence_and_c3_conservation():
+    mech = inputs.config_mechanism(0)
+    o = oracle.Oracle(mech, "f80")
+    st = inputs.config_states(0, n=64)
+    st["e"] = np.array([o.mixture_e(LD(st["T"][p]), st["Y"][:, p].astype(LD)) for p in range(64)], dtype=LD)
+    checked = 0
+    for p in range(64):
+        if not 1200.0 < st["T"][p] < 2500.0:
+            continue
+        s1 = {k: v[..., p:p + 1] for k, v in st.items() if k in ("rho", "T", "Y", "e")}
+        dt = stable_dt(o, s1, safety=0.2)
+        ref, _ = _run(o, st, p, dt / 16, 128)                         # RK4, 16 times finer
+        run = lambda h, n: o.reactor_cn(s1["rho"], s1["e"], s1["Y"], s1["T"], h, n, newton_iters=6, tol=LD(1e-9), max_iter=30)
+        Y1, _, Yb, lu1, bad1 = run(dt, 8)
+        Y2, _, _, lu2, bad2 = run(dt / 2, 16)
+        assert bad1 == bad2 == 0 and float(lu1[0]) < 1e-12 and float(lu2[0]) < 1e-12   # Newton converged
+        e1, e2 = np.max(np.abs(Y1[:, 0] - ref)), np.max(np.abs(Y2[:, 0] - ref))
+        if e2 < 1e-16:
+            continue
+        assert 3.0 < float(e1 / e2) < 5.5, (p, float(e1), float(e2))
+        # C3: linear invariants are kept by every Newton update
+        assert abs(float(Y1[:, 0].sum() - s1["Y"][:, 0].astype(LD).sum())) <= 1e-16 * float(Yb[:, 0].sum() + 1)
+        for el in range(mech.n_elements):
+            w = (mech.elem_comp[:, el] / mech.mol_weight).astype(LD)
+            assert abs(float((w * (Y1[:, 0] - s1["Y"][:, 0].astype(LD))).sum())) <= 1e-16 * float((w * (Yb[:, 0] + 1)).sum())
+        checked += 1
+    assert checked >= 5
