@@ -169,6 +169,22 @@ int pyro_source_terms(const pyro_mech *mech, int64_t n, int64_t ld, const double
 int pyro_reactor_rk4(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e, double *Y,
                      double *T, double dt, int32_t n_steps, double *work, int32_t *n_not_converged, void *cuda_stream);
 
+/* Implicit march of the same reactors (second half): Crank-Nicolson (A.32) PAPER.md:1043-1062,
+ *     Y^{m+1} - Y^m - dt/2 (s^{m+1} + s^m) = 0,   s_k = W_k omega_k / rho,
+ * each step solved by `newton_iters` Newton iterations (A.33)-(A.35) started from Y^m, with the analytic Jacobian
+ * (A.36) at fixed (rho, e) (pyro_get_jacobian, PYRO_JAC_FIXED_E) and a dense LU per point without pivoting (the matrix
+ * is I - dt/(2 rho) J).  The iteration count is fixed (data-independent control flow, no host synchronisation): a launch
+ * sequence of the library's own temperature, rates and Jacobian kernels plus the per-point linear algebra, all on
+ * `cuda_stream`.  Arguments as pyro_reactor_rk4, and
+ *   update_tol       a point whose last Newton update max_k |dY_k| of a step is not below it (or not finite) is counted
+ *   work             device scratch of *doubles doubles as pyro_reactor_cn_work_doubles(mech, ld, &doubles) reports; must not overlap Y
+ *   n_not_converged  += temperature solves that hit their cap + (point, step) pairs counted by update_tol
+ * Mechanisms of more than 127 species: PYRO_ERR_UNSUPPORTED. */
+int pyro_reactor_cn_work_doubles(const pyro_mech *mech, int64_t ld, int64_t *doubles);
+int pyro_reactor_cn(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e, double *Y,
+                    double *T, double dt, int32_t n_steps, int32_t newton_iters, double update_tol, double *work,
+                    int32_t *n_not_converged, void *cuda_stream);
+
 /* Chemical Jacobian (eq. (6); (A.36) PAPER.md:1057) of the source terms S_i = W_i omega_i
  * ((A.1) PAPER.md:888), analytic:
  *   J[(i*n_species + k)*ld + p] = dS_i/dY_k     [n_species*n_species][ld], device, out; must not overlap Y

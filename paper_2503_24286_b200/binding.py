@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libpyro.so")
 EXPORTS = (
     "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
     "pyro_get_temperature_from_enthalpy", "pyro_get_density", "pyro_get_pressure",
-    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak", "pyro_probe_dmma_peak", "pyro_probe_indexed_rmw",
+    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_reactor_cn", "pyro_reactor_cn_work_doubles", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak", "pyro_probe_dmma_peak", "pyro_probe_indexed_rmw",
     "pyro_status_string", "pyro_last_error_string", "pyro_transport_create", "pyro_transport_destroy",
     "pyro_get_transport",
 )
@@ -92,6 +92,8 @@ def load_library():
     lib.pyro_get_net_production_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_get_jacobian.argtypes = [vp, i64, i64, vp, vp, vp, C.c_int, vp, vp, vp]
     lib.pyro_reactor_rk4.argtypes = [vp, i64, i64, vp, vp, vp, vp, dbl, C.c_int32, vp, vp, vp]
+    lib.pyro_reactor_cn.argtypes = [vp, i64, i64, vp, vp, vp, vp, dbl, C.c_int32, C.c_int32, dbl, vp, vp, vp]
+    lib.pyro_reactor_cn_work_doubles.argtypes = [vp, i64, C.POINTER(i64)]
     lib.pyro_source_terms.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, vp]
     lib.pyro_source_terms_host.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, C.POINTER(i64)]
     lib.pyro_transport_create.argtypes = [C.POINTER(TransportDesc), C.c_int, C.POINTER(vp)]
@@ -268,6 +270,24 @@ class Mechanism:
         assert work.stride(0) == ld or n == 0
         _check(self._lib.pyro_reactor_rk4(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T), float(dt), int(n_steps),
                                           _ptr(work), _ptr(n_not_converged), _stream(stream)))
+        return Y, T
+
+    def reactor_cn(self, rho, e, Y, T, dt, n_steps, newton_iters=4, update_tol=1e-10, work=None, n_not_converged=None,
+                   stream=None):
+        """pyro_reactor_cn: marches Y (in place) by n_steps Crank-Nicolson steps; T: guess in, temperature of the last
+        Newton iterate out."""
+        import torch
+        n = rho.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        need = C.c_int64(0)
+        _check(self._lib.pyro_reactor_cn_work_doubles(self._h, ld, C.byref(need)))
+        need = int(need.value)
+        if work is None:
+            work = torch.empty(need, dtype=torch.float64, device=Y.device)
+        assert work.numel() >= need
+        _check(self._lib.pyro_reactor_cn(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T), float(dt), int(n_steps),
+                                         int(newton_iters), float(update_tol), _ptr(work), _ptr(n_not_converged),
+                                         _stream(stream)))
         return Y, T
 
     def get_jacobian(self, rho, T, Y, mode=0, out=None, dSdT=None, want_dSdT=True, stream=None):

@@ -734,6 +734,65 @@ int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *r
     return PYRO_OK;
 }
 
+namespace {
+int64_t cn_work_doubles(const pyro_mech *m, int64_t ld) {
+    const int64_t ns = m->packed.n_species;
+    return (ns * ns + 4 * ns) * ld + ld;   // J, omega, Ym, Sm, F, last update
+}
+}   // namespace
+
+int pyro_reactor_cn_work_doubles(const pyro_mech *m, int64_t ld, int64_t *doubles) {
+    if (!m || !doubles) return fail(PYRO_ERR_NULL, "NULL argument");
+    if (ld < 0) return fail(PYRO_ERR_BAD_SIZE, "ld < 0");
+    *doubles = cn_work_doubles(m, ld);
+    return PYRO_OK;
+}
+
+int pyro_reactor_cn(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e, double *Y, double *T,
+                    double dt, int32_t n_steps, int32_t newton_iters, double update_tol, double *work,
+                    int32_t *n_not_converged, void *cuda_stream) {
+    int st = check_fields(m, n, ld);
+    if (st != PYRO_OK) return st;
+    if (n_steps < 0 || newton_iters < 1 || !(dt == dt) || !(update_tol >= 0)) return fail(PYRO_ERR_BAD_SIZE, "n_steps >= 0, newton_iters >= 1, update_tol >= 0");
+    if (n == 0) return PYRO_OK;
+    if (!rho || !e || !Y || !T || !work) return fail(PYRO_ERR_NULL, "a field pointer is NULL");
+    if (!aligned8(rho) || !aligned8(e) || !aligned8(Y) || !aligned8(T) || !aligned8(work) ||
+        (reinterpret_cast<uintptr_t>(n_not_converged) & 3u))
+        return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
+    if (!m->jac_ok) return fail(PYRO_ERR_UNSUPPORTED, "the Jacobian kernel holds at most 127 species");
+    const int64_t ns = m->packed.n_species;
+    {
+        const uintptr_t ys = (uintptr_t)((ns - 1) * ld + n) * sizeof(double), ws = (uintptr_t)cn_work_doubles(m, ld) * sizeof(double);
+        const uintptr_t y0 = reinterpret_cast<uintptr_t>(Y), w0 = reinterpret_cast<uintptr_t>(work);
+        if (y0 < w0 + ws && w0 < y0 + ys) return fail(PYRO_ERR_BAD_SIZE, "work must not overlap Y");
+    }
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    double *J = work, *omega = J + ns * ns * ld, *Ym = omega + ns * ld, *Sm = Ym + ns * ld, *F = Sm + ns * ld, *lastu = F + ns * ld;
+    pyro::CnArgs a{};
+    a.n = n; a.ld = ld; a.rho = rho; a.omega = omega; a.Y = Y; a.Ym = Ym; a.Sm = Sm; a.F = F; a.J = J; a.last_update = lastu;
+    a.n_not_converged = n_not_converged; a.energy = m->d_energy; a.dt = dt; a.update_tol = update_tol; a.n_species = (int32_t)ns;
+    // rates at the initial state; then per step: old-level terms, newton_iters x (Jacobian, solve + update, temperature, rates)
+    if ((st = pyro_get_temperature(m, n, ld, rho, e, Y, T, T, n_not_converged, cuda_stream)) != PYRO_OK) return st;
+    if ((st = pyro_get_net_production_rates(m, n, ld, rho, T, Y, omega, cuda_stream)) != PYRO_OK) return st;
+    for (int32_t step = 0; step < n_steps; ++step) {
+        {
+            DeviceGuard guard(m->device);
+            PYRO_CUDA(pyro::launch_cn_begin_step(a, stream));
+        }
+        for (int32_t it = 0; it < newton_iters; ++it) {
+            if ((st = pyro_get_jacobian(m, n, ld, rho, T, Y, PYRO_JAC_FIXED_E, J, nullptr, cuda_stream)) != PYRO_OK) return st;
+            a.count_unconverged = (it == newton_iters - 1) ? 1 : 0;
+            {
+                DeviceGuard guard(m->device);
+                PYRO_CUDA(pyro::launch_cn_newton(a, stream));
+            }
+            if ((st = pyro_get_temperature(m, n, ld, rho, e, Y, T, T, n_not_converged, cuda_stream)) != PYRO_OK) return st;
+            if ((st = pyro_get_net_production_rates(m, n, ld, rho, T, Y, omega, cuda_stream)) != PYRO_OK) return st;
+        }
+    }
+    return PYRO_OK;
+}
+
 int pyro_source_terms_host(pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e,
                            const double *Y, const double *T_guess, double *T, double *omega,
                            int64_t *n_not_converged) {

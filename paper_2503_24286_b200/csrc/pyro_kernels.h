@@ -67,6 +67,21 @@ const void *reactor_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool singl
 cudaError_t launch_reactor(const ReactorArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem, bool singles,
                            size_t smem_bytes, cudaStream_t stream);
 
+struct CnArgs {                  // implicit (Crank-Nicolson) reactor march: per-point linear algebra (pyro_cn_kernels.cu)
+    int64_t n, ld;
+    const double *rho, *omega;   // [n], [n_species][ld] rates at the current Newton iterate
+    double *Y;                   // current iterate, updated in place
+    double *Ym, *Sm, *F;         // [n_species][ld] each: state and right-hand side at the old time level, Newton residual / update
+    double *J;                   // [n_species^2][ld]: Jacobian in, LU factors out
+    double *last_update;         // [n] or NULL: max_k |dY_k| of this iteration
+    int32_t *n_not_converged;
+    const EnergyRow *energy;     // W_k
+    double dt, update_tol;
+    int32_t n_species, count_unconverged;
+};
+cudaError_t launch_cn_begin_step(const CnArgs &a, cudaStream_t stream);
+cudaError_t launch_cn_newton(const CnArgs &a, cudaStream_t stream);
+
 constexpr int kJacMaxThreads = 128;
 constexpr size_t kJacRingBytes = 8192;  // per warp: two segments of 32 records of up to 128 bytes (RecordRing)     // threads (= points) per block of the Jacobian kernel: one warp per tensor-memory lane quarter
 

@@ -791,3 +791,66 @@ def test_two_points_per_thread_rates_kernel(mechs, monkeypatch):
         gm = binding.Mechanism(mech)
         om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
         parity.assert_omega_parity(gpu_rates(gm, rho, T, Y), om_ref, bound)
+
+
+# ------------------------------------------------------------------ implicit (Crank-Nicolson) reactor march (NEXT-4)
+@pytest.mark.parametrize("case,n", [("all_paths", 200), ("cfg0", 1000), ("cfg2", 150)])
+def test_reactor_cn_every_point(mechs, case, n):
+    """pyro_reactor_cn against the oracle's Crank-Nicolson march (same fixed number of Newton iterations per step), at
+    a step ten times the explicit one; ragged tails."""
+    if case == "all_paths":
+        mech = hand_cases.all_paths_mechanism()
+        rho, T, Y = hand_cases.random_states(mech, n)
+    else:
+        cfg = {"cfg0": 0, "cfg2": 2}[case]
+        mech = inputs.config_mechanism(cfg)
+        st = inputs.config_states(cfg, n=n)
+        rho, T, Y = st["rho"], st["T"], st["Y"]
+    orc = oracle.Oracle(mech)
+    gm = binding.Mechanism(mech)
+    e = np.array([orc.mixture_e(T[p], Y[:, p]) for p in range(n)])
+    Tg = T * 1.03
+    # ten times the explicit step of the stiffest reactor of the batch: I - dt/(2 rho) J stays a perturbation of the
+    # identity for every reactor (the kernel's LU does not pivot, reading G32)
+    dt = stable_dt(orc, rho, T, Y, safety=0.2)
+    for n_steps, iters in ((1, 1), (3, 4)):
+        Yr, Tr, Yb, lu, bad_r = orc.reactor_cn(rho, e, Y, Tg, dt, n_steps, newton_iters=iters)
+        ok = np.isfinite(Yr).all(axis=0) & np.isfinite(Tr) & (np.abs(Yr).max(axis=0) < 10.0) & (lu < 1e-3)
+        assert ok.sum() >= 0.5 * n
+        Yd, Td = dev(Y), dev(Tg)
+        gm.reactor_cn(dev(rho), dev(e), Yd, Td, dt, n_steps, newton_iters=iters)
+        torch.cuda.synchronize()
+        Yg, Tgpu = Yd.cpu().numpy(), Td.cpu().numpy()
+        rY = float(np.max(np.abs(Yg - Yr)[:, ok] / (Yb + np.abs(Yr) + 1e-300)[:, ok]))
+        rT = float(np.max(np.abs(Tgpu - Tr)[ok] / Tr[ok]))
+        print(f"{case} steps {n_steps} iters {iters}: max |dY|/scale = {rY:.2e}, max |dT|/T = {rT:.2e}, reactors compared {int(ok.sum())}/{n}")
+        assert rY <= 1e-9 and rT <= 1e-8
+
+
+def test_reactor_cn_linear_decay_closed_form_and_convergence_count():
+    """A -> B with a constant rate coefficient: the GPU march reproduces y (1 - z/2)/(1 + z/2) per step at z = 20,
+    where the explicit march diverges; the update tolerance counts unconverged (point, step) pairs."""
+    z4 = [0.0] * 4
+    sp = [dict(W=20.0, lo=[3.5, *z4, -1000.0, 2.0]), dict(W=20.0, lo=[3.0, *z4, -3000.0, 3.0])]
+    k, dt, steps = 2.5e5, 8e-5, 5
+    mech = inputs.simple_mechanism(sp, [dict(reac={0: 1}, prod={1: 1}, A=k, b=0.0, theta=0.0, reversible=0)])
+    gm, orc = binding.Mechanism(mech), oracle.Oracle(mech)
+    n = 100
+    Y = np.vstack([np.linspace(0.1, 0.9, n), 1 - np.linspace(0.1, 0.9, n)])
+    T = np.full(n, 1100.0)
+    rho = np.full(n, 0.4)
+    e = np.array([orc.mixture_e(T[p], Y[:, p]) for p in range(n)])
+    Yd, Td = dev(Y), dev(T)
+    bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+    gm.reactor_cn(dev(rho), dev(e), Yd, Td, dt, steps, newton_iters=2, update_tol=1e-12, n_not_converged=bad)
+    torch.cuda.synchronize()
+    g = ((1 - k * dt / 2) / (1 + k * dt / 2)) ** steps
+    assert np.max(np.abs(Yd.cpu().numpy()[0] - Y[0] * g)) < 1e-14 and int(bad.item()) == 0
+    Yd = dev(Y)
+    gm.reactor_cn(dev(rho), dev(e), Yd, dev(T), dt, steps, newton_iters=1, update_tol=1e-12, n_not_converged=bad)
+    torch.cuda.synchronize()
+    assert int(bad.item()) == n * steps     # one iteration: the (only) update is the whole step, far above the tolerance
+    Yr = dev(Y)
+    gm.reactor_rk4(dev(rho), dev(e), Yr, dev(T), dt, steps)
+    torch.cuda.synchronize()
+    assert not bool(torch.isfinite(Yr).all()) or float(Yr.abs().max().item()) > 1e10   # the explicit march diverges at z = 20
