@@ -680,8 +680,19 @@ int pyro_reactor_rk4(const pyro_mech *m, int64_t n, int64_t ld, const double *rh
     return PYRO_OK;
 }
 
+namespace {
+int jacobian_call(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y, int mode,
+                  double *J, double *dSdT, void *cuda_stream, int64_t jblock);
+}
+
 int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y,
                       int mode, double *J, double *dSdT, void *cuda_stream) {
+    return jacobian_call(m, n, ld, rho, T, Y, mode, J, dSdT, cuda_stream, 0);
+}
+
+namespace {
+int jacobian_call(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y, int mode,
+                  double *J, double *dSdT, void *cuda_stream, int64_t jblock) {
     int st = check_fields(m, n, ld);
     if (st != PYRO_OK) return st;
     if (mode != PYRO_JAC_FIXED_T && mode != PYRO_JAC_FIXED_E) return fail(PYRO_ERR_BAD_SIZE, "mode must be PYRO_JAC_FIXED_T or PYRO_JAC_FIXED_E");
@@ -713,6 +724,7 @@ int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *r
     a.planes_bytes = m->jac_planes_bytes;
     a.mode = mode;
     a.lay = m->jac.lay;
+    a.jblock = jblock;
     const int warps = m->jac_threads / 32;
     int64_t blocks = (int64_t)m->sm_count * m->jac_blocks_per_sm;
     if (blocks > (a.n_chunks + warps - 1) / warps) blocks = (a.n_chunks + warps - 1) / warps;
@@ -734,10 +746,9 @@ int pyro_get_jacobian(const pyro_mech *m, int64_t n, int64_t ld, const double *r
     return PYRO_OK;
 }
 
-namespace {
 int64_t cn_work_doubles(const pyro_mech *m, int64_t ld) {
-    const int64_t ns = m->packed.n_species;
-    return (ns * ns + 4 * ns) * ld + ld;   // J, omega, Ym, Sm, F, last update
+    const int64_t ns = m->packed.n_species, jb = pyro::cn_block_threads((int)ns);
+    return ns * ns * ((ld + jb - 1) / jb * jb) + 4 * ns * ld + ld;   // J (blocks of jb points), omega, Ym, Sm, F, last update
 }
 }   // namespace
 
@@ -767,10 +778,12 @@ int pyro_reactor_cn(const pyro_mech *m, int64_t n, int64_t ld, const double *rho
         if (y0 < w0 + ws && w0 < y0 + ys) return fail(PYRO_ERR_BAD_SIZE, "work must not overlap Y");
     }
     cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-    double *J = work, *omega = J + ns * ns * ld, *Ym = omega + ns * ld, *Sm = Ym + ns * ld, *F = Sm + ns * ld, *lastu = F + ns * ld;
+    const int64_t jb = pyro::cn_block_threads((int)ns);
+    double *J = work, *omega = J + ns * ns * ((ld + jb - 1) / jb * jb), *Ym = omega + ns * ld, *Sm = Ym + ns * ld, *F = Sm + ns * ld, *lastu = F + ns * ld;
     pyro::CnArgs a{};
     a.n = n; a.ld = ld; a.rho = rho; a.omega = omega; a.Y = Y; a.Ym = Ym; a.Sm = Sm; a.F = F; a.J = J; a.last_update = lastu;
     a.n_not_converged = n_not_converged; a.energy = m->d_energy; a.dt = dt; a.update_tol = update_tol; a.n_species = (int32_t)ns;
+    a.jblock = jb;
     // rates at the initial state; then per step: old-level terms, newton_iters x (Jacobian, solve + update, temperature, rates)
     if ((st = pyro_get_temperature(m, n, ld, rho, e, Y, T, T, n_not_converged, cuda_stream)) != PYRO_OK) return st;
     if ((st = pyro_get_net_production_rates(m, n, ld, rho, T, Y, omega, cuda_stream)) != PYRO_OK) return st;
@@ -780,7 +793,7 @@ int pyro_reactor_cn(const pyro_mech *m, int64_t n, int64_t ld, const double *rho
             PYRO_CUDA(pyro::launch_cn_begin_step(a, stream));
         }
         for (int32_t it = 0; it < newton_iters; ++it) {
-            if ((st = pyro_get_jacobian(m, n, ld, rho, T, Y, PYRO_JAC_FIXED_E, J, nullptr, cuda_stream)) != PYRO_OK) return st;
+            if ((st = jacobian_call(m, n, ld, rho, T, Y, PYRO_JAC_FIXED_E, J, nullptr, cuda_stream, jb)) != PYRO_OK) return st;
             a.count_unconverged = (it == newton_iters - 1) ? 1 : 0;
             {
                 DeviceGuard guard(m->device);

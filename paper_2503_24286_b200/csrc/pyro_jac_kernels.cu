@@ -218,12 +218,15 @@ template <bool kSmall> __global__ void __launch_bounds__(kJacMaxThreads, 1) jaco
         const int64_t pc = p < a.n ? p : a.n - 1;   // tail lanes recompute the last point and store nothing
         const bool live = p < a.n;
         const double *Yp = a.Y + pc;
-        double *Jp = a.J + pc;
+        // J[(i n_s + k) ld + p] -- or, for the implicit march, blocks of jblock points: element (i, k) of point p at
+        // ((p / jblock) n_s^2 + i n_s + k) jblock + p % jblock, so that the matrices of a block of points are contiguous
+        double *Jp = a.jblock ? a.J + (pc / a.jblock) * ((int64_t)ns * ns * a.jblock) + pc % a.jblock : a.J + pc;
+        const int64_t jstride = a.jblock ? a.jblock : a.ld;
         double *Tp = a.dSdT ? a.dSdT + pc : nullptr;
         jacobian_point(
             tab, a.lay, a.T[pc], a.rho[pc], a.mode, a.dSdT != nullptr, mem, [&](int k) { return __ldg(Yp + (int64_t)k * a.ld); },
             [&](int i, int k, double v) {
-                if (live) __stcs(Jp + ((int64_t)i * ns + k) * a.ld, v);
+                if (live) __stcs(Jp + ((int64_t)i * ns + k) * jstride, v);
             },
             [&](int i, double v) {
                 if (live) Tp[(int64_t)i * a.ld] = v;

@@ -72,13 +72,16 @@ struct CnArgs {                  // implicit (Crank-Nicolson) reactor march: per
     const double *rho, *omega;   // [n], [n_species][ld] rates at the current Newton iterate
     double *Y;                   // current iterate, updated in place
     double *Ym, *Sm, *F;         // [n_species][ld] each: state and right-hand side at the old time level, Newton residual / update
-    double *J;                   // [n_species^2][ld]: Jacobian in, LU factors out
+    double *J;                   // Jacobian in, LU factors out; blocked layout: element (i, k) of point p at
+                                 // ((p / jblock) n_s^2 + i n_s + k) jblock + p % jblock
+    int64_t jblock;
     double *last_update;         // [n] or NULL: max_k |dY_k| of this iteration
     int32_t *n_not_converged;
     const EnergyRow *energy;     // W_k
     double dt, update_tol;
     int32_t n_species, count_unconverged;
 };
+int cn_block_threads(int n_species);   // threads (= points) per block of cn_newton_kernel = the Jacobian's point block
 cudaError_t launch_cn_begin_step(const CnArgs &a, cudaStream_t stream);
 cudaError_t launch_cn_newton(const CnArgs &a, cudaStream_t stream);
 
@@ -97,6 +100,7 @@ struct JacArgs {                 // chemical Jacobian (pyro_jac_tables.h)
     uint32_t off_spec, tmem_cols;
     uint32_t planes_bytes;       // dynamic shared memory taken by the planes; the per-warp record rings (8 KB each) follow
     int32_t mode;                // 0: fixed (rho, T); 1: fixed (rho, e)
+    int64_t jblock;              // 0: J[(i n_s + k) ld + p]; else blocks of jblock points with contiguous matrices (implicit march)
     JacLayout lay;
 };
 
