@@ -854,3 +854,45 @@ def test_reactor_cn_linear_decay_closed_form_and_convergence_count():
     gm.reactor_rk4(dev(rho), dev(e), Yr, dev(T), dt, steps)
     torch.cuda.synchronize()
     assert not bool(torch.isfinite(Yr).all()) or float(Yr.abs().max().item()) > 1e10   # the explicit march diverges at z = 20
+
+
+# ------------------------------------------------------------------ widened rows at the sizes bench.py times, sampled
+def test_transport_and_reactors_at_bench_size_sampled(mechs):
+    """The launch configurations of bench.py's widened legs on configs[2]: transport on 2^20 points, the RK4 march on
+    2^20 reactors x 4 steps, the Crank-Nicolson march on 2^16 reactors x 1 step of 3 Newton iterations; sampled
+    reactors (first, last, random) against the oracle.  The step is the bench's: from the GPU Jacobian of the batch."""
+    mech, gm, orc = mechs(2)
+    n = 1 << 20
+    st = inputs.config_states(2, n=n)
+    rho, e, Y, Tg, T = (dev(st[k]) for k in ("rho", "e", "Y", "T_guess", "T"))
+    idx = _sample(n, 48)
+    # transport
+    tr = inputs.config_transport(2)
+    got = binding.Transport(tr).get_transport(T, Y)
+    torch.cuda.synchronize()
+    ref = oracle.TransportOracle(tr).get_transport(st["T"][idx], st["Y"][:, idx])
+    assert_transport_parity((got[0][idx], got[1][idx], got[2][:, idx]), ref)
+    # explicit march, step as in bench.py (largest Jacobian row sum over a slice of the batch)
+    m = 1 << 14
+    J, _ = gm.get_jacobian(rho[:m].contiguous(), T[:m].contiguous(), Y[:, :m].contiguous(), mode=1, want_dSdT=False)
+    dt = 1e-3 / float((J.abs().sum(dim=1) / rho[:m][None, :]).max().item())
+    del J
+    Yd, Td = Y.clone(), Tg.clone()
+    gm.reactor_rk4(rho, e, Yd, Td, dt, 4)
+    torch.cuda.synchronize()
+    Yr, Tr, Yb, _ = orc.reactor_rk4(st["rho"][idx], st["e"][idx], st["Y"][:, idx], st["T_guess"][idx], dt, 4)
+    ok = np.isfinite(Yr).all(axis=0) & (np.abs(Yr).max(axis=0) < 10.0)
+    assert ok.sum() >= 0.9 * len(idx)
+    assert_reactor_parity(Yd[:, idx].cpu().numpy()[:, ok], Td[idx].cpu().numpy()[ok], Yr[:, ok], Tr[ok], Yb[:, ok])
+    assert bool(torch.isfinite(Yd).all())
+    # implicit march at ten times that step
+    nc = 1 << 16
+    idc = _sample(nc, 32)
+    Yc, Tc = Y[:, :nc].clone(), Tg[:nc].clone()
+    gm.reactor_cn(rho[:nc].contiguous(), e[:nc].contiguous(), Yc, Tc, 10.0 * dt, 1, newton_iters=3)
+    torch.cuda.synchronize()
+    Yr, Tr, Yb, lu, _ = orc.reactor_cn(st["rho"][idc], st["e"][idc], st["Y"][:, idc], st["T_guess"][idc], 10.0 * dt, 1, newton_iters=3)
+    ok = np.isfinite(Yr).all(axis=0) & (np.abs(Yr).max(axis=0) < 10.0)
+    assert ok.sum() >= 0.9 * len(idc)
+    rY = float(np.max(np.abs(Yc[:, idc].cpu().numpy() - Yr)[:, ok] / (Yb + np.abs(Yr) + 1e-300)[:, ok]))
+    assert rY <= 1e-9, rY
