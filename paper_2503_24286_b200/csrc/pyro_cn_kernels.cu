@@ -124,12 +124,10 @@ cudaError_t launch_cn_begin_step(const CnArgs &a, cudaStream_t stream) {
 cudaError_t launch_cn_newton(const CnArgs &a, cudaStream_t stream) {
     const int tb = cn_block_threads(a.n_species);
     const size_t smem = (size_t)kCnPanel * a.n_species * tb * sizeof(double);
-    static bool attr_set = false;   // the limit is a property of the functions
-    if (!attr_set) {
-        cudaFuncSetAttribute(cn_newton_kernel<kCnPanel, 64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-        cudaFuncSetAttribute(cn_newton_kernel<kCnPanel, 32>, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-        attr_set = true;
-    }
+    // the limit is a property of the function on the current device: set it on every launch (cheap; no process-wide state)
+    const void *fn = tb == 64 ? (const void *)cn_newton_kernel<kCnPanel, 64> : (const void *)cn_newton_kernel<kCnPanel, 32>;
+    cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (ce != cudaSuccess) return ce;
     const dim3 grid((unsigned)((a.n + tb - 1) / tb));
     if (tb == 64) cn_newton_kernel<kCnPanel, 64><<<grid, dim3(64), smem, stream>>>(a);
     else cn_newton_kernel<kCnPanel, 32><<<grid, dim3(32), smem, stream>>>(a);
