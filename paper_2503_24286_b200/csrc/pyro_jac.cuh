@@ -75,6 +75,105 @@ PYRO_HD JacRates jac_reaction_rates(const JacRxn &r, const PointT &pt, const Mem
     return o;
 }
 
+struct JacExt {      // a third-body / falloff reaction at one point
+    double mul;      // multiplier of its incidence terms: [M] or L F
+    double g;        // dR/d[M]: the coefficient of the efficiency eff_k in dR/dC_k
+    double dRdT;     // dR/dT at fixed concentrations
+};
+
+// Third-body and falloff forms (readings G6-G8) and their derivatives with respect to [M] and T.
+template <class Tab, class Mem>
+PYRO_HD JacExt jac_ext_reaction(const Tab &tab, const JacRxn &r, const PointT &pt, double ctot, const Mem &mem) {
+    const JacRates q = jac_reaction_rates(r, pt, mem);
+    double M = r.eff_default * ctot;
+#pragma unroll 1
+    for (uint32_t e = r.eff_begin; e < r.eff_begin + r.eff_count; ++e) {
+        const EffEntry &en = tab.eff((int)e);
+        M = fma(en.delta, mem.ldC(en.species), M);
+    }
+    const double net = q.qf - q.qr;
+    const double dnet_dT = kLn2 * (q.qf * q.dyf - q.qr * (q.dyf + q.ddG));   // at fixed rate-coefficient multiplier
+    double mul, g, dRdT;
+    if (r.type == PYRO_THREE_BODY) {   // R = [M] (q_f - q_r)
+        mul = M;
+        g = net;
+        dRdT = M * dnet_dT;
+    } else {                           // R = L F (q_f - q_r), L = Pr/(1+Pr), Pr = k_0 [M]/k_inf
+        const RxnFall &fl = tab.rxn_fall((int)r.fall_index);
+        const double y0 = arrhenius_log2(fl.l[0], fl.l[1], fl.l[2], pt.L2T, pt.invT);
+        const double dy0 = arrhenius_log2_dT(fl.l[1], fl.l[2], pt.invT);
+        double e[4] = {y0 - q.yf, fl.troe_t3 * pt.T, fl.troe_t1 * pt.T, fl.troe_t2 * pt.invT};
+        exp2_poly_n<4>(e);
+        const double Pr = e[0] * M;
+        const double dlnL = rcp_newton(1.0 + Pr);   // d ln L / d ln Pr
+        double LF = Pr * dlnL, dlnF_dlnPr = 0.0, dlnF_dT = 0.0;
+        if (r.type == PYRO_FALLOFF_TROE) {
+            const double a3 = (1.0 - fl.troe_alpha) * e[1], a1 = fl.troe_alpha * e[2], a2 = fl.troe_has_t2 * e[3];
+            const double Fc = a3 + a1 + a2;
+            const double dFc = kLn2 * fma(fl.troe_t3, a3, fma(fl.troe_t1, a1, -fl.troe_t2 * pt.invT * pt.invT * a2));
+            const double l2Fc = log2_pos(Fc), lFc = l2Fc * kLog10of2;
+            const double dlFc = dFc * rcp_newton(Fc * kLn10);
+            const double cc = -0.4 - 0.67 * lFc, n = 0.75 - 1.27 * lFc;
+            const double xx = fma(log2_pos(Pr), kLog10of2, cc);
+            const double rden = rcp_newton(n - 0.14 * xx);
+            const double f1 = xx * rden;
+            const double gg = rcp_newton(fma(f1, f1, 1.0));
+            double z[1] = {l2Fc * gg};
+            exp2_poly_n<1>(z);
+            LF *= z[0];
+            const double df1_dx = n * rden * rden, df1_dn = -xx * rden * rden;
+            const double dgg = -2.0 * f1 * gg * gg;
+            dlnF_dlnPr = lFc * dgg * df1_dx;
+            dlnF_dT = kLn10 * dlFc * fma(lFc * dgg, fma(df1_dx, -0.67, df1_dn * -1.27), gg);
+        }
+        mul = LF;
+        const double s = dlnL + dlnF_dlnPr;
+        g = LF * s * rcp_newton(M) * net;
+        dRdT = LF * fma(fma(s, kLn2 * (dy0 - q.dyf), dlnF_dT), net, dnet_dT);
+    }
+    return JacExt{mul, g, dRdT};
+}
+
+// dR/dT of a reaction without [M]
+template <class Mem> PYRO_HD double jac_plain_dRdT(const JacRxn &r, const PointT &pt, const Mem &mem) {
+    const JacRates q = jac_reaction_rates(r, pt, mem);
+    return kLn2 * (q.qf * q.dyf - q.qr * (q.dyf + q.ddG));
+}
+
+// e_k(T) of the energy rows (A.26)
+PYRO_HD double jac_species_energy(const EnergyRow &er, double T) {
+    const double *ec = T < er.t_mid ? er.lo : er.hi;
+    double ek = fma(ec[5], T, ec[4]);
+    ek = fma(ek, T, ec[3]);
+    ek = fma(ek, T, ec[2]);
+    ek = fma(ek, T, ec[1]);
+    return fma(ek, T, ec[0]);
+}
+// c_v,k(T) = de_k/dT (A.29)-(A.31)
+PYRO_HD double jac_species_cv(const EnergyRow &er, double T) {
+    const double *ec = T < er.t_mid ? er.lo : er.hi;
+    double cvk = fma(5.0 * ec[5], T, 4.0 * ec[4]);
+    cvk = fma(cvk, T, 3.0 * ec[3]);
+    cvk = fma(cvk, T, 2.0 * ec[2]);
+    return fma(cvk, T, ec[1]);
+}
+
+// The incidences [begin, end) of one column: column[sc_species] += sc_w * d  (pyro_jac_tables.h)
+template <class Tab, class Mem>
+PYRO_HD void jac_column_accumulate(const Tab &tab, uint32_t begin, uint32_t end, const PointT &pt, const Mem &mem) {
+#pragma unroll 1
+    for (uint32_t q = begin; q < end; ++q) {
+        const JacInc &e = tab.inc((int)q);
+        double y[1] = {arrhenius_log2(e.f[0], e.f[1], e.f[2], pt.L2T, pt.invT) +
+                       (((mem.ldG(e.gslot[3]) + mem.ldG(e.gslot[4])) + mem.ldG(e.gslot[5])) -
+                        ((mem.ldG(e.gslot[0]) + mem.ldG(e.gslot[1])) + mem.ldG(e.gslot[2])))};
+        const double others = mem.ldC(e.other[0]) * mem.ldC(e.other[1]);
+        const double m = e.coef * mem.ld_ext(e.mul);
+        exp2_poly_n<1>(y);
+        jac_scatter<PW>(mem, e.sc_species, e.sc_w, (m * y[0]) * others);
+    }
+}
+
 // The whole Jacobian of one point.
 //   load_y(k)               mass fraction of species k at this point
 //   store_J(i, k, v)        J_ik = dS_i/dY_k;  store_T(i, v)  dS_i/dT (called only if want_T)
@@ -95,13 +194,7 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
         ctot += C;
         mem.fill((uint32_t)k, C, species_log2E(c, pt.T, pt.L2T, pt.invT), species_log2E_dT(c, pt.T, pt.invT));
         if (mode == 1) {   // c_v = sum_k Y_k de_k/dT  (A.29)-(A.31), energy rows of pyro_tables.h
-            const EnergyRow &er = tab.energy(k);
-            const double *ec = pt.T < er.t_mid ? er.lo : er.hi;
-            double cvk = fma(5.0 * ec[5], pt.T, 4.0 * ec[4]);
-            cvk = fma(cvk, pt.T, 3.0 * ec[3]);
-            cvk = fma(cvk, pt.T, 2.0 * ec[2]);
-            cvk = fma(cvk, pt.T, ec[1]);
-            cv = fma(y, cvk, cv);
+            cv = fma(y, jac_species_cv(tab.energy(k), pt.T), cv);
         }
     }
     mem.fill((uint32_t)ns, 1.0, 0.0, 0.0);
@@ -111,53 +204,8 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
 #pragma unroll 1
     for (int x = 0; x < lay.n_ext; ++x) {
         const JacRxn &r = tab.rxn(lay.n_plain + x);
-        const JacRates q = jac_reaction_rates(r, pt, mem);
-        double M = r.eff_default * ctot;
-#pragma unroll 1
-        for (uint32_t e = r.eff_begin; e < r.eff_begin + r.eff_count; ++e) {
-            const EffEntry &en = tab.eff((int)e);
-            M = fma(en.delta, mem.ldC(en.species), M);
-        }
-        const double net = q.qf - q.qr;
-        const double dnet_dT = kLn2 * (q.qf * q.dyf - q.qr * (q.dyf + q.ddG));   // at fixed rate-coefficient multiplier
-        double mul, g, dRdT;
-        if (r.type == PYRO_THREE_BODY) {   // R = [M] (q_f - q_r)
-            mul = M;
-            g = net;
-            dRdT = M * dnet_dT;
-        } else {                           // R = L F (q_f - q_r), L = Pr/(1+Pr), Pr = k_0 [M]/k_inf
-            const RxnFall &fl = tab.rxn_fall((int)r.fall_index);
-            const double y0 = arrhenius_log2(fl.l[0], fl.l[1], fl.l[2], pt.L2T, pt.invT);
-            const double dy0 = arrhenius_log2_dT(fl.l[1], fl.l[2], pt.invT);
-            double e[4] = {y0 - q.yf, fl.troe_t3 * pt.T, fl.troe_t1 * pt.T, fl.troe_t2 * pt.invT};
-            exp2_poly_n<4>(e);
-            const double Pr = e[0] * M;
-            const double dlnL = rcp_newton(1.0 + Pr);   // d ln L / d ln Pr
-            double LF = Pr * dlnL, dlnF_dlnPr = 0.0, dlnF_dT = 0.0;
-            if (r.type == PYRO_FALLOFF_TROE) {
-                const double a3 = (1.0 - fl.troe_alpha) * e[1], a1 = fl.troe_alpha * e[2], a2 = fl.troe_has_t2 * e[3];
-                const double Fc = a3 + a1 + a2;
-                const double dFc = kLn2 * fma(fl.troe_t3, a3, fma(fl.troe_t1, a1, -fl.troe_t2 * pt.invT * pt.invT * a2));
-                const double l2Fc = log2_pos(Fc), lFc = l2Fc * kLog10of2;
-                const double dlFc = dFc * rcp_newton(Fc * kLn10);
-                const double cc = -0.4 - 0.67 * lFc, n = 0.75 - 1.27 * lFc;
-                const double xx = fma(log2_pos(Pr), kLog10of2, cc);
-                const double rden = rcp_newton(n - 0.14 * xx);
-                const double f1 = xx * rden;
-                const double gg = rcp_newton(fma(f1, f1, 1.0));
-                double z[1] = {l2Fc * gg};
-                exp2_poly_n<1>(z);
-                LF *= z[0];
-                const double df1_dx = n * rden * rden, df1_dn = -xx * rden * rden;
-                const double dgg = -2.0 * f1 * gg * gg;
-                dlnF_dlnPr = lFc * dgg * df1_dx;
-                dlnF_dT = kLn10 * dlFc * fma(lFc * dgg, fma(df1_dx, -0.67, df1_dn * -1.27), gg);
-            }
-            mul = LF;
-            const double s = dlnL + dlnF_dlnPr;
-            g = LF * s * rcp_newton(M) * net;
-            dRdT = LF * fma(fma(s, kLn2 * (dy0 - q.dyf), dlnF_dT), net, dnet_dT);
-        }
+        const JacExt x_ = jac_ext_reaction(tab, r, pt, ctot, mem);
+        const double mul = x_.mul, g = x_.g, dRdT = x_.dRdT;
         mem.st_ext(1u + 2u * r.ext, mul);
         mem.st_ext(2u + 2u * r.ext, g);
         jac_scatter<PDT>(mem, r.sc_species, r.sc_w, dRdT);
@@ -168,8 +216,7 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
 #pragma unroll 1
     for (int j = 0; j < lay.n_plain; ++j) {
         const JacRxn &r = tab.rxn(j);
-        const JacRates q = jac_reaction_rates(r, pt, mem);
-        jac_scatter<PDT>(mem, r.sc_species, r.sc_w, kLn2 * (q.qf * q.dyf - q.qr * (q.dyf + q.ddG)));
+        jac_scatter<PDT>(mem, r.sc_species, r.sc_w, jac_plain_dRdT(r, pt, mem));
     }
     mem.fence_st();
     if (want_T) {
@@ -186,30 +233,13 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
 #pragma unroll 1
     for (int k = 0; k < ns; ++k) {
         const JacCol &col = tab.col(k);
-#pragma unroll 1
-        for (uint32_t q = col.inc_begin; q < col.inc_end; ++q) {
-            const JacInc &e = tab.inc((int)q);
-            double y[1] = {arrhenius_log2(e.f[0], e.f[1], e.f[2], pt.L2T, pt.invT) +
-                           (((mem.ldG(e.gslot[3]) + mem.ldG(e.gslot[4])) + mem.ldG(e.gslot[5])) -
-                            ((mem.ldG(e.gslot[0]) + mem.ldG(e.gslot[1])) + mem.ldG(e.gslot[2])))};
-            const double others = mem.ldC(e.other[0]) * mem.ldC(e.other[1]);
-            const double m = e.coef * mem.ld_ext(e.mul);
-            exp2_poly_n<1>(y);
-            jac_scatter<PW>(mem, e.sc_species, e.sc_w, (m * y[0]) * others);
-        }
+        jac_column_accumulate(tab, col.inc_begin, col.inc_end, pt, mem);
         mem.fence_st();
         // J_ik = (column_i + V_i) rho/W_k - dS_i/dT e_k/c_v ; the column accumulator is cleared for the next one
         const double scale = rho * tab.spec(k).inv_w;
         double ekcv = 0.0;
         if (mode == 1) {
-            const EnergyRow &er = tab.energy(k);
-            const double *ec = pt.T < er.t_mid ? er.lo : er.hi;
-            double ek = fma(ec[5], pt.T, ec[4]);
-            ek = fma(ek, pt.T, ec[3]);
-            ek = fma(ek, pt.T, ec[2]);
-            ek = fma(ek, pt.T, ec[1]);
-            ek = fma(ek, pt.T, ec[0]);
-            ekcv = ek * rcv;
+            ekcv = jac_species_energy(tab.energy(k), pt.T) * rcv;
         }
 #pragma unroll 1
         for (int i = 0; i < ns; i += 4) {   // four rows in flight per tensor-memory round trip
