@@ -15,10 +15,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 OBJ = os.path.join(_HERE, "build")
 LIB = os.path.join(_HERE, "libpyro.so")
-SOURCES = ["pyro_kernels.cu", "pyro_fused_kernels.cu", "pyro_rates2_kernels.cu", "pyro_jac_kernels.cu", "pyro_reactor_kernels.cu", "pyro_transport.cu", "pyro_probes.cu", "pyro_cn_kernels.cu", "pyro_api.cpp", "pyro_pack.cpp",
+SOURCES = ["pyro_kernels.cu", "pyro_fused_kernels.cu", "pyro_rates2_kernels.cu", "pyro_jac_kernels.cu", "pyro_jac_block_kernels.cu", "pyro_reactor_kernels.cu", "pyro_transport.cu", "pyro_probes.cu", "pyro_cn_kernels.cu", "pyro_api.cpp", "pyro_pack.cpp",
            "pyro_jac_pack.cpp"]
 HEADERS = ["pyro_kernels.h", "pyro_pack.h", "pyro_tables.h", "pyro_math.cuh", "pyro_point.cuh", "pyro_rates_kernel.cuh",
-           "pyro_jac.cuh", "pyro_jac_tables.h", os.path.join("..", "..", "include", "pyro.h")]
+           "pyro_jac.cuh", "pyro_jac_dev.cuh", "pyro_jac_tables.h", os.path.join("..", "..", "include", "pyro.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",
               "-Xptxas", "-v"]
 

@@ -105,6 +105,10 @@ struct pyro_mech {
     int jac_threads = 0, jac_blocks_per_sm = 0;
     size_t jac_smem = 0;
     uint32_t jac_planes_bytes = 0;
+    // block-cooperative Jacobian kernel (pyro_jac_block_kernels.cu): 0 = not used, else warps per block
+    int jac_block_warps = 0;
+    size_t jac_block_smem = 0;
+    uint32_t jac_block_planes_bytes = 0, jac_block_tmem_cols = 32;
     uint32_t jac_tmem_cols = 32;
     mutable std::mutex jac_mu;
     cudaEvent_t jac_done = nullptr;   // launches on one handle share the scratch: each waits for the one before
@@ -472,6 +476,31 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
             if (!std::strcmp(env, "shared")) m->jac_small = false;
         }
         const size_t planes = m->jac_small ? 3 : 4;
+        // The block-cooperative kernel (NW warps on one chunk of 32 points, planes once per chunk) when its shared
+        // memory fits: 5 planes + the [M] scratch + 2 NW reduction rows of 32 doubles, and NW record rings.
+        // (not for small mechanisms: with fewer columns than warps most of the block idles; measured at 9 species:
+        // 4.8 against 2.2 ns per point)
+        for (int nw : {16, 8}) {
+            if (lay.n_species < 24 && !std::getenv("PYRO_JAC_KERNEL")) break;
+            if (2 * rows * (size_t)(nw / 4) > 512) continue;
+            const size_t pl = (5 * rows + 1 + 2 * (size_t)jl.n_ext + 2 * (size_t)nw + 8 * (size_t)nw) * 32 * sizeof(double);   // + reduction scratch
+            const size_t need = pl + (size_t)nw * pyro::kJacBlockRingBytes;
+            cudaFuncAttributes fb{};
+            const void *bfn = pyro::jacobian_block_kernel_ptr(nw);
+            if ((ce = cudaFuncGetAttributes(&fb, bfn)) != cudaSuccess) return bail(ce, "cudaFuncGetAttributes(jacobian block)");
+            if (need + fb.sharedSizeBytes > (size_t)prop.sharedMemPerBlockOptin) continue;
+            if ((ce = cudaFuncSetAttribute(bfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)prop.sharedMemPerBlockOptin - fb.sharedSizeBytes))) != cudaSuccess)
+                return bail(ce, "cudaFuncSetAttribute(jacobian block)");
+            m->jac_block_warps = nw;
+            m->jac_block_smem = need;
+            m->jac_block_planes_bytes = (uint32_t)pl;
+            m->jac_block_tmem_cols = 32;
+            while (m->jac_block_tmem_cols < 2 * rows * (size_t)(nw / 4)) m->jac_block_tmem_cols *= 2;
+            break;
+        }
+        if (const char *env = std::getenv("PYRO_JAC_KERNEL")) {
+            if (!std::strcmp(env, "point")) m->jac_block_warps = 0;   // "block": also for small mechanisms (tests)
+        }
         cudaFuncAttributes fa{};
         const void *jfn = pyro::jacobian_kernel_ptr(m->jac_small);
         if ((ce = cudaFuncGetAttributes(&fa, jfn)) != cudaSuccess) return bail(ce, "cudaFuncGetAttributes(jacobian)");
@@ -737,7 +766,15 @@ int jacobian_call(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, 
     }
     PYRO_CUDA(cudaStreamWaitEvent(stream, m->jac_done, 0));   // the scratch is shared by the launches of one handle
     PYRO_CUDA(cudaMemsetAsync(a.work, 0, sizeof(unsigned long long), stream));
-    PYRO_CUDA(pyro::launch_jacobian(a, m->jac_small, m->jac_threads, (int)blocks, m->jac_smem, stream));
+    if (m->jac_block_warps) {
+        a.tmem_cols = m->jac_block_tmem_cols;
+        a.planes_bytes = m->jac_block_planes_bytes;
+        int64_t bb = m->sm_count;
+        if (bb > a.n_chunks) bb = a.n_chunks;
+        PYRO_CUDA(pyro::launch_jacobian_block(a, m->jac_block_warps, (int)bb, m->jac_block_smem, stream));
+    } else {
+        PYRO_CUDA(pyro::launch_jacobian(a, m->jac_small, m->jac_threads, (int)blocks, m->jac_smem, stream));
+    }
     PYRO_CUDA(cudaEventRecord(m->jac_done, stream));
     {
         std::lock_guard<std::mutex> wl(m->work_mu);

@@ -1,5 +1,6 @@
 // Packer of the chemical-Jacobian tables (pyro_jac_tables.h): transposes a validated mechanism into per-species
 // incidence lists.  Called by pyro_mech_create after pack_mechanism has accepted the description.
+#include <algorithm>
 #include <cmath>
 #include <cstring>
 #include <map>
@@ -148,6 +149,14 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
     off = align16j(off + (uint32_t)(falls.size() * sizeof(RxnFall)));
     lay.off_col = off;
     off = align16j(off + (uint32_t)(cols.size() * sizeof(JacCol)));
+    // the columns by decreasing list length: the block kernel hands them to its warps in this order (longest first)
+    std::vector<uint32_t> order(ns);
+    for (int k = 0; k < ns; ++k) order[k] = (uint32_t)k;
+    std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) {
+        return cols[x].inc_end - cols[x].inc_begin > cols[y].inc_end - cols[y].inc_begin;
+    });
+    lay.off_order = off;
+    off = align16j(off + (uint32_t)(order.size() * sizeof(uint32_t)));
     lay.bytes = off;
     out.blob.assign(off, 0);
     auto put = [&](uint32_t at, const void *src, size_t bytes) {
@@ -158,6 +167,7 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
     put(lay.off_eff, effs.data(), effs.size() * sizeof(EffEntry));
     put(lay.off_fall, falls.data(), falls.size() * sizeof(RxnFall));
     put(lay.off_col, cols.data(), cols.size() * sizeof(JacCol));
+    put(lay.off_order, order.data(), order.size() * sizeof(uint32_t));
     return PYRO_OK;
 }
 

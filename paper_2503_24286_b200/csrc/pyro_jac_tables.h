@@ -64,7 +64,7 @@ struct alignas(16) JacCol {
 };
 
 struct JacLayout {
-    uint32_t off_rxn, off_inc, off_eff, off_fall, off_col, bytes;
+    uint32_t off_rxn, off_inc, off_eff, off_fall, off_col, off_order, bytes;   // off_order: uint32[n_species], the columns by decreasing list length
     int32_t n_species, n_plain, n_ext, n_inc, n_eff, n_fall;
 };
 

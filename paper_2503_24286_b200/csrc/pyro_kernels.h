@@ -104,6 +104,9 @@ struct JacArgs {                 // chemical Jacobian (pyro_jac_tables.h)
     JacLayout lay;
 };
 
+constexpr size_t kJacBlockRingBytes = 4096;   // block kernel: per warp two segments of 16 records of up to 128 bytes
+const void *jacobian_block_kernel_ptr(int warps);   // 16 or 8 warps on one chunk of 32 points (pyro_jac_block_kernels.cu)
+cudaError_t launch_jacobian_block(const JacArgs &a, int warps, int blocks, size_t smem_bytes, cudaStream_t stream);
 const void *jacobian_kernel_ptr(bool small);
 cudaError_t launch_jacobian(const JacArgs &a, bool small, int threads, int blocks, size_t smem_bytes, cudaStream_t stream);
 

@@ -508,12 +508,13 @@ def test_jacobian_hand_mechanism_padded_ld_and_no_dSdT():
 
 
 def test_jacobian_v_plane_in_shared_memory_and_small_blocks(mechs, monkeypatch):
-    """The large-mechanism layout (V in shared memory, 4 tensor-memory columns per species) forced on configs[0],
-    and 32-thread blocks."""
+    """The one-thread-per-point kernel (the fallback of the block-cooperative one), its large-mechanism layout (V in
+    shared memory, 4 tensor-memory columns per species) forced on configs[0], and 32-thread blocks."""
     mech, _, orc = mechs(0)
     st = inputs.config_states(0, n=700)
     Jr, sTr, bJ, bT = orc.get_jacobian(st["rho"], st["T"], st["Y"], mode=0)
-    for env in ({"PYRO_JAC_V_PLANE": "shared"}, {"PYRO_JAC_BLOCK": "32"}):
+    for env in ({"PYRO_JAC_KERNEL": "block"}, {"PYRO_JAC_KERNEL": "point"}, {"PYRO_JAC_KERNEL": "point", "PYRO_JAC_V_PLANE": "shared"},
+                {"PYRO_JAC_KERNEL": "point", "PYRO_JAC_BLOCK": "32"}):
         for k, v in env.items():
             monkeypatch.setenv(k, v)
         gm = binding.Mechanism(mech)
