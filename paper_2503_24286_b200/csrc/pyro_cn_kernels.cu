@@ -8,6 +8,8 @@
 // counted in n_not_converged.
 #include <cuda_runtime.h>
 
+#include <cstdlib>
+
 #include "pyro_kernels.h"
 
 namespace pyro {
@@ -29,13 +31,45 @@ __global__ void __launch_bounds__(256) cn_begin_step_kernel(const CnArgs a) {
 // Left-looking LU in panels of NC columns.  A panel lives in shared memory as [column][row][thread] (conflict-free);
 // the factors already computed (columns left of the panel) are read from global memory once per panel -- one global
 // read serves NC multiply-adds, against three global accesses per multiply-add for the textbook in-place elimination
-// (measured at 53 species: 440 ns per solve in global memory).  Threads never touch one another's data: no barrier.
-#ifndef PYRO_CN_IN_FLIGHT
-#define PYRO_CN_IN_FLIGHT 8
-#endif
-constexpr int kCnInFlight = PYRO_CN_IN_FLIGHT;
+// (measured at 53 species: 440 ns per solve in global memory).  The right-hand side -F rides along as column n_s of the
+// matrix, so the forward substitution is the elimination of that column and reads nothing of its own.
+// Threads never touch one another's data: no barrier.
+//
+// Every global read of the factorisation has an address known in advance, and the kernel is bound by the latency of
+// these reads (first version, eight plain loads in flight per thread: issue 4 %, long scoreboard 72 %).  So they
+// stream through a per-thread ring in shared memory, filled by cp.async kCnGroups groups of kCnBatch elements ahead of
+// their use; the consumer waits once per group and then has kCnBatch x NC independent multiply-adds.
+constexpr int kCnBatch = 4;    // elements per cp.async group
+constexpr int kCnGroups = 8;   // groups requested ahead (a power of two)
+constexpr int kCnRing = kCnBatch * kCnGroups;
+
+template <int TB> struct CnRing {
+    uint32_t base;   // shared-memory byte address of this thread's element 0
+    int issued, taken;
+    __device__ __forceinline__ uint32_t at(int group, int e) const {
+        return base + (uint32_t)((group & (kCnGroups - 1)) * kCnBatch + e) * (TB * 8u);
+    }
+    __device__ __forceinline__ void request(int e, const double *src) const {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(at(issued, e)), "l"(src) : "memory");
+    }
+    __device__ __forceinline__ void commit() {   // one group per batch, empty past the end of the stream
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        ++issued;
+    }
+    __device__ __forceinline__ void wait_front() const { asm volatile("cp.async.wait_group %0;" ::"n"(kCnGroups - 1) : "memory"); }
+    __device__ __forceinline__ double take(int e) const {
+        double v;
+        asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(at(taken, e)));
+        return v;
+    }
+    __device__ __forceinline__ void drain() {
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        issued = taken = 0;
+    }
+};
+
 template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel(const CnArgs a) {
-    extern __shared__ double cn_cols[];   // [NC][n_species][TB]
+    extern __shared__ double cn_cols[];   // [NC][n_species][TB], then the ring [kCnRing][TB]
     const int tid = threadIdx.x;
     const int64_t p = (int64_t)blockIdx.x * TB + tid;
     if (p >= a.n) return;
@@ -46,76 +80,183 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
     const double inv_rho = 1.0 / a.rho[p], half = 0.5 * a.dt, c = half * inv_rho;
     auto S = [&](int col, int i) -> double & { return cn_cols[((size_t)col * ns + i) * TB + tid]; };
     auto G = [&](int i, int k) -> double & { return A[((int64_t)i * ns + k) * TB]; };
-    for (int j0 = 0; j0 < ns; j0 += NC) {
-        const int nc = ns - j0 < NC ? ns - j0 : NC;
+    const int64_t row_step = (int64_t)ns * TB;
+    CnRing<TB> ring{(uint32_t)__cvta_generic_to_shared(cn_cols + (size_t)NC * ns * TB) + 8u * (uint32_t)tid, 0, 0};
+
+    int rhs_col = 0;
+    for (int j0 = 0; j0 <= ns; j0 += NC) {   // columns 0 .. n_s - 1 of the matrix, column n_s = the right-hand side
+        // the panel: J straight into its place (all reads in flight at once), then A = I - c J in place
         for (int i = 0; i < ns; ++i)
 #pragma unroll
-            for (int cc = 0; cc < NC; ++cc) S(cc, i) = cc < nc ? (i == j0 + cc ? 1.0 : 0.0) - c * G(i, j0 + cc) : 0.0;
-        for (int k = 0; k < j0; ++k) {   // eliminations of the columns left of the panel
+            for (int cc = 0; cc < NC; ++cc)
+                if (j0 + cc < ns)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(&S(cc, i))), "l"(&G(i, j0 + cc)) : "memory");
+        // the factors left of the panel, L(i, k), k < j0, i > k: column after column, each in batches of kCnBatch rows
+        int gk = 0, gi = 1;
+        const double *gp = &G(1, 0);   // &G(gi, gk); a row further is row_step doubles on
+        auto request = [&]() {
+            if (gk < j0) {
+#pragma unroll
+                for (int e = 0; e < kCnBatch; ++e)
+                    if (gi + e < ns) ring.request(e, gp + e * row_step);
+                gi += kCnBatch;
+                gp += kCnBatch * row_step;
+                if (gi >= ns) {
+                    ++gk;
+                    gi = gk + 1;
+                    gp = &G(gi, gk);
+                }
+            }
+            ring.commit();
+        };
+        asm volatile("cp.async.commit_group;" ::: "memory");
+#pragma unroll 1
+        for (int u = 0; u < kCnGroups; ++u) request();
+        asm volatile("cp.async.wait_group %0;" ::"n"(kCnGroups) : "memory");   // the panel has landed
+        for (int i = 0; i < ns; ++i) {
+#pragma unroll
+            for (int cc = 0; cc < NC; ++cc) {
+                const int j = j0 + cc;
+                double v = 0.0;
+                if (j < ns) v = (i == j ? 1.0 : 0.0) - c * S(cc, i);
+                else if (j == ns) {
+                    const int64_t at = (int64_t)i * ld + p;
+                    v = -(a.Y[at] - a.Ym[at] - half * fma(a.energy[i].w * inv_rho, a.omega[at], a.Sm[at]));
+                    rhs_col = cc;
+                }
+                S(cc, i) = v;
+            }
+        }
+#pragma unroll 1
+        for (int k = 0; k < j0; ++k) {
             double ck[NC];
 #pragma unroll
             for (int cc = 0; cc < NC; ++cc) ck[cc] = S(cc, k);
-            // kCnInFlight factors in flight: with four warps per SM the loop is bound by the latency of these global reads
-            int i = k + 1;
-            for (; i + kCnInFlight <= ns; i += kCnInFlight) {
-                double l[kCnInFlight];
+            // loads first, then the multiply-adds, then the stores: written out, because the compiler cannot tell that
+            // the columns of the panel do not overlap and would otherwise wait for every load in turn
+            int i0 = k + 1;
+#pragma unroll 1
+            for (; i0 + kCnBatch <= ns; i0 += kCnBatch) {
+                ring.wait_front();
+                double l[kCnBatch], v[kCnBatch][NC];
 #pragma unroll
-                for (int u = 0; u < kCnInFlight; ++u) l[u] = G(i + u, k);
+                for (int e = 0; e < kCnBatch; ++e) l[e] = ring.take(e);
+                ++ring.taken;
 #pragma unroll
-                for (int u = 0; u < kCnInFlight; ++u)
+                for (int e = 0; e < kCnBatch; ++e)
 #pragma unroll
-                    for (int cc = 0; cc < NC; ++cc) S(cc, i + u) = fma(-l[u], ck[cc], S(cc, i + u));
+                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = S(cc, i0 + e);
+                request();
+#pragma unroll
+                for (int e = 0; e < kCnBatch; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = fma(-l[e], ck[cc], v[e][cc]);
+#pragma unroll
+                for (int e = 0; e < kCnBatch; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc) S(cc, i0 + e) = v[e][cc];
             }
-            for (; i < ns; ++i) {
-                const double l = G(i, k);
+            if (i0 < ns) {   // the ragged end of the column
+                ring.wait_front();
+                double l[kCnBatch], v[kCnBatch][NC];
 #pragma unroll
-                for (int cc = 0; cc < NC; ++cc) S(cc, i) = fma(-l, ck[cc], S(cc, i));
+                for (int e = 0; e < kCnBatch - 1; ++e) l[e] = i0 + e < ns ? ring.take(e) : 0.0;
+                ++ring.taken;
+#pragma unroll
+                for (int e = 0; e < kCnBatch - 1; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = i0 + e < ns ? S(cc, i0 + e) : 0.0;
+                request();
+#pragma unroll
+                for (int e = 0; e < kCnBatch - 1; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc)
+                        if (i0 + e < ns) S(cc, i0 + e) = fma(-l[e], ck[cc], v[e][cc]);
             }
         }
-        for (int jj = 0; jj < nc; ++jj) {   // the panel itself
+        ring.drain();
+        for (int jj = 0; jj < NC; ++jj) {   // the panel itself
             const int j = j0 + jj;
+            if (j > ns) break;
             for (int kk = 0; kk < jj; ++kk) {
                 const int k = j0 + kk;
                 const double ck = S(jj, k);
-                for (int i = k + 1; i < ns; ++i) S(jj, i) = fma(-S(kk, i), ck, S(jj, i));
+                int i = k + 1;
+                for (; i + 4 <= ns; i += 4) {
+                    double x[4], y[4];
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) x[e] = S(kk, i + e), y[e] = S(jj, i + e);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) S(jj, i + e) = fma(-x[e], ck, y[e]);
+                }
+                for (; i < ns; ++i) S(jj, i) = fma(-S(kk, i), ck, S(jj, i));
             }
-            const double piv = 1.0 / S(jj, j);
-            for (int i = j + 1; i < ns; ++i) S(jj, i) *= piv;
+            if (j < ns) {
+                const double piv = 1.0 / S(jj, j);
+                for (int i = j + 1; i < ns; ++i) S(jj, i) *= piv;
+            }
         }
         for (int i = 0; i < ns; ++i)
 #pragma unroll
             for (int cc = 0; cc < NC; ++cc)
-                if (cc < nc) G(i, j0 + cc) = S(cc, i);
+                if (j0 + cc < ns) G(i, j0 + cc) = S(cc, i);
     }
-    // right-hand side in column 0 of the panel store: forward substitution with L, back substitution with U
-    for (int i = 0; i < ns; ++i) {
-        const int64_t at = (int64_t)i * ld + p;
-        S(0, i) = -(a.Y[at] - a.Ym[at] - half * fma(a.energy[i].w * inv_rho, a.omega[at], a.Sm[at]));
+    // back substitution with U, row after row from the last: the diagonal element first, then the row right of it.
+    // y = L^-1 (-F) is in column rhs_col of the panel store; x overwrites it.
+    {
+        int gr = ns - 1, gj = ns - 1;
+        auto request = [&]() {
+            if (gr >= 0) {
+#pragma unroll
+                for (int e = 0; e < kCnBatch; ++e)
+                    if (gj + e < ns) ring.request(e, &G(gr, gj + e));
+                gj += kCnBatch;
+                if (gj >= ns) {
+                    --gr;
+                    gj = gr;
+                }
+            }
+            ring.commit();
+        };
+#pragma unroll 1
+        for (int u = 0; u < kCnGroups; ++u) request();
+        double worst = 0.0;
+        bool finite = true;
+#pragma unroll 1
+        for (int r = ns - 1; r >= 0; --r) {
+            double s = S(rhs_col, r), diag = 1.0;
+#pragma unroll 1
+            for (int j0 = r; j0 < ns; j0 += kCnBatch) {
+                ring.wait_front();
+                double u[kCnBatch];
+#pragma unroll
+                for (int e = 0; e < kCnBatch; ++e) u[e] = j0 + e < ns ? ring.take(e) : 0.0;
+                ++ring.taken;
+                request();
+#pragma unroll
+                for (int e = 0; e < kCnBatch; ++e) {
+                    if (j0 + e == r) diag = u[e];
+                    else if (j0 + e < ns) s = fma(-u[e], S(rhs_col, j0 + e), s);
+                }
+            }
+            s /= diag;
+            S(rhs_col, r) = s;
+            b[(int64_t)r * ld] = s;
+            a.Y[(int64_t)r * ld + p] += s;
+            worst = fmax(worst, fabs(s));
+            finite = finite && (s == s) && fabs(s) <= 1.7976931348623157e308;
+        }
+        ring.drain();
+        if (a.last_update) a.last_update[p] = worst;
+        if (a.count_unconverged && a.n_not_converged && (!finite || !(worst < a.update_tol))) atomicAdd(a.n_not_converged, 1);
     }
-    for (int k = 0; k < ns; ++k) {
-        const double bk = S(0, k);
-#pragma unroll 4
-        for (int i = k + 1; i < ns; ++i) S(0, i) = fma(-G(i, k), bk, S(0, i));
-    }
-    double worst = 0.0;
-    bool finite = true;
-    for (int r = ns - 1; r >= 0; --r) {
-        double s = S(0, r);
-#pragma unroll 4
-        for (int j = r + 1; j < ns; ++j) s = fma(-G(r, j), S(0, j), s);
-        s /= G(r, r);
-        S(0, r) = s;
-        b[(int64_t)r * ld] = s;
-        a.Y[(int64_t)r * ld + p] += s;
-        worst = fmax(worst, fabs(s));
-        finite = finite && (s == s) && fabs(s) <= 1.7976931348623157e308;
-    }
-    if (a.last_update) a.last_update[p] = worst;
-    if (a.count_unconverged && a.n_not_converged && (!finite || !(worst < a.update_tol))) atomicAdd(a.n_not_converged, 1);
 }
 
 constexpr int kCnPanel = 4;
-int cn_block_threads(int n_species) { return (size_t)kCnPanel * n_species * 64 * sizeof(double) <= 200 * 1024 ? 64 : 32; }
+int cn_block_threads(int n_species) {
+    if (const char *env = std::getenv("PYRO_CN_BLOCK")) return std::atoi(env) == 64 ? 64 : 32;
+    return 32;   // measured at 53 species: 271 ns per reactor-iteration against 300 with 64 (more blocks, more loads in flight)
+}
 
 cudaError_t launch_cn_begin_step(const CnArgs &a, cudaStream_t stream) {
     cn_begin_step_kernel<<<dim3((unsigned)((a.n + 255) / 256)), dim3(256), 0, stream>>>(a);
@@ -123,7 +264,7 @@ cudaError_t launch_cn_begin_step(const CnArgs &a, cudaStream_t stream) {
 }
 cudaError_t launch_cn_newton(const CnArgs &a, cudaStream_t stream) {
     const int tb = cn_block_threads(a.n_species);
-    const size_t smem = (size_t)kCnPanel * a.n_species * tb * sizeof(double);
+    const size_t smem = ((size_t)kCnPanel * a.n_species + kCnRing) * tb * sizeof(double);
     // the limit is a property of the function on the current device: set it on every launch (cheap; no process-wide state)
     const void *fn = tb == 64 ? (const void *)cn_newton_kernel<kCnPanel, 64> : (const void *)cn_newton_kernel<kCnPanel, 32>;
     cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
