@@ -39,7 +39,8 @@ __global__ void __launch_bounds__(256) cn_begin_step_kernel(const CnArgs a) {
 // these reads (first version, eight plain loads in flight per thread: issue 4 %, long scoreboard 72 %).  So they
 // stream through a per-thread ring in shared memory, filled by cp.async kCnGroups groups of kCnBatch elements ahead of
 // their use; the consumer waits once per group and then has kCnBatch x NC independent multiply-adds.
-constexpr int kCnBatch = 4;    // elements per cp.async group
+constexpr int kCnRows = 4;               // rows of two columns per cp.async group
+constexpr int kCnBatch = 2 * kCnRows;    // elements per cp.async group
 constexpr int kCnGroups = 8;   // groups requested ahead (a power of two)
 constexpr int kCnRing = kCnBatch * kCnGroups;
 
@@ -69,6 +70,7 @@ template <int TB> struct CnRing {
 };
 
 template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel(const CnArgs a) {
+    static_assert(NC % 2 == 0, "the eliminations left of a panel go by pairs of columns");
     extern __shared__ double cn_cols[];   // [NC][n_species][TB], then the ring [kCnRing][TB]
     const int tid = threadIdx.x;
     const int64_t p = (int64_t)blockIdx.x * TB + tid;
@@ -91,18 +93,29 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
             for (int cc = 0; cc < NC; ++cc)
                 if (j0 + cc < ns)
                     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(&S(cc, i))), "l"(&G(i, j0 + cc)) : "memory");
-        // the factors left of the panel, L(i, k), k < j0, i > k: column after column, each in batches of kCnBatch rows
+        // The factors left of the panel, L(i, k), k < j0, i > k, two columns (k, k + 1) at a time, so that an element of
+        // the panel is read and written once for two multiply-adds.  Order of the stream: L(k + 1, k) in a group of its
+        // own, then the rows i >= k + 2 in groups of kCnRows rows: L(i, k), L(i, k + 1), L(i + 1, k), ...
         int gk = 0, gi = 1;
-        const double *gp = &G(1, 0);   // &G(gi, gk); a row further is row_step doubles on
+        const double *gp = &G(1, 0);   // &G(gi, gk); a row further is row_step doubles on, a column further TB
         auto request = [&]() {
             if (gk < j0) {
+                if (gi == gk + 1) {
+                    ring.request(0, gp);
+                    gi += 1;
+                    gp += row_step;
+                } else {
 #pragma unroll
-                for (int e = 0; e < kCnBatch; ++e)
-                    if (gi + e < ns) ring.request(e, gp + e * row_step);
-                gi += kCnBatch;
-                gp += kCnBatch * row_step;
+                    for (int e = 0; e < kCnRows; ++e)
+                        if (gi + e < ns) {
+                            ring.request(2 * e, gp + e * row_step);
+                            ring.request(2 * e + 1, gp + e * row_step + TB);
+                        }
+                    gi += kCnRows;
+                    gp += kCnRows * row_step;
+                }
                 if (gi >= ns) {
-                    ++gk;
+                    gk += 2;
                     gi = gk + 1;
                     gp = &G(gi, gk);
                 }
@@ -115,63 +128,74 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
         asm volatile("cp.async.wait_group %0;" ::"n"(kCnGroups) : "memory");   // the panel has landed
         for (int i = 0; i < ns; ++i) {
 #pragma unroll
-            for (int cc = 0; cc < NC; ++cc) {
-                const int j = j0 + cc;
-                double v = 0.0;
-                if (j < ns) v = (i == j ? 1.0 : 0.0) - c * S(cc, i);
-                else if (j == ns) {
-                    const int64_t at = (int64_t)i * ld + p;
-                    v = -(a.Y[at] - a.Ym[at] - half * fma(a.energy[i].w * inv_rho, a.omega[at], a.Sm[at]));
-                    rhs_col = cc;
-                }
-                S(cc, i) = v;
+            for (int cc = 0; cc < NC; ++cc) S(cc, i) = j0 + cc < ns ? (i == j0 + cc ? 1.0 : 0.0) - c * S(cc, i) : 0.0;
+        }
+        if (j0 + NC > ns) {   // the last panel: the right-hand side -F behind the last column of the matrix
+            rhs_col = ns - j0;
+            for (int i = 0; i < ns; ++i) {
+                const int64_t at = (int64_t)i * ld + p;
+                S(rhs_col, i) = -(a.Y[at] - a.Ym[at] - half * fma(a.energy[i].w * inv_rho, a.omega[at], a.Sm[at]));
             }
         }
 #pragma unroll 1
-        for (int k = 0; k < j0; ++k) {
-            double ck[NC];
+        for (int k = 0; k < j0; k += 2) {   // j0 is a multiple of NC, NC is even
+            double ck[NC], ck1[NC];
+            ring.wait_front();
+            {
+                const double l0 = ring.take(0);
+                ++ring.taken;
+                request();
 #pragma unroll
-            for (int cc = 0; cc < NC; ++cc) ck[cc] = S(cc, k);
+                for (int cc = 0; cc < NC; ++cc) {
+                    ck[cc] = S(cc, k);
+                    ck1[cc] = fma(-l0, ck[cc], S(cc, k + 1));
+                    S(cc, k + 1) = ck1[cc];
+                }
+            }
             // loads first, then the multiply-adds, then the stores: written out, because the compiler cannot tell that
             // the columns of the panel do not overlap and would otherwise wait for every load in turn
-            int i0 = k + 1;
+            int i0 = k + 2;
 #pragma unroll 1
-            for (; i0 + kCnBatch <= ns; i0 += kCnBatch) {
+            for (; i0 + kCnRows <= ns; i0 += kCnRows) {
                 ring.wait_front();
-                double l[kCnBatch], v[kCnBatch][NC];
+                double l[kCnRows], l1[kCnRows], v[kCnRows][NC];
 #pragma unroll
-                for (int e = 0; e < kCnBatch; ++e) l[e] = ring.take(e);
+                for (int e = 0; e < kCnRows; ++e) l[e] = ring.take(2 * e), l1[e] = ring.take(2 * e + 1);
                 ++ring.taken;
 #pragma unroll
-                for (int e = 0; e < kCnBatch; ++e)
+                for (int e = 0; e < kCnRows; ++e)
 #pragma unroll
                     for (int cc = 0; cc < NC; ++cc) v[e][cc] = S(cc, i0 + e);
                 request();
 #pragma unroll
-                for (int e = 0; e < kCnBatch; ++e)
+                for (int e = 0; e < kCnRows; ++e)
 #pragma unroll
-                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = fma(-l[e], ck[cc], v[e][cc]);
+                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = fma(-l1[e], ck1[cc], fma(-l[e], ck[cc], v[e][cc]));
 #pragma unroll
-                for (int e = 0; e < kCnBatch; ++e)
+                for (int e = 0; e < kCnRows; ++e)
 #pragma unroll
                     for (int cc = 0; cc < NC; ++cc) S(cc, i0 + e) = v[e][cc];
             }
-            if (i0 < ns) {   // the ragged end of the column
+            if (i0 < ns) {   // the ragged end of the two columns
                 ring.wait_front();
-                double l[kCnBatch], v[kCnBatch][NC];
+                double l[kCnRows], l1[kCnRows], v[kCnRows][NC];
 #pragma unroll
-                for (int e = 0; e < kCnBatch - 1; ++e) l[e] = i0 + e < ns ? ring.take(e) : 0.0;
+                for (int e = 0; e < kCnRows - 1; ++e) {
+                    const bool in = i0 + e < ns;
+                    l[e] = in ? ring.take(2 * e) : 0.0;
+                    l1[e] = in ? ring.take(2 * e + 1) : 0.0;
+                }
                 ++ring.taken;
 #pragma unroll
-                for (int e = 0; e < kCnBatch - 1; ++e)
+                for (int e = 0; e < kCnRows - 1; ++e)
 #pragma unroll
                     for (int cc = 0; cc < NC; ++cc) v[e][cc] = i0 + e < ns ? S(cc, i0 + e) : 0.0;
                 request();
 #pragma unroll
-                for (int e = 0; e < kCnBatch - 1; ++e)
+                for (int e = 0; e < kCnRows - 1; ++e)
 #pragma unroll
                     for (int cc = 0; cc < NC; ++cc)
-                        if (i0 + e < ns) S(cc, i0 + e) = fma(-l[e], ck[cc], v[e][cc]);
+                        if (i0 + e < ns) S(cc, i0 + e) = fma(-l1[e], ck1[cc], fma(-l[e], ck[cc], v[e][cc]));
             }
         }
         ring.drain();
