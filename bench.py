@@ -251,14 +251,14 @@ def time_widened_rows(gm, mech, cfg, d, T, stream, device):
                 T_c.copy_(d["T_guess"][:nc])
                 gm.reactor_cn(rho_c, e_c, Y_c, T_c, 10.0 * dt, 1, newton_iters=iters, stream=stream)
             ms, mn = _event_times(cn, stream, 3, warm=1)
-            lu_bytes = 8.0 * (ns ** 3 / 12.0 + 3.0 * ns * ns)   # panel LU: one factor read per four multiply-adds + panel load/store + substitution
+            lu_bytes = 8.0 * (ns ** 3 / 12.0 + 2.5 * ns * ns)   # panel LU: one factor read per four multiply-adds + panel load/store + back substitution
             out["next4_reactor_cn"] = {
                 "reactors": nc, "steps": 1, "newton_iters": iters, "dt": 10.0 * dt, "ms": ms, "ms_min": mn,
                 "ns_per_reactor_iteration": ms * 1e6 / nc / iters,
                 "finite_fraction": float(torch.isfinite(Y_c).all(dim=0).float().mean().item()),
                 "roofline": {"bound": "hbm", "achieved": lu_bytes * nc * iters / (ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                              "frac": lu_bytes * nc * iters / (ms * 1e-3) / 1e9 / hbm_peak,
-                             "note": "the per-point panel LU dominates; bytes = factor reads of the left-looking LU as written (ns^3/12 + 3 ns^2 doubles per solve); compulsory traffic is 16 ns^2 bytes"}}
+                             "note": "the per-point panel LU dominates; bytes = factor reads of the left-looking LU as written (ns^3/12 + 2.5 ns^2 doubles per solve); compulsory traffic is 16 ns^2 bytes"}}
         except binding.PyroError as ex:
             out["next4_reactor_cn"] = {"unavailable": str(ex)}
     return out

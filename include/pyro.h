@@ -24,7 +24,7 @@
  *   the interface and change no result: PYRO_TABLES=shared|global, PYRO_RATES_BLOCK=<threads>,
  *   PYRO_B_PLANE=shared, PYRO_CARVEOUT=<percent>, PYRO_RATES_POINTS=2 (two grid points per thread), PYRO_RATES_TWO_BLOCKS=0|1, PYRO_PACK_SINGLES=0|1,
  *   PYRO_HOST_SLAB=<points> (pyro_source_terms_host), PYRO_JAC_KERNEL=point|block (the one-thread-per-point / the block-cooperative Jacobian kernel), PYRO_JAC_V_PLANE=shared, PYRO_JAC_BLOCK=<threads>
- *   (pyro_get_jacobian), PYRO_DEBUG=1 (prints the launch shape to stderr).
+ *   (pyro_get_jacobian), PYRO_CN_BLOCK=32|64 (points per block of the Crank-Nicolson LU kernel; read per call), PYRO_DEBUG=1 (prints the launch shape to stderr).
  */
 #ifndef PYRO_H
 #define PYRO_H
