@@ -88,6 +88,7 @@ struct pyro_mech {
     bool tab_smem2 = false;
     size_t smem2 = 0;
     uint32_t planes_off2 = 0, tmem_cols2 = 32;
+    int blocks_per_sm2 = 1;   // resident blocks of the two-points-per-thread kernel
     size_t reactor_smem = 0;         // its dynamic shared memory: that of the rates kernel + the staged energy table
     uint32_t reactor_energy_off = 0;
     int reactor_blocks_per_sm = 1;   // resident blocks of the reactor kernel (same block shape as the rates kernel)
@@ -150,7 +151,7 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
         args.n_chunks = (a.n + 63) / 64;
         args.planes_off = m->planes_off2;
         args.tmem_cols = m->tmem_cols2;
-        blocks = (int64_t)m->sm_count;
+        blocks = (int64_t)m->sm_count * m->blocks_per_sm2;
         const int64_t need = (args.n_chunks + pyro::kRates2Threads / 32 - 1) / (pyro::kRates2Threads / 32);
         if (blocks > need) blocks = need;
     }
@@ -162,7 +163,7 @@ int enqueue_rates(const pyro_mech *m, const pyro::RatesArgs &a, cudaStream_t str
     PYRO_CUDA(cudaStreamWaitEvent(stream, m->work_done[slot], 0));
     PYRO_CUDA(cudaMemsetAsync(args.work, 0, sizeof(unsigned long long), stream));
     if (two)
-        PYRO_CUDA(pyro::launch_rates2(args, pyro::kRates2Threads, (int)blocks, m->tab_smem2, m->smem2, stream));
+        PYRO_CUDA(pyro::launch_rates2(args, pyro::kRates2Threads, (int)blocks, m->tab_smem2, m->two_blocks, m->smem2, stream));
     else
         PYRO_CUDA(pyro::launch_rates(args, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem, m->two_blocks, m->smem_bytes, stream,
                                      fused));
@@ -365,9 +366,9 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
     // Two points per thread (pyro_rates2_kernels.cu): 128 threads hold the same 256 points; needs eight tensor-memory
     // columns per species row and the A plane of both points (16 bytes per row and thread) in shared memory.  Used for
     // mechanisms that run the one-block shape (not the two-block shape of small mechanisms).
-    if (!m->two_blocks && 8 * rows <= 512) {
+    if (8 * rows <= 512) {
         const size_t planes2 = 16 * rows * (size_t)pyro::kRates2Threads;
-        const void *fn2s = pyro::rates2_kernel_ptr(true), *fn2g = pyro::rates2_kernel_ptr(false);
+        const void *fn2s = pyro::rates2_kernel_ptr(true, m->two_blocks), *fn2g = pyro::rates2_kernel_ptr(false, m->two_blocks);
         cudaFuncAttributes fa2{};
         if ((ce = cudaFuncGetAttributes(&fa2, fn2s)) != cudaSuccess) return bail(ce, "cudaFuncGetAttributes(rates2)");
         const size_t smem_max2 = (size_t)prop.sharedMemPerBlockOptin - fa2.sharedSizeBytes;
@@ -386,15 +387,28 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         if (ok) {
             m->tmem_cols2 = 32;
             while (m->tmem_cols2 < 8 * rows) m->tmem_cols2 *= 2;
+            // small mechanisms: as many blocks per SM as shared memory, tensor memory and the register file hold
+            {
+                const size_t regs_block = (size_t)((fa2.numRegs + 7) / 8 * 8) * pyro::kRates2Threads;
+                int nb = (int)(prop.sharedMemPerMultiprocessor / (m->smem2 + fa2.sharedSizeBytes + 1024));
+                nb = std::min(nb, (int)(512 / m->tmem_cols2));
+                nb = std::min(nb, (int)((size_t)prop.regsPerMultiprocessor / regs_block));
+                m->blocks_per_sm2 = std::max(1, std::min(nb, 4));
+                if (std::getenv("PYRO_DEBUG"))
+                    std::fprintf(stderr, "pyro: two-point kernel regs %d smem %zu tmem_cols %u blocks per SM %d\n", fa2.numRegs, m->smem2, m->tmem_cols2, m->blocks_per_sm2);
+            }
             for (const void *f2 : {fn2s, fn2g}) {
                 if ((ce = cudaFuncSetAttribute(f2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_max2)) != cudaSuccess)
                     return bail(ce, "cudaFuncSetAttribute(rates2, MaxDynamicSharedMemorySize)");
                 if ((ce = cudaFuncSetAttribute(f2, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess)
                     return bail(ce, "cudaFuncSetAttribute(rates2, carveout)");
             }
-            // Measured slower than the one-point kernel (configs[2]: 7.58 against 7.09 ms -- 27 % fewer instructions, but
-            // one warp per scheduler issues on 45 % of the cycles against 66 % for two; profiles/r02_dead_ends.md):
-            // available to tests and measurements through PYRO_RATES_POINTS=2, not chosen by the library.
+            // Large mechanisms (one block per SM): measured slower than the one-point kernel (configs[2]: 7.58 against
+            // 7.09 ms -- 27 % fewer instructions, but one warp per scheduler issues on 45 % of the cycles against 66 % for
+            // two; profiles/r02_dead_ends.md).  Small mechanisms, where two blocks of it are resident per SM (two warps
+            // per scheduler, as the one-point kernel, with the fewer instructions): faster (configs[1]: 2.26 against
+            // 2.64 ms) and the library's choice.  PYRO_RATES_POINTS=1|2 forces either (tests, measurements).
+            m->two_points = m->two_blocks && m->blocks_per_sm2 >= 2;
             if (const char *env = std::getenv("PYRO_RATES_POINTS")) m->two_points = std::atoi(env) == 2;
         }
     }

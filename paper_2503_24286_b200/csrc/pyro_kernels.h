@@ -111,8 +111,8 @@ const void *jacobian_kernel_ptr(bool small);
 cudaError_t launch_jacobian(const JacArgs &a, bool small, int threads, int blocks, size_t smem_bytes, cudaStream_t stream);
 
 constexpr int kRates2Threads = 128;     // threads per block of the two-points-per-thread rates kernel (256 points)
-const void *rates2_kernel_ptr(bool tables_in_shared);
-cudaError_t launch_rates2(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, size_t smem_bytes, cudaStream_t stream);
+const void *rates2_kernel_ptr(bool tables_in_shared, bool singles);
+cudaError_t launch_rates2(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool singles, size_t smem_bytes, cudaStream_t stream);
 const void *rates_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks);
 const void *fused_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool two_blocks);
 const void *temperature_kernel_ptr();

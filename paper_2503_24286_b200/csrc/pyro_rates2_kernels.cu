@@ -71,7 +71,9 @@ struct DevMem2 {
     }
 };
 
-template <bool kTabSmem> __global__ void __launch_bounds__(kRates2Threads, 1) rates2_kernel(const RatesArgs a) {
+// kSingles: the tables hold reactions that run one at a time (small mechanisms, pyro_pack.cpp) -- the loops for them
+// are compiled in only then (instruction cache, as in the one-point kernel).
+template <bool kTabSmem, bool kSingles> __global__ void __launch_bounds__(kRates2Threads, 1) rates2_kernel(const RatesArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nthreads = blockDim.x;
@@ -122,7 +124,7 @@ template <bool kTabSmem> __global__ void __launch_bounds__(kRates2Threads, 1) ra
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)k * a.ld + pn + 32));
             }
         }
-        accumulate_reactions<false>(tab, a.groups, pt, ctot, mem);
+        accumulate_reactions<kSingles>(tab, a.groups, pt, ctot, mem);
         int k = 0;
 #pragma unroll 1
         for (; k < ns; k += 4) {
@@ -146,14 +148,15 @@ template <bool kTabSmem> __global__ void __launch_bounds__(kRates2Threads, 1) ra
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "r"(a.tmem_cols));
 }
 
-const void *rates2_kernel_ptr(bool tables_in_shared) {
-    return tables_in_shared ? (const void *)rates2_kernel<true> : (const void *)rates2_kernel<false>;
+const void *rates2_kernel_ptr(bool tables_in_shared, bool singles) {
+    if (singles) return tables_in_shared ? (const void *)rates2_kernel<true, true> : (const void *)rates2_kernel<false, true>;
+    return tables_in_shared ? (const void *)rates2_kernel<true, false> : (const void *)rates2_kernel<false, false>;
 }
 
-cudaError_t launch_rates2(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, size_t smem_bytes, cudaStream_t stream) {
+cudaError_t launch_rates2(const RatesArgs &a, int threads, int blocks, bool tables_in_shared, bool singles, size_t smem_bytes, cudaStream_t stream) {
     RatesArgs copy = a;
     void *params[] = {&copy};
-    return cudaLaunchKernel(rates2_kernel_ptr(tables_in_shared), dim3((unsigned)blocks), dim3((unsigned)threads), params, smem_bytes, stream);
+    return cudaLaunchKernel(rates2_kernel_ptr(tables_in_shared, singles), dim3((unsigned)blocks), dim3((unsigned)threads), params, smem_bytes, stream);
 }
 
 }   // namespace pyro

@@ -781,13 +781,17 @@ def test_abi_ld_and_alignment_on_every_entry_point(mechs):
     torch.cuda.synchronize()
 
 
-def test_two_points_per_thread_rates_kernel(mechs, monkeypatch):
-    """The two-points-per-thread variant of the rates kernel (PYRO_RATES_POINTS=2; measured slower, kept as a
-    variant): every entry against the oracle, ragged tail of a 64-point chunk, hand mechanism with every class."""
-    monkeypatch.setenv("PYRO_RATES_POINTS", "2")
-    st = inputs.config_states(2, n=2500 + 33)
+@pytest.mark.parametrize("points", ["1", "2"])
+def test_rates_kernel_points_per_thread(mechs, monkeypatch, points):
+    """Both rates kernels on every kind of mechanism, whichever the library would choose (PYRO_RATES_POINTS forces
+    one: the two-points-per-thread kernel is the default for small mechanisms, the one-point kernel for the others):
+    every entry against the oracle, ragged tail of a 64-point chunk, hand mechanism with every class."""
+    monkeypatch.setenv("PYRO_RATES_POINTS", points)
     hand = hand_cases.all_paths_mechanism()
-    cases = [(inputs.config_mechanism(2), (st["rho"], st["T"], st["Y"])), (hand, hand_cases.random_states(hand, 333))]
+    cases = [(hand, hand_cases.random_states(hand, 333))]
+    for cfg, n in ((0, 777), (1, 1000 + 33), (2, 2500 + 33)):
+        st = inputs.config_states(cfg, n=n)
+        cases.append((inputs.config_mechanism(cfg), (st["rho"], st["T"], st["Y"])))
     for mech, (rho, T, Y) in cases:
         gm = binding.Mechanism(mech)
         om_ref, bound = oracle.Oracle(mech).get_net_production_rates(rho, T, Y)
