@@ -23,7 +23,7 @@
  *   not choose by itself (they exist so that the parity tests reach every kernel variant); they are not part of
  *   the interface and change no result: PYRO_TABLES=shared|global, PYRO_RATES_BLOCK=<threads>,
  *   PYRO_B_PLANE=shared, PYRO_CARVEOUT=<percent>, PYRO_RATES_POINTS=1|2 (grid points per thread of the rates kernel), PYRO_RATES_TWO_BLOCKS=0|1, PYRO_PACK_SINGLES=0|1,
- *   PYRO_HOST_SLAB=<points> (pyro_source_terms_host), PYRO_JAC_KERNEL=point|block (the one-thread-per-point / the block-cooperative Jacobian kernel), PYRO_JAC_V_PLANE=shared, PYRO_JAC_BLOCK=<threads>
+ *   PYRO_HOST_SLAB=<points> (pyro_source_terms_host), PYRO_JAC_KERNEL=point|block (the one-thread-per-point / the block-cooperative Jacobian kernel), PYRO_JAC_V_PLANE=shared, PYRO_JAC_BLOCK=<threads>, PYRO_JAC_EXT=global
  *   (pyro_get_jacobian), PYRO_CN_BLOCK=32|64 (points per block of the Crank-Nicolson LU kernel; read per call), PYRO_DEBUG=1 (prints the launch shape to stderr).
  */
 #ifndef PYRO_H

@@ -108,6 +108,7 @@ struct pyro_mech {
     uint32_t jac_planes_bytes = 0;
     // block-cooperative Jacobian kernel (pyro_jac_block_kernels.cu): 0 = not used, else warps per block
     int jac_block_warps = 0;
+    bool jac_block_ext_global = false;   // its [M] scratch in global memory (mechanisms whose planes fill the shared memory)
     size_t jac_block_smem = 0;
     uint32_t jac_block_planes_bytes = 0, jac_block_tmem_cols = 32;
     uint32_t jac_tmem_cols = 32;
@@ -494,10 +495,15 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
         // memory fits: 5 planes + the [M] scratch + 2 NW reduction rows of 32 doubles, and NW record rings.
         // (not for small mechanisms: with fewer columns than warps most of the block idles; measured at 9 species:
         // 4.8 against 2.2 ns per point)
-        for (int nw : {16, 8}) {
+        for (int shape = 0; shape < 4 && !m->jac_block_warps; ++shape) {
+            const int nw = shape < 2 ? 16 : 8;
+            const bool ext_global = shape & 1;   // second choice: the [M] scratch in global memory
             if (lay.n_species < 24 && !std::getenv("PYRO_JAC_KERNEL")) break;
+            if (const char *env = std::getenv("PYRO_JAC_EXT")) {
+                if (!std::strcmp(env, "global") && !ext_global) continue;
+            }
             if (2 * rows * (size_t)(nw / 4) > 512) continue;
-            const size_t pl = (5 * rows + 1 + 2 * (size_t)jl.n_ext + 2 * (size_t)nw + 8 * (size_t)nw) * 32 * sizeof(double);   // + reduction scratch
+            const size_t pl = (5 * rows + (ext_global ? 0 : 1 + 2 * (size_t)jl.n_ext) + 2 * (size_t)nw + 8 * (size_t)nw) * 32 * sizeof(double);   // + reduction scratch
             const size_t need = pl + (size_t)nw * pyro::kJacBlockRingBytes;
             cudaFuncAttributes fb{};
             const void *bfn = pyro::jacobian_block_kernel_ptr(nw);
@@ -505,12 +511,12 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
             if (need + fb.sharedSizeBytes > (size_t)prop.sharedMemPerBlockOptin) continue;
             if ((ce = cudaFuncSetAttribute(bfn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)((size_t)prop.sharedMemPerBlockOptin - fb.sharedSizeBytes))) != cudaSuccess)
                 return bail(ce, "cudaFuncSetAttribute(jacobian block)");
+            m->jac_block_ext_global = ext_global;
             m->jac_block_warps = nw;
             m->jac_block_smem = need;
             m->jac_block_planes_bytes = (uint32_t)pl;
             m->jac_block_tmem_cols = 32;
             while (m->jac_block_tmem_cols < 2 * rows * (size_t)(nw / 4)) m->jac_block_tmem_cols *= 2;
-            break;
         }
         if (const char *env = std::getenv("PYRO_JAC_KERNEL")) {
             if (!std::strcmp(env, "point")) m->jac_block_warps = 0;   // "block": also for small mechanisms (tests)
@@ -783,6 +789,7 @@ int jacobian_call(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, 
     if (m->jac_block_warps) {
         a.tmem_cols = m->jac_block_tmem_cols;
         a.planes_bytes = m->jac_block_planes_bytes;
+        a.ext_global = m->jac_block_ext_global ? 1 : 0;
         int64_t bb = m->sm_count;
         if (bb > a.n_chunks) bb = a.n_chunks;
         PYRO_CUDA(pyro::launch_jacobian_block(a, m->jac_block_warps, (int)bb, m->jac_block_smem, stream));

@@ -94,8 +94,10 @@ template <int NW> __global__ void __launch_bounds__(32 * NW, 1) jacobian_block_k
     // reduction scratch [NW][8][32], NW rings
     double *sm = reinterpret_cast<double *>(smem_raw);
     double *pC = sm + lane, *pG = pC + rows * 32, *pDG = pG + rows * 32, *pV = pDG + rows * 32, *pDT = pV + rows * 32;
-    double *pExt = pDT + rows * 32;
-    double *red = sm + (5 * rows + 1 + 2 * a.lay.n_ext) * 32;   // [2][NW][32]
+    // (the [M] scratch moves to global memory -- L2 -- for mechanisms whose planes leave no room for it)
+    const int ext_rows = 1 + 2 * a.lay.n_ext;
+    double *pExt = a.ext_global ? a.ext + ((int64_t)blockIdx.x * ext_rows) * 32 + lane : pDT + rows * 32;
+    double *red = sm + (5 * rows + (a.ext_global ? 0 : ext_rows)) * 32;   // [2][NW][32]
     double *scratch = red + 2 * NW * 32;                         // [NW][8][32]: blk_reduce
     DevJacTab tab{a.gtab, a.off_spec, a.energy, a.jtab, a.lay.off_rxn, a.lay.off_inc, a.lay.off_eff, a.lay.off_fall, a.lay.off_col,
                   (uint32_t)a.lay.n_inc};

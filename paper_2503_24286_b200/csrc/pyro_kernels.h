@@ -100,6 +100,7 @@ struct JacArgs {                 // chemical Jacobian (pyro_jac_tables.h)
     uint32_t off_spec, tmem_cols;
     uint32_t planes_bytes;       // dynamic shared memory taken by the planes; the per-warp record rings (8 KB each) follow
     int32_t mode;                // 0: fixed (rho, T); 1: fixed (rho, e)
+    int32_t ext_global;          // block kernel: the [M] scratch is ext[block][slot][32] in global memory, not in shared memory
     int64_t jblock;              // 0: J[(i n_s + k) ld + p]; else blocks of jblock points with contiguous matrices (implicit march)
     JacLayout lay;
 };

@@ -525,6 +525,20 @@ def test_jacobian_v_plane_in_shared_memory_and_small_blocks(mechs, monkeypatch):
             monkeypatch.delenv(k)
 
 
+def test_jacobian_block_kernel_scratch_in_global_memory(mechs, monkeypatch):
+    """The block-cooperative kernel with the scratch of the [M] reactions in global memory (its shape for mechanisms
+    whose planes fill the shared memory: configs[3] by itself), forced on configs[2] and on the hand mechanism."""
+    monkeypatch.setenv("PYRO_JAC_KERNEL", "block")
+    monkeypatch.setenv("PYRO_JAC_EXT", "global")
+    hand = hand_cases.all_paths_mechanism()
+    st = inputs.config_states(2, n=333)
+    for mech, (rho, T, Y) in ((inputs.config_mechanism(2), (st["rho"], st["T"], st["Y"])), (hand, hand_cases.random_states(hand, 99))):
+        Jr, sTr, bJ, bT = oracle.Oracle(mech).get_jacobian(rho, T, Y, mode=1)
+        J, sT = gpu_jacobian(binding.Mechanism(mech), rho, T, Y, 1)
+        parity.assert_jacobian_parity(J, Jr, bJ)
+        parity.assert_jacobian_parity(sT, sTr, bT)
+
+
 def test_jacobian_full_size_sampled_columns(mechs):
     """configs[2] at the size bench.py times the Jacobian on (2^18 points): sampled points against the oracle."""
     mech, gm, orc = mechs(2)
