@@ -168,10 +168,17 @@ PYRO_HD void plain_reactions(const Tab &tab, int j0, int count, const PT &pt, co
 // couples two in lockstep, the rest one at a time.
 // kSingles = false leaves the one-at-a-time loops out (the packer then stores no singles): for
 // large mechanisms their code alone costs 8 % (measured on configs[2]: instruction cache).
-template <int NR, int NP, bool kSingles, class Tab, class Mem, class PT>
+// kQuads = false runs the groups of eight and of four two in lockstep as well (they are stored as consecutive
+// disjoint couples): small mechanisms hardly have such groups, and without the four-in-lockstep loops the
+// two-points-per-thread kernel is half the code and far fewer registers.
+template <int NR, int NP, bool kSingles, bool kQuads, class Tab, class Mem, class PT>
 PYRO_HD int plain_shape(const Tab &tab, int j, int g8, int g4, int g2, int g1, const PT &pt, const Mem &mem) {
-    plain_reactions<NR, NP, 4>(tab, j, g8 + g4, pt, mem);
-    plain_reactions<NR, NP, 2>(tab, j + g8 + g4, g2, pt, mem);
+    if (kQuads) {
+        plain_reactions<NR, NP, 4>(tab, j, g8 + g4, pt, mem);
+        plain_reactions<NR, NP, 2>(tab, j + g8 + g4, g2, pt, mem);
+    } else {
+        plain_reactions<NR, NP, 2>(tab, j, g8 + g4 + g2, pt, mem);
+    }
     if (kSingles) plain_reactions<NR, NP, 1>(tab, j + g8 + g4 + g2, g1, pt, mem);
     return j + g8 + g4 + g2 + g1;
 }
@@ -311,12 +318,18 @@ PYRO_HD void extended_reactions(const Tab &tab, int j0, int count, const PT &pt,
     }
 }
 
-template <int KIND, bool kSingles, class Tab, class Mem, class PT, class V>
+template <int KIND, bool kSingles, bool kCouples, class Tab, class Mem, class PT, class V>
 PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, int g1, const PT &pt, V ctot, const Mem &mem) {
     // groups of four and couples alike run two in lockstep, in ONE loop per kind: four in lockstep
-    // gains less than the second copy of the loop costs (instruction cache; measured on configs[2])
-    extended_reactions<KIND, 2>(tab, j, g4 + g2, pt, ctot, mem);
-    if (kSingles) extended_reactions<KIND, 1>(tab, j + g4 + g2, g1, pt, ctot, mem);
+    // gains less than the second copy of the loop costs (instruction cache; measured on configs[2]).
+    // kCouples = false (small mechanisms in the two-points-per-thread kernel, where a reaction already is two chains):
+    // every record one at a time -- one loop per kind and the registers of one reaction.
+    if (kCouples) {
+        extended_reactions<KIND, 2>(tab, j, g4 + g2, pt, ctot, mem);
+        if (kSingles) extended_reactions<KIND, 1>(tab, j + g4 + g2, g1, pt, ctot, mem);
+    } else {
+        extended_reactions<KIND, 1>(tab, j, g4 + g2 + g1, pt, ctot, mem);
+    }
     return j + g4 + g2 + g1;
 }
 
@@ -324,23 +337,23 @@ PYRO_HD int extended_kind(const Tab &tab, int j, int g4, int g2, int g1, const P
 // accumulation into plane W, (A.5)-(A.10) PAPER.md:908-934.  The planes hold n_species + 1
 // entries: the last one is the dummy species (A = B = 1, omega = sink) that pads the
 // extended records and the efficiency lists.
-template <bool kSingles, class Tab, class Mem, class PT, class V>
+template <bool kSingles, bool kQuads = true, class Tab, class Mem, class PT, class V>
 PYRO_HD void accumulate_reactions(const Tab &tab, const GroupCounts &g, const PT &pt, V ctot, const Mem &mem) {
     int j = 0;
-    j = plain_shape<1, 1, kSingles>(tab, j, g.shape_g8[0], g.shape_g4[0], g.shape_g2[0], g.shape_g1[0], pt, mem);
-    j = plain_shape<1, 2, kSingles>(tab, j, g.shape_g8[1], g.shape_g4[1], g.shape_g2[1], g.shape_g1[1], pt, mem);
-    j = plain_shape<1, 3, kSingles>(tab, j, g.shape_g8[2], g.shape_g4[2], g.shape_g2[2], g.shape_g1[2], pt, mem);
-    j = plain_shape<2, 1, kSingles>(tab, j, g.shape_g8[3], g.shape_g4[3], g.shape_g2[3], g.shape_g1[3], pt, mem);
-    j = plain_shape<2, 2, kSingles>(tab, j, g.shape_g8[4], g.shape_g4[4], g.shape_g2[4], g.shape_g1[4], pt, mem);
-    j = plain_shape<2, 3, kSingles>(tab, j, g.shape_g8[5], g.shape_g4[5], g.shape_g2[5], g.shape_g1[5], pt, mem);
-    j = plain_shape<3, 1, kSingles>(tab, j, g.shape_g8[6], g.shape_g4[6], g.shape_g2[6], g.shape_g1[6], pt, mem);
-    j = plain_shape<3, 2, kSingles>(tab, j, g.shape_g8[7], g.shape_g4[7], g.shape_g2[7], g.shape_g1[7], pt, mem);
-    j = plain_shape<3, 3, kSingles>(tab, j, g.shape_g8[8], g.shape_g4[8], g.shape_g2[8], g.shape_g1[8], pt, mem);
+    j = plain_shape<1, 1, kSingles, kQuads>(tab, j, g.shape_g8[0], g.shape_g4[0], g.shape_g2[0], g.shape_g1[0], pt, mem);
+    j = plain_shape<1, 2, kSingles, kQuads>(tab, j, g.shape_g8[1], g.shape_g4[1], g.shape_g2[1], g.shape_g1[1], pt, mem);
+    j = plain_shape<1, 3, kSingles, kQuads>(tab, j, g.shape_g8[2], g.shape_g4[2], g.shape_g2[2], g.shape_g1[2], pt, mem);
+    j = plain_shape<2, 1, kSingles, kQuads>(tab, j, g.shape_g8[3], g.shape_g4[3], g.shape_g2[3], g.shape_g1[3], pt, mem);
+    j = plain_shape<2, 2, kSingles, kQuads>(tab, j, g.shape_g8[4], g.shape_g4[4], g.shape_g2[4], g.shape_g1[4], pt, mem);
+    j = plain_shape<2, 3, kSingles, kQuads>(tab, j, g.shape_g8[5], g.shape_g4[5], g.shape_g2[5], g.shape_g1[5], pt, mem);
+    j = plain_shape<3, 1, kSingles, kQuads>(tab, j, g.shape_g8[6], g.shape_g4[6], g.shape_g2[6], g.shape_g1[6], pt, mem);
+    j = plain_shape<3, 2, kSingles, kQuads>(tab, j, g.shape_g8[7], g.shape_g4[7], g.shape_g2[7], g.shape_g1[7], pt, mem);
+    j = plain_shape<3, 3, kSingles, kQuads>(tab, j, g.shape_g8[8], g.shape_g4[8], g.shape_g2[8], g.shape_g1[8], pt, mem);
     int x = 0;
-    x = extended_kind<kExtGeneral, kSingles>(tab, x, g.ext_g4[0], g.ext_g2[0], g.ext_g1[0], pt, ctot, mem);
-    x = extended_kind<kExtThreeBody, kSingles>(tab, x, g.ext_g4[1], g.ext_g2[1], g.ext_g1[1], pt, ctot, mem);
-    x = extended_kind<kExtLindemann, kSingles>(tab, x, g.ext_g4[2], g.ext_g2[2], g.ext_g1[2], pt, ctot, mem);
-    x = extended_kind<kExtTroe, kSingles>(tab, x, g.ext_g4[3], g.ext_g2[3], g.ext_g1[3], pt, ctot, mem);
+    x = extended_kind<kExtGeneral, kSingles, kQuads>(tab, x, g.ext_g4[0], g.ext_g2[0], g.ext_g1[0], pt, ctot, mem);
+    x = extended_kind<kExtThreeBody, kSingles, kQuads>(tab, x, g.ext_g4[1], g.ext_g2[1], g.ext_g1[1], pt, ctot, mem);
+    x = extended_kind<kExtLindemann, kSingles, kQuads>(tab, x, g.ext_g4[2], g.ext_g2[2], g.ext_g1[2], pt, ctot, mem);
+    x = extended_kind<kExtTroe, kSingles, kQuads>(tab, x, g.ext_g4[3], g.ext_g2[3], g.ext_g1[3], pt, ctot, mem);
     mem.fence_st();
 }
 

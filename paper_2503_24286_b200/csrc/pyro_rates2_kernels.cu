@@ -73,7 +73,7 @@ struct DevMem2 {
 
 // kSingles: the tables hold reactions that run one at a time (small mechanisms, pyro_pack.cpp) -- the loops for them
 // are compiled in only then (instruction cache, as in the one-point kernel).
-template <bool kTabSmem, bool kSingles> __global__ void __launch_bounds__(kRates2Threads, 1) rates2_kernel(const RatesArgs a) {
+template <bool kTabSmem, bool kSingles> __global__ void __launch_bounds__(kRates2Threads, kSingles ? 3 : 1) rates2_kernel(const RatesArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_tmem_base;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nthreads = blockDim.x;
@@ -124,7 +124,7 @@ template <bool kTabSmem, bool kSingles> __global__ void __launch_bounds__(kRates
                 asm volatile("prefetch.global.L2 [%0];" ::"l"(a.Y + (int64_t)k * a.ld + pn + 32));
             }
         }
-        accumulate_reactions<kSingles>(tab, a.groups, pt, ctot, mem);
+        accumulate_reactions<kSingles, !kSingles>(tab, a.groups, pt, ctot, mem);   // small mechanisms: no four-in-lockstep loops
         int k = 0;
 #pragma unroll 1
         for (; k < ns; k += 4) {
