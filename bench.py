@@ -467,12 +467,13 @@ def main():
                 "block_threads": info["block_threads"], "blocks_per_sm": info["blocks_per_sm"],
                 "smem_bytes_per_block": info["smem_bytes"], "tables_in_shared": info["tables_in_shared"], "tmem_columns": info["tmem_columns"],
                 "registers": info["registers"], "spill_bytes": info["local_bytes"],
+                "points_per_thread": info["points_per_thread"],
                 "newton_not_converged": not_converged,
             },
             "kernels_ms": {"temperature": temp_ms, "rates": rates_ms, "temperature_min": float(min(temp_all)),
                            "rates_min": float(min(rates_all)), "statistic": "median and min of the per-launch event times"},
             "roofline": {
-                "bound": "alu", "kernel": "rates_kernel", "achieved": achieved_tflops, "peak": FP64_PEAK_TFLOPS,
+                "bound": "alu", "kernel": "rates2_kernel" if info["points_per_thread"] == 2 else "rates_kernel", "achieved": achieved_tflops, "peak": FP64_PEAK_TFLOPS,
                 "unit": "TFLOP/s", "frac": achieved_tflops / FP64_PEAK_TFLOPS,
                 "traffic": NCU_RATES_DRAM_BYTES_PER_POINT_53SP * n if ns == 53 else None,
                 "traffic_note": "bytes per launch, ncu dram read + write of one profiled launch scaled by points; "

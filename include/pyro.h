@@ -240,10 +240,11 @@ int pyro_source_terms_host(pyro_mech *mech, int64_t n, int64_t ld, const double 
 /* Facts about a packed mechanism, for reports: fills up to `cap` int64 values
  *   [0] n_species  [1] n_reactions  [2] reactions in the plain class  [3] in the extended class
  *   [4] table bytes  [5] 1 if the rates kernel stages the tables in shared memory, 0 if it reads
- *   them from global memory  [6] threads (= points) per block of the rates kernel
+ *   them from global memory  [6] threads per block of the rates kernel (points per block: [6] x [12])
  *   [7] dynamic shared memory per block (bytes)  [8] resident (persistent) blocks per SM
  *   [9] registers per thread of the rates kernel  [10] local (spill) bytes per thread
- *   [11] SM count of the device  [12] grid points per thread of the rates kernel (1)
+ *   [11] SM count of the device  [12] grid points per thread of the rates kernel
+ *   (1; 2 for small mechanisms: the two-points-per-thread kernel)
  *   [13] tensor-memory columns a block allocates  [14] 1 if B_k = 1/E_k is kept in tensor memory
  *   beside omega_k (else in a second shared-memory plane)
  * returns the number of values written (negative pyro_status on error). */

@@ -409,7 +409,7 @@ int pyro_mech_create(const pyro_mech_desc *desc, int device, pyro_mech **out) {
             // two; profiles/r02_dead_ends.md).  Small mechanisms, where two blocks of it are resident per SM (two warps
             // per scheduler, as the one-point kernel, with the fewer instructions): faster (configs[1]: 2.26 against
             // 2.64 ms) and the library's choice.  PYRO_RATES_POINTS=1|2 forces either (tests, measurements).
-            m->two_points = m->two_blocks && m->blocks_per_sm2 >= 2;
+            m->two_points = m->two_blocks && m->b_tmem && m->blocks_per_sm2 >= 2;   // (b_tmem false: the PYRO_B_PLANE hook asks for the one-point variant)
             if (const char *env = std::getenv("PYRO_RATES_POINTS")) m->two_points = std::atoi(env) == 2;
         }
     }
@@ -955,11 +955,24 @@ int pyro_mech_info(const pyro_mech *m, int64_t *out, int cap) {
     if (!m || !out) return -fail(PYRO_ERR_NULL, "NULL argument");
     DeviceGuard guard(m->device);
     cudaFuncAttributes fa{};
-    cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks));
-    const int64_t v[15] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
-                           (int64_t)m->packed.lay.bytes, m->tab_smem ? 1 : 0, m->block_threads,
-                           (int64_t)m->smem_bytes, m->blocks_per_sm, fa.numRegs, (int64_t)fa.localSizeBytes,
-                           m->sm_count, 1, (int64_t)m->tmem_cols, m->b_tmem ? 1 : 0};
+    int64_t v[15] = {m->packed.n_species, m->packed.n_reactions, m->packed.lay.n_p, m->packed.lay.n_x,
+                     (int64_t)m->packed.lay.bytes, m->tab_smem ? 1 : 0, m->block_threads,
+                     (int64_t)m->smem_bytes, m->blocks_per_sm, 0, 0,
+                     m->sm_count, 1, (int64_t)m->tmem_cols, m->b_tmem ? 1 : 0};
+    if (m->two_points) {   // the kernel pyro_get_net_production_rates launches: two grid points per thread
+        cudaFuncGetAttributes(&fa, pyro::rates2_kernel_ptr(m->tab_smem2, m->two_blocks));
+        v[5] = m->tab_smem2 ? 1 : 0;
+        v[6] = pyro::kRates2Threads;
+        v[7] = (int64_t)m->smem2;
+        v[8] = m->blocks_per_sm2;
+        v[12] = 2;
+        v[13] = (int64_t)m->tmem_cols2;
+        v[14] = 1;
+    } else {
+        cudaFuncGetAttributes(&fa, pyro::rates_kernel_ptr(m->tab_smem, m->b_tmem, m->two_blocks));
+    }
+    v[9] = fa.numRegs;
+    v[10] = (int64_t)fa.localSizeBytes;
     int cnt = cap < 15 ? cap : 15;
     for (int i = 0; i < cnt; ++i) out[i] = v[i];
     return cnt;
