@@ -40,12 +40,19 @@ PYRO_HD double species_log2E_dT(const double *c, double T, double invT) {
 template <int P, class Mem>
 PYRO_HD void jac_scatter(const Mem &mem, const uint16_t (&sp)[6], const double (&w)[6], double d) {
     typename Mem::Raw r[6];
+    uint32_t s[6];   // read once: the fences below are compiler barriers, behind which the record would be read again
+    double c[6];
+#pragma unroll
+    for (int m = 0; m < 6; ++m) {
+        s[m] = sp[m];
+        c[m] = w[m];
+    }
     mem.fence_st();
 #pragma unroll
-    for (int m = 0; m < 6; ++m) r[m] = mem.template ld_acc<P>(sp[m]);
+    for (int m = 0; m < 6; ++m) r[m] = mem.template ld_acc<P>(s[m]);
     mem.fence_ld();
 #pragma unroll
-    for (int m = 0; m < 6; ++m) mem.template st_acc<P>(sp[m], fma(w[m], d, mem.value(r[m])));
+    for (int m = 0; m < 6; ++m) mem.template st_acc<P>(s[m], fma(c[m], d, mem.value(r[m])));
 }
 
 struct JacRates {   // what phases 1 and 2 need of one reaction at one point

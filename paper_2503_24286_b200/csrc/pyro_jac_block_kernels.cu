@@ -197,17 +197,37 @@ template <int NW> __global__ void __launch_bounds__(32 * NW, 1) jacobian_block_k
             mem.fence_st();
             const double scale = rho * tab.spec(k).inv_w;
             const double ekcv = a.mode == 1 ? jac_species_energy(tab.energy(k), pt.T) * rcv : 0.0;
+            // four rows per tensor-memory round trip; the row pointer advances by n_s planes of J per row
+            double *jp = Jp + (int64_t)k * jstride;
+            const int64_t rstep = (int64_t)ns * jstride;
+            const double *v = pV, *dt = pDT;
+            int i = 0;
 #pragma unroll 1
-            for (int i = 0; i < ns; i += 4) {
+            for (; i + 4 <= ns; i += 4, jp += 4 * rstep, v += 128, dt += 128) {
                 BlkJacMem::Raw r[4];
 #pragma unroll
-                for (int u = 0; u < 4; ++u) r[u] = mem.ld_acc<PW>((uint32_t)(i + u < ns ? i + u : ns));
+                for (int u = 0; u < 4; ++u) r[u] = mem.ld_acc<PW>((uint32_t)(i + u));
+                double pv[4], pd[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) pv[u] = v[u * 32], pd[u] = dt[u * 32];
                 mem.fence_ld();
 #pragma unroll
-                for (int u = 0; u < 4; ++u)
+                for (int u = 0; u < 4; ++u) {
+                    const double val = fma(mem.value(r[u]) + pv[u], scale, -(pd[u] * ekcv));
+                    if (live) __stcs(jp + u * rstep, val);
+                    mem.st_acc<PW>((uint32_t)(i + u), 0.0);
+                }
+            }
+            if (i < ns) {   // the last one to three rows (the dummy row n_s stands in for the rows beyond)
+                BlkJacMem::Raw r[3];
+#pragma unroll
+                for (int u = 0; u < 3; ++u) r[u] = mem.ld_acc<PW>((uint32_t)(i + u < ns ? i + u : ns));
+                mem.fence_ld();
+#pragma unroll
+                for (int u = 0; u < 3; ++u)
                     if (i + u < ns) {
-                        const double v = fma(mem.value(r[u]) + pV[(i + u) * 32], scale, -(pDT[(i + u) * 32] * ekcv));
-                        if (live) __stcs(Jp + ((int64_t)(i + u) * ns + k) * jstride, v);
+                        const double val = fma(mem.value(r[u]) + v[u * 32], scale, -(dt[u * 32] * ekcv));
+                        if (live) __stcs(jp + u * rstep, val);
                         mem.st_acc<PW>((uint32_t)(i + u), 0.0);
                     }
             }
