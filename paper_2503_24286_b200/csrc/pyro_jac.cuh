@@ -169,15 +169,21 @@ PYRO_HD double jac_species_cv(const EnergyRow &er, double T) {
 template <class Tab, class Mem>
 PYRO_HD void jac_column_accumulate(const Tab &tab, uint32_t begin, uint32_t end, const PointT &pt, const Mem &mem) {
 #pragma unroll 1
-    for (uint32_t q = begin; q < end; ++q) {
-        const JacInc &e = tab.inc((int)q);
-        double y[1] = {arrhenius_log2(e.f[0], e.f[1], e.f[2], pt.L2T, pt.invT) +
-                       (((mem.ldG(e.gslot[3]) + mem.ldG(e.gslot[4])) + mem.ldG(e.gslot[5])) -
-                        ((mem.ldG(e.gslot[0]) + mem.ldG(e.gslot[1])) + mem.ldG(e.gslot[2])))};
-        const double others = mem.ldC(e.other[0]) * mem.ldC(e.other[1]);
-        const double m = e.coef * mem.ld_ext(e.mul);
-        exp2_poly_n<1>(y);
-        jac_scatter<PW>(mem, e.sc_species, e.sc_w, (m * y[0]) * others);
+    for (uint32_t q = begin; q < end;) {
+        uint32_t n;
+        const JacInc *run = tab.inc_run(q, end, n);   // the records the table has at consecutive addresses
+        q += n;
+#pragma unroll 1
+        for (const JacInc *stop = run + n; run != stop; ++run) {
+            const JacInc &e = *run;
+            double y[1] = {arrhenius_log2(e.f[0], e.f[1], e.f[2], pt.L2T, pt.invT) +
+                           (((mem.ldG(e.gslot[3]) + mem.ldG(e.gslot[4])) + mem.ldG(e.gslot[5])) -
+                            ((mem.ldG(e.gslot[0]) + mem.ldG(e.gslot[1])) + mem.ldG(e.gslot[2])))};
+            const double others = mem.ldC(e.other[0]) * mem.ldC(e.other[1]);
+            const double m = e.coef * mem.ld_ext(e.mul);
+            exp2_poly_n<1>(y);
+            jac_scatter<PW>(mem, e.sc_species, e.sc_w, (m * y[0]) * others);
+        }
     }
 }
 

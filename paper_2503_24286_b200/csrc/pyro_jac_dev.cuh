@@ -59,6 +59,13 @@ struct RecordRing {
         }
         return gen + (uint32_t)(seg & 1) * seg_bytes + (q - (uint32_t)seg * seg_recs) * rec_bytes;
     }
+    // record q and how many records from q on (below limit) lie contiguous in the ring: a loop over them only steps a pointer
+    __device__ __forceinline__ const unsigned char *get_run(uint32_t q, uint32_t limit, uint32_t &n) {
+        const unsigned char *p = get(q);
+        const uint32_t seg_end = (q / seg_recs + 1u) * seg_recs;
+        n = (limit < seg_end ? limit : seg_end) - q;
+        return p;
+    }
 };
 
 struct DevJacTab {
@@ -85,6 +92,10 @@ struct DevJacTab {
     }
     __device__ __forceinline__ const JacRxn &rxn(int j) const { return *reinterpret_cast<const JacRxn *>(ring.get((uint32_t)(j - rxn_first))); }
     __device__ __forceinline__ const JacInc &inc(int q) const { return *reinterpret_cast<const JacInc *>(ring.get((uint32_t)(q - inc_first))); }
+    // incidences q .. q + n - 1 (n >= 1, q + n <= end) at consecutive addresses
+    __device__ __forceinline__ const JacInc *inc_run(uint32_t q, uint32_t end, uint32_t &n) const {
+        return reinterpret_cast<const JacInc *>(ring.get_run(q - (uint32_t)inc_first, end - (uint32_t)inc_first, n));
+    }
     __device__ __forceinline__ const EffEntry &eff(int q) const { return reinterpret_cast<const EffEntry *>(jbase + off_eff)[q]; }
     __device__ __forceinline__ const RxnFall &rxn_fall(int j) const { return reinterpret_cast<const RxnFall *>(jbase + off_fall)[j]; }
     __device__ __forceinline__ const JacCol &col(int k) const { return reinterpret_cast<const JacCol *>(jbase + off_col)[k]; }

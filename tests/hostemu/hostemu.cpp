@@ -34,6 +34,10 @@ struct HostJacTab {
     const pyro::EnergyRow &energy(int k) const { return en[k]; }
     const pyro::JacRxn &rxn(int j) const { return reinterpret_cast<const pyro::JacRxn *>(jbase + jl.off_rxn)[j]; }
     const pyro::JacInc &inc(int q) const { return reinterpret_cast<const pyro::JacInc *>(jbase + jl.off_inc)[q]; }
+    const pyro::JacInc *inc_run(uint32_t q, uint32_t end, uint32_t &n) const {
+        n = end - q;
+        return &inc((int)q);
+    }
     const pyro::EffEntry &eff(int q) const { return reinterpret_cast<const pyro::EffEntry *>(jbase + jl.off_eff)[q]; }
     const pyro::RxnFall &rxn_fall(int j) const { return reinterpret_cast<const pyro::RxnFall *>(jbase + jl.off_fall)[j]; }
     const pyro::JacCol &col(int k) const { return reinterpret_cast<const pyro::JacCol *>(jbase + jl.off_col)[k]; }
