@@ -39,9 +39,9 @@ __global__ void __launch_bounds__(256) cn_begin_step_kernel(const CnArgs a) {
 // these reads (first version, eight plain loads in flight per thread: issue 4 %, long scoreboard 72 %).  So they
 // stream through a per-thread ring in shared memory, filled by cp.async kCnGroups groups of kCnBatch elements ahead of
 // their use; the consumer waits once per group and then has kCnBatch x NC independent multiply-adds.
-constexpr int kCnRows = 4;               // rows of two columns per cp.async group
-constexpr int kCnBatch = 2 * kCnRows;    // elements per cp.async group
-constexpr int kCnGroups = 8;   // groups requested ahead (a power of two)
+constexpr int kCnRows = 4;               // rows of four columns per cp.async group
+constexpr int kCnBatch = 4 * kCnRows;    // elements per cp.async group
+constexpr int kCnGroups = 4;   // groups requested ahead (a power of two)
 constexpr int kCnRing = kCnBatch * kCnGroups;
 
 template <int TB> struct CnRing {
@@ -70,7 +70,7 @@ template <int TB> struct CnRing {
 };
 
 template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel(const CnArgs a) {
-    static_assert(NC % 2 == 0, "the eliminations left of a panel go by pairs of columns");
+    static_assert(NC % 4 == 0 && kCnBatch >= 6, "the eliminations left of a panel go by four columns");
     extern __shared__ double cn_cols[];   // [NC][n_species][TB], then the ring [kCnRing][TB]
     const int tid = threadIdx.x;
     const int64_t p = (int64_t)blockIdx.x * TB + tid;
@@ -93,29 +93,35 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
             for (int cc = 0; cc < NC; ++cc)
                 if (j0 + cc < ns)
                     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(&S(cc, i))), "l"(&G(i, j0 + cc)) : "memory");
-        // The factors left of the panel, L(i, k), k < j0, i > k, two columns (k, k + 1) at a time, so that an element of
-        // the panel is read and written once for two multiply-adds.  Order of the stream: L(k + 1, k) in a group of its
-        // own, then the rows i >= k + 2 in groups of kCnRows rows: L(i, k), L(i, k + 1), L(i + 1, k), ...
+        // The factors left of the panel, L(i, k), k < j0, i > k, four columns (k .. k + 3) at a time, so that an element
+        // of the panel is read and written once for four multiply-adds.  Order of the stream: the triangle
+        // L(k+1,k); L(k+2,k), L(k+2,k+1); L(k+3,k), L(k+3,k+1), L(k+3,k+2) in a group of its own, then the rows i >= k + 4
+        // in groups of kCnRows rows of four: L(i, k .. k+3), L(i + 1, k .. k+3), ...
         int gk = 0, gi = 1;
         const double *gp = &G(1, 0);   // &G(gi, gk); a row further is row_step doubles on, a column further TB
         auto request = [&]() {
             if (gk < j0) {
                 if (gi == gk + 1) {
                     ring.request(0, gp);
-                    gi += 1;
-                    gp += row_step;
+                    ring.request(1, gp + row_step);
+                    ring.request(2, gp + row_step + TB);
+                    ring.request(3, gp + 2 * row_step);
+                    ring.request(4, gp + 2 * row_step + TB);
+                    ring.request(5, gp + 2 * row_step + 2 * TB);
+                    gi += 3;
+                    gp += 3 * row_step;
                 } else {
 #pragma unroll
                     for (int e = 0; e < kCnRows; ++e)
                         if (gi + e < ns) {
-                            ring.request(2 * e, gp + e * row_step);
-                            ring.request(2 * e + 1, gp + e * row_step + TB);
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) ring.request(4 * e + q, gp + e * row_step + q * TB);
                         }
                     gi += kCnRows;
                     gp += kCnRows * row_step;
                 }
                 if (gi >= ns) {
-                    gk += 2;
+                    gk += 4;
                     gi = gk + 1;
                     gp = &G(gi, gk);
                 }
@@ -138,29 +144,37 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
             }
         }
 #pragma unroll 1
-        for (int k = 0; k < j0; k += 2) {   // j0 is a multiple of NC, NC is even
-            double ck[NC], ck1[NC];
+        for (int k = 0; k < j0; k += 4) {   // j0 is a multiple of NC, NC a multiple of four
+            double c0[NC], c1[NC], c2[NC], c3[NC];   // rows k .. k + 3 of the panel, final after the triangle
             ring.wait_front();
             {
-                const double l0 = ring.take(0);
+                double t[6];
+#pragma unroll
+                for (int e = 0; e < 6; ++e) t[e] = ring.take(e);
                 ++ring.taken;
+#pragma unroll
+                for (int cc = 0; cc < NC; ++cc) c0[cc] = S(cc, k), c1[cc] = S(cc, k + 1), c2[cc] = S(cc, k + 2), c3[cc] = S(cc, k + 3);
                 request();
 #pragma unroll
                 for (int cc = 0; cc < NC; ++cc) {
-                    ck[cc] = S(cc, k);
-                    ck1[cc] = fma(-l0, ck[cc], S(cc, k + 1));
-                    S(cc, k + 1) = ck1[cc];
+                    c1[cc] = fma(-t[0], c0[cc], c1[cc]);
+                    c2[cc] = fma(-t[2], c1[cc], fma(-t[1], c0[cc], c2[cc]));
+                    c3[cc] = fma(-t[5], c2[cc], fma(-t[4], c1[cc], fma(-t[3], c0[cc], c3[cc])));
                 }
+#pragma unroll
+                for (int cc = 0; cc < NC; ++cc) S(cc, k + 1) = c1[cc], S(cc, k + 2) = c2[cc], S(cc, k + 3) = c3[cc];
             }
             // loads first, then the multiply-adds, then the stores: written out, because the compiler cannot tell that
             // the columns of the panel do not overlap and would otherwise wait for every load in turn
-            int i0 = k + 2;
+            int i0 = k + 4;
 #pragma unroll 1
             for (; i0 + kCnRows <= ns; i0 += kCnRows) {
                 ring.wait_front();
-                double l[kCnRows], l1[kCnRows], v[kCnRows][NC];
+                double l[kCnRows][4], v[kCnRows][NC];
 #pragma unroll
-                for (int e = 0; e < kCnRows; ++e) l[e] = ring.take(2 * e), l1[e] = ring.take(2 * e + 1);
+                for (int e = 0; e < kCnRows; ++e)
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) l[e][q] = ring.take(4 * e + q);
                 ++ring.taken;
 #pragma unroll
                 for (int e = 0; e < kCnRows; ++e)
@@ -170,32 +184,29 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
 #pragma unroll
                 for (int e = 0; e < kCnRows; ++e)
 #pragma unroll
-                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = fma(-l1[e], ck1[cc], fma(-l[e], ck[cc], v[e][cc]));
+                    for (int cc = 0; cc < NC; ++cc)
+                        v[e][cc] = fma(-l[e][3], c3[cc], fma(-l[e][2], c2[cc], fma(-l[e][1], c1[cc], fma(-l[e][0], c0[cc], v[e][cc]))));
 #pragma unroll
                 for (int e = 0; e < kCnRows; ++e)
 #pragma unroll
                     for (int cc = 0; cc < NC; ++cc) S(cc, i0 + e) = v[e][cc];
             }
-            if (i0 < ns) {   // the ragged end of the two columns
+            if (i0 < ns) {   // the ragged end of the four columns
                 ring.wait_front();
-                double l[kCnRows], l1[kCnRows], v[kCnRows][NC];
 #pragma unroll
-                for (int e = 0; e < kCnRows - 1; ++e) {
-                    const bool in = i0 + e < ns;
-                    l[e] = in ? ring.take(2 * e) : 0.0;
-                    l1[e] = in ? ring.take(2 * e + 1) : 0.0;
-                }
+                for (int e = 0; e < kCnRows - 1; ++e)
+                    if (i0 + e < ns) {
+                        double l[4], v[NC];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) l[q] = ring.take(4 * e + q);
+#pragma unroll
+                        for (int cc = 0; cc < NC; ++cc) v[cc] = S(cc, i0 + e);
+#pragma unroll
+                        for (int cc = 0; cc < NC; ++cc)
+                            S(cc, i0 + e) = fma(-l[3], c3[cc], fma(-l[2], c2[cc], fma(-l[1], c1[cc], fma(-l[0], c0[cc], v[cc]))));
+                    }
                 ++ring.taken;
-#pragma unroll
-                for (int e = 0; e < kCnRows - 1; ++e)
-#pragma unroll
-                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = i0 + e < ns ? S(cc, i0 + e) : 0.0;
                 request();
-#pragma unroll
-                for (int e = 0; e < kCnRows - 1; ++e)
-#pragma unroll
-                    for (int cc = 0; cc < NC; ++cc)
-                        if (i0 + e < ns) S(cc, i0 + e) = fma(-l1[e], ck1[cc], fma(-l[e], ck[cc], v[e][cc]));
             }
         }
         ring.drain();
