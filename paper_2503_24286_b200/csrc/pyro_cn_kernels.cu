@@ -132,9 +132,23 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
 #pragma unroll 1
         for (int u = 0; u < kCnGroups; ++u) request();
         asm volatile("cp.async.wait_group %0;" ::"n"(kCnGroups) : "memory");   // the panel has landed
-        for (int i = 0; i < ns; ++i) {
+        {   // A = I - c J in place, four rows at a time (loads first: see below)
+            int i = 0;
+            for (; i + 4 <= ns; i += 4) {
+                double v[4][NC];
 #pragma unroll
-            for (int cc = 0; cc < NC; ++cc) S(cc, i) = j0 + cc < ns ? (i == j0 + cc ? 1.0 : 0.0) - c * S(cc, i) : 0.0;
+                for (int e = 0; e < 4; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = S(cc, i + e);
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc) S(cc, i + e) = j0 + cc < ns ? (i + e == j0 + cc ? 1.0 : 0.0) - c * v[e][cc] : 0.0;
+            }
+            for (; i < ns; ++i) {
+#pragma unroll
+                for (int cc = 0; cc < NC; ++cc) S(cc, i) = j0 + cc < ns ? (i == j0 + cc ? 1.0 : 0.0) - c * S(cc, i) : 0.0;
+            }
         }
         if (j0 + NC > ns) {   // the last panel: the right-hand side -F behind the last column of the matrix
             rhs_col = ns - j0;
@@ -231,10 +245,25 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
                 for (int i = j + 1; i < ns; ++i) S(jj, i) *= piv;
             }
         }
-        for (int i = 0; i < ns; ++i)
+        {   // the panel's columns back to their place in global memory, four rows at a time
+            int i = 0;
+            for (; i + 4 <= ns; i += 4) {
+                double v[4][NC];
 #pragma unroll
-            for (int cc = 0; cc < NC; ++cc)
-                if (j0 + cc < ns) G(i, j0 + cc) = S(cc, i);
+                for (int e = 0; e < 4; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc) v[e][cc] = S(cc, i + e);
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+#pragma unroll
+                    for (int cc = 0; cc < NC; ++cc)
+                        if (j0 + cc < ns) G(i + e, j0 + cc) = v[e][cc];
+            }
+            for (; i < ns; ++i)
+#pragma unroll
+                for (int cc = 0; cc < NC; ++cc)
+                    if (j0 + cc < ns) G(i, j0 + cc) = S(cc, i);
+        }
     }
     // back substitution with U, row after row from the last: the diagonal element first, then the row right of it.
     // y = L^-1 (-F) is in column rhs_col of the panel store; x overwrites it.
@@ -276,12 +305,28 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
             }
             s /= diag;
             S(rhs_col, r) = s;
-            b[(int64_t)r * ld] = s;
-            a.Y[(int64_t)r * ld + p] += s;
             worst = fmax(worst, fabs(s));
             finite = finite && (s == s) && fabs(s) <= 1.7976931348623157e308;
         }
         ring.drain();
+        {   // dY out, Y += dY: four rows at a time, so that the reads of Y do not wait for one another
+            int i = 0;
+            for (; i + 4 <= ns; i += 4) {
+                double y[4], d[4];
+#pragma unroll
+                for (int e = 0; e < 4; ++e) y[e] = a.Y[(int64_t)(i + e) * ld + p], d[e] = S(rhs_col, i + e);
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    b[(int64_t)(i + e) * ld] = d[e];
+                    a.Y[(int64_t)(i + e) * ld + p] = y[e] + d[e];
+                }
+            }
+            for (; i < ns; ++i) {
+                const double d = S(rhs_col, i);
+                b[(int64_t)i * ld] = d;
+                a.Y[(int64_t)i * ld + p] += d;
+            }
+        }
         if (a.last_update) a.last_update[p] = worst;
         if (a.count_unconverged && a.n_not_converged && (!finite || !(worst < a.update_tol))) atomicAdd(a.n_not_converged, 1);
     }
