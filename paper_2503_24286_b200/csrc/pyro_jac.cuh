@@ -36,23 +36,27 @@ PYRO_HD double species_log2E_dT(const double *c, double T, double invT) {
     return fma(invT, fma(-c[2], invT, c[1] * kLog2e), h);
 }
 
-// column[sc_species[m]] += sc_w[m] * d  for the six scatter entries (unused entries name the dummy species)
-template <int P, class Mem>
-PYRO_HD void jac_scatter(const Mem &mem, const uint16_t (&sp)[6], const double (&w)[6], double d) {
-    typename Mem::Raw r[6];
-    uint32_t s[6];   // read once: the fences below are compiler barriers, behind which the record would be read again
-    double c[6];
+// column[sc_species[m]] += sc_w[m] * d  for the first N scatter entries (unused entries name the dummy species)
+template <int P, int N, class Mem>
+PYRO_HD void jac_scatter_n(const Mem &mem, const uint16_t (&sp)[6], const double (&w)[6], double d) {
+    typename Mem::Raw r[N];
+    uint32_t s[N];   // read once: the fences below are compiler barriers, behind which the record would be read again
+    double c[N];
 #pragma unroll
-    for (int m = 0; m < 6; ++m) {
+    for (int m = 0; m < N; ++m) {
         s[m] = sp[m];
         c[m] = w[m];
     }
     mem.fence_st();
 #pragma unroll
-    for (int m = 0; m < 6; ++m) r[m] = mem.template ld_acc<P>(s[m]);
+    for (int m = 0; m < N; ++m) r[m] = mem.template ld_acc<P>(s[m]);
     mem.fence_ld();
 #pragma unroll
-    for (int m = 0; m < 6; ++m) mem.template st_acc<P>(s[m], fma(c[m], d, mem.value(r[m])));
+    for (int m = 0; m < N; ++m) mem.template st_acc<P>(s[m], fma(c[m], d, mem.value(r[m])));
+}
+template <int P, class Mem>
+PYRO_HD void jac_scatter(const Mem &mem, const uint16_t (&sp)[6], const double (&w)[6], double d) {
+    jac_scatter_n<P, 6>(mem, sp, w, d);
 }
 
 struct JacRates {   // what phases 1 and 2 need of one reaction at one point
@@ -165,8 +169,9 @@ PYRO_HD double jac_species_cv(const EnergyRow &er, double T) {
     return fma(cvk, T, ec[1]);
 }
 
-// The incidences [begin, end) of one column: column[sc_species] += sc_w * d  (pyro_jac_tables.h)
-template <class Tab, class Mem>
+// The incidences [begin, end) of one class of one column: column[sc_species] += sc_w * d  (pyro_jac_tables.h)
+// kGibbs: the records have a Gibbs sum (product side); N: scatter entries in use (4 or 6)
+template <bool kGibbs, int N, class Tab, class Mem>
 PYRO_HD void jac_column_accumulate(const Tab &tab, uint32_t begin, uint32_t end, const PointT &pt, const Mem &mem) {
 #pragma unroll 1
     for (uint32_t q = begin; q < end;) {
@@ -176,15 +181,29 @@ PYRO_HD void jac_column_accumulate(const Tab &tab, uint32_t begin, uint32_t end,
 #pragma unroll 1
         for (const JacInc *stop = run + n; run != stop; ++run) {
             const JacInc &e = *run;
-            double y[1] = {arrhenius_log2(e.f[0], e.f[1], e.f[2], pt.L2T, pt.invT) +
-                           (((mem.ldG(e.gslot[3]) + mem.ldG(e.gslot[4])) + mem.ldG(e.gslot[5])) -
-                            ((mem.ldG(e.gslot[0]) + mem.ldG(e.gslot[1])) + mem.ldG(e.gslot[2])))};
+            double y[1] = {arrhenius_log2(e.f[0], e.f[1], e.f[2], pt.L2T, pt.invT)};
+            if (kGibbs)
+                y[0] += ((mem.ldG(e.gslot[3]) + mem.ldG(e.gslot[4])) + mem.ldG(e.gslot[5])) -
+                        ((mem.ldG(e.gslot[0]) + mem.ldG(e.gslot[1])) + mem.ldG(e.gslot[2]));
             const double others = mem.ldC(e.other[0]) * mem.ldC(e.other[1]);
             const double m = e.coef * mem.ld_ext(e.mul);
             exp2_poly_n<1>(y);
-            jac_scatter<PW>(mem, e.sc_species, e.sc_w, (m * y[0]) * others);
+            jac_scatter_n<PW, N>(mem, e.sc_species, e.sc_w, (m * y[0]) * others);
         }
     }
+}
+
+// One column: its four classes of records one after the other.
+template <class Tab, class Mem>
+PYRO_HD void jac_column(const Tab &tab, const JacCol &col, const PointT &pt, const Mem &mem) {
+    uint32_t q = col.inc_begin;
+    jac_column_accumulate<false, 4>(tab, q, q + col.n_class[0], pt, mem);
+    q += col.n_class[0];
+    jac_column_accumulate<false, 6>(tab, q, q + col.n_class[1], pt, mem);
+    q += col.n_class[1];
+    jac_column_accumulate<true, 4>(tab, q, q + col.n_class[2], pt, mem);
+    q += col.n_class[2];
+    jac_column_accumulate<true, 6>(tab, q, q + col.n_class[3], pt, mem);
 }
 
 // The whole Jacobian of one point.
@@ -246,7 +265,7 @@ PYRO_HD void jacobian_point(const Tab &tab, const JacLayout &lay, double T, doub
 #pragma unroll 1
     for (int k = 0; k < ns; ++k) {
         const JacCol &col = tab.col(k);
-        jac_column_accumulate(tab, col.inc_begin, col.inc_end, pt, mem);
+        jac_column(tab, col, pt, mem);
         mem.fence_st();
         // J_ik = (column_i + V_i) rho/W_k - dS_i/dT e_k/c_v ; the column accumulator is cleared for the next one
         const double scale = rho * tab.spec(k).inv_w;

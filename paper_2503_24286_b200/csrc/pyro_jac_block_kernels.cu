@@ -193,7 +193,7 @@ template <int NW> __global__ void __launch_bounds__(32 * NW, 1) jacobian_block_k
             const int k = (int)order[cidx];
             const JacCol &col = tab.col(k);
             tab.begin_inc_range(col.inc_begin, col.inc_end - col.inc_begin);
-            jac_column_accumulate(tab, col.inc_begin, col.inc_end, pt, mem);
+            jac_column(tab, col, pt, mem);
             mem.fence_st();
             const double scale = rho * tab.spec(k).inv_w;
             const double ekcv = a.mode == 1 ? jac_species_energy(tab.energy(k), pt.T) * rcv : 0.0;

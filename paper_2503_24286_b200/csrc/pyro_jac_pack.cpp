@@ -129,10 +129,30 @@ int pack_jacobian(const pyro_mech_desc *d, JacPacked &out, std::string &err) {
     lay.n_fall = (int)falls.size();
     std::vector<JacCol> cols(ns);
     std::vector<JacInc> inc_all;
+    auto inc_class = [&](const JacInc &e) {
+        bool gibbs = false;
+        for (int m = 0; m < 6; ++m) gibbs = gibbs || e.gslot[m] != dummy;
+        const bool wide = e.sc_species[4] != dummy || e.sc_species[5] != dummy;   // the scatter list is filled from the front
+        return 2 * (gibbs ? 1 : 0) + (wide ? 1 : 0);
+    };
     for (int k = 0; k < ns; ++k) {
+        std::vector<JacInc> list(inc[k]);
+        list.insert(list.end(), effinc[k].begin(), effinc[k].end());
+        std::memset(&cols[k], 0, sizeof cols[k]);
         cols[k].inc_begin = (uint32_t)inc_all.size();
-        inc_all.insert(inc_all.end(), inc[k].begin(), inc[k].end());
-        inc_all.insert(inc_all.end(), effinc[k].begin(), effinc[k].end());
+        for (int c = 0; c < 4; ++c) {
+            size_t n = 0;
+            for (const JacInc &e : list)
+                if (inc_class(e) == c) {
+                    inc_all.push_back(e);
+                    ++n;
+                }
+            if (n > 65535) {
+                err = "too many incidences of one species for the Jacobian tables";
+                return PYRO_ERR_TOO_LARGE;
+            }
+            cols[k].n_class[c] = (uint16_t)n;
+        }
         cols[k].inc_end = (uint32_t)inc_all.size();
     }
     lay.n_inc = (int)inc_all.size();

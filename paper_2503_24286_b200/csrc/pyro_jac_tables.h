@@ -58,9 +58,15 @@ struct alignas(16) JacInc {
 // The incidence list of one species: records [inc_begin, inc_end) of the JacInc table, in the order the kernel walks
 // them (the whole table is read front to back once per point).  A species that is listed in the efficiency list of
 // an [M]-reaction x has one more incidence for it: d = delta * scratch[g_x], stored as a JacInc whose exponent is 0
-// (2^0 = 1 exactly), whose other molecules are the dummy species and whose multiplier slot is g_x.  16 bytes.
+// (2^0 = 1 exactly), whose other molecules are the dummy species and whose multiplier slot is g_x.
+// Within a list the records are sorted into four classes, each with a loop of its own in the kernel (no per-record
+// branch): class = 2 * (has a Gibbs sum: product-side incidence) + (more than four scatter entries); n_class[c] records
+// of class c follow one another in the order 0, 1, 2, 3.  A record of a class without a Gibbs sum has all its gslot =
+// dummy, one with at most four scatter entries has sc_species[4..5] = dummy: the short loops skip work whose result
+// is exactly zero.  16 bytes.
 struct alignas(16) JacCol {
-    uint32_t inc_begin, inc_end, pad0, pad1;
+    uint32_t inc_begin, inc_end;
+    uint16_t n_class[4];
 };
 
 struct JacLayout {
