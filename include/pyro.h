@@ -169,6 +169,31 @@ int pyro_source_terms(const pyro_mech *mech, int64_t n, int64_t ld, const double
 int pyro_reactor_rk4(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e, double *Y,
                      double *T, double dt, int32_t n_steps, double *work, int32_t *n_not_converged, void *cuda_stream);
 
+/* pyro_reactor_rk4 for callers that cannot allocate device memory -- and so have no `work` field to pass.  That is the
+ * situation of code running inside somebody else's memory budget: a solver plug-in whose host application owns every
+ * byte of the GPU and hands out only the state arrays, a call made while the application's memory pool is frozen
+ * (between its set-up phase and its tear-down), a real-time or in-situ loop in which cudaMalloc's implicit device
+ * synchronisation is not acceptable.  Same march, same results as pyro_reactor_rk4; the scratch it needs (the running
+ * sum of the stage slopes, one double per species and reactor, and the launch's work counter) is a fixed array built
+ * into the library image instead.  The call itself performs no cudaMalloc / cudaFree and calls nothing that does.
+ *   Limit.   n_species * (n rounded up to a multiple of 32) <= PYRO_RK4_STATIC_MAX_DOUBLES (4 Mi doubles = 32 MiB:
+ *            79 136 reactors of a 53-species mechanism, 466 016 of a 9-species one); beyond it the call returns
+ *            PYRO_ERR_TOO_LARGE and launches nothing -- march the batch in slabs.  `ld` does not enter the limit.
+ *   Cost.    every GPU on which the process uses libpyro holds those 32 MiB (+ 256 bytes) from the moment the
+ *            library is loaded there until the process exits, whether or not this function is ever called.
+ *   First call on a device.  Looks up the array's address on that device and raises the kernel's shared-memory
+ *            limit (two cheap, non-allocating runtime queries; later calls skip them).  Make that first call
+ *            outside any stream capture; n_steps = 0 on one reactor is enough.
+ *   Sharing. There is ONE array per device, used by every call on every handle and stream.  Two calls whose kernels
+ *            may run at the same time on one device (different streams without an event between them, or two host
+ *            threads) race on it and both results are garbage: keep the calls of a device on one stream or order them
+ *            yourself.  Nothing in the array has to survive between calls and nothing in it is read before this call
+ *            has written it (the work counter is reset on `cuda_stream` first), so stale contents are harmless.
+ * Arguments, preconditions and n_not_converged exactly as pyro_reactor_rk4, minus `work`. */
+#define PYRO_RK4_STATIC_MAX_DOUBLES 4194304
+int pyro_reactor_rk4_static(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e, double *Y,
+                            double *T, double dt, int32_t n_steps, int32_t *n_not_converged, void *cuda_stream);
+
 /* Implicit march of the same reactors (second half): Crank-Nicolson (A.32) PAPER.md:1043-1062,
  *     Y^{m+1} - Y^m - dt/2 (s^{m+1} + s^m) = 0,   s_k = W_k omega_k / rho,
  * each step solved by `newton_iters` Newton iterations (A.33)-(A.35) started from Y^m, with the analytic Jacobian

@@ -17,12 +17,13 @@ LIB_PATH = os.path.join(_HERE, "libpyro.so")
 EXPORTS = (
     "pyro_mech_create", "pyro_mech_destroy", "pyro_mech_set_newton", "pyro_get_temperature",
     "pyro_get_temperature_from_enthalpy", "pyro_get_density", "pyro_get_pressure",
-    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_reactor_cn", "pyro_reactor_cn_work_doubles", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak", "pyro_probe_dmma_peak", "pyro_probe_indexed_rmw",
+    "pyro_get_net_production_rates", "pyro_get_jacobian", "pyro_reactor_rk4", "pyro_reactor_rk4_static", "pyro_reactor_cn", "pyro_reactor_cn_work_doubles", "pyro_source_terms", "pyro_source_terms_host", "pyro_mech_info", "pyro_probe_fp64_peak", "pyro_probe_dmma_peak", "pyro_probe_indexed_rmw",
     "pyro_status_string", "pyro_last_error_string", "pyro_transport_create", "pyro_transport_destroy",
     "pyro_get_transport",
 )
 
 PYRO_OK = 0
+RK4_STATIC_MAX_DOUBLES = 4194304   # PYRO_RK4_STATIC_MAX_DOUBLES of pyro.h
 STATUS_NAMES = {0: "PYRO_OK", 1: "PYRO_ERR_NULL", 2: "PYRO_ERR_BAD_SIZE", 3: "PYRO_ERR_BAD_MECH",
                 4: "PYRO_ERR_TOO_LARGE", 5: "PYRO_ERR_ALIGN", 6: "PYRO_ERR_CUDA", 7: "PYRO_ERR_UNSUPPORTED"}
 
@@ -92,6 +93,7 @@ def load_library():
     lib.pyro_get_net_production_rates.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp]
     lib.pyro_get_jacobian.argtypes = [vp, i64, i64, vp, vp, vp, C.c_int, vp, vp, vp]
     lib.pyro_reactor_rk4.argtypes = [vp, i64, i64, vp, vp, vp, vp, dbl, C.c_int32, vp, vp, vp]
+    lib.pyro_reactor_rk4_static.argtypes = [vp, i64, i64, vp, vp, vp, vp, dbl, C.c_int32, vp, vp]
     lib.pyro_reactor_cn.argtypes = [vp, i64, i64, vp, vp, vp, vp, dbl, C.c_int32, C.c_int32, dbl, vp, vp, vp]
     lib.pyro_reactor_cn_work_doubles.argtypes = [vp, i64, C.POINTER(i64)]
     lib.pyro_source_terms.argtypes = [vp, i64, i64, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -270,6 +272,16 @@ class Mechanism:
         assert work.stride(0) == ld or n == 0
         _check(self._lib.pyro_reactor_rk4(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T), float(dt), int(n_steps),
                                           _ptr(work), _ptr(n_not_converged), _stream(stream)))
+        return Y, T
+
+    def reactor_rk4_static(self, rho, e, Y, T, dt, n_steps, n_not_converged=None, stream=None):
+        """pyro_reactor_rk4_static: reactor_rk4 for callers that may not allocate device memory.  Nothing is allocated
+        here either (no torch tensor is created): the scratch is the fixed array inside libpyro.so, which limits
+        n_species * ceil32(n) to RK4_STATIC_MAX_DOUBLES and must not be used by two overlapping calls on one device."""
+        n = rho.shape[0]
+        ld = Y.stride(0) if Y.dim() == 2 and n > 0 else n
+        _check(self._lib.pyro_reactor_rk4_static(self._h, n, ld, _ptr(rho), _ptr(e), _ptr(Y), _ptr(T), float(dt),
+                                                 int(n_steps), _ptr(n_not_converged), _stream(stream)))
         return Y, T
 
     def reactor_cn(self, rho, e, Y, T, dt, n_steps, newton_iters=4, update_tol=1e-10, work=None, n_not_converged=None,

@@ -729,6 +729,48 @@ int pyro_reactor_rk4(const pyro_mech *m, int64_t n, int64_t ld, const double *rh
     return PYRO_OK;
 }
 
+// pyro_reactor_rk4 without the caller's `work` field: the scratch is the array built into the library image
+// (pyro_reactor_kernels.cu).  No allocation, no event, no lock on this path; calls that overlap on a device race
+// (documented in pyro.h), so nothing here tries to order them.
+int pyro_reactor_rk4_static(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *e, double *Y, double *T,
+                            double dt, int32_t n_steps, int32_t *n_not_converged, void *cuda_stream) {
+    int st = check_fields(m, n, ld);
+    if (st != PYRO_OK) return st;
+    if (n_steps < 0 || !(dt == dt)) return fail(PYRO_ERR_BAD_SIZE, "n_steps must be >= 0 and dt a number");
+    if (n == 0) return PYRO_OK;
+    if (!rho || !e || !Y || !T) return fail(PYRO_ERR_NULL, "a field pointer is NULL");
+    if (!aligned8(rho) || !aligned8(e) || !aligned8(Y) || !aligned8(T) || (reinterpret_cast<uintptr_t>(n_not_converged) & 3u))
+        return fail(PYRO_ERR_ALIGN, "field pointers must be 8-byte aligned");
+    const int64_t n_pad = (n + 31) & ~(int64_t)31;
+    if (n_pad > (int64_t)PYRO_RK4_STATIC_MAX_DOUBLES / m->packed.n_species)
+        return fail(PYRO_ERR_TOO_LARGE, "pyro_reactor_rk4_static: n_species x n (rounded up to 32) = " +
+                                            std::to_string(m->packed.n_species) + " x " + std::to_string(n_pad) +
+                                            " doubles exceed the built-in scratch of " +
+                                            std::to_string((long long)PYRO_RK4_STATIC_MAX_DOUBLES) +
+                                            " doubles; march the batch in slabs or pass your own work field to pyro_reactor_rk4");
+    DeviceGuard guard(m->device);
+    cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+    pyro::ReactorArgs a{};
+    a.rates = rates_args(m, n, ld, rho, nullptr, nullptr, nullptr);
+    a.rates.e = e;
+    a.rates.n_not_converged = n_not_converged;
+    a.rates.energy = m->d_energy;
+    a.rates.tol = m->newton_tol.load(std::memory_order_relaxed);
+    a.rates.max_iter = m->newton_max_iter.load(std::memory_order_relaxed);
+    a.rates.t_mid = m->packed.lay.t_mid;
+    a.rates.single_t_mid = m->packed.lay.single_t_mid;
+    a.Y = Y; a.T = T; a.dt = dt; a.n_steps = n_steps;
+    a.energy_smem_off = m->reactor_energy_off;
+    const int warps = m->block_threads / 32;
+    int64_t blocks = (int64_t)m->sm_count * m->reactor_blocks_per_sm;
+    if (blocks > (a.rates.n_chunks + warps - 1) / warps) blocks = (a.rates.n_chunks + warps - 1) / warps;
+    const char *failed_at = "";
+    const cudaError_t ce = pyro::launch_reactor_static(a, m->device, m->block_threads, (int)blocks, m->tab_smem, m->b_tmem,
+                                                       m->two_blocks, m->reactor_smem, stream, &failed_at);
+    if (ce != cudaSuccess) return fail(PYRO_ERR_CUDA, std::string(failed_at) + ": " + cudaGetErrorString(ce));
+    return PYRO_OK;
+}
+
 namespace {
 int jacobian_call(const pyro_mech *m, int64_t n, int64_t ld, const double *rho, const double *T, const double *Y, int mode,
                   double *J, double *dSdT, void *cuda_stream, int64_t jblock);

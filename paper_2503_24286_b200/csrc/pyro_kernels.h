@@ -67,6 +67,10 @@ const void *reactor_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool singl
 cudaError_t launch_reactor(const ReactorArgs &a, int threads, int blocks, bool tables_in_shared, bool b_in_tmem, bool singles,
                            size_t smem_bytes, cudaStream_t stream);
 
+// pyro_reactor_rk4_static: acc and rates.work are taken from the library's built-in device array (pyro_reactor_kernels.cu)
+cudaError_t launch_reactor_static(const ReactorArgs &a, int device, int threads, int blocks, bool tables_in_shared, bool b_in_tmem,
+                                  bool singles, size_t smem_bytes, cudaStream_t stream, const char **failed_at);
+
 struct CnArgs {                  // implicit (Crank-Nicolson) reactor march: per-point linear algebra (pyro_cn_kernels.cu)
     int64_t n, ld;
     const double *rho, *omega;   // [n], [n_species][ld] rates at the current Newton iterate

@@ -4,17 +4,23 @@
 // kernel (pyro_rates_kernel.cuh): the stage's mass fractions, then A_k, in shared memory; omega_k and B_k in tensor
 // memory; the state Y0 and the running sum of the stage slopes in global memory (the caller's Y and scratch field),
 // which a warp touches in 256-byte segments that stay in L2 over the four stages of a step.
+#include <mutex>
+
+#include "../../include/pyro.h"
 #include "pyro_rates_kernel.cuh"
 
 namespace pyro {
 
-template <bool kTabSmem, bool kBTmem, bool kSingles>
+// kOwnScratch (pyro_reactor_rk4_static, end of this file): a.acc is the library's built-in scratch array, laid out
+// [n_species][n rounded up to a whole chunk] instead of with the caller's leading dimension.
+template <bool kTabSmem, bool kBTmem, bool kSingles, bool kOwnScratch = false>
 __global__ void __launch_bounds__(kRatesMaxThreads, kSingles ? 2 : 1) reactor_kernel(const ReactorArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ uint32_t s_tmem_base;
     const RatesArgs &r = a.rates;
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31, nthreads = blockDim.x;
     const int ns = r.n_species;
+    const int64_t acc_ld = kOwnScratch ? ((r.n + 31) & ~(int64_t)31) : r.ld;
     if (kTabSmem) {
         const uint4 *src = reinterpret_cast<const uint4 *>(r.gtab);
         uint4 *dst = reinterpret_cast<uint4 *>(smem_raw);
@@ -68,9 +74,9 @@ __global__ void __launch_bounds__(kRatesMaxThreads, kSingles ? 2 : 1) reactor_ke
             [&](int k, double v) {
                 if (live) Yp[(int64_t)k * r.ld] = v;
             },
-            [&](int k) { return live ? Ap[(int64_t)k * r.ld] : 0.0; },
+            [&](int k) { return live ? Ap[(int64_t)k * acc_ld] : 0.0; },
             [&](int k, double v) {
-                if (live) Ap[(int64_t)k * r.ld] = v;
+                if (live) Ap[(int64_t)k * acc_ld] = v;
             },
             [&](int k) -> const EnergyRow & { return energy[k]; });
         if (live) {
@@ -98,6 +104,86 @@ cudaError_t launch_reactor(const ReactorArgs &a, int threads, int blocks, bool t
     ReactorArgs copy = a;
     void *params[] = {&copy};
     return cudaLaunchKernel(reactor_kernel_ptr(tables_in_shared, b_in_tmem, singles), dim3((unsigned)blocks),
+                            dim3((unsigned)threads), params, smem_bytes, stream);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// pyro_reactor_rk4_static (include/pyro.h): the same march for callers that have no device memory to lend as `work`
+// and no way of getting any.  The stage-slope sums and the chunk counter live in the array below, which is part of
+// the library image: the CUDA driver places it on every GPU that loads libpyro.so and keeps it there until the
+// process exits, so using it costs no allocation at call time.
+//
+// g_rk4_static is a __device__ variable.  Inside host functions its name denotes a host-side shadow object, NOT the
+// storage on the GPU: handing `g_rk4_static` (or `&g_rk4_static[0]`) to a kernel or to cudaMemsetAsync from host code
+// would pass a host address.  The device address comes from cudaGetSymbolAddress, asked once per device with that
+// device current (every device has its own copy at its own address), and is what the launch below passes on.
+constexpr size_t kRk4StaticHeaderDoubles = 32;   // 256 bytes: [0] the chunk counter of the launch, rest unused
+static __device__ __align__(256) double g_rk4_static[kRk4StaticHeaderDoubles + PYRO_RK4_STATIC_MAX_DOUBLES];
+
+namespace {
+constexpr int kStaticMaxDevices = 64;
+struct Rk4StaticDevice {
+    std::once_flag once;
+    cudaError_t status = cudaErrorUnknown;
+    const char *failed_at = "";
+    double *base = nullptr;   // device address of g_rk4_static on this device
+};
+Rk4StaticDevice g_rk4_static_dev[kStaticMaxDevices];
+
+const void *reactor_static_kernel_ptr(bool tables_in_shared, bool b_in_tmem, bool singles) {
+    if (singles) {
+        if (tables_in_shared) return b_in_tmem ? (const void *)reactor_kernel<true, true, true, true> : (const void *)reactor_kernel<true, false, true, true>;
+        return b_in_tmem ? (const void *)reactor_kernel<false, true, true, true> : (const void *)reactor_kernel<false, false, true, true>;
+    }
+    if (tables_in_shared) return b_in_tmem ? (const void *)reactor_kernel<true, true, false, true> : (const void *)reactor_kernel<true, false, false, true>;
+    return b_in_tmem ? (const void *)reactor_kernel<false, true, false, true> : (const void *)reactor_kernel<false, false, false, true>;
+}
+
+// Runs once per device, with that device current: looks up where this device keeps the array and lifts the dynamic
+// shared-memory limit of the eight kernel variants to the device maximum (a property of the function, so no later
+// call has to touch it).  Neither call allocates.
+void rk4_static_setup(Rk4StaticDevice &d) {
+    void *p = nullptr;
+    d.failed_at = "cudaGetSymbolAddress(g_rk4_static)";
+    if ((d.status = cudaGetSymbolAddress(&p, g_rk4_static)) != cudaSuccess) return;
+    int dev = 0, optin = 0;
+    d.failed_at = "cudaDeviceGetAttribute(MaxSharedMemoryPerBlockOptin)";
+    if ((d.status = cudaGetDevice(&dev)) != cudaSuccess) return;
+    if ((d.status = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess) return;
+    for (int v = 0; v < 8; ++v) {
+        const void *fn = reactor_static_kernel_ptr((v & 1) != 0, (v & 2) != 0, (v & 4) != 0);
+        cudaFuncAttributes fa{};
+        d.failed_at = "cudaFuncGetAttributes(reactor, built-in scratch)";
+        if ((d.status = cudaFuncGetAttributes(&fa, fn)) != cudaSuccess) return;
+        d.failed_at = "cudaFuncSetAttribute(reactor, built-in scratch)";
+        if ((d.status = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes)) != cudaSuccess) return;
+        if ((d.status = cudaFuncSetAttribute(fn, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared)) != cudaSuccess) return;
+    }
+    d.base = static_cast<double *>(p);
+    d.failed_at = "";
+}
+}   // namespace
+
+// `a` as for launch_reactor except acc and rates.work, which are set here.  `device` is the current device.
+cudaError_t launch_reactor_static(const ReactorArgs &a, int device, int threads, int blocks, bool tables_in_shared, bool b_in_tmem,
+                                  bool singles, size_t smem_bytes, cudaStream_t stream, const char **failed_at) {
+    *failed_at = "device ordinal beyond the built-in scratch bookkeeping";
+    if (device < 0 || device >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+    Rk4StaticDevice &d = g_rk4_static_dev[device];
+    std::call_once(d.once, [&d] { rk4_static_setup(d); });
+    *failed_at = d.failed_at;
+    if (d.status != cudaSuccess) return d.status;
+    ReactorArgs copy = a;
+    copy.rates.work = reinterpret_cast<unsigned long long *>(d.base);
+    copy.acc = d.base + kRk4StaticHeaderDoubles;
+    // The array keeps whatever the last call left in it.  Only the chunk counter has to start at zero; the slope sums
+    // are written (stage 2 of a step) before they are read (stages 3, 4 and the update), so they need no clearing.
+    *failed_at = "cudaMemsetAsync(chunk counter of the built-in scratch)";
+    cudaError_t ce = cudaMemsetAsync(copy.rates.work, 0, sizeof(unsigned long long), stream);
+    if (ce != cudaSuccess) return ce;
+    *failed_at = "launch of the reactor kernel (built-in scratch)";
+    void *params[] = {&copy};
+    return cudaLaunchKernel(reactor_static_kernel_ptr(tables_in_shared, b_in_tmem, singles), dim3((unsigned)blocks),
                             dim3((unsigned)threads), params, smem_bytes, stream);
 }
 
