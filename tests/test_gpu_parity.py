@@ -875,6 +875,149 @@ def test_reactor_cn_linear_decay_closed_form_and_convergence_count():
     assert not bool(torch.isfinite(Yr).all()) or float(Yr.abs().max().item()) > 1e10   # the explicit march diverges at z = 20
 
 
+# ------------------------------------------------------------------ marches on which most reactors move
+# The synthetic mechanisms span more than a hundred decades of chemical time scale from one state to the next, so one
+# step size for a whole batch leaves almost every reactor where it started (and an unchanged Y then passes any
+# comparison).  The tests below group the reactors by their OWN time scale and march every group at its own step.
+def stiffness_groups(orc, rho, T, Y, ratio=10.0):
+    """[(indices, lambda_max)]: the reactors sorted by lambda_p = largest row sum of |dS/dY|/rho at fixed (rho, e) (the
+    oracle's Jacobian), cut into runs whose lambda stay within `ratio` of one another."""
+    J, _, _, _ = orc.get_jacobian(rho, T, Y, mode=1)
+    lam = (np.abs(J).sum(axis=1) / np.asarray(rho)[None, :]).max(axis=0)
+    order = np.argsort(lam)
+    groups, cur = [], [order[0]]
+    for p in order[1:]:
+        if lam[p] <= ratio * lam[cur[0]]:
+            cur.append(p)
+        else:
+            groups.append(np.array(cur))
+            cur = [p]
+    groups.append(np.array(cur))
+    return [(g, float(lam[g].max())) for g in groups]
+
+
+def moved_fraction(Y0, Y1, threshold):
+    """Share of the reactors of which some mass fraction changed by more than `threshold`, relatively."""
+    return float(np.mean(np.max(np.abs(Y1 - Y0) / (np.abs(Y0) + 1e-30), axis=0) > threshold))
+
+
+def tempered_residual(Yg, Yr, Yb):
+    """max |dY| / scale with a scale an unchanged Y cannot meet: the size Yb of the terms added into an entry wherever
+    those are visible in it (Yb >= 1e-4 |Y|: the entry moved in the fifth digit or before), else Yb + |Y| (there the
+    rounding of Y itself, 1e-16 |Y|, is what bounds the agreement)."""
+    scale = np.where(Yb >= 1e-4 * np.abs(Yr), Yb, Yb + np.abs(Yr)) + 1e-300
+    return float(np.max(np.abs(Yg - Yr) / scale))
+
+
+def tempered_case(case, n):
+    if case == "all_paths":
+        mech = hand_cases.all_paths_mechanism()
+        rho, T, Y = hand_cases.random_states(mech, n)
+    else:
+        cfg = {"cfg0": 0, "cfg2": 2, "cfg3": 3}[case]
+        mech = inputs.config_mechanism(cfg)
+        st = inputs.config_states(cfg, n=n)
+        rho, T, Y = st["rho"], st["T"], st["Y"]
+    orc = oracle.Oracle(mech)
+    e = np.array([orc.mixture_e(T[p], Y[:, p]) for p in range(n)])
+    return mech, orc, rho, T, Y, e
+
+
+@pytest.mark.parametrize("case,n", [("cfg0", 3001), ("cfg2", 700), ("cfg3", 120), ("all_paths", 333)])
+def test_reactor_rk4_tempered_most_reactors_move(case, n):
+    """pyro_reactor_rk4 against the oracle, one launch per stiffness group at dt = 0.2 / lambda_max of the group, 7 steps:
+    in every launch at least 80 % of the reactors change some Y_k by more than 1e-6 (asserted), over the batch at least
+    80 % by more than 1e-3, and every entry is compared on the scale of the terms the march added to it."""
+    mech, orc, rho, T, Y, e = tempered_case(case, n)
+    gm = binding.Mechanism(mech)
+    Tg = T * 1.03
+    worst, worst_T, moved3, launches = 0.0, 0.0, 0.0, 0
+    for g, lam_max in stiffness_groups(orc, rho, T, Y):
+        dt = 0.2 / lam_max
+        Yr, Tr, Yb, bad_r = orc.reactor_rk4(rho[g], e[g], Y[:, g], Tg[g], dt, 7)
+        assert np.isfinite(Yr).all() and np.isfinite(Tr).all() and np.abs(Yr).max() < 10.0   # stable for every reactor of the group
+        Yd, Td = dev(Y[:, g]), dev(Tg[g])
+        bad = torch.zeros(1, dtype=torch.int32, device="cuda")
+        gm.reactor_rk4(dev(rho[g]), dev(e[g]), Yd, Td, dt, 7, n_not_converged=bad)
+        torch.cuda.synchronize()
+        Yg, Tgpu = Yd.cpu().numpy(), Td.cpu().numpy()
+        assert np.isfinite(Yg).all() and np.isfinite(Tgpu).all()
+        m6 = moved_fraction(Y[:, g], Yr, 1e-6)
+        assert m6 >= 0.8, f"{case}: only {m6:.2f} of the {len(g)} reactors of a launch moved (dt {dt:.3e})"
+        assert moved_fraction(Y[:, g], Yg, 1e-6) >= 0.8
+        moved3 += moved_fraction(Y[:, g], Yr, 1e-3) * len(g)
+        worst = max(worst, tempered_residual(Yg, Yr, Yb))
+        worst_T = max(worst_T, float(np.max(np.abs(Tgpu - Tr) / Tr)))
+        assert int(bad.item()) == bad_r
+        launches += 1
+    print(f"{case}: {launches} launches, moved by > 1e-3: {moved3 / n:.3f} of {n} reactors, max |dY|/scale = {worst:.2e}, max |dT|/T = {worst_T:.2e}")
+    assert moved3 >= 0.8 * n
+    assert worst <= REACTOR_TOL and worst_T <= 1e-9
+
+
+@pytest.mark.parametrize("z", [0.1, 1.0, 2.5])
+def test_reactor_rk4_linear_decay_taylor_polynomial(z):
+    """GPU twin of oracle pin R1: A -> B at a constant rate coefficient k; one RK4 step of size z/k multiplies Y_A by
+    the degree-4 Taylor polynomial of exp(-z) -- every reactor, 5 steps, to 1e-14."""
+    z4 = [0.0] * 4
+    sp = [dict(W=20.0, lo=[3.5, *z4, -1000.0, 2.0]), dict(W=20.0, lo=[3.0, *z4, -3000.0, 3.0])]
+    k, steps, n = 2.5e5, 5, 4099
+    mech = inputs.simple_mechanism(sp, [dict(reac={0: 1}, prod={1: 1}, A=k, b=0.0, theta=0.0, reversible=0)])
+    gm, orc = binding.Mechanism(mech), oracle.Oracle(mech)
+    ya = np.linspace(0.1, 0.9, n)
+    Y = np.vstack([ya, 1 - ya])
+    T = np.full(n, 1100.0)
+    rho = np.full(n, 0.4)
+    e = np.array([orc.mixture_e(T[p], Y[:, p]) for p in range(n)])
+    Yd, Td = dev(Y), dev(T)
+    gm.reactor_rk4(dev(rho), dev(e), Yd, Td, z / k, steps)
+    torch.cuda.synchronize()
+    growth = (1 - z + z**2 / 2 - z**3 / 6 + z**4 / 24) ** steps
+    Yg = Yd.cpu().numpy()
+    assert np.max(np.abs(Yg[0] - ya * growth)) < 1e-14
+    assert np.max(np.abs(Yg[1] - (1 - ya * growth))) < 1e-14     # mass is conserved: Y_B = 1 - Y_A
+
+
+@pytest.mark.parametrize("case,n", [("cfg0", 1000), ("cfg2", 300), ("all_paths", 200)])
+@pytest.mark.parametrize("factor", [10.0, 100.0])
+def test_reactor_cn_tempered_far_from_the_identity(case, n, factor):
+    """pyro_reactor_cn against the oracle's Crank-Nicolson march (partial pivoting) per stiffness group, at `factor`
+    times the group's explicit step 0.2 / lambda_max, 2 steps of 4 Newton iterations.  At factor 100 the matrix the
+    kernel factors WITHOUT pivoting, I - dt/(2 rho) J, has |dt/(2 rho) J| up to 10 for every group: the reactors lost to
+    that (or to a Newton iteration that diverges at such a step on either side) are counted and reported."""
+    mech, orc, rho, T, Y, e = tempered_case(case, n)
+    gm = binding.Mechanism(mech)
+    Tg = T * 1.03
+    compared, lost, worst, moved, norm_min = 0, 0, 0.0, 0.0, np.inf
+    for g, lam_max in stiffness_groups(orc, rho, T, Y):
+        dt = factor * 0.2 / lam_max
+        norm_min = min(norm_min, 0.5 * dt * lam_max)
+        Yr, Tr, Yb, lu, _ = orc.reactor_cn(rho[g], e[g], Y[:, g], Tg[g], dt, 2, newton_iters=4)
+        ok = np.isfinite(Yr).all(axis=0) & np.isfinite(Tr) & (np.abs(Yr).max(axis=0) < 10.0)
+        Yd, Td = dev(Y[:, g]), dev(Tg[g])
+        gm.reactor_cn(dev(rho[g]), dev(e[g]), Yd, Td, dt, 2, newton_iters=4)
+        torch.cuda.synchronize()
+        Yg, Tgpu = Yd.cpu().numpy(), Td.cpu().numpy()
+        if not ok.any():
+            continue
+        scale = (np.where(Yb >= 1e-4 * np.abs(Yr), Yb, Yb + np.abs(Yr)) + 1e-300)[:, ok]
+        with np.errstate(invalid="ignore"):
+            r = np.max(np.abs(Yg[:, ok] - Yr[:, ok]) / scale, axis=0)
+            rT = np.abs(Tgpu[ok] - Tr[ok]) / Tr[ok]
+        good = (r <= 1e-9) & (rT <= 1e-8)
+        compared += int(ok.sum())
+        lost += int((~good).sum())
+        if good.any():
+            worst = max(worst, float(r[good].max()))
+        moved += moved_fraction(Y[:, g][:, ok], Yr[:, ok], 1e-3) * int(ok.sum())
+    print(f"{case} x{factor:g}: |dt/(2 rho) J| >= {norm_min:.1f} in every launch, reactors compared {compared}/{n}, "
+          f"lost to the LU without pivoting or a diverging Newton iteration {lost}, moved by > 1e-3: {moved / max(compared, 1):.3f}, "
+          f"max |dY|/scale of the rest = {worst:.2e}")
+    assert compared >= 0.8 * n
+    assert moved >= 0.8 * compared
+    assert lost == 0
+
+
 # ------------------------------------------------------------------ widened rows at the sizes bench.py times, sampled
 def test_transport_and_reactors_at_bench_size_sampled(mechs):
     """The launch configurations of bench.py's widened legs on configs[2]: transport on 2^20 points, the RK4 march on
