@@ -48,6 +48,45 @@ def test_two_ranks_own_disjoint_work_and_share_only_the_step_time():
     assert v0 == v1 == 2 * 257 / 15e-3
 
 
+def _slab_worker(rank, world, port, out):
+    """What `bench.py --scaling strong` does on every rank, with the oracle in place of the GPU: the same seeded field,
+    this rank's slab of it, the rates of the slab's points."""
+    from oracle import oracle
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        full = inputs.config_states(0, n=1000, seed=sharding.rank_state_seed(0, 0))
+        lo, cnt = sharding.rank_slab(1000, rank, world)
+        st = {k: np.ascontiguousarray(v[..., lo:lo + cnt]) for k, v in full.items()}
+        om = oracle.Oracle(inputs.config_mechanism(0)).get_net_production_rates(st["rho"], st["T"], st["Y"], want_bound=False)
+        om = om[0] if isinstance(om, tuple) else om
+        out.put((rank, lo, cnt, np.asarray(om)))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_strong_sharding_slabs_reproduce_the_single_rank_field():
+    """The ranks' slab results, laid side by side, are the single-rank result of the whole field: every point computed
+    exactly once, none skipped, bit for bit (points are independent)."""
+    from oracle import oracle
+    world, port = 2, _free_port()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    procs = [ctx.Process(target=_slab_worker, args=(r, world, port, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = sorted((q.get(timeout=120) for _ in procs), key=lambda r: r[0])
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    full = inputs.config_states(0, n=1000, seed=sharding.rank_state_seed(0, 0))
+    whole = oracle.Oracle(inputs.config_mechanism(0)).get_net_production_rates(full["rho"], full["T"], full["Y"], want_bound=False)
+    whole = whole[0] if isinstance(whole, tuple) else whole
+    assert res[0][1] == 0 and res[0][1] + res[0][2] == res[1][1] and res[1][1] + res[1][2] == 1000
+    joined = np.concatenate([r[3] for r in res], axis=1)
+    assert joined.shape == whole.shape and np.array_equal(joined, whole)
+
+
 def test_slabs_partition_any_size():
     for n in (0, 1, 31, 32, 33, 1000, 4096 + 5):
         for world in (1, 2, 3, 8):
