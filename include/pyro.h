@@ -24,7 +24,7 @@
  *   the interface and change no result: PYRO_TABLES=shared|global, PYRO_RATES_BLOCK=<threads>,
  *   PYRO_B_PLANE=shared, PYRO_CARVEOUT=<percent>, PYRO_RATES_POINTS=1|2 (grid points per thread of the rates kernel), PYRO_RATES_TWO_BLOCKS=0|1, PYRO_PACK_SINGLES=0|1,
  *   PYRO_HOST_SLAB=<points> (pyro_source_terms_host), PYRO_JAC_KERNEL=point|block (the one-thread-per-point / the block-cooperative Jacobian kernel), PYRO_JAC_V_PLANE=shared, PYRO_JAC_BLOCK=<threads>, PYRO_JAC_EXT=global
- *   (pyro_get_jacobian), PYRO_CN_BLOCK=32|64 (points per block of the Crank-Nicolson LU kernel; read per call), PYRO_DEBUG=1 (prints the launch shape to stderr).
+ *   (pyro_get_jacobian), PYRO_CN_BLOCK=32|64 (points per block of the Crank-Nicolson LU kernel; read once per process at the first Crank-Nicolson call; 64 only up to 97 species), PYRO_DEBUG=1 (prints the launch shape to stderr).
  */
 #ifndef PYRO_H
 #define PYRO_H
@@ -204,7 +204,13 @@ int pyro_reactor_rk4_static(const pyro_mech *mech, int64_t n, int64_t ld, const 
  *   update_tol       a point whose last Newton update max_k |dY_k| of a step is not below it (or not finite) is counted
  *   work             device scratch of *doubles doubles as pyro_reactor_cn_work_doubles(mech, ld, &doubles) reports; must not overlap Y
  *   n_not_converged  += temperature solves that hit their cap + (point, step) pairs counted by update_tol
- * Mechanisms of more than 127 species: PYRO_ERR_UNSUPPORTED. */
+ * Mechanisms of more than 127 species: PYRO_ERR_UNSUPPORTED.
+ * Step-size regime of the LU.  The elimination takes the pivots in the given order and inverts them without a magnitude
+ * check.  That is safe while I - dt/(2 rho) J is diagonally dominated and has been verified beyond it, against an
+ * elimination with partial pivoting, up to |dt/(2 rho) J|_inf = 10 (100 times the explicit stability step; no reactor
+ * of the test batches lost a digit there).  Above that regime element growth is neither bounded nor detected as such: the
+ * only report is n_not_converged (a non-finite or too large last update), so march stiffer steps with a tolerance that
+ * means something, or in several smaller steps. */
 int pyro_reactor_cn_work_doubles(const pyro_mech *mech, int64_t ld, int64_t *doubles);
 int pyro_reactor_cn(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *e, double *Y,
                     double *T, double dt, int32_t n_steps, int32_t newton_iters, double update_tol, double *work,

@@ -23,24 +23,35 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xptxas", "-v"]
 
 
-def _stale():
-    if not os.path.exists(LIB):
+STAMP = os.path.join(OBJ, "defines.txt")   # the -D options the objects and the library on disk were built with
+
+
+def _built_defines():
+    try:
+        return open(STAMP).read()
+    except OSError:
+        return None
+
+
+def _stale(defines=()):
+    if not os.path.exists(LIB) or _built_defines() != " ".join(defines):
         return True
     t = os.path.getmtime(LIB)
     return any(os.path.getmtime(os.path.join(CSRC, f)) > t for f in SOURCES + HEADERS)
 
 
 def build_libpyro(force=False, defines=(), verbose=False):
-    if not (force or _stale()):
+    if not (force or _stale(defines)):
         return LIB
     nvcc = os.environ.get("NVCC", "nvcc")
     os.makedirs(OBJ, exist_ok=True)
+    same_defines = _built_defines() == " ".join(defines)   # objects compiled with other -D options are never reused
     newest_header = max(os.path.getmtime(os.path.join(CSRC, h)) for h in HEADERS)
 
     def compile_one(src):
         obj = os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
         path = os.path.join(CSRC, src)
-        if (not force and not defines and os.path.exists(obj)
+        if (not force and same_defines and os.path.exists(obj)
                 and os.path.getmtime(obj) > max(os.path.getmtime(path), newest_header)):
             return obj, None, ""
         cmd = [nvcc, *NVCC_FLAGS, *defines, "-c", "-o", obj, path]
@@ -62,6 +73,8 @@ def build_libpyro(force=False, defines=(), verbose=False):
         raise RuntimeError("nvcc failed building libpyro.so")
     with open(os.path.join(_HERE, "libpyro.build.log"), "w") as f:
         f.write(log)
+    with open(STAMP, "w") as f:
+        f.write(" ".join(defines))
     return LIB
 
 

@@ -10,6 +10,8 @@
 
 #include <cstdlib>
 
+#include <mutex>
+
 #include "pyro_kernels.h"
 
 namespace pyro {
@@ -333,8 +335,16 @@ template <int NC, int TB> __global__ void __launch_bounds__(TB) cn_newton_kernel
 }
 
 constexpr int kCnPanel = 4;
+constexpr size_t kCnSmemLimit = 227 * 1024;   // dynamic shared memory a block can get on sm_100
+static size_t cn_smem_bytes(int n_species, int tb) { return ((size_t)kCnPanel * n_species + kCnRing) * tb * sizeof(double); }
 int cn_block_threads(int n_species) {
-    if (const char *env = std::getenv("PYRO_CN_BLOCK")) return std::atoi(env) == 64 ? 64 : 32;
+    // PYRO_CN_BLOCK is a test hook, read once per process (not per call: getenv is not safe against a concurrent setenv)
+    static const int forced = [] {
+        const char *env = std::getenv("PYRO_CN_BLOCK");
+        return env ? (std::atoi(env) == 64 ? 64 : 32) : 0;
+    }();
+    // 64 points per block only where their panels fit the shared memory of one block (up to 97 species)
+    if (forced == 64 && cn_smem_bytes(n_species, 64) <= kCnSmemLimit) return 64;
     return 32;   // measured at 53 species: 271 ns per reactor-iteration against 300 with 64 (more blocks, more loads in flight)
 }
 
@@ -342,13 +352,35 @@ cudaError_t launch_cn_begin_step(const CnArgs &a, cudaStream_t stream) {
     cn_begin_step_kernel<<<dim3((unsigned)((a.n + 255) / 256)), dim3(256), 0, stream>>>(a);
     return cudaGetLastError();
 }
+namespace {
+// The dynamic shared-memory limit is a property of the function on a device, shared by every mechanism and host thread:
+// raised once per device to the device maximum, so that no launch ever lowers it under a concurrent one.
+struct CnDeviceSetup {
+    std::once_flag once;
+    cudaError_t status = cudaSuccess;
+};
+CnDeviceSetup g_cn_setup[64];
+void cn_setup_device(CnDeviceSetup &d, int dev) {
+    int optin = 0;
+    if ((d.status = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev)) != cudaSuccess) return;
+    for (const void *fn : {(const void *)cn_newton_kernel<kCnPanel, 64>, (const void *)cn_newton_kernel<kCnPanel, 32>}) {
+        cudaFuncAttributes fa{};
+        if ((d.status = cudaFuncGetAttributes(&fa, fn)) != cudaSuccess) return;
+        if ((d.status = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, optin - (int)fa.sharedSizeBytes)) != cudaSuccess) return;
+    }
+}
+}   // namespace
+
 cudaError_t launch_cn_newton(const CnArgs &a, cudaStream_t stream) {
     const int tb = cn_block_threads(a.n_species);
-    const size_t smem = ((size_t)kCnPanel * a.n_species + kCnRing) * tb * sizeof(double);
-    // the limit is a property of the function on the current device: set it on every launch (cheap; no process-wide state)
-    const void *fn = tb == 64 ? (const void *)cn_newton_kernel<kCnPanel, 64> : (const void *)cn_newton_kernel<kCnPanel, 32>;
-    cudaError_t ce = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = cn_smem_bytes(a.n_species, tb);
+    int dev = 0;
+    cudaError_t ce = cudaGetDevice(&dev);
     if (ce != cudaSuccess) return ce;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    CnDeviceSetup &d = g_cn_setup[dev];
+    std::call_once(d.once, [&d, dev] { cn_setup_device(d, dev); });
+    if (d.status != cudaSuccess) return d.status;
     const dim3 grid((unsigned)((a.n + tb - 1) / tb));
     if (tb == 64) cn_newton_kernel<kCnPanel, 64><<<grid, dim3(64), smem, stream>>>(a);
     else cn_newton_kernel<kCnPanel, 32><<<grid, dim3(32), smem, stream>>>(a);
