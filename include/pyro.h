@@ -227,8 +227,12 @@ int pyro_reactor_cn(const pyro_mech *mech, int64_t n, int64_t ld, const double *
  *   PYRO_JAC_FIXED_E   rho and the internal energy e (an adiabatic isochoric reactor (A.1); what the paper's listing 23
  *                      differentiates, through the temperature inversion):  J_ik - dS_i/dT e_k(T)/c_v(T,Y)
  * The derivatives of the third-body and Lindemann / Troe forms are included (through [M] and through T).
- * Mechanisms of more than 127 species: PYRO_ERR_UNSUPPORTED.  Launches on one handle share a scratch buffer and are
- * ordered after one another (also across streams). */
+ * Mechanisms of more than 127 species: PYRO_ERR_UNSUPPORTED.  The limit is the tensor memory of an SM: per species row the
+ * kernel keeps two FP64 accumulators for each of a warp's points (the column dS_i/dY_k being built and dS_i/dT), four of the
+ * 512 columns a block can hold, so 127 species + the [M] row fill it; the rates path needs half of that and goes to 255.
+ * (The dense output is 8 n_species^2 bytes per point -- 131 KB at 128 species -- so larger mechanisms want a sparse
+ * output format before they want a larger kernel.)  Launches on one handle share a scratch buffer and are ordered after
+ * one another (also across streams). */
 enum { PYRO_JAC_FIXED_T = 0, PYRO_JAC_FIXED_E = 1 };
 int pyro_get_jacobian(const pyro_mech *mech, int64_t n, int64_t ld, const double *rho, const double *T,
                       const double *Y, int mode, double *J, double *dSdT, void *cuda_stream);
