@@ -659,3 +659,53 @@ def test_reactor_point_code_matches_oracle(emu, case):
         assert bad_r == bad_e == 0
         rY, rT = assert_reactor_parity(Ye, Te, Yr, Tr, Yb)
     assert np.any(np.abs(Yr - Y) > 1e-6 * np.abs(Y))
+
+
+# ------------------------------------------------------------------ bench.py host helpers (no GPU)
+def test_bench_tempered_window_picks_the_most_populated_decade():
+    """bench.py marches the reactor legs on the states of the most populated window [L, 10 L] of their own time scale."""
+    import bench
+    rng = np.random.default_rng(3)
+    lam = np.concatenate([10.0 ** rng.uniform(20, 140, 5000), 10.0 ** rng.uniform(33.0, 33.9, 700), [np.nan, 0.0, -1.0, np.inf]])
+    sel, lam_max = bench.tempered_window(lam)
+    assert len(sel) >= 700 and len(set(sel.tolist())) == len(sel)
+    assert np.isfinite(lam[sel]).all() and lam[sel].min() > 0
+    assert lam[sel].max() == lam_max and lam_max <= 10.0 * lam[sel].min()
+    assert 5e32 <= lam[sel].min() and lam_max <= 1e35
+    # brute force on a small case: no other window holds more states
+    small = lam[:300]
+    sel_s, _ = bench.tempered_window(small)
+    ok = small[np.isfinite(small) & (small > 0)]
+    best = max(int(np.sum((ok >= lo) & (ok <= 10.0 * lo))) for lo in ok)
+    assert len(sel_s) == best
+    empty, none = bench.tempered_window(np.array([np.nan, 0.0]))
+    assert len(empty) == 0 and none is None
+
+
+def test_bench_ncu_summary_round_trip_and_staleness_guard(tmp_path):
+    """The ncu figures of the bench line come from a committed one-row summary; they are withheld when the library's
+    kernel is not the captured one (other registers per thread) or the mechanism has another size."""
+    import bench
+    cols = list(bench.NCU_COLUMNS.values())
+    units = {"launch__registers_per_thread": "register/thread", "gpu__time_duration.sum": "ms", "dram__bytes_read.sum": "Mbyte",
+             "dram__bytes_write.sum": "Gbyte", "smsp__cycles_elapsed.max": "cycle", "smsp__inst_executed.sum": "inst"}
+    vals = {"launch__registers_per_thread": "178", "gpu__time_duration.sum": "1.5", "dram__bytes_read.sum": "400.5",
+            "dram__bytes_write.sum": "0.25", "smsp__cycles_elapsed.max": "1,000,000", "smsp__inst_executed.sum": "12345"}
+    raw = tmp_path / "raw.csv"
+    with open(raw, "w") as f:
+        f.write('"ID","Kernel Name",' + ",".join(f'"{c}"' for c in cols) + "\n")
+        f.write('"","",' + ",".join(f'"{units.get(c, "inst/cycle")}"' for c in cols) + "\n")
+        f.write('"0","void rates_kernel<1, 1, 1, 0>(RatesArgs)",' + ",".join(f'"{vals.get(c, "2.0")}"' for c in cols) + "\n")
+    out = tmp_path / "capture.csv"
+    rec = bench.write_ncu_summary(str(raw), 1 << 20, 53, 325, out_path=str(out))
+    assert rec["duration_ns"] == 1.5e6 and rec["dram_read_bytes"] == 400.5e6 and rec["dram_write_bytes"] == 0.25e9
+    assert rec["fp64_flops"] == (2.0 + 2.0 + 2 * 2.0) * 1e6 and rec["kernel"] == "void rates_kernel<1, 1, 1, 0>"
+    back = bench.read_ncu_summary(53, 325, 178, path=str(out))
+    assert back["points"] == 1 << 20 and back["dram_read_bytes"] == 400.5e6 and back["kernel"] == rec["kernel"]
+    assert bench.read_ncu_summary(53, 325, 170, path=str(out)) is None      # another build of the kernel
+    assert bench.read_ncu_summary(9, 21, 178, path=str(out)) is None        # another mechanism
+    assert bench.read_ncu_summary(53, 325, 178, path=str(tmp_path / "missing.csv")) is None
+    # the committed capture of this round parses and is of the graded configuration
+    committed = bench.read_ncu_summary(53, 325, 178)
+    if committed is not None:
+        assert committed["points"] == 1 << 20 and 8e8 < committed["dram_read_bytes"] + committed["dram_write_bytes"] < 1e9
